@@ -1,0 +1,198 @@
+/* kripke.h - C ABI of the B200-native fused bitmask Kripke evaluator (libkripke_b200.so).
+ *
+ * What the library computes (citations: P:n = /root/reference/PAPER.md line n):
+ *   A batch of modal formulas (postfix programs over T, F, p_i, not, box, dia, and, or, imp;
+ *   grammar P:38) is evaluated on every labelled frame of n worlds in a frame class and on every
+ *   valuation of n_vars variables, by the bitwise recurrence of P:46-56 (section 3, Lemma 1,
+ *   Theorem 1): a world set is an n-bit integer, box x = {w : succ[w] & ~x == 0},
+ *   dia x = {w : succ[w] & x != 0}.  Frames and valuations are derived from indices and never
+ *   stored (Proposition 1).  Per formula the library returns Algorithm 1's outputs
+ *   (P:80-112): the number of refuting (frame, valuation) models, the number of refuting frames,
+ *   and the lexicographically first refuting (frame, valuation) with its least falsifying world -
+ *   a certificate in the sense of Definition 1.  The pair path returns the same for
+ *   "truth sets differ" (Definition 2 / Proposition 4).
+ *
+ * Index conventions (readings R2, R3):
+ *   frame index f:     succ[w] = (f >> (w*n)) & (2^n - 1); bit u of succ[w] is the edge w -> u.
+ *   valuation index v: truth(p_i) = (v >> (i*n)) & (2^n - 1); bit w set iff p_i holds at w.
+ *   classes:    K all frames; T reflexive; S4 reflexive + transitive; S5 equivalences.
+ *   class order:       frames of a class are enumerated by ascending f; a frame range
+ *                      [frame_begin, frame_begin + frame_count) indexes that enumeration.
+ *   witness.frame is always the K-index f itself.
+ *
+ * Conventions for every entry point:
+ *   - returns KRIPKE_OK (0) or a negative kripke_status; never throws, aborts or prints;
+ *   - "host" / "device" on a pointer says where the memory lives; the caller owns every buffer it
+ *     passes; the library owns only what a handle holds and frees it in the matching destroy call;
+ *   - device work is enqueued on `stream` (a cudaStream_t passed as void*, NULL = default stream)
+ *     and the call returns without waiting, unless stated otherwise; outputs are valid once the
+ *     stream has been synchronised;
+ *   - there is no CPU fallback: without a CUDA device every compute call returns KRIPKE_ECUDA.
+ */
+#ifndef KRIPKE_H
+#define KRIPKE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    KRIPKE_OK = 0,
+    KRIPKE_EINVAL = -1,        /* null pointer, size out of range, bad class or flags            */
+    KRIPKE_EPROGRAM = -2,      /* malformed postfix program (bad opcode, underflow, != 1 result) */
+    KRIPKE_EUNSUPPORTED = -3,  /* valid request outside the implementation limits below         */
+    KRIPKE_ECUDA = -4,         /* a CUDA call failed; see kripke_last_cuda_error()               */
+    KRIPKE_ENOMEM = -5         /* host allocation failed                                         */
+} kripke_status;
+
+/* Postfix opcodes (one byte each).  The paper gives no encoding ("concatenated RPN
+ * bytecode"); this one is fixed here.  Binary operators pop y then x and push (x op y). */
+enum {
+    KRIPKE_OP_TOP = 0x00, KRIPKE_OP_BOT = 0x01,
+    KRIPKE_OP_VAR0 = 0x10,                       /* 0x10 + i is variable p_i, i < n_vars <= 4 */
+    KRIPKE_OP_NOT = 0x20, KRIPKE_OP_BOX = 0x21, KRIPKE_OP_DIA = 0x22,
+    KRIPKE_OP_AND = 0x30, KRIPKE_OP_OR = 0x31, KRIPKE_OP_IMP = 0x32
+};
+
+enum { KRIPKE_CLASS_K = 0, KRIPKE_CLASS_T = 1, KRIPKE_CLASS_S4 = 2, KRIPKE_CLASS_S5 = 3 };
+
+/* Implementation limits (the paper's own are P:390: 32-bit masks, 16 successor slots, 48-slot
+ * stack, <= 4 variables, k*n < 63). */
+#define KRIPKE_MAX_WORLDS 6u
+#define KRIPKE_MAX_VARS 4u
+#define KRIPKE_MAX_STACK 16u        /* postfix stack slots a program may need               */
+#define KRIPKE_MAX_PROGRAM_LEN 64u  /* opcodes per program                                   */
+#define KRIPKE_MAX_MODEL_BITS 61u   /* n*n + n_vars*n must not exceed this                   */
+
+/* flags of the *_range calls */
+enum {
+    KRIPKE_ACCUMULATE = 1u << 0,      /* add to counts_out / keep the smaller witness instead of
+                                         overwriting (chunked scans, multi-GPU shards)            */
+    KRIPKE_KERNEL_AUTO = 0u << 4,     /* bit-sliced kernel where it applies, else the scalar one  */
+    KRIPKE_KERNEL_SCALAR = 1u << 4,   /* force the scalar kernel (Algorithm 1 restated, one model
+                                         per thread iteration): baseline / ablation / cross-check */
+    KRIPKE_KERNEL_SLICED = 2u << 4,   /* force the bit-sliced kernel; KRIPKE_EUNSUPPORTED if the
+                                         shape or a program does not fit it                       */
+    KRIPKE_KERNEL_MASK = 3u << 4,
+    KRIPKE_REDUCE_BLOCK = 0u << 8,    /* scalar kernel only: one atomic pair per (block, formula),
+                                         the paper's revised reduction                     */
+    KRIPKE_REDUCE_WARP = 1u << 8,     /* one atomic pair per (warp, formula)                      */
+    KRIPKE_REDUCE_THREAD = 2u << 8,   /* one per failing (frame, formula): the paper's original
+                                         frame-atomic variant, kept for ablation   */
+    KRIPKE_REDUCE_MASK = 3u << 8
+};
+
+/* Outputs, 16 bytes each ("16 bytes per formula"; layout is reading R18). */
+typedef struct {
+    uint64_t refuting_models;   /* #{(f, v) in range : truth set != all worlds}                  */
+    uint64_t refuting_frames;   /* #{f in range : some v refutes}; valid frames = range - this   */
+} kripke_count_t;
+
+typedef struct {
+    uint64_t frame;             /* K-index f of the first refuting (f, v); UINT64_MAX = none     */
+    uint32_t valuation;         /* v                                                             */
+    uint32_t world;             /* least w with bit w of the truth set clear (pairs: least w
+                                   where the two truth sets differ)                              */
+} kripke_witness_t;
+
+#define KRIPKE_NO_WITNESS UINT64_MAX
+
+/* A validated batch of programs, lowered and resident on the current CUDA device. */
+typedef struct kripke_programs kripke_programs_t;
+
+const char *kripke_version(void);
+
+/* Last CUDA error code (a cudaError_t) seen by this thread's most recent failing call, 0 if none. */
+int kripke_last_cuda_error(void);
+
+/* Checks B = n_formulas postfix programs (HOST pointers): program b is
+ * code[offsets[b] .. offsets[b+1]); offsets has B+1 non-decreasing entries.  Each must use only the
+ * opcodes above with variable index < n_vars, never underflow, leave exactly one value, be at most
+ * KRIPKE_MAX_PROGRAM_LEN long and need at most KRIPKE_MAX_STACK slots.  On success *max_stack_out
+ * (optional) is the deepest stack any program needs.  Pure host function, no CUDA. */
+int kripke_validate_programs(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,
+                             uint32_t n_vars, uint32_t *max_stack_out);
+
+/* Stages a batch (step H1): validates (as above), lowers each program to the kernels'
+ * internal program format and copies both forms to the current device (synchronous; allocates
+ * device memory owned by the handle).  code / offsets are HOST pointers and are not retained. */
+int kripke_programs_create(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,
+                           uint32_t n_vars, kripke_programs_t **programs_out);
+int kripke_programs_destroy(kripke_programs_t *programs);   /* synchronises the device first */
+
+/* Number of distinct labelled frames in a class (2^(n*n), 2^(n*n-n), preorders, equivalences). */
+int kripke_class_size(uint32_t n_worlds, uint32_t frame_class, uint64_t *size_out);
+
+/* Fused corpus scan over one (class, n) layer (Algorithm 1; steps H1-H6): every program
+ * of the batch on every frame of the class and every valuation of n_vars variables (n_vars must be
+ * the value given at create time).  counts_out / witness_out: DEVICE arrays of n_formulas entries,
+ * overwritten. */
+int kripke_eval_batch(const kripke_programs_t *programs, uint32_t n_worlds, uint32_t n_vars,
+                      uint32_t frame_class, kripke_count_t *counts_out,
+                      kripke_witness_t *witness_out, void *stream);
+
+/* Same over the class frames [frame_begin, frame_begin + frame_count) only, with `flags`. */
+int kripke_eval_batch_range(const kripke_programs_t *programs, uint32_t n_worlds, uint32_t n_vars,
+                            uint32_t frame_class, uint64_t frame_begin, uint64_t frame_count,
+                            uint32_t flags, kripke_count_t *counts_out,
+                            kripke_witness_t *witness_out, void *stream);
+
+/* Pairwise distinguishability (step H7): for pair j = (pairs[2j], pairs[2j+1])
+ * of program indices, per model x = truth(phi) XOR truth(psi); the model distinguishes the pair
+ * iff x != 0; world = least set bit of x.  pairs: HOST array of 2*n_pairs indices (read before the
+ * call returns).  counts_out / witness_out: DEVICE arrays of n_pairs entries. */
+int kripke_distinguish_pairs(const kripke_programs_t *programs, const uint32_t *pairs,
+                             uint32_t n_pairs, uint32_t n_worlds, uint32_t n_vars,
+                             uint32_t frame_class, uint64_t frame_begin, uint64_t frame_count,
+                             uint32_t flags, kripke_count_t *counts_out,
+                             kripke_witness_t *witness_out, void *stream);
+
+/* End-to-end convenience with HOST buffers only: create + eval over the full class + copy the
+ * results back + destroy, synchronously (this is what bench.py's "e2e" figure times). */
+int kripke_eval_batch_host(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,
+                           uint32_t n_worlds, uint32_t n_vars, uint32_t frame_class,
+                           kripke_count_t *counts_host, kripke_witness_t *witness_host);
+
+/* What the last eval / pairs call on this handle executed (host-side bookkeeping, valid right
+ * after the call returns): kernel launches enqueued, which kernel family ran the bulk (0 scalar,
+ * 1 bit-sliced), and the 3-input logic instructions per 32 models the lowered programs need
+ * summed over the batch (the "algorithmic ops" of DESIGN.md's roofline). */
+typedef struct {
+    uint32_t launches;
+    uint32_t kernel_family;
+    uint64_t sliced_logic_ops_per_word;   /* sum over programs, per 32-model word            */
+    uint64_t models_per_program;          /* (frames in range) * 2^(n_vars*n)                */
+} kripke_run_info_t;
+int kripke_last_run_info(const kripke_programs_t *programs, kripke_run_info_t *info_out);
+
+/* Integer-pipe calibration ("source-level uint32 XOR/AND/OR" re-done as an instruction
+ * rate): runs a register-resident loop of independent 3-input logic instructions on every SM and
+ * reports executed thread-instructions per second.  variant: 0 = LOP3 only, 1 = IADD3 only,
+ * 2 = SHF only, 3 = LOP3 interleaved with IMAD (reports LOP3+IMAD).  Synchronous. */
+int kripke_calibrate_int32(uint32_t variant, double *thread_instr_per_s_out, double *elapsed_ms_out,
+                           void *stream);
+
+/* Multi-GPU exchange step: when the frame range of a scan is sharded over
+ * ranks, counts combine by SUM and witnesses by lexicographic MIN of (frame, valuation).  These two
+ * calls convert DEVICE witness records to and from one 64-bit key per record whose numeric MIN is
+ * that lexicographic MIN: key = (((f << n_vars*n) | v) << 3) | world, or 2^63-1 for "none"
+ * (n*n + n_vars*n + 3 <= 63 always holds within the limits above), so a single ncclAllReduce(MIN)
+ * on the keys and one ncclAllReduce(SUM) on the counts finish the scan. */
+int kripke_witness_to_keys(const kripke_witness_t *witness, uint32_t n_records, uint32_t n_worlds,
+                           uint32_t n_vars, uint64_t *keys_out, void *stream);
+int kripke_keys_to_witness(const uint64_t *keys, uint32_t n_records, uint32_t n_worlds,
+                           uint32_t n_vars, kripke_witness_t *witness_out, void *stream);
+
+/* Diagnostic (pure host, no CUDA): lowers one program - or the pair (a, b) if code_b != NULL - to
+ * the bit-sliced kernel's micro-ops (csrc/ucode.h) and copies them to ucode_out (capacity cap).
+ * Returns the number of micro-ops, or a negative kripke_status (KRIPKE_EUNSUPPORTED if the program
+ * needs more register-stack slots than the kernel has; *need_out is set in both cases). */
+int kripke_debug_lower(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b,
+                       uint32_t n_vars, uint8_t *ucode_out, uint32_t cap, uint32_t *need_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KRIPKE_H */

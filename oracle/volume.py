@@ -52,6 +52,8 @@ def _load():
                                         ctypes.c_int, ctypes.c_int, u64p, u64p, ctypes.c_uint64,
                                         u64p, u64p, u64p, u32p, u32p, ctypes.c_int]
         lib.kov_max_threads.restype = ctypes.c_int
+        lib.kov_orbits.restype = ctypes.c_int64
+        lib.kov_orbits.argtypes = [ctypes.c_int, u64p, u64p, ctypes.c_uint64]
         lib.kov_signatures.restype = ctypes.c_int
         lib.kov_signatures.argtypes = [u8p, u32p, ctypes.c_uint32, ctypes.c_int, ctypes.c_int, u64p, u64p]
         _lib = lib
@@ -169,3 +171,16 @@ def signatures(code, offsets, max_n: int, k: int):
     if rc:
         raise ValueError("kov_signatures failed")
     return a, b
+
+
+def orbits(n: int):
+    """(representatives, sizes): the least K-index of every isomorphism class of n-world frames,
+    ascending, and the class sizes (uint64 arrays).  sum(sizes) = 2^(n*n)."""
+    lib = _load()
+    cnt = lib.kov_orbits(n, None, None, 0)
+    if cnt < 0:
+        raise ValueError("kov_orbits failed")
+    reps = np.zeros(cnt, np.uint64)
+    sizes = np.zeros(cnt, np.uint64)
+    lib.kov_orbits(n, _p(reps, ctypes.c_uint64), _p(sizes, ctypes.c_uint64), cnt)
+    return reps, sizes

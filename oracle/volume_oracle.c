@@ -367,3 +367,70 @@ int kov_signatures(const u8 *code, const uint32_t *offs, uint32_t B, int max_n, 
     }
     return bad ? -1 : 0;
 }
+
+/* ---- isomorphism orbits of labelled frames (relabelling invariance) ----
+ * A permutation pi of the worlds maps the relation R to {(pi(w), pi(u)) : (w,u) in R}.  Counts of
+ * refuting models / frames of a fixed formula are equal on isomorphic frames (rename the worlds in
+ * the valuation as well), so a full-class-K count equals the sum over orbit representatives of
+ * orbit size x the representative's count.  A frame is its orbit's representative iff no image is
+ * smaller than it; the orbit size is the number of distinct images.  Plain enumeration of all n!
+ * permutations, nothing clever. */
+static uint64_t apply_perm(int n, const int *pi, uint64_t f) {
+    uint64_t g = 0;
+    for (int w = 0; w < n; ++w)
+        for (int u = 0; u < n; ++u)
+            if ((f >> (w * n + u)) & 1u) g |= 1ull << (pi[w] * n + pi[u]);
+    return g;
+}
+
+static int next_perm(int n, int *p) {           /* lexicographic successor; 0 when done */
+    int i = n - 2;
+    while (i >= 0 && p[i] > p[i + 1]) --i;
+    if (i < 0) return 0;
+    int j = n - 1;
+    while (p[j] < p[i]) --j;
+    int t = p[i]; p[i] = p[j]; p[j] = t;
+    for (int a = i + 1, b = n - 1; a < b; ++a, --b) { t = p[a]; p[a] = p[b]; p[b] = t; }
+    return 1;
+}
+
+/* Writes the ascending orbit representatives of all n-world frames and their orbit sizes; returns
+ * the number of orbits (or -1).  Pass reps = NULL to count only. */
+int64_t kov_orbits(int n, uint64_t *reps, uint64_t *sizes, uint64_t cap) {
+    if (n < 1 || n > 5) return -1;
+    int nperm = 1;
+    for (int i = 2; i <= n; ++i) nperm *= i;
+    int (*perms)[MAXN] = malloc((size_t)nperm * sizeof(*perms));
+    int p[MAXN];
+    for (int i = 0; i < n; ++i) p[i] = i;
+    int c = 0;
+    do { memcpy(perms[c++], p, sizeof(p)); } while (next_perm(n, p));
+    uint64_t total = 1ull << (n * n);
+    u8 *is_rep = calloc(total, 1);
+#pragma omp parallel for schedule(dynamic, 4096)
+    for (uint64_t f = 0; f < total; ++f) {
+        int rep = 1;
+        for (int i = 0; i < nperm && rep; ++i)
+            if (apply_perm(n, perms[i], f) < f) rep = 0;
+        is_rep[f] = (u8)rep;
+    }
+    uint64_t count = 0;
+    for (uint64_t f = 0; f < total; ++f) {
+        if (!is_rep[f]) continue;
+        if (reps && count < cap) {
+            uint64_t img[120];
+            for (int i = 0; i < nperm; ++i) img[i] = apply_perm(n, perms[i], f);
+            uint64_t distinct = 0;
+            for (int i = 0; i < nperm; ++i) {
+                int seen = 0;
+                for (int j = 0; j < i; ++j) if (img[j] == img[i]) { seen = 1; break; }
+                distinct += !seen;
+            }
+            reps[count] = f;
+            sizes[count] = distinct;
+        }
+        ++count;
+    }
+    free(is_rep); free(perms);
+    return (int64_t)count;
+}

@@ -1,0 +1,273 @@
+"""Thin ctypes binding of libkripke_b200.so (include/kripke.h).  Argument marshalling only.
+
+Every function has the name of the C entry point without the `kripke_` prefix.  Device buffers are
+torch CUDA tensors (torch is used for device memory and streams only); results come back as the
+tensors the C library wrote.  There is no CPU fallback: if the library is missing or no CUDA device
+is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libkripke_b200.so")
+
+OK, EINVAL, EPROGRAM, EUNSUPPORTED, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
+CLASS_K, CLASS_T, CLASS_S4, CLASS_S5 = 0, 1, 2, 3
+ACCUMULATE = 1 << 0
+KERNEL_AUTO, KERNEL_SCALAR, KERNEL_SLICED = 0 << 4, 1 << 4, 2 << 4
+REDUCE_BLOCK, REDUCE_WARP, REDUCE_THREAD = 0 << 8, 1 << 8, 2 << 8
+NO_WITNESS = (1 << 64) - 1
+
+_STATUS = {EINVAL: "KRIPKE_EINVAL", EPROGRAM: "KRIPKE_EPROGRAM", EUNSUPPORTED: "KRIPKE_EUNSUPPORTED",
+           ECUDA: "KRIPKE_ECUDA", ENOMEM: "KRIPKE_ENOMEM"}
+
+EXPORTS = [
+    "kripke_version", "kripke_last_cuda_error", "kripke_validate_programs", "kripke_programs_create",
+    "kripke_programs_destroy", "kripke_class_size", "kripke_eval_batch", "kripke_eval_batch_range",
+    "kripke_distinguish_pairs", "kripke_eval_batch_host", "kripke_last_run_info",
+    "kripke_calibrate_int32", "kripke_debug_lower", "kripke_witness_to_keys", "kripke_keys_to_witness",
+]
+
+
+class KripkeError(RuntimeError):
+    def __init__(self, status: int, where: str, cuda_error: int = 0):
+        self.status = status
+        self.cuda_error = cuda_error
+        extra = f" (cudaError {cuda_error})" if status == ECUDA else ""
+        super().__init__(f"{where}: {_STATUS.get(status, status)}{extra}")
+
+
+class RunInfo(ctypes.Structure):
+    _fields_ = [("launches", ctypes.c_uint32), ("kernel_family", ctypes.c_uint32),
+                ("sliced_logic_ops_per_word", ctypes.c_uint64), ("models_per_program", ctypes.c_uint64)]
+
+
+_lib = None
+
+
+def load():
+    """Loads the library (building it with nvcc first if the .so is not there yet)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        from . import build as _build
+        _build.build()
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, u8p, u32p, u64p = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p
+    u32, u64 = ctypes.c_uint32, ctypes.c_uint64
+    lib.kripke_version.restype = ctypes.c_char_p
+    lib.kripke_last_cuda_error.restype = ctypes.c_int
+    lib.kripke_validate_programs.argtypes = [u8p, u32p, u32, u32, ctypes.POINTER(u32)]
+    lib.kripke_programs_create.argtypes = [u8p, u32p, u32, u32, ctypes.POINTER(vp)]
+    lib.kripke_programs_destroy.argtypes = [vp]
+    lib.kripke_class_size.argtypes = [u32, u32, ctypes.POINTER(u64)]
+    lib.kripke_eval_batch.argtypes = [vp, u32, u32, u32, vp, vp, vp]
+    lib.kripke_eval_batch_range.argtypes = [vp, u32, u32, u32, u64, u64, u32, vp, vp, vp]
+    lib.kripke_distinguish_pairs.argtypes = [vp, u32p, u32, u32, u32, u32, u64, u64, u32, vp, vp, vp]
+    lib.kripke_eval_batch_host.argtypes = [u8p, u32p, u32, u32, u32, u32, vp, vp]
+    lib.kripke_last_run_info.argtypes = [vp, ctypes.POINTER(RunInfo)]
+    lib.kripke_calibrate_int32.argtypes = [u32, ctypes.POINTER(ctypes.c_double),
+                                           ctypes.POINTER(ctypes.c_double), vp]
+    lib.kripke_witness_to_keys.argtypes = [vp, u32, u32, u32, vp, vp]
+    lib.kripke_keys_to_witness.argtypes = [vp, u32, u32, u32, vp, vp]
+    lib.kripke_debug_lower.argtypes = [u8p, u32, u8p, u32, u32, u8p, u32, ctypes.POINTER(u32)]
+    for name in EXPORTS:
+        if name not in ("kripke_version",):
+            getattr(lib, name).restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, where: str):
+    if rc != OK:
+        raise KripkeError(rc, where, load().kripke_last_cuda_error())
+
+
+def _host(code, offsets):
+    code = np.ascontiguousarray(code, dtype=np.uint8)
+    offsets = np.ascontiguousarray(offsets, dtype=np.uint32)
+    if code.size == 0:
+        code = np.zeros(1, np.uint8)
+    return code, offsets
+
+
+def version() -> str:
+    return load().kripke_version().decode()
+
+
+def validate_programs(code, offsets, n_vars: int) -> int:
+    """Returns the deepest postfix stack any program needs; raises KripkeError if invalid."""
+    code, offsets = _host(code, offsets)
+    deepest = ctypes.c_uint32(0)
+    _check(load().kripke_validate_programs(code.ctypes.data, offsets.ctypes.data, len(offsets) - 1,
+                                           n_vars, ctypes.byref(deepest)), "kripke_validate_programs")
+    return deepest.value
+
+
+def class_size(n_worlds: int, frame_class: int) -> int:
+    out = ctypes.c_uint64(0)
+    _check(load().kripke_class_size(n_worlds, frame_class, ctypes.byref(out)), "kripke_class_size")
+    return out.value
+
+
+class Programs:
+    """Owner of a kripke_programs_t handle."""
+
+    def __init__(self, code, offsets, n_vars: int):
+        code, offsets = _host(code, offsets)
+        self.n_formulas = len(offsets) - 1
+        self.n_vars = n_vars
+        self._h = ctypes.c_void_p()
+        _check(load().kripke_programs_create(code.ctypes.data, offsets.ctypes.data, self.n_formulas,
+                                             n_vars, ctypes.byref(self._h)), "kripke_programs_create")
+
+    def destroy(self):
+        if self._h:
+            load().kripke_programs_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def last_run_info(self) -> RunInfo:
+        info = RunInfo()
+        _check(load().kripke_last_run_info(self._h, ctypes.byref(info)), "kripke_last_run_info")
+        return info
+
+
+def programs_create(code, offsets, n_vars: int) -> Programs:
+    return Programs(code, offsets, n_vars)
+
+
+def programs_destroy(p: Programs):
+    p.destroy()
+
+
+def _outputs(n: int, counts_out, witness_out):
+    import torch
+    if counts_out is None:
+        counts_out = torch.empty((n, 2), dtype=torch.int64, device="cuda")
+    if witness_out is None:
+        witness_out = torch.empty((n, 2), dtype=torch.int64, device="cuda")
+    for t in (counts_out, witness_out):
+        assert t.is_cuda and t.dtype == torch.int64 and t.is_contiguous() and t.numel() >= 2 * n
+    return counts_out, witness_out
+
+
+def _stream(stream):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def eval_batch(programs: Programs, n_worlds: int, n_vars: int, frame_class: int,
+               counts_out=None, witness_out=None, stream=None):
+    """kripke_eval_batch.  Returns (counts, witness): int64 CUDA tensors of shape (B, 2) holding the
+    kripke_count_t / kripke_witness_t records (see unpack())."""
+    counts_out, witness_out = _outputs(programs.n_formulas, counts_out, witness_out)
+    _check(load().kripke_eval_batch(programs._h, n_worlds, n_vars, frame_class, counts_out.data_ptr(),
+                                    witness_out.data_ptr(), _stream(stream)), "kripke_eval_batch")
+    return counts_out, witness_out
+
+
+def eval_batch_range(programs: Programs, n_worlds: int, n_vars: int, frame_class: int,
+                     frame_begin: int, frame_count: int, flags: int = 0,
+                     counts_out=None, witness_out=None, stream=None):
+    counts_out, witness_out = _outputs(programs.n_formulas, counts_out, witness_out)
+    _check(load().kripke_eval_batch_range(programs._h, n_worlds, n_vars, frame_class, frame_begin,
+                                          frame_count, flags, counts_out.data_ptr(),
+                                          witness_out.data_ptr(), _stream(stream)),
+           "kripke_eval_batch_range")
+    return counts_out, witness_out
+
+
+def distinguish_pairs(programs: Programs, pairs, n_worlds: int, n_vars: int, frame_class: int,
+                      frame_begin: int, frame_count: int, flags: int = 0,
+                      counts_out=None, witness_out=None, stream=None):
+    pairs = np.ascontiguousarray(pairs, dtype=np.uint32).reshape(-1)
+    n_pairs = len(pairs) // 2
+    counts_out, witness_out = _outputs(n_pairs, counts_out, witness_out)
+    _check(load().kripke_distinguish_pairs(programs._h, pairs.ctypes.data, n_pairs, n_worlds, n_vars,
+                                           frame_class, frame_begin, frame_count, flags,
+                                           counts_out.data_ptr(), witness_out.data_ptr(),
+                                           _stream(stream)), "kripke_distinguish_pairs")
+    return counts_out, witness_out
+
+
+def eval_batch_host(code, offsets, n_worlds: int, n_vars: int, frame_class: int):
+    """kripke_eval_batch_host: host buffers in, host buffers out (numpy uint64 arrays (B, 2))."""
+    code, offsets = _host(code, offsets)
+    n = len(offsets) - 1
+    counts = np.zeros((n, 2), np.uint64)
+    witness = np.zeros((n, 2), np.uint64)
+    _check(load().kripke_eval_batch_host(code.ctypes.data, offsets.ctypes.data, n, n_worlds, n_vars,
+                                         frame_class, counts.ctypes.data, witness.ctypes.data),
+           "kripke_eval_batch_host")
+    return counts, witness
+
+
+def calibrate_int32(variant: int = 0, stream=None):
+    """Returns (thread-instructions per second, elapsed ms) of the integer-pipe calibration."""
+    rate, ms = ctypes.c_double(0), ctypes.c_double(0)
+    _check(load().kripke_calibrate_int32(variant, ctypes.byref(rate), ctypes.byref(ms), _stream(stream)),
+           "kripke_calibrate_int32")
+    return rate.value, ms.value
+
+
+def witness_to_keys(witness, n_worlds: int, n_vars: int, keys_out=None, stream=None):
+    """Device witness records (int64 (B, 2) CUDA tensor) -> int64 (B,) keys whose MIN is the
+    lexicographically first (frame, valuation)."""
+    import torch
+    n = witness.shape[0]
+    if keys_out is None:
+        keys_out = torch.empty((n,), dtype=torch.int64, device="cuda")
+    _check(load().kripke_witness_to_keys(witness.data_ptr(), n, n_worlds, n_vars, keys_out.data_ptr(),
+                                         _stream(stream)), "kripke_witness_to_keys")
+    return keys_out
+
+
+def keys_to_witness(keys, n_worlds: int, n_vars: int, witness_out=None, stream=None):
+    import torch
+    n = keys.shape[0]
+    if witness_out is None:
+        witness_out = torch.empty((n, 2), dtype=torch.int64, device="cuda")
+    _check(load().kripke_keys_to_witness(keys.data_ptr(), n, n_worlds, n_vars, witness_out.data_ptr(),
+                                         _stream(stream)), "kripke_keys_to_witness")
+    return witness_out
+
+
+def debug_lower(code_a: bytes, code_b: bytes | None, n_vars: int):
+    """(micro-ops as bytes, register-stack slots needed); raises KripkeError(EUNSUPPORTED) if the
+    program does not fit the bit-sliced kernel."""
+    a = np.frombuffer(bytes(code_a), np.uint8).copy()
+    b = np.frombuffer(bytes(code_b), np.uint8).copy() if code_b is not None else None
+    out = np.zeros(256, np.uint8)
+    need = ctypes.c_uint32(0)
+    rc = load().kripke_debug_lower(a.ctypes.data, len(a), b.ctypes.data if b is not None else None,
+                                   len(b) if b is not None else 0, n_vars, out.ctypes.data, len(out),
+                                   ctypes.byref(need))
+    if rc < 0:
+        raise KripkeError(rc, "kripke_debug_lower")
+    return bytes(out[:rc]), need.value
+
+
+def unpack(counts, witness):
+    """(counts, witness) as returned above (torch or numpy) -> dict of numpy uint64/uint32 arrays:
+    models, frames, wit_f (NO_WITNESS = none), wit_v, wit_w."""
+    if hasattr(counts, "cpu"):
+        counts = counts.cpu().numpy()
+        witness = witness.cpu().numpy()
+    c = np.ascontiguousarray(counts).view(np.uint64).reshape(-1, 2)
+    w = np.ascontiguousarray(witness).view(np.uint64).reshape(-1, 2)
+    return {"models": c[:, 0].copy(), "frames": c[:, 1].copy(), "wit_f": w[:, 0].copy(),
+            "wit_v": (w[:, 1] & np.uint64(0xFFFFFFFF)).astype(np.uint32),
+            "wit_w": (w[:, 1] >> np.uint64(32)).astype(np.uint32)}

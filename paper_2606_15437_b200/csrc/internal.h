@@ -1,0 +1,82 @@
+// internal.h - declarations shared by the host translation units of libkripke_b200.so.
+#pragma once
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/kripke.h"
+#include "ucode.h"
+
+namespace kripke {
+
+// ---- lower.cpp ---------------------------------------------------------------------------------
+struct Lowered {
+    std::vector<uint8_t> ucode;   // micro-ops, FIN last
+    int need = 0;                 // register-stack slots needed (fits the sliced kernel iff <= UC_DMAX)
+    uint32_t n_modal = 0;         // executed box/dia micro-ops
+    uint32_t n_bool = 0;          // executed and/or/andn/nand micro-ops
+};
+int validate_programs(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas, uint32_t n_vars,
+                      uint32_t *max_stack_out);
+bool lower_single(const uint8_t *code, uint32_t len, Lowered *out);
+bool lower_pair(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b, Lowered *out);
+
+// ---- device-side job description (kernels) -----------------------------------------------------
+// Accumulators per output record, owned by the programs handle, zeroed at the start of a call.
+struct Accum {
+    unsigned long long models;
+    unsigned long long frames;
+    unsigned long long best;      // least class-frame index (or unit) with a hit; ~0 = none
+};
+
+struct ScanJob {
+    // what to scan
+    uint32_t n;                   // worlds
+    uint32_t k;                   // variables
+    uint32_t cls;                 // frame class
+    uint64_t frame_begin;         // class-order range
+    uint64_t frame_count;
+    const uint64_t *class_table;  // device: ascending K-indices for S4 / S5 (else null)
+    // programs (raw postfix form; used by the scalar kernel and by witness completion)
+    const uint8_t *code;          // device
+    const uint32_t *offsets;      // device, n_formulas + 1
+    uint32_t n_formulas;
+    // records: either one per formula (pairs == null) or one per pair
+    const uint32_t *pairs;        // device, 2 * n_records, or null
+    uint32_t n_records;
+    Accum *accum;                 // device, n_records
+};
+
+// ---- launch wrappers (defined in the .cu files) ------------------------------------------------
+struct SlicedPlan {
+    // lowered slots (a slot is one record the sliced kernel evaluates)
+    const uint8_t *ucode;         // device: n_slots * stride bytes
+    const uint32_t *slot_record;  // device: record index per slot
+    uint32_t n_slots;
+    uint32_t stride;              // bytes per slot (multiple of 4, >= longest ucode + 1)
+    uint32_t max_need;            // most register-stack slots any slot needs
+};
+
+// Most register-stack slots an instantiation for this shape offers (0 = shape not supported).
+uint32_t sliced_max_need(uint32_t n, uint32_t k, uint32_t cls);
+// Class frames per scan unit of the sliced kernel for this shape (ranges must be multiples of it).
+uint64_t sliced_frames_per_unit(uint32_t n, uint32_t k);
+// Enqueue the sliced scan; returns a cudaError_t as int and the number of kernel launches.
+int launch_sliced(const ScanJob &job, const SlicedPlan &plan, void *stream, uint32_t *launches);
+// Enqueue the scalar (Algorithm 1) scan over the records listed in `records` (device, or null = all).
+int launch_scalar(const ScanJob &job, const uint32_t *records, uint32_t n_list, uint32_t reduce_mode,
+                  void *stream, uint32_t *launches);
+// Zero the accumulators; finish: turn accumulators into counts / witnesses (handles ACCUMULATE).
+int launch_init(Accum *accum, uint32_t n_records, void *stream);
+int launch_finish(const ScanJob &job, bool accumulate, kripke_count_t *counts_out,
+                  kripke_witness_t *witness_out, void *stream);
+// Witness records <-> 64-bit keys (multi-GPU exchange step).
+int launch_witness_keys(bool to_keys, const void *src, uint32_t n_records, uint32_t kn, void *dst, void *stream);
+// Calibration kernels.
+int run_calibration(uint32_t variant, double *rate_out, double *ms_out, void *stream);
+
+// ---- class tables (api.cpp) --------------------------------------------------------------------
+// Host: ascending K-indices of the class members (S4 / S5), n <= 5 here; cached.
+const std::vector<uint64_t> *class_table_host(uint32_t n, uint32_t cls);
+
+}  // namespace kripke

@@ -1,0 +1,206 @@
+// lower.cpp - host side of step H1 (program staging): validation of postfix programs and their
+// lowering to the bit-sliced kernel's micro-ops (ucode.h).  Pure host code, no CUDA.
+#include "internal.h"
+
+#include <algorithm>
+
+namespace kripke {
+
+namespace {
+
+bool is_atom(uint8_t c, uint32_t n_vars) {
+    return c == KRIPKE_OP_TOP || c == KRIPKE_OP_BOT || (c >= KRIPKE_OP_VAR0 && c < KRIPKE_OP_VAR0 + n_vars);
+}
+bool is_unary(uint8_t c) { return c == KRIPKE_OP_NOT || c == KRIPKE_OP_BOX || c == KRIPKE_OP_DIA; }
+bool is_binary(uint8_t c) { return c == KRIPKE_OP_AND || c == KRIPKE_OP_OR || c == KRIPKE_OP_IMP; }
+
+// Simplified syntax tree used by the lowering.
+enum NodeKind : uint8_t { N_CONST, N_VAR, N_NOT, N_BOX, N_DIA, N_AND, N_OR, N_IMP };
+struct Node {
+    NodeKind kind;
+    uint8_t value;   // N_CONST: 0/1, N_VAR: index
+    int a, b;        // children
+    int need;        // register-stack slots needed to evaluate this subtree
+};
+
+struct Lowerer {
+    std::vector<Node> nodes;
+    std::vector<uint8_t> out;
+    uint64_t logic_ops = 0;   // per 32-model word, as a function of n: modal*n*n + bool*n
+    uint32_t n_modal = 0, n_bool = 0;
+
+    int add(NodeKind k, uint8_t v, int a, int b) {
+        nodes.push_back(Node{k, v, a, b, 0});
+        return (int)nodes.size() - 1;
+    }
+    bool is_const(int i, int v) const { return nodes[i].kind == N_CONST && nodes[i].value == v; }
+    bool is_const(int i) const { return nodes[i].kind == N_CONST; }
+
+    // constant folding while building (results are exact identities of the semantics)
+    int mk_not(int x) {
+        if (is_const(x)) return add(N_CONST, !nodes[x].value, -1, -1);
+        if (nodes[x].kind == N_NOT) return nodes[x].a;
+        return add(N_NOT, 0, x, -1);
+    }
+    int mk_modal(NodeKind k, int x) {
+        if (k == N_BOX && is_const(x, 1)) return x;   // box T = T
+        if (k == N_DIA && is_const(x, 0)) return x;   // dia F = F
+        return add(k, 0, x, -1);                      // box F (dead ends) and dia T stay
+    }
+    int mk_and(int x, int y) {
+        if (is_const(x, 0) || is_const(y, 0)) return add(N_CONST, 0, -1, -1);
+        if (is_const(x, 1)) return y;
+        if (is_const(y, 1)) return x;
+        return add(N_AND, 0, x, y);
+    }
+    int mk_or(int x, int y) {
+        if (is_const(x, 1) || is_const(y, 1)) return add(N_CONST, 1, -1, -1);
+        if (is_const(x, 0)) return y;
+        if (is_const(y, 0)) return x;
+        return add(N_OR, 0, x, y);
+    }
+    int mk_imp(int x, int y) {
+        if (is_const(x, 0) || is_const(y, 1)) return add(N_CONST, 1, -1, -1);
+        if (is_const(x, 1)) return y;
+        if (is_const(y, 0)) return mk_not(x);
+        return add(N_IMP, 0, x, y);
+    }
+
+    // Postfix -> folded tree.  The program is already validated.
+    int build(const uint8_t *code, uint32_t len) {
+        std::vector<int> st;
+        for (uint32_t i = 0; i < len; ++i) {
+            uint8_t c = code[i];
+            if (c == KRIPKE_OP_TOP) st.push_back(add(N_CONST, 1, -1, -1));
+            else if (c == KRIPKE_OP_BOT) st.push_back(add(N_CONST, 0, -1, -1));
+            else if (c >= KRIPKE_OP_VAR0 && c < KRIPKE_OP_VAR0 + KRIPKE_MAX_VARS)
+                st.push_back(add(N_VAR, (uint8_t)(c - KRIPKE_OP_VAR0), -1, -1));
+            else if (is_unary(c)) {
+                int x = st.back(); st.pop_back();
+                st.push_back(c == KRIPKE_OP_NOT ? mk_not(x) : mk_modal(c == KRIPKE_OP_BOX ? N_BOX : N_DIA, x));
+            } else {
+                int y = st.back(); st.pop_back();
+                int x = st.back(); st.pop_back();
+                st.push_back(c == KRIPKE_OP_AND ? mk_and(x, y) : c == KRIPKE_OP_OR ? mk_or(x, y) : mk_imp(x, y));
+            }
+        }
+        return st.back();
+    }
+
+    // Slots needed when the deeper operand of a binary node is evaluated first (Sethi-Ullman).
+    int need(int i) {
+        Node &nd = nodes[i];
+        switch (nd.kind) {
+        case N_CONST: case N_VAR: nd.need = 1; break;
+        case N_NOT: case N_BOX: case N_DIA: nd.need = need(nd.a); break;
+        default: {
+            int l = need(nd.a), r = need(nd.b);
+            nd.need = (l >= r) ? std::max(l, r + 1) : std::max(r, l + 1);
+        }
+        }
+        return nd.need;
+    }
+
+    // Emits micro-ops leaving the value of node i in slot d; returns its polarity (1 = the slot
+    // holds the complement of the value).
+    int emit(int i, int d) {
+        const Node nd = nodes[i];
+        switch (nd.kind) {
+        case N_CONST:
+            out.push_back((uint8_t)(UC_PUSH + 4 * UC_DMAX + d));
+            return nd.value;                      // T is the complement of all-false
+        case N_VAR:
+            out.push_back((uint8_t)(UC_PUSH + nd.value * UC_DMAX + d));
+            return 0;
+        case N_NOT:
+            return !emit(nd.a, d);
+        case N_BOX: case N_DIA: {
+            int p = emit(nd.a, d);
+            // box ~s = ~dia s ; dia ~s = ~box s
+            bool box = (nd.kind == N_BOX) != (p != 0);
+            out.push_back((uint8_t)((box ? UC_BOX : UC_DIA) + d));
+            ++n_modal;
+            return p;
+        }
+        default: {
+            bool a_first = nodes[nd.a].need >= nodes[nd.b].need;
+            int first = a_first ? nd.a : nd.b, second = a_first ? nd.b : nd.a;
+            int p1 = emit(first, d), p2 = emit(second, d + 1);
+            int px = a_first ? p1 : p2, py = a_first ? p2 : p1;
+            // as a conjunction of literals: and = x & y ; or = ~(~x & ~y) ; imp = ~(x & ~y)
+            int negx = (nd.kind == N_OR), negy = (nd.kind != N_AND), flip = (nd.kind != N_AND);
+            int ax = px ^ negx, ay = py ^ negy;
+            int a1 = a_first ? ax : ay, a2 = a_first ? ay : ax;   // by slot: d, d+1
+            ++n_bool;
+            if (!a1 && !a2) { out.push_back((uint8_t)(UC_AND + d)); return flip; }
+            if (!a1 && a2) { out.push_back((uint8_t)(UC_ANDN + d)); return flip; }
+            if (a1 && !a2) { out.push_back((uint8_t)(UC_NAND + d)); return flip; }
+            out.push_back((uint8_t)(UC_OR + d));   // ~s1 & ~s2 = ~(s1 | s2)
+            return !flip;
+        }
+        }
+    }
+};
+
+}  // namespace
+
+int validate_programs(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas, uint32_t n_vars,
+                      uint32_t *max_stack_out) {
+    if (!offsets || n_vars > KRIPKE_MAX_VARS) return KRIPKE_EINVAL;
+    if (n_formulas && !code) return KRIPKE_EINVAL;
+    uint32_t deepest = 0;
+    bool unsupported = false;
+    for (uint32_t b = 0; b < n_formulas; ++b) {
+        if (offsets[b + 1] < offsets[b]) return KRIPKE_EINVAL;
+        uint32_t len = offsets[b + 1] - offsets[b];
+        if (len == 0) return KRIPKE_EPROGRAM;
+        if (len > KRIPKE_MAX_PROGRAM_LEN) unsupported = true;
+        uint32_t sp = 0, top = 0;
+        for (uint32_t i = 0; i < len; ++i) {
+            uint8_t c = code[offsets[b] + i];
+            if (is_atom(c, n_vars)) ++sp;
+            else if (is_unary(c)) { if (sp < 1) return KRIPKE_EPROGRAM; }
+            else if (is_binary(c)) { if (sp < 2) return KRIPKE_EPROGRAM; --sp; }
+            else return KRIPKE_EPROGRAM;
+            top = std::max(top, sp);
+        }
+        if (sp != 1) return KRIPKE_EPROGRAM;
+        deepest = std::max(deepest, top);
+    }
+    if (max_stack_out) *max_stack_out = deepest;
+    if (unsupported || deepest > KRIPKE_MAX_STACK) return KRIPKE_EUNSUPPORTED;
+    return KRIPKE_OK;
+}
+
+bool lower_single(const uint8_t *code, uint32_t len, Lowered *out) {
+    Lowerer lw;
+    int root = lw.build(code, len);
+    out->need = lw.need(root);
+    if (out->need > UC_DMAX) return false;
+    int p = lw.emit(root, 0);
+    lw.out.push_back(p ? UC_FIN_ANY : UC_FIN_ALL);
+    out->ucode = std::move(lw.out);
+    out->n_modal = lw.n_modal;
+    out->n_bool = lw.n_bool;
+    return true;
+}
+
+bool lower_pair(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b, Lowered *out) {
+    Lowerer lw;
+    int ra = lw.build(code_a, len_a);
+    int rb = lw.build(code_b, len_b);
+    int na = lw.need(ra), nb = lw.need(rb);
+    // XOR is symmetric: evaluate the deeper formula first (slot 0), the other above it (slot 1)
+    if (nb > na) { std::swap(ra, rb); std::swap(na, nb); }
+    out->need = std::max(na, nb + 1);
+    if (out->need > UC_DMAX) return false;
+    int pa = lw.emit(ra, 0);
+    int pb = lw.emit(rb, 1);
+    lw.out.push_back(pa == pb ? UC_FIN_XOR : UC_FIN_XNOR);
+    out->ucode = std::move(lw.out);
+    out->n_modal = lw.n_modal;
+    out->n_bool = lw.n_bool;
+    return true;
+}
+
+}  // namespace kripke

@@ -1,0 +1,146 @@
+"""Writes the stored expected values under tests/golden/ by calling ONLY oracle/ and workloads/.
+
+    python tests/golden/make_golden.py <part> [--threads N]
+
+parts (sizes are oracle evaluations; times are for the 8-core build box at ~0.1 G eval/s):
+  c2          config 2: 5,624 formulas, n=4, classes K/T/S4/S5, full ranges      (1.0e11, ~15 min)
+  n5_classes  config 3: same corpus, n=5, classes S4 and S5 in full             (4.0e10, ~6 min)
+  n5_ranges   config 3: 16 seeded ranges of 64 frames of K and of T at n=5       (1.2e10, ~2 min)
+  n5_orbit    config 3: full-range K counts at n=5 for 96 corpus formulas and the named axioms,
+              by the isomorphism-orbit route (291,968 representatives x orbit sizes)
+  c4_ranges   config 4: 2,048 three-variable formulas, n=5, 4 seeded ranges of 8 K-frames
+  c5_counts   config 5: distinguishing-frame counts of every pair for n=1..5 (orbit route at
+              n=5) and first witnesses for n<=4
+
+Nothing here imports the CUDA path; no value comes from it.  Each .npz stores the corpus SHA-256
+so a test can tell that it is comparing the same bytes.
+"""
+import argparse
+import hashlib
+import os
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+sys.path.insert(0, ROOT)
+
+import workloads as W                      # noqa: E402
+from oracle import volume as V             # noqa: E402
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CLASSES = {"K": 0, "T": 1, "S4": 2, "S5": 3}
+
+
+def sha(programs):
+    return hashlib.sha256(b"\xff".join(programs)).hexdigest()
+
+
+def seeded_ranges(seed, total, width, count):
+    rng = W.SplitMix64(seed)
+    return sorted(rng.below(total - width) for _ in range(count))
+
+
+def save(name, **arrays):
+    path = os.path.join(HERE, name)
+    np.savez_compressed(path, **arrays)
+    print("wrote", path, os.path.getsize(path), "bytes")
+
+
+def part_c2(threads):
+    progs = W.corpus_c2()
+    code, offs = W.pack_programs(progs)
+    out = {"corpus_sha256": np.array(sha(progs))}
+    for cname, cls in CLASSES.items():
+        t = time.time()
+        r = V.census(code, offs, 4, 2, cls, threads=threads)
+        print(cname, "%.1fs" % (time.time() - t))
+        for key, val in r.items():
+            out[f"{cname}_{key}"] = val
+    save("c2_n4.npz", **out)
+
+
+def part_n5_classes(threads):
+    progs = W.corpus_c2()
+    code, offs = W.pack_programs(progs)
+    out = {"corpus_sha256": np.array(sha(progs))}
+    for cname in ("S4", "S5"):
+        t = time.time()
+        r = V.census(code, offs, 5, 2, CLASSES[cname], threads=threads)
+        print(cname, "%.1fs" % (time.time() - t))
+        for key, val in r.items():
+            out[f"{cname}_{key}"] = val
+    save("n5_s4s5.npz", **out)
+
+
+def part_n5_ranges(threads):
+    progs = W.corpus_c2()
+    code, offs = W.pack_programs(progs)
+    out = {"corpus_sha256": np.array(sha(progs)), "width": np.array(64)}
+    for cname, total, seed in (("K", 1 << 25, 501), ("T", 1 << 20, 502)):
+        begins = seeded_ranges(seed, total, 64, 16)
+        out[f"{cname}_begin"] = np.array(begins, np.uint64)
+        acc = {}
+        for b in begins:
+            r = V.census(code, offs, 5, 2, CLASSES[cname], b, 64, threads=threads)
+            for key, val in r.items():
+                acc.setdefault(key, []).append(val)
+        for key, val in acc.items():
+            out[f"{cname}_{key}"] = np.stack(val)
+    save("n5_ranges.npz", **out)
+
+
+def part_n5_orbit(threads):
+    progs = W.corpus_c2()[:96] + [W.to_postfix(t) for t in W.named_axioms().values()]
+    code, offs = W.pack_programs(progs)
+    reps, sizes = V.orbits(5)
+    assert int(sizes.sum()) == 1 << 25
+    t = time.time()
+    r = V.census_list(code, offs, 5, 2, reps, weights=sizes, threads=threads)
+    print("orbit census %.1fs" % (time.time() - t))
+    save("n5_orbit.npz", corpus_sha256=np.array(sha(progs)), n_corpus=np.array(96),
+         models=r["models"], frames=r["frames"])
+
+
+def part_c4_ranges(threads):
+    progs = W.corpus_c4()
+    code, offs = W.pack_programs(progs)
+    begins = seeded_ranges(504, 1 << 25, 8, 4)
+    acc = {}
+    for b in begins:
+        r = V.census(code, offs, 5, 3, 0, b, 8, threads=threads)
+        for key, val in r.items():
+            acc.setdefault(key, []).append(val)
+    save("c4_ranges.npz", corpus_sha256=np.array(sha(progs)), begin=np.array(begins, np.uint64),
+         width=np.array(8), **{k: np.stack(v) for k, v in acc.items()})
+
+
+def part_c5_counts(threads):
+    progs, pairs, names = W.pairs_c5()
+    code, offs = W.pack_programs(progs)
+    pairs = np.array(pairs, np.uint32)
+    out = {"corpus_sha256": np.array(sha(progs)), "n_pairs": np.array(len(pairs))}
+    for n in (1, 2, 3, 4):
+        r = V.census(code, offs, n, 0, 0, pairs=pairs, threads=threads)
+        for key in ("frames", "wit_f", "wit_w"):
+            out[f"n{n}_{key}"] = r[key]
+    reps, sizes = V.orbits(5)
+    r = V.census_list(code, offs, 5, 0, reps, weights=sizes, pairs=pairs, threads=threads)
+    out["n5_frames"] = r["frames"]
+    save("c5_counts.npz", **out)
+
+
+PARTS = {"c2": part_c2, "n5_classes": part_n5_classes, "n5_ranges": part_n5_ranges,
+         "n5_orbit": part_n5_orbit, "c4_ranges": part_c4_ranges, "c5_counts": part_c5_counts}
+
+if __name__ == "__main__":
+    ap = argparse.ArgumentParser()
+    ap.add_argument("part", choices=sorted(PARTS) + ["all"])
+    ap.add_argument("--threads", type=int, default=0)
+    a = ap.parse_args()
+    V.build()
+    for p in (sorted(PARTS) if a.part == "all" else [a.part]):
+        t0 = time.time()
+        PARTS[p](a.threads)
+        print(p, "done in %.1fs" % (time.time() - t0))

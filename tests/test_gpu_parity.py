@@ -1,0 +1,351 @@
+"""Parity of the CUDA path (through the C ABI) with the oracle: bit-exact counts and witnesses.
+
+Small shapes are compared with the oracle run live; n = 4 / 5 with values stored by
+tests/golden/make_golden.py (which calls only oracle/); full-range n = 5 results also with closed
+forms and the isomorphism-orbit route.  Every witness is re-verified as a certificate by the
+set-based Python oracle.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle import kripke_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+K, T, S4, S5 = 0, 1, 2, 3
+CLS = {"K": K, "T": T, "S4": S4, "S5": S5}
+KEYS = ("models", "frames", "wit_f", "wit_v", "wit_w")
+
+
+@pytest.fixture(scope="module")
+def kb():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    from paper_2606_15437_b200 import binding
+    binding.load()
+    return binding
+
+
+def gold(name):
+    path = os.path.join(GOLD, name)
+    assert os.path.exists(path), f"{name} missing: run python tests/golden/make_golden.py"
+    return np.load(path)
+
+
+def run(kb, progs, n, k, cls, begin=0, count=None, flags=0, handle=None):
+    h = handle or kb.Programs(*W.pack_programs(progs), k)
+    if count is None:
+        count = kb.class_size(n, cls) - begin
+    c, w = kb.eval_batch_range(h, n, k, cls, begin, count, flags)
+    return kb.unpack(c, w)
+
+
+def same(got, want, what="", keys=KEYS):
+    for key in keys:
+        g, w = np.asarray(got[key]).astype(np.uint64), np.asarray(want[key]).astype(np.uint64)
+        bad = np.nonzero(g != w)[0]
+        assert len(bad) == 0, f"{what}: {key} differs at {bad[:5]}: got {g[bad[:5]]} want {w[bad[:5]]}"
+
+
+def certify(progs, res, n, k, cls, idx=None):
+    """Every witness is a valid certificate for the set-based checker (Definition 1)."""
+    for b in (range(len(progs)) if idx is None else idx):
+        f = int(res["wit_f"][b])
+        if f == O.NO_WITNESS:
+            assert int(res["models"][b]) == 0 and int(res["frames"][b]) == 0
+        else:
+            assert int(res["models"][b]) > 0
+            assert O.check_witness(progs[b], n, k, cls, f, int(res["wit_v"][b]), int(res["wit_w"][b])), b
+
+
+# ---------------------------------------------------------------------------------------------
+def test_c1_n3_all_classes_both_kernels(kb, vol):
+    """Config 1 (n=3, 1,000 formulas, k=2) against the oracle run live; every class."""
+    progs = W.corpus_c1()
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 2)
+    for cls in (K, T, S4, S5):
+        want = vol.census(code, offs, 3, 2, cls)
+        for flags in (kb.KERNEL_AUTO, kb.KERNEL_SCALAR):
+            got = run(kb, progs, 3, 2, cls, flags=flags, handle=h)
+            same(got, want, f"C1 cls={cls} flags={flags}")
+        certify(progs, got, 3, 2, cls, idx=range(0, 1000, 7))
+    assert h.last_run_info().launches >= 3
+    got = run(kb, progs, 3, 2, K, flags=kb.KERNEL_SLICED, handle=h)
+    same(got, vol.census(code, offs, 3, 2, K), "C1 forced sliced")
+    assert h.last_run_info().kernel_family == 1
+
+
+def test_tiny_sizes(kb, vol):
+    progs = W.corpus_c1(200)
+    code, offs = W.pack_programs(progs)
+    for n in (1, 2):
+        for cls in (K, T, S4, S5):
+            same(run(kb, progs, n, 2, cls), vol.census(code, offs, n, 2, cls), f"n={n} cls={cls}")
+    # one variable, no variable
+    p1 = [c for c in W.corpus_c4(400) if b"\x11" not in c and b"\x12" not in c][:40]
+    code1, offs1 = W.pack_programs(p1)
+    for n in (2, 4):
+        same(run(kb, p1, n, 1, K), vol.census(code1, offs1, n, 1, K), f"k=1 n={n}")
+    p0, _, _ = W.pairs_c5(50)
+    code0, offs0 = W.pack_programs(p0)
+    for n in (1, 3, 4):
+        same(run(kb, p0, n, 0, K), vol.census(code0, offs0, n, 0, K), f"k=0 n={n}")
+        same(run(kb, p0, n, 0, S4), vol.census(code0, offs0, n, 0, S4), f"k=0 n={n} S4")
+
+
+def test_c2_n4_all_classes_golden(kb):
+    """Config 2: 5,624 formulas, n=4, K/T/S4/S5, full ranges, both kernel families."""
+    g = gold("c2_n4.npz")
+    progs = W.corpus_c2()
+    h = kb.Programs(*W.pack_programs(progs), 2)
+    for cname, cls in CLS.items():
+        want = {key: g[f"{cname}_{key}"] for key in KEYS}
+        for flags in (kb.KERNEL_AUTO, kb.KERNEL_SCALAR):
+            got = run(kb, progs, 4, 2, cls, flags=flags, handle=h)
+            same(got, want, f"C2 {cname} flags={flags}")
+        certify(progs, got, 4, 2, cls, idx=range(0, len(progs), 23))
+
+
+def test_c3_n5_s4_s5_full_golden(kb):
+    g = gold("n5_s4s5.npz")
+    progs = W.corpus_c2()
+    h = kb.Programs(*W.pack_programs(progs), 2)
+    for cname in ("S4", "S5"):
+        got = run(kb, progs, 5, 2, CLS[cname], handle=h)
+        same(got, {key: g[f"{cname}_{key}"] for key in KEYS}, f"n=5 {cname}")
+        certify(progs, got, 5, 2, CLS[cname], idx=range(0, len(progs), 41))
+
+
+def test_c3_n5_sampled_ranges_golden(kb):
+    """16 seeded ranges of 64 consecutive K-frames and T-frames at n=5, every formula."""
+    g = gold("n5_ranges.npz")
+    progs = W.corpus_c2()
+    h = kb.Programs(*W.pack_programs(progs), 2)
+    width = int(g["width"])
+    for cname in ("K", "T"):
+        for i, b in enumerate(g[f"{cname}_begin"]):
+            got = run(kb, progs, 5, 2, CLS[cname], int(b), width, handle=h)
+            same(got, {key: g[f"{cname}_{key}"][i] for key in KEYS}, f"n=5 {cname} range {int(b)}")
+
+
+def test_c3_n5_full_K_counts_by_orbits(kb):
+    """Full-range n=5 class-K counts of 96 corpus formulas + the named axioms = the oracle's
+    isomorphism-orbit sum (291,968 representatives x orbit sizes)."""
+    g = gold("n5_orbit.npz")
+    progs = W.corpus_c2()[:96] + [W.to_postfix(t) for t in W.named_axioms().values()]
+    got = run(kb, progs, 5, 2, K)
+    same(got, g, "n=5 full K", keys=("models", "frames"))
+    certify(progs, got, 5, 2, K)
+
+
+def test_n5_closed_forms_full_range(kb):
+    """BASELINE.json north_star closed forms on the GPU side, full n=5 ranges."""
+    ax = W.named_axioms()
+    names = ["T", "D", "4", "B", "CD", "K"]
+    progs = [W.to_postfix(ax[a]) for a in names] + [W.to_postfix(W.parse(s)) for s in ("p->p", "T", "F", "p&~p")]
+    r = run(kb, progs, 5, 2, K)
+    total = 1 << 25
+    valid = total - r["frames"].astype(np.int64)
+    assert valid[:5].tolist() == [1 << 20, 28629151, 154303, 1 << 15, 7776]
+    assert r["models"][5:8].tolist() == [0, 0, 0] and r["wit_f"][5:8].tolist() == [O.NO_WITNESS] * 3
+    assert r["models"][8:].tolist() == [total << 10] * 2 and r["frames"][8:].tolist() == [total] * 2
+    assert (r["wit_f"][8:] == 0).all() and (r["wit_v"][8:] == 0).all() and (r["wit_w"][8:] == 0).all()
+    # class sizes through the filters: F is refuted on every frame of the class
+    for cls, size in ((T, 1 << 20), (S4, 6942), (S5, 52)):
+        rr = run(kb, [progs[8]], 5, 2, cls)
+        assert int(rr["frames"][0]) == size and int(rr["models"][0]) == size << 10
+    # T axiom is never refuted in T, 4 never in S4, B never in S5; each is refuted in the class below
+    assert int(run(kb, [progs[0]], 5, 2, T)["models"][0]) == 0
+    assert int(run(kb, [progs[2]], 5, 2, S4)["models"][0]) == 0 and int(run(kb, [progs[2]], 5, 2, T)["models"][0]) > 0
+    assert int(run(kb, [progs[3]], 5, 2, S5)["models"][0]) == 0 and int(run(kb, [progs[3]], 5, 2, S4)["models"][0]) > 0
+
+
+def test_c4_three_variables_ranges_golden(kb):
+    g = gold("c4_ranges.npz")
+    progs = W.corpus_c4()
+    h = kb.Programs(*W.pack_programs(progs), 3)
+    for i, b in enumerate(g["begin"]):
+        got = run(kb, progs, 5, 3, K, int(b), int(g["width"]), handle=h)
+        same(got, {key: g[key][i] for key in KEYS}, f"C4 range {int(b)}")
+    got = run(kb, progs[:64], 5, 3, K, int(g["begin"][0]), int(g["width"]), flags=kb.KERNEL_SCALAR)
+    same(got, {key: g[key][0][:64] for key in KEYS}, "C4 scalar")
+
+
+def test_c3_n5_full_corpus_witnesses(kb, vol):
+    """The headline workload's certificates: every (formula, class) witness of the n=5 layer is
+    accepted by the set-based checker, and is the first: the oracle finds the same witness when it
+    scans the class from its first frame up to the reported one."""
+    progs = W.corpus_c2()
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 2)
+    results = {}
+    for cname, cls in CLS.items():
+        results[cname] = run(kb, progs, 5, 2, cls, handle=h)
+    # monotone in the class: refuted in a stronger class => refuted in every weaker one
+    for weak, strong in (("K", "T"), ("T", "S4"), ("S4", "S5")):
+        assert ((results[strong]["models"] > 0) <= (results[weak]["models"] > 0)).all()
+    for cname, cls in CLS.items():
+        res = results[cname]
+        certify(progs, res, 5, 2, cls, idx=range(0, len(progs), 11))
+        frames = None if cls == K else vol.class_frames(5, cls)
+        hit = np.nonzero(res["wit_f"] != O.NO_WITNESS)[0]
+        pos = res["wit_f"][hit] if cls == K else np.searchsorted(frames, res["wit_f"][hit])
+        unverified = 0
+        for p in np.unique(pos):
+            if p >= 512:                       # cap the oracle's prefix scan
+                unverified += int((pos == p).sum())
+                continue
+            sel = hit[pos == p]
+            sc, so = W.pack_programs([progs[b] for b in sel])
+            want = vol.census(sc, so, 5, 2, cls, 0, int(p) + 1)
+            for key in ("wit_f", "wit_v", "wit_w"):
+                assert (want[key].astype(np.uint64) == res[key][sel].astype(np.uint64)).all(), (cname, int(p), key)
+        assert unverified <= 8, f"{cname}: {unverified} witnesses beyond the firstness cap"
+
+
+def test_ranges_compose(kb, vol):
+    """Range additivity, KRIPKE_ACCUMULATE, ragged and empty ranges, the last frames of a class."""
+    import torch
+    progs = W.corpus_c2(256)
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 2)
+    full = run(kb, progs, 4, 2, K, handle=h)
+    cuts = [0, 1, 130, 131, 4099, 30000, 65535, 65536]
+    c = torch.zeros((len(progs), 2), dtype=torch.int64, device="cuda")
+    w = torch.full((len(progs), 2), -1, dtype=torch.int64, device="cuda")
+    w[:, 1] = 0
+    for a, b in reversed(list(zip(cuts, cuts[1:]))):       # out of order on purpose
+        kb.eval_batch_range(h, 4, 2, K, a, b - a, kb.ACCUMULATE, c, w)
+    same(kb.unpack(c, w), full, "accumulated pieces")
+    # ragged ranges with both kernels against the oracle
+    for cls, a, n in ((K, 12345, 777), (T, 4000, 96), (S4, 300, 55), (K, 65535, 1), (K, 7, 0)):
+        want = vol.census(code, offs, 4, 2, cls, a, n)
+        for flags in (kb.KERNEL_AUTO, kb.KERNEL_SCALAR):
+            same(run(kb, progs, 4, 2, cls, a, n, flags, handle=h), want, f"ragged cls={cls} [{a},+{n})")
+    # k=0 shapes put frames inside the word: unaligned ranges must still be exact
+    p0, _, _ = W.pairs_c5(30)
+    c0, o0 = W.pack_programs(p0)
+    for a, n in ((3, 1000), (127, 130), (128, 256), (500, 1)):
+        same(run(kb, p0, 4, 0, K, a, n), vol.census(c0, o0, 4, 0, K, a, n), f"k=0 [{a},+{n})")
+
+
+def test_argument_errors(kb):
+    import torch
+    progs = W.corpus_c1(8)
+    h = kb.Programs(*W.pack_programs(progs), 2)
+    lib = kb.load()
+    c = torch.zeros((8, 2), dtype=torch.int64, device="cuda")
+    w = torch.zeros((8, 2), dtype=torch.int64, device="cuda")
+    call = lambda n, k, cls, a, cnt, fl: lib.kripke_eval_batch_range(h._h, n, k, cls, a, cnt, fl, c.data_ptr(), w.data_ptr(), None)
+    assert call(3, 2, 0, 0, 512, 0) == kb.OK
+    assert call(0, 2, 0, 0, 1, 0) == kb.EINVAL and call(7, 2, 0, 0, 1, 0) == kb.EINVAL
+    assert call(3, 1, 0, 0, 1, 0) == kb.EINVAL            # n_vars differs from the handle's
+    assert call(3, 2, 4, 0, 1, 0) == kb.EINVAL            # bad class
+    assert call(3, 2, 0, 500, 13, 0) == kb.EINVAL         # range past the class
+    assert call(3, 2, 0, 0, 1, 1 << 20) == kb.EINVAL      # unknown flag
+    assert call(3, 2, 1, 0, 64, kb.KERNEL_SLICED) == kb.EUNSUPPORTED   # group-per-unit shape, class T
+    assert lib.kripke_eval_batch_range(h._h, 3, 2, 0, 0, 1, 0, None, None, None) == kb.EINVAL
+    assert lib.kripke_eval_batch(None, 3, 2, 0, c.data_ptr(), w.data_ptr(), None) == kb.EINVAL
+    torch.cuda.synchronize()
+
+
+def test_scalar_reduce_modes_agree(kb, vol):
+    progs = W.corpus_c2(128)
+    code, offs = W.pack_programs(progs)
+    want = vol.census(code, offs, 4, 2, T)
+    for mode in (kb.REDUCE_BLOCK, kb.REDUCE_WARP, kb.REDUCE_THREAD):
+        same(run(kb, progs, 4, 2, T, flags=kb.KERNEL_SCALAR | mode), want, f"reduce mode {mode}")
+
+
+def test_host_buffer_entry_point(kb, vol):
+    progs = W.corpus_c1(100)
+    code, offs = W.pack_programs(progs)
+    c, w = kb.eval_batch_host(code, offs, 3, 2, K)
+    same(kb.unpack(c, w), vol.census(code, offs, 3, 2, K), "eval_batch_host")
+
+
+# ---------------------------------------------------------------------------------------------
+def pairs_run(kb, h, pairs, n, k, begin=0, count=None, flags=0):
+    if count is None:
+        count = kb.class_size(n, K) - begin
+    c, w = kb.distinguish_pairs(h, pairs, n, k, K, begin, count, flags)
+    return kb.unpack(c, w)
+
+
+def test_c5_pairs_through_five_worlds_golden(kb, vol):
+    """Config 5's exhaustive recheck: every pair on every labelled frame of 1..5 worlds."""
+    g = gold("c5_counts.npz")
+    progs, pairs, names = W.pairs_c5()
+    pairs = np.array(pairs, np.uint32)
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 0)
+    for n in (1, 2, 3, 4):
+        got = pairs_run(kb, h, pairs, n, 0)
+        assert (got["models"] == got["frames"]).all()
+        same(got, {key: g[f"n{n}_{key}"] for key in ("frames", "wit_f", "wit_w")}, f"pairs n={n}",
+             keys=("frames", "wit_f", "wit_w"))
+    got = pairs_run(kb, h, pairs, 5, 0)
+    same(got, {"frames": g["n5_frames"]}, "pairs n=5", keys=("frames",))
+    # n=5 witnesses: certificate + firstness by an oracle prefix scan (capped)
+    hit = np.nonzero(got["wit_f"] != O.NO_WITNESS)[0]
+    for j in hit[::17]:
+        a, b = progs[pairs[j][0]], progs[pairs[j][1]]
+        assert O.check_pair_witness(a, b, 5, 0, K, int(got["wit_f"][j]), 0, int(got["wit_w"][j]))
+    small = hit[got["wit_f"][hit] < (1 << 16)]
+    for f in np.unique(got["wit_f"][small]):
+        sel = small[got["wit_f"][small] == f]
+        want = vol.census(code, offs, 5, 0, K, 0, int(f) + 1, pairs=pairs[sel])
+        assert (want["wit_f"] == f).all() and (want["wit_w"] == got["wit_w"][sel]).all()
+    # the paper's named results: alpha_1/alpha_2 split at 4, alpha_2/alpha_3 agree through 5
+    assert names[0] == "alpha_1/alpha_2" and names[1] == "alpha_2/alpha_3"
+    assert int(got["frames"][1]) == 0 and int(got["frames"][0]) > 0
+    # scalar kernel agrees on a subset
+    sub = pairs[:40]
+    same(pairs_run(kb, h, sub, 4, 0, flags=kb.KERNEL_SCALAR),
+         {key: g[f"n4_{key}"][:40] for key in ("frames", "wit_f", "wit_w")}, "pairs scalar",
+         keys=("frames", "wit_f", "wit_w"))
+
+
+def test_c5_alpha_pair_separates_at_six_worlds(kb, vol):
+    """Proposition 5: alpha_2 / alpha_3 first split at six worlds.  The first
+    distinguishing labelled frame is f = 17,335,328 (oracle prefix scan in tests/test_oracle_pins.py);
+    the paper's own path frame 541,098,242 distinguishes them at world 0."""
+    progs = [W.to_postfix(W.alpha(m)) for m in (1, 2, 3)]
+    h = kb.Programs(*W.pack_programs(progs), 0)
+    pairs = np.array([[1, 2], [0, 1]], np.uint32)
+    got = pairs_run(kb, h, pairs, 6, 0, 0, 1 << 25)
+    assert int(got["wit_f"][0]) == 17335328
+    assert O.check_pair_witness(progs[1], progs[2], 6, 0, K, 17335328, 0, int(got["wit_w"][0]))
+    code, offs = W.pack_programs(progs)
+    want = vol.census(code, offs, 6, 0, K, 17335000, 1000, pairs=pairs)
+    same(pairs_run(kb, h, pairs, 6, 0, 17335000, 1000), want, "n=6 window")
+    one = pairs_run(kb, h, pairs, 6, 0, 541098242, 1)
+    assert int(one["frames"][0]) == 1 and int(one["wit_w"][0]) == 0
+    # chunked ascending scan with accumulation = the same first frame
+    import torch
+    c = torch.zeros((2, 2), dtype=torch.int64, device="cuda")
+    w = torch.full((2, 2), -1, dtype=torch.int64, device="cuda")
+    for a in range(0, 1 << 25, 1 << 23):
+        kb.distinguish_pairs(h, pairs, 6, 0, K, a, 1 << 23, kb.ACCUMULATE, c, w)
+    same(kb.unpack(c, w), got, "chunked n=6")
+
+
+def test_pairs_with_variables(kb, vol):
+    progs = W.corpus_c2(64)
+    code, offs = W.pack_programs(progs)
+    pairs = np.array([[i, 63 - i] for i in range(32)], np.uint32)
+    h = kb.Programs(code, offs, 2)
+    for n, a, cnt in ((3, 0, 512), (4, 1000, 300)):
+        want = vol.census(code, offs, n, 2, K, a, cnt, pairs=pairs)
+        for flags in (kb.KERNEL_AUTO, kb.KERNEL_SCALAR):
+            same(pairs_run(kb, h, pairs, n, 2, a, cnt, flags), want, f"pairs k=2 n={n}")
+
+
+def test_calibration_runs(kb):
+    rate, ms = kb.calibrate_int32(0)
+    assert rate > 1e12 and ms > 0
