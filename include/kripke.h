@@ -186,11 +186,14 @@ int kripke_keys_to_witness(const uint64_t *keys, uint32_t n_records, uint32_t n_
                            uint32_t n_vars, kripke_witness_t *witness_out, void *stream);
 
 /* Diagnostic (pure host, no CUDA): lowers one program - or the pair (a, b) if code_b != NULL - to
- * the bit-sliced kernel's micro-ops (csrc/ucode.h) and copies them to ucode_out (capacity cap).
+ * the bit-sliced kernel's 16-bit micro-ops (csrc/ucode.h: low byte op, high byte argument) and
+ * copies them to ucode_out (capacity cap entries).  leaf_mode: bit 0 = "box F / dia T is a leaf",
+ * bit 1 = "p_0, box p_0, dia p_0 are leaves" (what the kernel instantiation for a shape provides).
  * Returns the number of micro-ops, or a negative kripke_status (KRIPKE_EUNSUPPORTED if the program
  * needs more register-stack slots than the kernel has; *need_out is set in both cases). */
 int kripke_debug_lower(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b,
-                       uint32_t n_vars, uint8_t *ucode_out, uint32_t cap, uint32_t *need_out);
+                       uint32_t n_vars, uint32_t leaf_mode, uint16_t *ucode_out, uint32_t cap,
+                       uint32_t *need_out);
 
 #ifdef __cplusplus
 }

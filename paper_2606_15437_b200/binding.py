@@ -75,7 +75,7 @@ def load():
                                            ctypes.POINTER(ctypes.c_double), vp]
     lib.kripke_witness_to_keys.argtypes = [vp, u32, u32, u32, vp, vp]
     lib.kripke_keys_to_witness.argtypes = [vp, u32, u32, u32, vp, vp]
-    lib.kripke_debug_lower.argtypes = [u8p, u32, u8p, u32, u32, u8p, u32, ctypes.POINTER(u32)]
+    lib.kripke_debug_lower.argtypes = [u8p, u32, u8p, u32, u32, u32, u8p, u32, ctypes.POINTER(u32)]
     for name in EXPORTS:
         if name not in ("kripke_version",):
             getattr(lib, name).restype = ctypes.c_int
@@ -245,19 +245,19 @@ def keys_to_witness(keys, n_worlds: int, n_vars: int, witness_out=None, stream=N
     return witness_out
 
 
-def debug_lower(code_a: bytes, code_b: bytes | None, n_vars: int):
-    """(micro-ops as bytes, register-stack slots needed); raises KripkeError(EUNSUPPORTED) if the
+def debug_lower(code_a: bytes, code_b: bytes | None, n_vars: int, leaf_mode: int = 0):
+    """([(op, arg), ...], register-stack slots needed); raises KripkeError(EUNSUPPORTED) if the
     program does not fit the bit-sliced kernel."""
     a = np.frombuffer(bytes(code_a), np.uint8).copy()
     b = np.frombuffer(bytes(code_b), np.uint8).copy() if code_b is not None else None
-    out = np.zeros(256, np.uint8)
+    out = np.zeros(256, np.uint16)
     need = ctypes.c_uint32(0)
     rc = load().kripke_debug_lower(a.ctypes.data, len(a), b.ctypes.data if b is not None else None,
-                                   len(b) if b is not None else 0, n_vars, out.ctypes.data, len(out),
-                                   ctypes.byref(need))
+                                   len(b) if b is not None else 0, n_vars, leaf_mode, out.ctypes.data,
+                                   len(out), ctypes.byref(need))
     if rc < 0:
         raise KripkeError(rc, "kripke_debug_lower")
-    return bytes(out[:rc]), need.value
+    return [(int(x) & 0xFF, int(x) >> 8) for x in out[:rc]], need.value
 
 
 def unpack(counts, witness):

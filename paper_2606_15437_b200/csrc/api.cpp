@@ -39,10 +39,10 @@ int upload(T **dst, const std::vector<T> &src) {
 
 // A lowered set of records for the sliced kernel plus the list of records it cannot run.
 struct HostPlan {
-    std::vector<uint8_t> ucode;
+    std::vector<uint16_t> ucode;
     std::vector<uint32_t> slot_record;
     std::vector<uint32_t> unfit;
-    uint32_t stride = 4;
+    uint32_t stride = 2;
     uint32_t max_need = 0;
     uint64_t n_modal = 0, n_bool = 0;
 };
@@ -51,13 +51,13 @@ void build_plan(const std::vector<Lowered> &low, const std::vector<bool> &fits, 
     size_t longest = 1;
     for (size_t i = 0; i < low.size(); ++i)
         if (fits[i]) longest = std::max(longest, low[i].ucode.size());
-    hp->stride = (uint32_t)((longest + 1 + 3) / 4 * 4);        // one spare byte after FIN (prefetch)
+    hp->stride = (uint32_t)((longest + 1 + 1) / 2 * 2);        // one spare entry after FIN (prefetch)
     for (size_t i = 0; i < low.size(); ++i) {
         if (!fits[i]) { hp->unfit.push_back((uint32_t)i); continue; }
         hp->slot_record.push_back((uint32_t)i);
         size_t at = hp->ucode.size();
-        hp->ucode.resize(at + hp->stride, (uint8_t)UC_FIN_ALL);
-        std::memcpy(&hp->ucode[at], low[i].ucode.data(), low[i].ucode.size());
+        hp->ucode.resize(at + hp->stride, (uint16_t)UC_FIN_ALL);
+        std::memcpy(&hp->ucode[at], low[i].ucode.data(), low[i].ucode.size() * sizeof(uint16_t));
         hp->max_need = std::max(hp->max_need, (uint32_t)low[i].need);
         hp->n_modal += low[i].n_modal;
         hp->n_bool += low[i].n_bool;
@@ -65,10 +65,10 @@ void build_plan(const std::vector<Lowered> &low, const std::vector<bool> &fits, 
 }
 
 struct DevicePlan {
-    uint8_t *ucode = nullptr;
+    uint16_t *ucode = nullptr;
     uint32_t *slot_record = nullptr;
     uint32_t *unfit = nullptr;
-    uint32_t n_slots = 0, n_unfit = 0, stride = 4, max_need = 0;
+    uint32_t n_slots = 0, n_unfit = 0, stride = 2, max_need = 0;
     uint64_t n_modal = 0, n_bool = 0;
     void release() {
         cudaFree(ucode); cudaFree(slot_record); cudaFree(unfit);
@@ -188,7 +188,7 @@ struct kripke_programs {
     std::vector<uint32_t> h_offsets;
     uint8_t *d_code = nullptr;
     uint32_t *d_offsets = nullptr;
-    DevicePlan single;                 // one record per formula
+    std::map<uint32_t, DevicePlan> single;   // one record per formula, per lowering mode (built on first use)
     DevicePlan pair;                   // rebuilt by each kripke_distinguish_pairs call
     uint32_t *d_pairs = nullptr;
     uint32_t pairs_cap = 0;
@@ -205,6 +205,25 @@ int ensure_accum(kripke_programs *h, uint32_t n) {
     h->d_accum = nullptr; h->accum_cap = 0;
     CU(cudaMalloc((void **)&h->d_accum, (size_t)n * sizeof(Accum)));
     h->accum_cap = n;
+    return KRIPKE_OK;
+}
+
+// The batch lowered for one set of derived leaves (cached in the handle; synchronous upload).
+int single_plan(kripke_programs *h, uint32_t mode, const DevicePlan **out) {
+    auto it = h->single.find(mode);
+    if (it == h->single.end()) {
+        std::vector<Lowered> low(h->n_formulas);
+        std::vector<bool> fits(h->n_formulas);
+        for (uint32_t b = 0; b < h->n_formulas; ++b)
+            fits[b] = lower_single(&h->h_code[h->h_offsets[b]], h->h_offsets[b + 1] - h->h_offsets[b], mode, &low[b]);
+        HostPlan hp;
+        build_plan(low, fits, &hp);
+        DevicePlan dp;
+        int rc = upload_plan(hp, &dp);
+        if (rc) { dp.release(); return rc; }
+        it = h->single.emplace(mode, dp).first;
+    }
+    *out = &it->second;
     return KRIPKE_OK;
 }
 
@@ -243,11 +262,11 @@ int run_scan(kripke_programs *h, const DevicePlan &plan, const uint32_t *d_pairs
     uint32_t launches = 1;
 
     // the sliced kernel runs the batch if an instantiation for this shape keeps enough stack slots
+    uint64_t fpu = 1;
     bool use_sliced = family != KRIPKE_KERNEL_SCALAR && plan.n_slots > 0 &&
-                      sliced_max_need(n, k, cls) >= plan.max_need;
+                      sliced_select(n, k, cls, plan.max_need, &fpu);
     uint64_t ab = begin, ae = begin;          // aligned sub-range for the sliced kernel
     if (use_sliced) {
-        const uint64_t fpu = sliced_frames_per_unit(n, k);
         ab = (begin + fpu - 1) / fpu * fpu;
         ae = (begin + count) / fpu * fpu;
         if (ae <= ab) { use_sliced = false; ab = ae = begin; }
@@ -311,15 +330,8 @@ int kripke_programs_create(const uint8_t *code, const uint32_t *offsets, uint32_
     h->h_code.assign(code + offsets[0], code + offsets[n_formulas]);
     const uint32_t base = offsets[0];
     for (auto &o : h->h_offsets) o -= base;
-    std::vector<Lowered> low(n_formulas);
-    std::vector<bool> fits(n_formulas);
-    for (uint32_t b = 0; b < n_formulas; ++b)
-        fits[b] = lower_single(&h->h_code[h->h_offsets[b]], h->h_offsets[b + 1] - h->h_offsets[b], &low[b]);
-    HostPlan hp;
-    build_plan(low, fits, &hp);
     if (h->h_code.empty()) h->h_code.push_back(0);
-    if ((rc = upload(&h->d_code, h->h_code)) || (rc = upload(&h->d_offsets, h->h_offsets)) ||
-        (rc = upload_plan(hp, &h->single))) {
+    if ((rc = upload(&h->d_code, h->h_code)) || (rc = upload(&h->d_offsets, h->h_offsets))) {
         kripke_programs_destroy(h);
         return rc;
     }
@@ -330,7 +342,7 @@ int kripke_programs_create(const uint8_t *code, const uint32_t *offsets, uint32_
 int kripke_programs_destroy(kripke_programs_t *h) {
     if (!h) return KRIPKE_OK;
     cudaDeviceSynchronize();
-    h->single.release();
+    for (auto &kv : h->single) kv.second.release();
     h->pair.release();
     cudaFree(h->d_code); cudaFree(h->d_offsets); cudaFree(h->d_pairs); cudaFree(h->d_accum);
     delete h;
@@ -343,7 +355,10 @@ int kripke_eval_batch_range(const kripke_programs_t *programs, uint32_t n_worlds
                             void *stream) {
     if (!programs) return KRIPKE_EINVAL;
     kripke_programs *h = const_cast<kripke_programs *>(programs);
-    return run_scan(h, h->single, nullptr, h->n_formulas, n_worlds, n_vars, frame_class, frame_begin,
+    const DevicePlan *plan = nullptr;
+    int rc = single_plan(h, sliced_lower_mode(n_worlds, n_vars), &plan);
+    if (rc) return rc;
+    return run_scan(h, *plan, nullptr, h->n_formulas, n_worlds, n_vars, frame_class, frame_begin,
                     frame_count, flags, counts_out, witness_out, stream);
 }
 
@@ -365,12 +380,13 @@ int kripke_distinguish_pairs(const kripke_programs_t *programs, const uint32_t *
     kripke_programs *h = const_cast<kripke_programs *>(programs);
     for (uint32_t i = 0; i < 2 * n_pairs; ++i)
         if (pairs[i] >= h->n_formulas) return KRIPKE_EINVAL;
+    const uint32_t mode = sliced_lower_mode(n_worlds, n_vars);
     std::vector<Lowered> low(n_pairs);
     std::vector<bool> fits(n_pairs);
     for (uint32_t j = 0; j < n_pairs; ++j) {
         const uint32_t a = pairs[2 * j], b = pairs[2 * j + 1];
         fits[j] = lower_pair(&h->h_code[h->h_offsets[a]], h->h_offsets[a + 1] - h->h_offsets[a],
-                             &h->h_code[h->h_offsets[b]], h->h_offsets[b + 1] - h->h_offsets[b], &low[j]);
+                             &h->h_code[h->h_offsets[b]], h->h_offsets[b + 1] - h->h_offsets[b], mode, &low[j]);
     }
     HostPlan hp;
     build_plan(low, fits, &hp);
@@ -444,18 +460,21 @@ int kripke_keys_to_witness(const uint64_t *keys, uint32_t n_records, uint32_t n_
 }
 
 int kripke_debug_lower(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b,
-                       uint32_t n_vars, uint8_t *ucode_out, uint32_t cap, uint32_t *need_out) {
+                       uint32_t n_vars, uint32_t leaf_mode, uint16_t *ucode_out, uint32_t cap,
+                       uint32_t *need_out) {
     if (!code_a || !ucode_out) return KRIPKE_EINVAL;
     const uint32_t offs_a[2] = {0, len_a}, offs_b[2] = {0, len_b};
     int rc = validate_programs(code_a, offs_a, 1, n_vars, nullptr);
     if (rc == KRIPKE_OK && code_b) rc = validate_programs(code_b, offs_b, 1, n_vars, nullptr);
     if (rc) return rc;
     Lowered low;
-    const bool fits = code_b ? lower_pair(code_a, len_a, code_b, len_b, &low) : lower_single(code_a, len_a, &low);
+    if (leaf_mode > 3) return KRIPKE_EINVAL;
+    const bool fits = code_b ? lower_pair(code_a, len_a, code_b, len_b, leaf_mode, &low)
+                             : lower_single(code_a, len_a, leaf_mode, &low);
     if (need_out) *need_out = (uint32_t)low.need;
     if (!fits) return KRIPKE_EUNSUPPORTED;
     if (low.ucode.size() > cap) return KRIPKE_EINVAL;
-    std::memcpy(ucode_out, low.ucode.data(), low.ucode.size());
+    std::memcpy(ucode_out, low.ucode.data(), low.ucode.size() * sizeof(uint16_t));
     return (int)low.ucode.size();
 }
 

@@ -11,15 +11,16 @@ namespace kripke {
 
 // ---- lower.cpp ---------------------------------------------------------------------------------
 struct Lowered {
-    std::vector<uint8_t> ucode;   // micro-ops, FIN last
+    std::vector<uint16_t> ucode;  // micro-ops (op | arg << 8), FIN last
     int need = 0;                 // register-stack slots needed (fits the sliced kernel iff <= UC_DMAX)
     uint32_t n_modal = 0;         // executed box/dia micro-ops
     uint32_t n_bool = 0;          // executed and/or/andn/nand micro-ops
 };
 int validate_programs(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas, uint32_t n_vars,
                       uint32_t *max_stack_out);
-bool lower_single(const uint8_t *code, uint32_t len, Lowered *out);
-bool lower_pair(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b, Lowered *out);
+bool lower_single(const uint8_t *code, uint32_t len, uint32_t mode, Lowered *out);
+bool lower_pair(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b, uint32_t mode,
+                Lowered *out);
 
 // ---- device-side job description (kernels) -----------------------------------------------------
 // Accumulators per output record, owned by the programs handle, zeroed at the start of a call.
@@ -50,17 +51,18 @@ struct ScanJob {
 // ---- launch wrappers (defined in the .cu files) ------------------------------------------------
 struct SlicedPlan {
     // lowered slots (a slot is one record the sliced kernel evaluates)
-    const uint8_t *ucode;         // device: n_slots * stride bytes
+    const uint16_t *ucode;        // device: n_slots * stride micro-ops
     const uint32_t *slot_record;  // device: record index per slot
     uint32_t n_slots;
-    uint32_t stride;              // bytes per slot (multiple of 4, >= longest ucode + 1)
+    uint32_t stride;              // micro-ops per slot (even, >= longest program + 1)
     uint32_t max_need;            // most register-stack slots any slot needs
 };
 
-// Most register-stack slots an instantiation for this shape offers (0 = shape not supported).
-uint32_t sliced_max_need(uint32_t n, uint32_t k, uint32_t cls);
-// Class frames per scan unit of the sliced kernel for this shape (ranges must be multiples of it).
-uint64_t sliced_frames_per_unit(uint32_t n, uint32_t k);
+// Is there a sliced instantiation for this shape and class that keeps `need` stack slots?  If so
+// *frames_per_unit is the alignment frame ranges must have for it.
+bool sliced_select(uint32_t n, uint32_t k, uint32_t cls, uint32_t need, uint64_t *frames_per_unit);
+// LOWER_LEAF_* flags of the derived leaves the instantiations for this shape provide (0 = no shape).
+uint32_t sliced_lower_mode(uint32_t n, uint32_t k);
 // Enqueue the sliced scan; returns a cudaError_t as int and the number of kernel launches.
 int launch_sliced(const ScanJob &job, const SlicedPlan &plan, void *stream, uint32_t *launches);
 // Enqueue the scalar (Algorithm 1) scan over the records listed in `records` (device, or null = all).

@@ -23,10 +23,17 @@ struct Node {
     int need;        // register-stack slots needed to evaluate this subtree
 };
 
+struct Leaf {
+    bool is = false;      // the subtree is read as an operand, it never occupies a slot
+    bool is_var = false;  // true: variable p_id (LOADV / BOOLV); false: leaf-table entry id (LOADL / BOOLL)
+    uint8_t id = 0;
+    int pol = 0;          // 1 = the subtree's value is the complement of the leaf
+};
+
 struct Lowerer {
+    uint32_t mode = 0;               // LOWER_LEAF_* flags
     std::vector<Node> nodes;
-    std::vector<uint8_t> out;
-    uint64_t logic_ops = 0;   // per 32-model word, as a function of n: modal*n*n + bool*n
+    std::vector<uint16_t> out;
     uint32_t n_modal = 0, n_bool = 0;
 
     int add(NodeKind k, uint8_t v, int a, int b) {
@@ -87,30 +94,85 @@ struct Lowerer {
         return st.back();
     }
 
-    // Slots needed when the deeper operand of a binary node is evaluated first (Sethi-Ullman).
+    // Is the subtree an atom or a derived leaf of the target kernel?
+    Leaf leaf_of(int i) const {
+        Leaf lf;
+        int pol = 0;
+        while (nodes[i].kind == N_NOT) { pol ^= 1; i = nodes[i].a; }
+        const Node &nd = nodes[i];
+        if (nd.kind == N_VAR) {
+            lf.is = true; lf.pol = pol;
+            if (nd.value == 0 && (mode & LOWER_LEAF_P)) { lf.is_var = false; lf.id = LEAF_P; }
+            else { lf.is_var = true; lf.id = nd.value; }
+            return lf;
+        }
+        if (nd.kind != N_BOX && nd.kind != N_DIA) return lf;
+        int j = nd.a, cp = 0;
+        while (nodes[j].kind == N_NOT) { cp ^= 1; j = nodes[j].a; }
+        const bool box = nd.kind == N_BOX;
+        if (nodes[j].kind == N_CONST && (mode & LOWER_LEAF_DEAD)) {
+            const int c = nodes[j].value ^ cp;
+            // box F = "no successor" ; dia T = ~(box F).  (box T and dia F were folded away.)
+            if (box && c == 0) { lf.is = true; lf.id = LEAF_DEAD; lf.pol = pol; }
+            else if (!box && c == 1) { lf.is = true; lf.id = LEAF_DEAD; lf.pol = pol ^ 1; }
+            return lf;
+        }
+        if (nodes[j].kind == N_VAR && nodes[j].value == 0 && (mode & LOWER_LEAF_P)) {
+            // box ~p = ~dia p ; dia ~p = ~box p
+            lf.is = true;
+            lf.id = (box != (cp != 0)) ? LEAF_BOXP : LEAF_DIAP;
+            lf.pol = pol ^ cp;
+            return lf;
+        }
+        return lf;
+    }
+
+    // Register-stack slots needed to leave the subtree's value in a slot; leaves used as operands
+    // need none.  The deeper operand of a binary node is evaluated first (Sethi-Ullman).
     int need(int i) {
+        if (leaf_of(i).is) return nodes[i].need = 0;
         Node &nd = nodes[i];
         switch (nd.kind) {
         case N_CONST: case N_VAR: nd.need = 1; break;
-        case N_NOT: case N_BOX: case N_DIA: nd.need = need(nd.a); break;
+        case N_NOT: nd.need = need(nd.a); break;
+        case N_BOX: case N_DIA: nd.need = std::max(1, need(nd.a)); break;
         default: {
             int l = need(nd.a), r = need(nd.b);
-            nd.need = (l >= r) ? std::max(l, r + 1) : std::max(r, l + 1);
+            if (l == 0 && r == 0) nd.need = 1;
+            else if (l == 0 || r == 0) nd.need = std::max(l, r);
+            else nd.need = (l >= r) ? std::max(l, r + 1) : std::max(r, l + 1);
         }
         }
         return nd.need;
     }
 
+    void op(uint32_t code, uint32_t arg = 0) { out.push_back((uint16_t)(code | (arg << 8))); }
+
+    void load_leaf(const Leaf &lf, int d) {
+        if (lf.is_var) op(UC_LOADV + lf.id * 4 + d);
+        else op(UC_LOADL + d, lf.id);
+    }
+    // D[d] <- (D[d] ^ a1) & (leaf ^ a2) up to the returned polarity
+    int bool_leaf(const Leaf &lf, int d, int a1, int a2, int flip) {
+        const int f = (!a1 && !a2) ? BF_AND : (!a1 && a2) ? BF_ANDN : (a1 && !a2) ? BF_NAND : BF_OR;
+        if (lf.is_var) op(UC_BOOLV + (f * 4 + lf.id) * 4 + d);
+        else op(UC_BOOLL + f * 4 + d, lf.id);
+        ++n_bool;
+        return (f == BF_OR) ? !flip : flip;          // ~s1 & ~s2 = ~(s1 | s2)
+    }
+
     // Emits micro-ops leaving the value of node i in slot d; returns its polarity (1 = the slot
     // holds the complement of the value).
     int emit(int i, int d) {
+        const Leaf self = leaf_of(i);
+        if (self.is) { load_leaf(self, d); return self.pol; }
         const Node nd = nodes[i];
         switch (nd.kind) {
         case N_CONST:
-            out.push_back((uint8_t)(UC_PUSH + 4 * UC_DMAX + d));
+            op(UC_LOADZ + d);
             return nd.value;                      // T is the complement of all-false
-        case N_VAR:
-            out.push_back((uint8_t)(UC_PUSH + nd.value * UC_DMAX + d));
+        case N_VAR:                               // (always a leaf; kept for completeness)
+            op(UC_LOADV + nd.value * 4 + d);
             return 0;
         case N_NOT:
             return !emit(nd.a, d);
@@ -118,25 +180,32 @@ struct Lowerer {
             int p = emit(nd.a, d);
             // box ~s = ~dia s ; dia ~s = ~box s
             bool box = (nd.kind == N_BOX) != (p != 0);
-            out.push_back((uint8_t)((box ? UC_BOX : UC_DIA) + d));
+            op((box ? UC_BOX : UC_DIA) + d);
             ++n_modal;
             return p;
         }
         default: {
+            // as a conjunction of literals: and = x & y ; or = ~(~x & ~y) ; imp = ~(x & ~y)
+            const int negx = (nd.kind == N_OR), negy = (nd.kind != N_AND), flip = (nd.kind != N_AND);
+            const Leaf la = leaf_of(nd.a), lb = leaf_of(nd.b);
+            if (lb.is) {                          // y is read as an operand (x may be a leaf too)
+                int px = emit(nd.a, d);
+                return bool_leaf(lb, d, px ^ negx, lb.pol ^ negy, flip);
+            }
+            if (la.is) {
+                int py = emit(nd.b, d);
+                return bool_leaf(la, d, py ^ negy, la.pol ^ negx, flip);
+            }
             bool a_first = nodes[nd.a].need >= nodes[nd.b].need;
             int first = a_first ? nd.a : nd.b, second = a_first ? nd.b : nd.a;
             int p1 = emit(first, d), p2 = emit(second, d + 1);
             int px = a_first ? p1 : p2, py = a_first ? p2 : p1;
-            // as a conjunction of literals: and = x & y ; or = ~(~x & ~y) ; imp = ~(x & ~y)
-            int negx = (nd.kind == N_OR), negy = (nd.kind != N_AND), flip = (nd.kind != N_AND);
             int ax = px ^ negx, ay = py ^ negy;
             int a1 = a_first ? ax : ay, a2 = a_first ? ay : ax;   // by slot: d, d+1
+            const int f = (!a1 && !a2) ? BF_AND : (!a1 && a2) ? BF_ANDN : (a1 && !a2) ? BF_NAND : BF_OR;
+            op(UC_BOOL + f * 4 + d);
             ++n_bool;
-            if (!a1 && !a2) { out.push_back((uint8_t)(UC_AND + d)); return flip; }
-            if (!a1 && a2) { out.push_back((uint8_t)(UC_ANDN + d)); return flip; }
-            if (a1 && !a2) { out.push_back((uint8_t)(UC_NAND + d)); return flip; }
-            out.push_back((uint8_t)(UC_OR + d));   // ~s1 & ~s2 = ~(s1 | s2)
-            return !flip;
+            return (f == BF_OR) ? !flip : flip;
         }
         }
     }
@@ -172,31 +241,34 @@ int validate_programs(const uint8_t *code, const uint32_t *offsets, uint32_t n_f
     return KRIPKE_OK;
 }
 
-bool lower_single(const uint8_t *code, uint32_t len, Lowered *out) {
+bool lower_single(const uint8_t *code, uint32_t len, uint32_t mode, Lowered *out) {
     Lowerer lw;
+    lw.mode = mode;
     int root = lw.build(code, len);
-    out->need = lw.need(root);
+    out->need = std::max(1, lw.need(root));
     if (out->need > UC_DMAX) return false;
     int p = lw.emit(root, 0);
-    lw.out.push_back(p ? UC_FIN_ANY : UC_FIN_ALL);
+    lw.op(p ? UC_FIN_ANY : UC_FIN_ALL);
     out->ucode = std::move(lw.out);
     out->n_modal = lw.n_modal;
     out->n_bool = lw.n_bool;
     return true;
 }
 
-bool lower_pair(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b, Lowered *out) {
+bool lower_pair(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b, uint32_t mode,
+                Lowered *out) {
     Lowerer lw;
+    lw.mode = mode;
     int ra = lw.build(code_a, len_a);
     int rb = lw.build(code_b, len_b);
-    int na = lw.need(ra), nb = lw.need(rb);
+    int na = std::max(1, lw.need(ra)), nb = std::max(1, lw.need(rb));
     // XOR is symmetric: evaluate the deeper formula first (slot 0), the other above it (slot 1)
     if (nb > na) { std::swap(ra, rb); std::swap(na, nb); }
     out->need = std::max(na, nb + 1);
     if (out->need > UC_DMAX) return false;
     int pa = lw.emit(ra, 0);
     int pb = lw.emit(rb, 1);
-    lw.out.push_back(pa == pb ? UC_FIN_XOR : UC_FIN_XNOR);
+    lw.op(pa == pb ? UC_FIN_XOR : UC_FIN_XNOR);
     out->ucode = std::move(lw.out);
     out->n_modal = lw.n_modal;
     out->n_bool = lw.n_bool;

@@ -45,10 +45,10 @@ struct SlicedParams {
     const uint64_t *class_table;
     uint64_t unit_begin;            // first scan unit
     uint64_t unit_count;
-    const uint8_t *ucode;           // n_slots * stride
+    const uint16_t *ucode;          // n_slots * stride micro-ops
     const uint32_t *slot_record;
     uint32_t n_slots;
-    uint32_t stride;
+    uint32_t stride;                // micro-ops per slot (even)
     uint32_t chunk;                 // slots per work item
     uint32_t n_chunks;
     uint32_t tiles_per_item;        // tiles of TPB (threads per block) units per work item
@@ -66,6 +66,13 @@ struct SlicedCfg {
     static constexpr bool FRAME_PER_UNIT = KN >= LOW;
     static constexpr int PASS_BITS = FRAME_PER_UNIT ? KN - LOW : 0;
     static constexpr int UNIT_FRAME_BITS = FRAME_PER_UNIT ? 0 : LOW - KN;   // log2 frames per unit
+    // p_0 lies entirely inside the 32-model word and the frame is thread-uniform: p_0, box p_0 and
+    // dia p_0 are the same N words for every word the thread holds -> leaf-table entries
+    static constexpr bool P_LEAF = FRAME_PER_UNIT && K >= 1 && N <= 5;
+    // leaf table words per thread: frame-per-unit: LEAF_COUNT leaves x N words (the same for all M
+    // words of the thread); group-per-unit: the dead-end leaf only, one copy per word (M x N)
+    static constexpr int LEAF_WORDS = FRAME_PER_UNIT ? LEAF_COUNT * N : M * N;
+    static constexpr uint32_t LOWER_MODE = LOWER_LEAF_DEAD | (P_LEAF ? LOWER_LEAF_P : 0u);
     static_assert(N >= 1 && N <= 6 && K >= 0 && K <= 4 && DMAX >= 2 && DMAX <= UC_DMAX, "shape");
     static_assert(N * N + KN >= LOW, "too few models for one group");
 };
@@ -75,13 +82,18 @@ __device__ __forceinline__ constexpr uint32_t lane_pattern(int pos) {
          : pos == 3 ? 0xFF00FF00u : 0xFFFF0000u;
 }
 
-template <class C>
+template <int F> __device__ __forceinline__ uint32_t bool_fn(uint32_t a, uint32_t b) {
+    return (F == BF_AND) ? (a & b) : (F == BF_OR) ? (a | b) : (F == BF_ANDN) ? (a & ~b) : (~a & b);
+}
+
+template <class C, int TPB>
 struct SlicedThread {
     static constexpr int N = C::N, M = C::M;
     static constexpr int DMAX = C::DMAX;
     uint32_t D[DMAX][M][N];           // register stack
     uint32_t E[N * N];                // thread-uniform edge masks (where not constant)
     uint32_t VH[C::PASS_BITS > 0 ? C::PASS_BITS : 1];   // pass-dependent valuation masks
+    const uint32_t *leaf;             // this thread's column of the shared-memory leaf table
 
     // word of the edge w->u for the thread's m-th word
     __device__ __forceinline__ uint32_t edge(int m, int w, int u) const {
@@ -98,16 +110,99 @@ struct SlicedThread {
         if (pos < C::LOW) return ((m >> (pos - 5)) & 1) ? 0xFFFFFFFFu : 0u;
         return VH[(pos - C::LOW) < C::PASS_BITS ? (pos - C::LOW) : 0];
     }
+    // leaf-table word (entry l, world w) - frame-per-unit layout; (word m, world w) otherwise
+    __device__ __forceinline__ uint32_t leaf_word(uint32_t l, int m, int w) const {
+        if (C::FRAME_PER_UNIT) return leaf[(l * N + w) * TPB];
+        return leaf[(m * N + w) * TPB];
+    }
 
-    template <int d> __device__ __forceinline__ void push_var(int i) {
-        if (d >= DMAX || i >= C::K) return;      // never emitted for this instantiation
+    // Once per scan unit: the derived leaves go to the leaf table.
+    __device__ __forceinline__ void store_leaves(uint32_t *col) const {
+        if (C::FRAME_PER_UNIT) {
+#pragma unroll
+            for (int w = 0; w < N; ++w) {
+                uint32_t none = 0xFFFFFFFFu, boxp = 0xFFFFFFFFu, diap = 0u;
+#pragma unroll
+                for (int u = 0; u < N; ++u) {
+                    none &= ~E[w * N + u];                                   // box F: no successor
+                    if (C::P_LEAF) {
+                        boxp &= (lane_pattern(u) | ~E[w * N + u]);           // box p_0
+                        diap |= (lane_pattern(u) & E[w * N + u]);            // dia p_0
+                    }
+                }
+                col[(LEAF_DEAD * N + w) * TPB] = none;
+                if (C::P_LEAF) {
+                    col[(LEAF_P * N + w) * TPB] = lane_pattern(w);
+                    col[(LEAF_BOXP * N + w) * TPB] = boxp;
+                    col[(LEAF_DIAP * N + w) * TPB] = diap;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int m = 0; m < M; ++m)
+#pragma unroll
+                for (int w = 0; w < N; ++w) {
+                    uint32_t none = 0xFFFFFFFFu;
+#pragma unroll
+                    for (int u = 0; u < N; ++u) none &= ~edge(m, w, u);
+                    col[(m * N + w) * TPB] = none;
+                }
+        }
+    }
+
+    template <int d> __device__ __forceinline__ void load_var(int i) {
+        if (d >= DMAX || i >= C::K || (C::P_LEAF && i == 0)) return;   // never emitted for this instantiation
         constexpr int dd = d < DMAX ? d : 0;
 #pragma unroll
         for (int m = 0; m < M; ++m)
 #pragma unroll
             for (int w = 0; w < N; ++w) D[dd][m][w] = atom(i, m, w);
     }
-    template <int d> __device__ __forceinline__ void push_zero() {
+    template <int d, int F> __device__ __forceinline__ void bool_var(int i) {
+        if (d >= DMAX || i >= C::K || (C::P_LEAF && i == 0)) return;
+        constexpr int dd = d < DMAX ? d : 0;
+#pragma unroll
+        for (int m = 0; m < M; ++m)
+#pragma unroll
+            for (int w = 0; w < N; ++w) D[dd][m][w] = bool_fn<F>(D[dd][m][w], atom(i, m, w));
+    }
+    template <int d> __device__ __forceinline__ void load_leaf(uint32_t l) {
+        if (d >= DMAX) return;
+        constexpr int dd = d < DMAX ? d : 0;
+        if (C::FRAME_PER_UNIT) {
+            uint32_t v[N];
+#pragma unroll
+            for (int w = 0; w < N; ++w) v[w] = leaf_word(l, 0, w);
+#pragma unroll
+            for (int m = 0; m < M; ++m)
+#pragma unroll
+                for (int w = 0; w < N; ++w) D[dd][m][w] = v[w];
+        } else {
+#pragma unroll
+            for (int m = 0; m < M; ++m)
+#pragma unroll
+                for (int w = 0; w < N; ++w) D[dd][m][w] = leaf_word(l, m, w);
+        }
+    }
+    template <int d, int F> __device__ __forceinline__ void bool_leaf(uint32_t l) {
+        if (d >= DMAX) return;
+        constexpr int dd = d < DMAX ? d : 0;
+        if (C::FRAME_PER_UNIT) {
+            uint32_t v[N];
+#pragma unroll
+            for (int w = 0; w < N; ++w) v[w] = leaf_word(l, 0, w);
+#pragma unroll
+            for (int m = 0; m < M; ++m)
+#pragma unroll
+                for (int w = 0; w < N; ++w) D[dd][m][w] = bool_fn<F>(D[dd][m][w], v[w]);
+        } else {
+#pragma unroll
+            for (int m = 0; m < M; ++m)
+#pragma unroll
+                for (int w = 0; w < N; ++w) D[dd][m][w] = bool_fn<F>(D[dd][m][w], leaf_word(l, m, w));
+        }
+    }
+    template <int d> __device__ __forceinline__ void load_zero() {
         if (d >= DMAX) return;
         constexpr int dd = d < DMAX ? d : 0;
 #pragma unroll
@@ -155,10 +250,7 @@ struct SlicedThread {
 #pragma unroll
         for (int m = 0; m < M; ++m)
 #pragma unroll
-            for (int w = 0; w < N; ++w) {
-                const uint32_t a = D[dd][m][w], b = D[d1][m][w];
-                D[dd][m][w] = (F == 0) ? (a & b) : (F == 1) ? (a | b) : (F == 2) ? (a & ~b) : (~a & b);
-            }
+            for (int w = 0; w < N; ++w) D[dd][m][w] = bool_fn<F>(D[dd][m][w], D[d1][m][w]);
     }
     template <int F> __device__ __forceinline__ void fin(uint32_t (&r)[M]) const {
 #pragma unroll
@@ -176,51 +268,80 @@ struct SlicedThread {
     }
 
     // Runs one lowered program on the thread's M words; r[m] = models that refute / distinguish.
-    __device__ __forceinline__ void run(const uint8_t *__restrict__ uc, uint32_t (&r)[M]) {
+    __device__ __forceinline__ void run(const uint16_t *__restrict__ uc, uint32_t (&r)[M]) {
         uint32_t pc = 0;
         uint32_t nxt = uc[0];
         for (;;) {
-            const uint32_t op = nxt;
-            nxt = uc[++pc];          // prefetch (the slot's stride leaves a byte after FIN)
+            const uint32_t op = nxt & 0xFFu, arg = nxt >> 8;
+            nxt = uc[++pc];          // prefetch (the slot's stride leaves an entry after FIN)
             switch (op) {
 #define KRIPKE_CASE4(base, call) \
     case (base) + 0: call(0); break; case (base) + 1: call(1); break; \
     case (base) + 2: call(2); break; case (base) + 3: call(3); break;
 #define KRIPKE_CASE3(base, call) \
     case (base) + 0: call(0); break; case (base) + 1: call(1); break; case (base) + 2: call(2); break;
-#define PUSH0(d) push_var<d>(0)
-#define PUSH1(d) push_var<d>(1)
-#define PUSH2(d) push_var<d>(2)
-#define PUSH3(d) push_var<d>(3)
-#define PUSHZ(d) push_zero<d>()
+#define LV0(d) load_var<d>(0)
+#define LV1(d) load_var<d>(1)
+#define LV2(d) load_var<d>(2)
+#define LV3(d) load_var<d>(3)
+                KRIPKE_CASE4(UC_LOADV + 0, LV0) KRIPKE_CASE4(UC_LOADV + 4, LV1)
+                KRIPKE_CASE4(UC_LOADV + 8, LV2) KRIPKE_CASE4(UC_LOADV + 12, LV3)
+#define BV(f, i) KRIPKE_CASE4(UC_BOOLV + ((f) * 4 + (i)) * 4, BVD_##f##_##i)
+#define BVD_0_0(d) bool_var<d, 0>(0)
+#define BVD_0_1(d) bool_var<d, 0>(1)
+#define BVD_0_2(d) bool_var<d, 0>(2)
+#define BVD_0_3(d) bool_var<d, 0>(3)
+#define BVD_1_0(d) bool_var<d, 1>(0)
+#define BVD_1_1(d) bool_var<d, 1>(1)
+#define BVD_1_2(d) bool_var<d, 1>(2)
+#define BVD_1_3(d) bool_var<d, 1>(3)
+#define BVD_2_0(d) bool_var<d, 2>(0)
+#define BVD_2_1(d) bool_var<d, 2>(1)
+#define BVD_2_2(d) bool_var<d, 2>(2)
+#define BVD_2_3(d) bool_var<d, 2>(3)
+#define BVD_3_0(d) bool_var<d, 3>(0)
+#define BVD_3_1(d) bool_var<d, 3>(1)
+#define BVD_3_2(d) bool_var<d, 3>(2)
+#define BVD_3_3(d) bool_var<d, 3>(3)
+                BV(0, 0) BV(0, 1) BV(0, 2) BV(0, 3) BV(1, 0) BV(1, 1) BV(1, 2) BV(1, 3)
+                BV(2, 0) BV(2, 1) BV(2, 2) BV(2, 3) BV(3, 0) BV(3, 1) BV(3, 2) BV(3, 3)
+#define LL(d) load_leaf<d>(arg)
+#define BL0(d) bool_leaf<d, 0>(arg)
+#define BL1(d) bool_leaf<d, 1>(arg)
+#define BL2(d) bool_leaf<d, 2>(arg)
+#define BL3(d) bool_leaf<d, 3>(arg)
+                KRIPKE_CASE4(UC_LOADL, LL)
+                KRIPKE_CASE4(UC_BOOLL + 0, BL0) KRIPKE_CASE4(UC_BOOLL + 4, BL1)
+                KRIPKE_CASE4(UC_BOOLL + 8, BL2) KRIPKE_CASE4(UC_BOOLL + 12, BL3)
+#define BB0(d) boolean<d, 0>()
+#define BB1(d) boolean<d, 1>()
+#define BB2(d) boolean<d, 2>()
+#define BB3(d) boolean<d, 3>()
+                KRIPKE_CASE3(UC_BOOL + 0, BB0) KRIPKE_CASE3(UC_BOOL + 4, BB1)
+                KRIPKE_CASE3(UC_BOOL + 8, BB2) KRIPKE_CASE3(UC_BOOL + 12, BB3)
 #define BOXD(d) box<d>()
 #define DIAD(d) dia<d>()
-#define ANDD(d) boolean<d, 0>()
-#define ORD(d) boolean<d, 1>()
-#define ANDND(d) boolean<d, 2>()
-#define NANDD(d) boolean<d, 3>()
-                KRIPKE_CASE4(UC_PUSH + 0 * UC_DMAX, PUSH0)
-                KRIPKE_CASE4(UC_PUSH + 1 * UC_DMAX, PUSH1)
-                KRIPKE_CASE4(UC_PUSH + 2 * UC_DMAX, PUSH2)
-                KRIPKE_CASE4(UC_PUSH + 3 * UC_DMAX, PUSH3)
-                KRIPKE_CASE4(UC_PUSH + 4 * UC_DMAX, PUSHZ)
+#define LZ(d) load_zero<d>()
                 KRIPKE_CASE4(UC_BOX, BOXD)
                 KRIPKE_CASE4(UC_DIA, DIAD)
-                KRIPKE_CASE3(UC_AND, ANDD)
-                KRIPKE_CASE3(UC_OR, ORD)
-                KRIPKE_CASE3(UC_ANDN, ANDND)
-                KRIPKE_CASE3(UC_NAND, NANDD)
-#undef PUSH0
-#undef PUSH1
-#undef PUSH2
-#undef PUSH3
-#undef PUSHZ
+                KRIPKE_CASE4(UC_LOADZ, LZ)
+#undef LV0
+#undef LV1
+#undef LV2
+#undef LV3
+#undef BV
+#undef LL
+#undef BL0
+#undef BL1
+#undef BL2
+#undef BL3
+#undef BB0
+#undef BB1
+#undef BB2
+#undef BB3
 #undef BOXD
 #undef DIAD
-#undef ANDD
-#undef ORD
-#undef ANDND
-#undef NANDD
+#undef LZ
 #undef KRIPKE_CASE4
 #undef KRIPKE_CASE3
             case UC_FIN_ALL: fin<0>(r); return;
@@ -265,15 +386,18 @@ __global__ void __launch_bounds__(TPB, MINB) scan_sliced_kernel(SlicedParams p) 
     constexpr int N = C::N, M = C::M;
     constexpr int SLICED_THREADS = TPB;
     extern __shared__ __align__(16) unsigned char smem[];
-    unsigned long long *s_models = reinterpret_cast<unsigned long long *>(smem);
+    // [leaf table: LEAF_WORDS x TPB words][models u64 x chunk][frames u32 x chunk][best u32 x chunk][ucode]
+    uint32_t *s_leaf = reinterpret_cast<uint32_t *>(smem);
+    unsigned long long *s_models = reinterpret_cast<unsigned long long *>(s_leaf + C::LEAF_WORDS * TPB);
     uint32_t *s_frames = reinterpret_cast<uint32_t *>(s_models + p.chunk);
     uint32_t *s_best = s_frames + p.chunk;
-    uint8_t *s_ucode = reinterpret_cast<uint8_t *>(s_best + p.chunk);
+    uint16_t *s_ucode = reinterpret_cast<uint16_t *>(s_best + p.chunk);
 
     const uint32_t lane = threadIdx.x & 31u;
     const uint32_t n_items = p.n_ranges * p.n_chunks;
     const uint64_t units_per_item = (uint64_t)p.tiles_per_item * SLICED_THREADS;
-    SlicedThread<C> T;
+    SlicedThread<C, TPB> T;
+    T.leaf = s_leaf + threadIdx.x;
 
     for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
         const uint32_t chunk_id = item % p.n_chunks;
@@ -289,7 +413,7 @@ __global__ void __launch_bounds__(TPB, MINB) scan_sliced_kernel(SlicedParams p) 
             s_models[i] = 0ull; s_frames[i] = 0u; s_best[i] = 0xFFFFFFFFu;
         }
         {
-            const uint32_t words = nslots * (p.stride / 4);
+            const uint32_t words = nslots * (p.stride / 2);
             const uint32_t *src = reinterpret_cast<const uint32_t *>(p.ucode + (size_t)slot0 * p.stride);
             uint32_t *dst = reinterpret_cast<uint32_t *>(s_ucode);
             for (uint32_t i = threadIdx.x; i < words; i += SLICED_THREADS) dst[i] = src[i];
@@ -302,7 +426,6 @@ __global__ void __launch_bounds__(TPB, MINB) scan_sliced_kernel(SlicedParams p) 
             const uint64_t rel = warp_rel + lane;
             const bool valid = rel < item_units;
             const uint64_t unit = u0 + (valid ? rel : 0);
-            const uint32_t vmask = valid ? 0xFFFFFFFFu : 0u;
 
             // steps H2/H3: the thread-uniform index bits become all-0 / all-1 words
             if (C::FRAME_PER_UNIT) {
@@ -316,9 +439,10 @@ __global__ void __launch_bounds__(TPB, MINB) scan_sliced_kernel(SlicedParams p) 
                     if (pos >= C::LOW) T.E[e] = 0u - (uint32_t)((unit >> (pos - C::LOW)) & 1ull);
                 }
             }
+            T.store_leaves(s_leaf + threadIdx.x);              // private column: no barrier needed
 
             for (uint32_t s = 0; s < nslots; ++s) {
-                const uint8_t *uc = s_ucode + s * p.stride;
+                const uint16_t *uc = s_ucode + s * p.stride;
                 uint32_t cnt = 0, fcnt = 0;
 #pragma unroll 1
                 for (uint32_t pass = 0; pass < (1u << C::PASS_BITS); ++pass) {
@@ -327,9 +451,10 @@ __global__ void __launch_bounds__(TPB, MINB) scan_sliced_kernel(SlicedParams p) 
                     uint32_t r[M];
                     T.run(uc, r);                               // step H4
 #pragma unroll
-                    for (int m = 0; m < M; ++m) { r[m] &= vmask; cnt += __popc(r[m]); }   // step H5
+                    for (int m = 0; m < M; ++m) cnt += __popc(r[m]);              // step H5
                     if (!C::FRAME_PER_UNIT) fcnt += frames_in_group<C>(r);
                 }
+                if (!valid) { cnt = 0; fcnt = 0; }
                 // step H6, warp level
                 const uint32_t bal = __ballot_sync(0xFFFFFFFFu, cnt != 0u);
                 if (bal) {
@@ -364,18 +489,19 @@ int launch_sliced_inst(const ScanJob &job, const SlicedPlan &plan, void *stream,
     static int blocks_per_sm = 0, sm_count = 0;
     constexpr int SLICED_THREADS = TPB;
     auto kern = scan_sliced_kernel<C, TPB, MINB>;
-    const size_t per_slot = 16 + plan.stride;
-    const size_t max_smem = 96 * 1024;
+    const size_t per_slot = 16 + 2 * (size_t)plan.stride;
+    const size_t leaf_bytes = (size_t)C::LEAF_WORDS * TPB * sizeof(uint32_t);
+    const size_t slot_budget = 32 * 1024;
     if (!blocks_per_sm) {
         int dev = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return (int)e;
         e = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return (int)e;
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_smem);
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(leaf_bytes + slot_budget + 16));
         if (e != cudaSuccess) return (int)e;
         int b = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, kern, SLICED_THREADS, 32 * 1024);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, kern, SLICED_THREADS, leaf_bytes + slot_budget + 16);
         if (e != cudaSuccess) return (int)e;
         blocks_per_sm = b > 0 ? b : 1;
     }
@@ -392,7 +518,7 @@ int launch_sliced_inst(const ScanJob &job, const SlicedPlan &plan, void *stream,
 
     const uint32_t grid_full = (uint32_t)(sm_count * blocks_per_sm);
     const uint64_t tiles = (p.unit_count + SLICED_THREADS - 1) / SLICED_THREADS;
-    const uint32_t chunk_cap = (uint32_t)std::min<size_t>(2048, (32 * 1024) / per_slot);
+    const uint32_t chunk_cap = (uint32_t)std::max<size_t>(1, std::min<size_t>(2048, slot_budget / per_slot));
     // Work items: enough of them to balance the grid, each as large as that allows.
     uint32_t chunk;
     uint64_t tiles_per_item;
@@ -421,7 +547,7 @@ int launch_sliced_inst(const ScanJob &job, const SlicedPlan &plan, void *stream,
         q.n_ranges = (uint32_t)nr;
         const uint64_t items = nr * p.n_chunks;
         const uint32_t grid = (uint32_t)std::min<uint64_t>(items, grid_full);
-        const size_t smem = (size_t)chunk * per_slot + 16;
+        const size_t smem = leaf_bytes + (size_t)chunk * per_slot + 16;
         kern<<<grid, SLICED_THREADS, smem, (cudaStream_t)stream>>>(q);
         if (launches) ++*launches;
         cudaError_t e = cudaGetLastError();

@@ -86,34 +86,40 @@ def _run_ucode(uc, n, succ, vals):
     def dia(x):
         return sum(1 << w for w in range(n) if succ[w] & x)
 
-    for op in uc:
-        if op < 20:
-            atom, d = divmod(op, 4)
-            D[d] = vals[atom] if atom < 4 else 0
-        elif op < 24:
-            D[op - 20] = box(D[op - 20])
-        elif op < 28:
-            D[op - 24] = dia(D[op - 24])
-        elif op < 31:
-            d = op - 28
-            D[d] = D[d] & D[d + 1]
-        elif op < 34:
-            d = op - 31
-            D[d] = D[d] | D[d + 1]
-        elif op < 37:
-            d = op - 34
-            D[d] = D[d] & ~D[d + 1] & full
-        elif op < 40:
-            d = op - 37
-            D[d] = ~D[d] & D[d + 1] & full
-        elif op == 40:
+    leaves = {0: vals[0], 1: box(0), 2: box(vals[0]), 3: dia(vals[0])}   # p, box F, box p, dia p
+    fn = [lambda a, b: a & b, lambda a, b: a | b, lambda a, b: a & ~b & full, lambda a, b: ~a & b & full]
+    for op, arg in uc:
+        if op < 16:
+            i, d = divmod(op, 4)
+            D[d] = vals[i]
+        elif op < 80:
+            fi, d = divmod(op - 16, 4)
+            f, i = divmod(fi, 4)
+            D[d] = fn[f](D[d], vals[i])
+        elif op < 84:
+            D[op - 80] = leaves[arg]
+        elif op < 100:
+            f, d = divmod(op - 84, 4)
+            D[d] = fn[f](D[d], leaves[arg])
+        elif op < 116:
+            f, d = divmod(op - 100, 4)
+            D[d] = fn[f](D[d], D[d + 1])
+        elif op < 120:
+            D[op - 116] = box(D[op - 116])
+        elif op < 124:
+            D[op - 120] = dia(D[op - 120])
+        elif op == 124:
             return D[0] != full                      # refuted: truth set = D0
-        elif op == 41:
+        elif op == 125:
             return D[0] != 0                         # refuted: truth set = ~D0
-        elif op == 42:
+        elif op == 126:
             return (D[0] ^ D[1]) != 0
-        elif op == 43:
+        elif op == 127:
             return (~(D[0] ^ D[1]) & full) != 0
+        elif 128 <= op < 132:
+            D[op - 128] = 0
+        else:
+            raise AssertionError(f"bad micro-op {op}")
     raise AssertionError("no FIN op")
 
 
@@ -128,36 +134,57 @@ def _models(rng, n, k, count):
     return out
 
 
-def test_lowering_matches_oracle_truth(vol):
-    """Refuted-or-not of the lowered program == truth set != W from the oracle, on random models."""
-    rng = W.SplitMix64(2024)
+@pytest.mark.parametrize("mode", [0, 1, 3])
+def test_lowering_matches_oracle_truth(vol, mode):
+    """Refuted-or-not of the lowered program == truth set != W from the oracle, on random models,
+    for every leaf mode the kernel instantiations use."""
+    rng = W.SplitMix64(2024 + mode)
     sets = [(W.corpus_c1(300), 2), (W.corpus_c2(600)[300:], 2), (W.corpus_c4(300), 3)]
+    if mode != 3:
+        sets.append((W.pairs_c5(100)[0], 0))
     for progs, k in sets:
         for c in progs:
-            uc, need = kb.debug_lower(c, None, k)
-            assert 1 <= need <= 4 and uc[-1] in (40, 41)
+            uc, need = kb.debug_lower(c, None, k, mode)
+            assert 1 <= need <= 4 and uc[-1][0] in (124, 125)
+            if mode == 3:
+                assert all(op >= 4 and not (16 <= op < 80 and ((op - 16) // 4) % 4 == 0) for op, _ in uc), \
+                    "p_0 must be read through the leaf table in this mode"
             for n in (3, 5):
-                for f, v, succ, vals in _models(rng, n, k, 6):
+                for f, v, succ, vals in _models(rng, n, k, 5):
                     want = vol.truth(c, n, f, k, v) != [1] * n
                     assert _run_ucode(uc, n, succ, vals) == want, (W.to_text(W.from_postfix(c)), n, f, v)
 
 
-def test_pair_lowering_matches_oracle_truth(vol):
-    rng = W.SplitMix64(7)
+@pytest.mark.parametrize("mode", [0, 1, 3])
+def test_pair_lowering_matches_oracle_truth(vol, mode):
+    rng = W.SplitMix64(7 + mode)
     progs, pairs, _ = W.pairs_c5(200)
     extra = W.corpus_c2(60)
-    cases = [(progs[a], progs[b], 0) for a, b in pairs] + list(zip(extra[:30], extra[30:], [2] * 30))
+    cases = list(zip(extra[:30], extra[30:], [2] * 30))
+    if mode != 3:
+        cases += [(progs[a], progs[b], 0) for a, b in pairs]
     for a, b, k in cases:
         try:
-            uc, need = kb.debug_lower(a, b, k)
+            uc, need = kb.debug_lower(a, b, k, mode)
         except kb.KripkeError as e:
             assert e.status == kb.EUNSUPPORTED
             continue
-        assert uc[-1] in (42, 43)
+        assert uc[-1][0] in (126, 127) and need >= 2
         for n in (4, 6):
             for f, v, succ, vals in _models(rng, n, k, 5):
                 want = vol.truth(a, n, f, k, v) != vol.truth(b, n, f, k, v)
                 assert _run_ucode(uc, n, succ, vals) == want
+
+
+def test_lowering_uses_no_slot_for_atom_operands():
+    """<= 7-node formulas need at most 2 register-stack slots once atoms are operands; the derived
+    leaves make []p, <>p, []F, <>T free."""
+    needs = [kb.debug_lower(c, None, 2, 3)[1] for c in W.corpus_c2()]
+    assert max(needs) <= 2
+    uc, need = kb.debug_lower(W.to_postfix(W.parse("[]p->(<>T&~<>~p)")), None, 2, 3)
+    assert need == 1 and all(not (116 <= op < 124) for op, _ in uc)      # no box/dia micro-op left
+    uc, need = kb.debug_lower(W.to_postfix(W.parse("[](p->q)->(<>p-><>q)")), None, 2, 3)
+    assert need == 2
 
 
 def test_deep_program_does_not_fit_register_stack():
@@ -167,8 +194,8 @@ def test_deep_program_does_not_fit_register_stack():
         assert need <= 4
     except kb.KripkeError as e:
         assert e.status == kb.EUNSUPPORTED
-    # a perfectly balanced tree of 16 leaves needs 5 slots: must be refused by the lowering
-    t = [("var", i % 2) for i in range(16)]
+    # a perfectly balanced tree of 32 leaves needs 5 slots (atoms are operands): must be refused
+    t = [("var", i % 2) for i in range(32)]
     ops = ["and", "or"]
     lvl = 0
     while len(t) > 1:
