@@ -149,6 +149,25 @@ int kripke_distinguish_pairs(const kripke_programs_t *programs, const uint32_t *
                              uint32_t flags, kripke_count_t *counts_out,
                              kripke_witness_t *witness_out, void *stream);
 
+/* Size loop and records (step H8; Theorem 2(2)): runs kripke_eval_batch for n = 1..n_max
+ * on the full class and keeps, per formula, the least n with a refuting model ("minimal countermodel
+ * size", 0 = no countermodel through n_max worlds - never "valid"), the counts of that layer
+ * and its first countermodel.  All three outputs are DEVICE arrays of n_formulas entries; enqueued
+ * on `stream`. */
+int kripke_minimal_refutation(const kripke_programs_t *programs, uint32_t n_vars, uint32_t frame_class,
+                              uint32_t n_max, uint32_t *size_out, kripke_count_t *counts_out,
+                              kripke_witness_t *witness_out, void *stream);
+
+/* Separation size of formula pairs (Definition 2): for n = 1..n_max scans class K in ascending
+ * chunks of at most chunk_frames frames and records, per pair, the least n at which some frame
+ * distinguishes it (0 = k-indistinguishable through n_max) and the first distinguishing
+ * (frame, valuation, world) of that size.  A pair leaves the scan as soon as it is separated, so
+ * the later chunks only carry the survivors.  pairs, size_out, witness_out: HOST arrays
+ * (2*n_pairs, n_pairs, n_pairs).  Synchronous. */
+int kripke_pairs_separation(const kripke_programs_t *programs, const uint32_t *pairs, uint32_t n_pairs,
+                            uint32_t n_vars, uint32_t n_max, uint64_t chunk_frames,
+                            uint32_t *size_out, kripke_witness_t *witness_out, void *stream);
+
 /* End-to-end convenience with HOST buffers only: create + eval over the full class + copy the
  * results back + destroy, synchronously (this is what bench.py's "e2e" figure times). */
 int kripke_eval_batch_host(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,

@@ -30,6 +30,7 @@ EXPORTS = [
     "kripke_programs_destroy", "kripke_class_size", "kripke_eval_batch", "kripke_eval_batch_range",
     "kripke_distinguish_pairs", "kripke_eval_batch_host", "kripke_last_run_info",
     "kripke_calibrate_int32", "kripke_debug_lower", "kripke_witness_to_keys", "kripke_keys_to_witness",
+    "kripke_minimal_refutation", "kripke_pairs_separation",
 ]
 
 
@@ -73,6 +74,8 @@ def load():
     lib.kripke_last_run_info.argtypes = [vp, ctypes.POINTER(RunInfo)]
     lib.kripke_calibrate_int32.argtypes = [u32, ctypes.POINTER(ctypes.c_double),
                                            ctypes.POINTER(ctypes.c_double), vp]
+    lib.kripke_minimal_refutation.argtypes = [vp, u32, u32, u32, vp, vp, vp, vp]
+    lib.kripke_pairs_separation.argtypes = [vp, u32p, u32, u32, u32, u64, vp, vp, vp]
     lib.kripke_witness_to_keys.argtypes = [vp, u32, u32, u32, vp, vp]
     lib.kripke_keys_to_witness.argtypes = [vp, u32, u32, u32, vp, vp]
     lib.kripke_debug_lower.argtypes = [u8p, u32, u8p, u32, u32, u32, u8p, u32, ctypes.POINTER(u32)]
@@ -201,6 +204,34 @@ def distinguish_pairs(programs: Programs, pairs, n_worlds: int, n_vars: int, fra
                                            counts_out.data_ptr(), witness_out.data_ptr(),
                                            _stream(stream)), "kripke_distinguish_pairs")
     return counts_out, witness_out
+
+
+def minimal_refutation(programs: Programs, n_vars: int, frame_class: int, n_max: int,
+                       size_out=None, counts_out=None, witness_out=None, stream=None):
+    """kripke_minimal_refutation.  Returns (size int32 (B,), counts int64 (B,2), witness int64 (B,2))
+    CUDA tensors; size 0 = no countermodel through n_max worlds."""
+    import torch
+    n = programs.n_formulas
+    if size_out is None:
+        size_out = torch.empty((n,), dtype=torch.int32, device="cuda")
+    counts_out, witness_out = _outputs(n, counts_out, witness_out)
+    _check(load().kripke_minimal_refutation(programs._h, n_vars, frame_class, n_max, size_out.data_ptr(),
+                                            counts_out.data_ptr(), witness_out.data_ptr(), _stream(stream)),
+           "kripke_minimal_refutation")
+    return size_out, counts_out, witness_out
+
+
+def pairs_separation(programs: Programs, pairs, n_vars: int, n_max: int, chunk_frames: int = 1 << 30,
+                     stream=None):
+    """kripke_pairs_separation.  Returns (size uint32 (P,), witness uint64 (P,2)) numpy arrays."""
+    pairs = np.ascontiguousarray(pairs, dtype=np.uint32).reshape(-1)
+    n_pairs = len(pairs) // 2
+    size = np.zeros(n_pairs, np.uint32)
+    witness = np.zeros((n_pairs, 2), np.uint64)
+    _check(load().kripke_pairs_separation(programs._h, pairs.ctypes.data, n_pairs, n_vars, n_max,
+                                          chunk_frames, size.ctypes.data, witness.ctypes.data,
+                                          _stream(stream)), "kripke_pairs_separation")
+    return size, witness
 
 
 def eval_batch_host(code, offsets, n_worlds: int, n_vars: int, frame_class: int):

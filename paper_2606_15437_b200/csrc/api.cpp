@@ -194,6 +194,9 @@ struct kripke_programs {
     uint32_t pairs_cap = 0;
     Accum *d_accum = nullptr;
     uint32_t accum_cap = 0;
+    kripke_count_t *d_tmp_counts = nullptr;   // per-layer scratch of the size loop
+    kripke_witness_t *d_tmp_wit = nullptr;
+    uint32_t tmp_cap = 0;
     kripke_run_info_t last = {};
 };
 
@@ -345,6 +348,7 @@ int kripke_programs_destroy(kripke_programs_t *h) {
     for (auto &kv : h->single) kv.second.release();
     h->pair.release();
     cudaFree(h->d_code); cudaFree(h->d_offsets); cudaFree(h->d_pairs); cudaFree(h->d_accum);
+    cudaFree(h->d_tmp_counts); cudaFree(h->d_tmp_wit);
     delete h;
     return KRIPKE_OK;
 }
@@ -403,6 +407,88 @@ int kripke_distinguish_pairs(const kripke_programs_t *programs, const uint32_t *
     if (n_pairs) CU(cudaMemcpy(h->d_pairs, pairs, (size_t)2 * n_pairs * sizeof(uint32_t), cudaMemcpyHostToDevice));
     return run_scan(h, h->pair, h->d_pairs, n_pairs, n_worlds, n_vars, frame_class, frame_begin,
                     frame_count, flags, counts_out, witness_out, stream);
+}
+
+int kripke_minimal_refutation(const kripke_programs_t *programs, uint32_t n_vars, uint32_t frame_class,
+                              uint32_t n_max, uint32_t *size_out, kripke_count_t *counts_out,
+                              kripke_witness_t *witness_out, void *stream) {
+    if (!programs || n_max < 1 || n_max > KRIPKE_MAX_WORLDS) return KRIPKE_EINVAL;
+    kripke_programs *h = const_cast<kripke_programs *>(programs);
+    const uint32_t B = h->n_formulas;
+    if (B && (!size_out || !counts_out || !witness_out)) return KRIPKE_EINVAL;
+    if (B > h->tmp_cap) {
+        cudaFree(h->d_tmp_counts); cudaFree(h->d_tmp_wit);
+        h->d_tmp_counts = nullptr; h->d_tmp_wit = nullptr; h->tmp_cap = 0;
+        CU(cudaMalloc((void **)&h->d_tmp_counts, (size_t)B * sizeof(kripke_count_t)));
+        CU(cudaMalloc((void **)&h->d_tmp_wit, (size_t)B * sizeof(kripke_witness_t)));
+        h->tmp_cap = B;
+    }
+    for (uint32_t n = 1; n <= n_max; ++n) {
+        int rc = kripke_eval_batch(h, n, n_vars, frame_class, h->d_tmp_counts, h->d_tmp_wit, stream);
+        if (rc) return rc;
+        int e = launch_record_size(n, B, h->d_tmp_counts, h->d_tmp_wit, size_out, counts_out, witness_out, stream);
+        if (e) return cuda_fail(e);
+    }
+    return KRIPKE_OK;
+}
+
+int kripke_pairs_separation(const kripke_programs_t *programs, const uint32_t *pairs, uint32_t n_pairs,
+                            uint32_t n_vars, uint32_t n_max, uint64_t chunk_frames,
+                            uint32_t *size_out, kripke_witness_t *witness_out, void *stream) {
+    if (!programs || n_max < 1 || n_max > KRIPKE_MAX_WORLDS || chunk_frames == 0) return KRIPKE_EINVAL;
+    if (n_pairs && (!pairs || !size_out || !witness_out)) return KRIPKE_EINVAL;
+    kripke_programs *h = const_cast<kripke_programs *>(programs);
+    std::vector<uint32_t> active(n_pairs);          // indices of the pairs not separated yet
+    for (uint32_t j = 0; j < n_pairs; ++j) {
+        active[j] = j;
+        size_out[j] = 0;
+        witness_out[j].frame = KRIPKE_NO_WITNESS; witness_out[j].valuation = 0; witness_out[j].world = 0;
+    }
+    kripke_count_t *d_counts = nullptr;
+    kripke_witness_t *d_wit = nullptr;
+    if (n_pairs) {
+        CU(cudaMalloc((void **)&d_counts, (size_t)n_pairs * sizeof(kripke_count_t)));
+        cudaError_t e = cudaMalloc((void **)&d_wit, (size_t)n_pairs * sizeof(kripke_witness_t));
+        if (e != cudaSuccess) { cudaFree(d_counts); return cuda_fail((int)e); }
+    }
+    std::vector<kripke_count_t> hc(n_pairs);
+    std::vector<kripke_witness_t> hw(n_pairs);
+    std::vector<uint32_t> sub;
+    int rc = KRIPKE_OK;
+    for (uint32_t n = 1; n <= n_max && rc == KRIPKE_OK && !active.empty(); ++n) {
+        const uint64_t total = 1ull << (n * n);
+        for (uint64_t begin = 0; begin < total && rc == KRIPKE_OK && !active.empty(); begin += chunk_frames) {
+            const uint64_t count = std::min<uint64_t>(chunk_frames, total - begin);
+            sub.resize(2 * active.size());
+            for (size_t a = 0; a < active.size(); ++a) {
+                sub[2 * a] = pairs[2 * active[a]];
+                sub[2 * a + 1] = pairs[2 * active[a] + 1];
+            }
+            rc = kripke_distinguish_pairs(h, sub.data(), (uint32_t)active.size(), n, n_vars, KRIPKE_CLASS_K, begin,
+                                          count, 0, d_counts, d_wit, stream);
+            if (rc) break;
+            cudaError_t e = cudaMemcpyAsync(hc.data(), d_counts, active.size() * sizeof(kripke_count_t),
+                                            cudaMemcpyDeviceToHost, (cudaStream_t)stream);
+            if (e == cudaSuccess)
+                e = cudaMemcpyAsync(hw.data(), d_wit, active.size() * sizeof(kripke_witness_t),
+                                    cudaMemcpyDeviceToHost, (cudaStream_t)stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+            if (e != cudaSuccess) { rc = cuda_fail((int)e); break; }
+            std::vector<uint32_t> still;
+            for (size_t a = 0; a < active.size(); ++a) {
+                if (hc[a].refuting_models != 0) {
+                    size_out[active[a]] = n;
+                    witness_out[active[a]] = hw[a];
+                } else {
+                    still.push_back(active[a]);
+                }
+            }
+            active.swap(still);
+        }
+    }
+    cudaFree(d_counts);
+    cudaFree(d_wit);
+    return rc;
 }
 
 int kripke_eval_batch_host(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,

@@ -72,6 +72,9 @@ int launch_scalar(const ScanJob &job, const uint32_t *records, uint32_t n_list, 
 int launch_init(Accum *accum, uint32_t n_records, void *stream);
 int launch_finish(const ScanJob &job, bool accumulate, kripke_count_t *counts_out,
                   kripke_witness_t *witness_out, void *stream);
+// Size record of step H8.
+int launch_record_size(uint32_t n, uint32_t n_records, const kripke_count_t *cnt, const kripke_witness_t *wit,
+                       uint32_t *size_out, kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream);
 // Witness records <-> 64-bit keys (multi-GPU exchange step).
 int launch_witness_keys(bool to_keys, const void *src, uint32_t n_records, uint32_t kn, void *dst, void *stream);
 // Calibration kernels.

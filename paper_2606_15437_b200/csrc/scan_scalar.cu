@@ -221,7 +221,32 @@ __global__ void keys_to_witness_kernel(const unsigned long long *keys, uint32_t 
     wit[i] = w;
 }
 
+// step H8: keep the first size at which a formula is refuted
+__global__ void record_size_kernel(uint32_t n, uint32_t n_records, const kripke_count_t *cnt, const kripke_witness_t *wit,
+                                   uint32_t *size_out, kripke_count_t *counts_out, kripke_witness_t *witness_out) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_records) return;
+    if (n == 1) {
+        size_out[i] = 0;
+        counts_out[i].refuting_models = 0; counts_out[i].refuting_frames = 0;
+        witness_out[i].frame = KRIPKE_NO_WITNESS; witness_out[i].valuation = 0; witness_out[i].world = 0;
+    }
+    if (size_out[i] == 0 && cnt[i].refuting_models != 0) {
+        size_out[i] = n;
+        counts_out[i] = cnt[i];
+        witness_out[i] = wit[i];
+    }
+}
+
 }  // namespace
+
+int launch_record_size(uint32_t n, uint32_t n_records, const kripke_count_t *cnt, const kripke_witness_t *wit,
+                       uint32_t *size_out, kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream) {
+    if (n_records == 0) return 0;
+    record_size_kernel<<<(n_records + 255) / 256, 256, 0, (cudaStream_t)stream>>>(n, n_records, cnt, wit, size_out,
+                                                                                  counts_out, witness_out);
+    return (int)cudaGetLastError();
+}
 
 int launch_witness_keys(bool to_keys, const void *src, uint32_t n_records, uint32_t kn, void *dst, void *stream) {
     if (n_records == 0) return 0;

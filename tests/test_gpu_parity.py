@@ -349,3 +349,86 @@ def test_pairs_with_variables(kb, vol):
 def test_calibration_runs(kb):
     rate, ms = kb.calibrate_int32(0)
     assert rate > 1e12 and ms > 0
+
+
+# ---------------------------------------------------------------------------------------------
+def test_h8_minimal_refutation_size_records(kb, vol):
+    """Step H8 (Theorem 2(2)): least n with a countermodel, its counts and certificate, per class."""
+    g = gold("c2_n4.npz")
+    progs = W.corpus_c2()[:600]
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 2)
+    for cname, cls in CLS.items():
+        layers = [vol.census(code, offs, n, 2, cls) for n in (1, 2, 3)]
+        layers.append({key: g[f"{cname}_{key}"][:600] for key in KEYS})
+        size, c, w = kb.minimal_refutation(h, 2, cls, 4)
+        got = kb.unpack(c, w)
+        size = size.cpu().numpy()
+        for b in range(len(progs)):
+            first = next((n for n in (1, 2, 3, 4) if int(layers[n - 1]["models"][b]) > 0), 0)
+            assert int(size[b]) == first, (cname, b)
+            if first:
+                for key in KEYS:
+                    assert int(got[key][b]) == int(layers[first - 1][key][b]), (cname, b, key)
+                if b % 29 == 0:
+                    assert O.check_witness(progs[b], first, 2, cls, int(got["wit_f"][b]), int(got["wit_v"][b]),
+                                           int(got["wit_w"][b]))
+            else:
+                assert int(got["wit_f"][b]) == O.NO_WITNESS
+
+
+def test_h8_paper_frontier_on_gpu(kb, vol):
+    """P:143-147 end to end on the GPU: the 44,678 enumerated formulas reduce to 5,621 semantic
+    classes (oracle signatures); the K frontier of the representatives is 5,084 at one world, 536 at
+    two and exactly one formula (p -> p) unrefuted through five worlds."""
+    forms = W.enumerate_constant_free(7, 2)
+    progs = [W.to_postfix(t) for t in forms]
+    a, b = vol.signatures(*W.pack_programs(progs), 3, 2)
+    first = {}
+    for i, s in enumerate(zip(a.tolist(), b.tolist())):
+        first.setdefault(s, i)
+    reps = [progs[i] for i in sorted(first.values())]
+    assert len(reps) == 5621
+    h = kb.Programs(*W.pack_programs(reps), 2)
+    size, c, w = kb.minimal_refutation(h, 2, K, 5)
+    size = size.cpu().numpy()
+    assert [int((size == n).sum()) for n in (1, 2, 3, 4, 5, 0)] == [5084, 536, 0, 0, 0, 1]
+    assert W.to_text(W.from_postfix(reps[int(np.nonzero(size == 0)[0][0])])) == "(p->p)"
+    # bounded survivors in the stronger classes are supersets (class monotonicity, P:157)
+    surv = {}
+    for cname, cls in CLS.items():
+        s, _, _ = kb.minimal_refutation(h, 2, cls, 5)
+        surv[cname] = set(np.nonzero(s.cpu().numpy() == 0)[0].tolist())
+    assert surv["K"] <= surv["T"] <= surv["S4"] <= surv["S5"]
+    assert len(surv["K"]) == 1
+
+
+def test_c5_pairs_separation_sizes(kb, vol):
+    """Config 5 driver: separation size of every pair through five worlds against the stored oracle
+    counts, and the paper's late separations at six worlds."""
+    g = gold("c5_counts.npz")
+    progs, pairs, names = W.pairs_c5()
+    pairs = np.array(pairs, np.uint32)
+    h = kb.Programs(*W.pack_programs(progs), 0)
+    size, wit = kb.pairs_separation(h, pairs, 0, 5, 1 << 22)
+    frames = np.stack([g[f"n{n}_frames"] for n in (1, 2, 3, 4, 5)])
+    want = np.array([next((n + 1 for n in range(5) if frames[n][j] > 0), 0) for j in range(len(pairs))])
+    assert (size == want).all()
+    for n in (1, 2, 3, 4):
+        sel = np.nonzero(size == n)[0]
+        assert (wit[sel, 0] == g[f"n{n}_wit_f"][sel]).all()
+        assert ((wit[sel, 1] >> np.uint64(32)) == g[f"n{n}_wit_w"][sel]).all()
+    # the pairs that agree through five worlds go on to six (full 2^36 scan for the ones that never split)
+    late = np.nonzero(size == 0)[0]
+    named_late = [j for j in late if names[j]]
+    assert "alpha_2/alpha_3" in [names[j] for j in named_late]
+    size6, wit6 = kb.pairs_separation(h, pairs[named_late], 0, 6, 1 << 30)
+    by_name = {names[j]: (int(size6[i]), int(wit6[i, 0]), int(wit6[i, 1] >> np.uint64(32))) for i, j in enumerate(named_late)}
+    for name in ("alpha_2/alpha_3", "<>^5T/<>^6T", "[]^5F/[]^6F", "(<>[])^2F/(<>[])^3F"):
+        assert by_name[name][0] == 6 and by_name[name][1] == 17335328, (name, by_name[name])
+    for i, j in enumerate(named_late):
+        if size6[i]:
+            a, b = progs[pairs[j][0]], progs[pairs[j][1]]
+            assert O.check_pair_witness(a, b, 6, 0, K, int(wit6[i, 0]), 0, int(wit6[i, 1] >> np.uint64(32))), names[j]
+    # Lemma 2: alpha_3 / alpha_4 need eight worlds, so they survive the complete six-world scan
+    assert by_name["([]<>)^3T/([]<>)^4T"][0] == 0
