@@ -159,7 +159,8 @@ def run_ours(args):
     keys = {c: torch.zeros((B,), dtype=torch.int64, device="cuda") for c, _ in CLASSES}
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
     launches = [0]
-    k_ops_per_word = [0]
+    k_info = {}
+    executed = [0]
 
     def step(ev_k=None):
         for cname, cls in CLASSES:
@@ -171,8 +172,10 @@ def run_ours(args):
                 ev_k[1].record()
             info = h.last_run_info()
             launches[0] += info.launches
+            executed[0] += info.executed_models
             if cname == "K":
-                k_ops_per_word[0] = info.sliced_logic_ops_per_word
+                k_info["instr_per_frame"] = info.logic_instr_per_frame
+                k_info["frames"] = count
         if world > 1:                                                   # the one exchange step
             for cname, _ in CLASSES:
                 kb.witness_to_keys(wits[cname], N_WORLDS, N_VARS, keys[cname])
@@ -197,6 +200,7 @@ def run_ours(args):
     sampler = ClockSampler(local_rank)
     sampler.start()
     launches[0] = 0
+    executed[0] = 0
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     evk = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
@@ -238,8 +242,7 @@ def run_ours(args):
                "h2d_bytes_per_step": int(4 * (code.nbytes + offs.nbytes)), "d2h_bytes_per_step": int(4 * 32 * B)}
 
     if rank == 0:
-        words = (sizes["K"] // world) * nval // 32
-        k_instr = k_ops_per_word[0] * words                       # executed 3-input logic thread-instructions
+        k_instr = k_info["instr_per_frame"] * k_info["frames"]    # executed 3-input logic thread-instructions
         achieved = k_instr / (k_ms * 1e-3) / 1e12
         peak = SM_COUNT * INT_LANES_PER_SM * 1.965e9 / 1e12        # derived ALU-pipe peak at max clock
         cpu_rate, cpu_dt, cores, cpu_evals = oracle_sample(progs, args.ref_frames)
@@ -253,7 +256,11 @@ def run_ours(args):
                              "K/T/S4/S5 frames of 5 worlds x 1,024 valuations") if args.workload == "c3"
                             else "c3_small: C3 with K cut to 2^20 and T to 2^16 frames (debug only)",
                 "formulas": B, "n_worlds": N_WORLDS, "n_vars": N_VARS, "classes": [c for c, _ in CLASSES],
-                "evaluations_per_step": evals_per_step, "parallelism": f"frame-range shard x{world}",
+                "evaluations_per_step": evals_per_step,
+                "executed_evaluations_per_step": executed[0] // args.steps,
+                "valuation_sweep": "per-formula variable support (PAPER.md:93 k_b), counts scaled; "
+                                   "KRIPKE_FULL_SWEEP evaluates every valuation",
+                "parallelism": f"frame-range shard x{world}",
                 "l2": "flushed between iterations (256 MiB fill); the kernels read < 100 KB of input",
             },
             "clocks": clocks,
@@ -266,8 +273,8 @@ def run_ours(args):
                 "peak_source": "derived: 148 SMs x 4 x 16 ALU lanes/clk x 1.965 GHz (DESIGN.md)",
                 "peak_measured_calibration": {k: v / 1e12 for k, v in cal.items()},
                 "frac_of_measured_lop3": achieved / (cal["lop3"] / 1e12),
-                "algorithmic_ops": "executed 3-input logic instr of the lowered programs: "
-                                   "sum_b (modal*n^2 + bool*n + n+1) per 32-model word",
+                "algorithmic_ops": "executed 3-input logic instr of the lowered programs: sum_b (modal*n^2 + "
+                                   "bool*n + n+1) x 2^(k_b*n)/32 per frame (k_b = variables formula b mentions)",
             },
             "cpu_baseline": {"value": cpu_rate, "unit": "evaluations/s", "cores": cores, "kind": "oracle",
                              "sample": f"first {args.ref_frames} K-frames of n=5 x 1024 valuations x {B} formulas "
@@ -278,18 +285,101 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_c4(args):
+    """--workload c4: BASELINE.json configs[3] ablations: formula batch size (fusion)
+    on the bit-sliced kernel, fused vs separate launches, and per-block / per-warp / per-thread atomics
+    on the scalar (Algorithm 1) kernel under mixed and adversarial contention.  n=5, 3 variables."""
+    import torch
+    from paper_2606_15437_b200 import binding as kb
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    kb.load()
+    n, k = 5, 3
+    progs = W.corpus_c4()
+    nval = 1 << (k * n)
+    reps = max(1, args.steps)
+
+    def timed(fn):
+        for _ in range(max(1, args.warmup > 0)):
+            fn()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b) * 1e-3)
+        return float(np.median(ts))
+
+    out = {"batch": {}, "fusion": {}, "contention": {}}
+    clock = ClockSampler(0)
+    clock.start()
+    # A. batch size (fusion) on the bit-sliced kernel
+    for B, begin, count in ((1, 0, 1 << 25), (32, 0, 1 << 25), (256, 1 << 24, 1 << 20), (2048, 1 << 24, 1 << 20)):
+        h = kb.Programs(*W.pack_programs(progs[:B]), k)
+        c = torch.zeros((B, 2), dtype=torch.int64, device="cuda")
+        w = torch.zeros((B, 2), dtype=torch.int64, device="cuda")
+        t = timed(lambda: kb.eval_batch_range(h, n, k, 0, begin, count, 0, c, w))
+        info = h.last_run_info()
+        ev = B * count * nval
+        out["batch"][str(B)] = {"frames": count, "seconds": t, "evaluations_per_s": ev / t,
+                                "logic_instr_per_s": info.sliced_logic_ops_per_word * (count * nval // 32) / t}
+        h.destroy()
+    # B. one fused launch of 32 formulas vs 32 separate launches (2^20-frame range)
+    begin, count = 1 << 24, 1 << 20
+    hs = [kb.Programs(*W.pack_programs([p]), k) for p in progs[:32]]
+    c1 = torch.zeros((1, 2), dtype=torch.int64, device="cuda")
+    w1 = torch.zeros((1, 2), dtype=torch.int64, device="cuda")
+    t_sep = timed(lambda: [kb.eval_batch_range(hh, n, k, 0, begin, count, 0, c1, w1) for hh in hs])
+    h32 = kb.Programs(*W.pack_programs(progs[:32]), k)
+    c = torch.zeros((32, 2), dtype=torch.int64, device="cuda")
+    w = torch.zeros((32, 2), dtype=torch.int64, device="cuda")
+    t_fused = timed(lambda: kb.eval_batch_range(h32, n, k, 0, begin, count, 0, c, w))
+    out["fusion"] = {"formulas": 32, "frames": count, "separate_s": t_sep, "fused_s": t_fused,
+                     "fused_speedup": t_sep / t_fused}
+    # C. atomic contention on the scalar kernel (the paper's layout), 2^12-frame range
+    begin, count = 1 << 24, 1 << 12
+    mixed = progs[:64]
+    adversarial = [W.to_postfix(("and", ("bot",), W.from_postfix(p))) for p in progs[:64]]   # every model refutes
+    for name, batch in (("mixed", mixed), ("adversarial", adversarial)):
+        h = kb.Programs(*W.pack_programs(batch), k)
+        c = torch.zeros((64, 2), dtype=torch.int64, device="cuda")
+        w = torch.zeros((64, 2), dtype=torch.int64, device="cuda")
+        res = {}
+        for mname, mode in (("block", kb.REDUCE_BLOCK), ("warp", kb.REDUCE_WARP), ("thread", kb.REDUCE_THREAD)):
+            t = timed(lambda: kb.eval_batch_range(h, n, k, 0, begin, count, kb.KERNEL_SCALAR | mode, c, w))
+            res[mname] = {"seconds": t, "evaluations_per_s": 64 * count * nval / t}
+        res["block_vs_thread"] = res["thread"]["seconds"] / res["block"]["seconds"]
+        t = timed(lambda: kb.eval_batch_range(h, n, k, 0, begin, count, 0, c, w))
+        res["sliced"] = {"seconds": t, "evaluations_per_s": 64 * count * nval / t}
+        out["contention"][name] = res
+        h.destroy()
+    clocks = clock.result()
+    b2048 = out["batch"]["2048"]
+    print(json.dumps({
+        "metric": "formula-model evaluations/sec at n=5", "value": b2048["evaluations_per_s"],
+        "unit": "evaluations/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": b2048["seconds"] * 1e3, "higher_is_better": True, "scaling": "strong",
+        "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": "C4 ablation (BASELINE.json configs[3]): n=5, 3 variables, 2,048 seeded formulas of "
+                               "9-15 nodes; value = batch 2,048 on K-frames [2^24, 2^24+2^20) (the paper's stress shape)"},
+        "clocks": clocks, "ablation": out,
+    }))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c3", "c3_small"])
+    ap.add_argument("--workload", default="c3", choices=["c3", "c3_small", "c4"])
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--ref-frames", type=int, default=256)
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.workload == "c4":
+        run_c4(args)
     else:
         run_ours(args)
 

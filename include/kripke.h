@@ -70,6 +70,11 @@ enum { KRIPKE_CLASS_K = 0, KRIPKE_CLASS_T = 1, KRIPKE_CLASS_S4 = 2, KRIPKE_CLASS
 enum {
     KRIPKE_ACCUMULATE = 1u << 0,      /* add to counts_out / keep the smaller witness instead of
                                          overwriting (chunked scans, multi-GPU shards)            */
+    KRIPKE_FULL_SWEEP = 1u << 1,      /* evaluate every program on all 2^(n_vars*n) valuations even if it
+                                         ignores a variable (default: a program is scanned over the
+                                         valuations of the variables it mentions - the paper's
+                                         per-formula k_b, P:93 - and its model count scaled; results
+                                         are identical either way)                                 */
     KRIPKE_KERNEL_AUTO = 0u << 4,     /* bit-sliced kernel where it applies, else the scalar one  */
     KRIPKE_KERNEL_SCALAR = 1u << 4,   /* force the scalar kernel (Algorithm 1 restated, one model
                                          per thread iteration): baseline / ablation / cross-check */
@@ -175,14 +180,18 @@ int kripke_eval_batch_host(const uint8_t *code, const uint32_t *offsets, uint32_
                            kripke_count_t *counts_host, kripke_witness_t *witness_host);
 
 /* What the last eval / pairs call on this handle executed (host-side bookkeeping, valid right
- * after the call returns): kernel launches enqueued, which kernel family ran the bulk (0 scalar,
- * 1 bit-sliced), and the 3-input logic instructions per 32 models the lowered programs need
- * summed over the batch (the "algorithmic ops" of DESIGN.md's roofline). */
+ * after the call returns). */
 typedef struct {
-    uint32_t launches;
-    uint32_t kernel_family;
-    uint64_t sliced_logic_ops_per_word;   /* sum over programs, per 32-model word            */
-    uint64_t models_per_program;          /* (frames in range) * 2^(n_vars*n)                */
+    uint32_t launches;                    /* kernel launches enqueued                                  */
+    uint32_t kernel_family;               /* which family ran the bulk: 0 scalar, 1 bit-sliced         */
+    uint64_t sliced_logic_ops_per_word;   /* 3-input logic instructions per 32-model word the lowered
+                                             programs need, summed over the batch                      */
+    uint64_t models_per_program;          /* definitional: (frames in range) * 2^(n_vars*n)            */
+    uint64_t executed_models;             /* models actually evaluated, summed over programs (a program
+                                             that mentions g variables is scanned on 2^(g*n) valuations) */
+    double logic_instr_per_frame;         /* 3-input logic thread-instructions the sliced kernel executes
+                                             per frame of the range, summed over programs: the
+                                             "algorithmic ops" of DESIGN.md's roofline                 */
 } kripke_run_info_t;
 int kripke_last_run_info(const kripke_programs_t *programs, kripke_run_info_t *info_out);
 

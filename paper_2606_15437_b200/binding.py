@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libkripke_b200.so")
 OK, EINVAL, EPROGRAM, EUNSUPPORTED, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 CLASS_K, CLASS_T, CLASS_S4, CLASS_S5 = 0, 1, 2, 3
 ACCUMULATE = 1 << 0
+FULL_SWEEP = 1 << 1
 KERNEL_AUTO, KERNEL_SCALAR, KERNEL_SLICED = 0 << 4, 1 << 4, 2 << 4
 REDUCE_BLOCK, REDUCE_WARP, REDUCE_THREAD = 0 << 8, 1 << 8, 2 << 8
 NO_WITNESS = (1 << 64) - 1
@@ -44,7 +45,8 @@ class KripkeError(RuntimeError):
 
 class RunInfo(ctypes.Structure):
     _fields_ = [("launches", ctypes.c_uint32), ("kernel_family", ctypes.c_uint32),
-                ("sliced_logic_ops_per_word", ctypes.c_uint64), ("models_per_program", ctypes.c_uint64)]
+                ("sliced_logic_ops_per_word", ctypes.c_uint64), ("models_per_program", ctypes.c_uint64),
+                ("executed_models", ctypes.c_uint64), ("logic_instr_per_frame", ctypes.c_double)]
 
 
 _lib = None

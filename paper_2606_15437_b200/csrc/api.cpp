@@ -37,13 +37,15 @@ int upload(T **dst, const std::vector<T> &src) {
     return KRIPKE_OK;
 }
 
-// A lowered set of records for the sliced kernel plus the list of records it cannot run.
+// A lowered set of records for the sliced kernel plus the list of records it cannot run.  Slots are
+// sorted by the number of register-stack slots they need, so that each need class can run on the
+// kernel instantiation with the fewest slots (more words per thread, more resident warps).
 struct HostPlan {
     std::vector<uint16_t> ucode;
     std::vector<uint32_t> slot_record;
     std::vector<uint32_t> unfit;
     uint32_t stride = 2;
-    uint32_t max_need = 0;
+    uint32_t need_end[UC_DMAX + 1] = {0, 0, 0, 0, 0};   // slots with need <= d are [0, need_end[d])
     uint64_t n_modal = 0, n_bool = 0;
 };
 
@@ -52,15 +54,19 @@ void build_plan(const std::vector<Lowered> &low, const std::vector<bool> &fits, 
     for (size_t i = 0; i < low.size(); ++i)
         if (fits[i]) longest = std::max(longest, low[i].ucode.size());
     hp->stride = (uint32_t)((longest + 1 + 1) / 2 * 2);        // one spare entry after FIN (prefetch)
-    for (size_t i = 0; i < low.size(); ++i) {
-        if (!fits[i]) { hp->unfit.push_back((uint32_t)i); continue; }
-        hp->slot_record.push_back((uint32_t)i);
-        size_t at = hp->ucode.size();
-        hp->ucode.resize(at + hp->stride, (uint16_t)UC_FIN_ALL);
-        std::memcpy(&hp->ucode[at], low[i].ucode.data(), low[i].ucode.size() * sizeof(uint16_t));
-        hp->max_need = std::max(hp->max_need, (uint32_t)low[i].need);
-        hp->n_modal += low[i].n_modal;
-        hp->n_bool += low[i].n_bool;
+    for (size_t i = 0; i < low.size(); ++i)
+        if (!fits[i]) hp->unfit.push_back((uint32_t)i);
+    for (int need = 1; need <= UC_DMAX; ++need) {
+        for (size_t i = 0; i < low.size(); ++i) {
+            if (!fits[i] || low[i].need != need) continue;
+            hp->slot_record.push_back((uint32_t)i);
+            size_t at = hp->ucode.size();
+            hp->ucode.resize(at + hp->stride, (uint16_t)UC_FIN_ALL);
+            std::memcpy(&hp->ucode[at], low[i].ucode.data(), low[i].ucode.size() * sizeof(uint16_t));
+            hp->n_modal += low[i].n_modal;
+            hp->n_bool += low[i].n_bool;
+        }
+        hp->need_end[need] = (uint32_t)hp->slot_record.size();
     }
 }
 
@@ -68,7 +74,8 @@ struct DevicePlan {
     uint16_t *ucode = nullptr;
     uint32_t *slot_record = nullptr;
     uint32_t *unfit = nullptr;
-    uint32_t n_slots = 0, n_unfit = 0, stride = 2, max_need = 0;
+    uint32_t n_slots = 0, n_unfit = 0, stride = 2;
+    uint32_t need_end[UC_DMAX + 1] = {0, 0, 0, 0, 0};
     uint64_t n_modal = 0, n_bool = 0;
     void release() {
         cudaFree(ucode); cudaFree(slot_record); cudaFree(unfit);
@@ -85,11 +92,27 @@ int upload_plan(const HostPlan &hp, DevicePlan *dp) {
     dp->n_slots = (uint32_t)hp.slot_record.size();
     dp->n_unfit = (uint32_t)hp.unfit.size();
     dp->stride = hp.stride;
-    dp->max_need = hp.max_need;
+    std::memcpy(dp->need_end, hp.need_end, sizeof(dp->need_end));
     dp->n_modal = hp.n_modal;
     dp->n_bool = hp.n_bool;
     return KRIPKE_OK;
 }
+
+// The records of one scan grouped by the number of variables their programs mention (after
+// constant folding).  A program that ignores a variable has the same truth set for every value of
+// it, so group g is scanned over the 2^(g*n) valuations of its own variables only - Algorithm 1's
+// per-formula k_b - and its model count is multiplied by 2^((k-g)*n) (reading R8).
+struct GroupPlan {
+    uint32_t k_eff = 0;
+    DevicePlan dp;
+};
+struct ScanPlan {
+    std::vector<GroupPlan> groups;
+    void release() {
+        for (auto &g : groups) g.dp.release();
+        groups.clear();
+    }
+};
 
 // ---- class tables (step H2) ----------------------------------------------------------------------
 // Ascending K-indices of the preorders (S4) / equivalences (S5) on n worlds.  Rows are chosen from
@@ -188,8 +211,8 @@ struct kripke_programs {
     std::vector<uint32_t> h_offsets;
     uint8_t *d_code = nullptr;
     uint32_t *d_offsets = nullptr;
-    std::map<uint32_t, DevicePlan> single;   // one record per formula, per lowering mode (built on first use)
-    DevicePlan pair;                   // rebuilt by each kripke_distinguish_pairs call
+    std::map<uint64_t, ScanPlan> single;     // one record per formula; cached per (n, usable reduced shapes)
+    ScanPlan pair;                     // rebuilt by each kripke_distinguish_pairs call
     uint32_t *d_pairs = nullptr;
     uint32_t pairs_cap = 0;
     Accum *d_accum = nullptr;
@@ -211,33 +234,29 @@ int ensure_accum(kripke_programs *h, uint32_t n) {
     return KRIPKE_OK;
 }
 
-// The batch lowered for one set of derived leaves (cached in the handle; synchronous upload).
-int single_plan(kripke_programs *h, uint32_t mode, const DevicePlan **out) {
-    auto it = h->single.find(mode);
-    if (it == h->single.end()) {
-        std::vector<Lowered> low(h->n_formulas);
-        std::vector<bool> fits(h->n_formulas);
-        for (uint32_t b = 0; b < h->n_formulas; ++b)
-            fits[b] = lower_single(&h->h_code[h->h_offsets[b]], h->h_offsets[b + 1] - h->h_offsets[b], mode, &low[b]);
-        HostPlan hp;
-        build_plan(low, fits, &hp);
-        DevicePlan dp;
-        int rc = upload_plan(hp, &dp);
-        if (rc) { dp.release(); return rc; }
-        it = h->single.emplace(mode, dp).first;
-    }
-    *out = &it->second;
-    return KRIPKE_OK;
+// Which reduced shapes (n, g), g < k, the sliced kernel can run for this class: bit g.
+uint32_t reduced_shapes(uint32_t n, uint32_t k, uint32_t cls, uint32_t flags) {
+    uint32_t mask = 0;
+    if ((flags & KRIPKE_FULL_SWEEP) || (flags & KRIPKE_KERNEL_MASK) == KRIPKE_KERNEL_SCALAR) return 0;
+    if (n < 1 || n > KRIPKE_MAX_WORLDS || k > KRIPKE_MAX_VARS) return 0;
+    if (!sliced_select(n, k, cls, 1, nullptr)) return 0;
+    for (uint32_t g = 0; g < k; ++g)
+        if (sliced_select(n, g, cls, 1, nullptr)) mask |= 1u << g;
+    return mask;
 }
 
-// The common scan: zero accumulators, run the sliced kernel on the aligned part of the range for
-// the records it can take and the scalar kernel on the rest, then finish.
-int run_scan(kripke_programs *h, const DevicePlan &plan, const uint32_t *d_pairs, uint32_t n_records,
+// Lowers the records (formulas, or pairs if `pairs` != null) into one GroupPlan per variable count.
+int build_scan_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
+                    uint32_t shapes, ScanPlan *out);
+
+// The common scan: zero accumulators, run every group on the sliced kernel where an instantiation
+// exists (aligned part of the range) and on the scalar kernel elsewhere, then finish.
+int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *d_pairs, uint32_t n_records,
              uint32_t n, uint32_t k, uint32_t cls, uint64_t begin, uint64_t count, uint32_t flags,
              kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream) {
     if (n < 1 || n > KRIPKE_MAX_WORLDS || k != h->n_vars || cls > KRIPKE_CLASS_S5) return KRIPKE_EINVAL;
     if (n * n + k * n > KRIPKE_MAX_MODEL_BITS) return KRIPKE_EUNSUPPORTED;
-    if (flags & ~(KRIPKE_ACCUMULATE | KRIPKE_KERNEL_MASK | KRIPKE_REDUCE_MASK)) return KRIPKE_EINVAL;
+    if (flags & ~(KRIPKE_ACCUMULATE | KRIPKE_FULL_SWEEP | KRIPKE_KERNEL_MASK | KRIPKE_REDUCE_MASK)) return KRIPKE_EINVAL;
     const uint32_t family = flags & KRIPKE_KERNEL_MASK, reduce = (flags & KRIPKE_REDUCE_MASK) >> 8;
     if (family == KRIPKE_KERNEL_MASK || reduce > 2) return KRIPKE_EINVAL;
     if (n_records && (!counts_out || !witness_out)) return KRIPKE_EINVAL;
@@ -247,8 +266,14 @@ int run_scan(kripke_programs *h, const DevicePlan &plan, const uint32_t *d_pairs
     if (begin > csize || count > csize - begin) return KRIPKE_EINVAL;
     h->last = kripke_run_info_t{};
     h->last.models_per_program = count << (k * n);
-    h->last.sliced_logic_ops_per_word =
-        plan.n_modal * n * n + plan.n_bool * n + (uint64_t)plan.n_slots * (n + 1);
+    for (const GroupPlan &g : plan.groups) {
+        h->last.sliced_logic_ops_per_word += g.dp.n_modal * n * n + g.dp.n_bool * n + (uint64_t)g.dp.n_slots * (n + 1);
+        // thread-instructions the sliced kernel executes per frame of the range, summed over programs
+        h->last.logic_instr_per_frame +=
+            (double)(g.dp.n_modal * n * n + g.dp.n_bool * n + (uint64_t)g.dp.n_slots * (n + 1)) *
+            ((double)(1ull << (g.k_eff * n)) / 32.0);
+        h->last.executed_models += (uint64_t)(g.dp.n_slots + g.dp.n_unfit) * (count << (g.k_eff * n));
+    }
     if (n_records == 0) return KRIPKE_OK;
 
     if ((rc = ensure_accum(h, n_records))) return rc;
@@ -264,40 +289,133 @@ int run_scan(kripke_programs *h, const DevicePlan &plan, const uint32_t *d_pairs
     if (e) return cuda_fail(e);
     uint32_t launches = 1;
 
-    // the sliced kernel runs the batch if an instantiation for this shape keeps enough stack slots
-    uint64_t fpu = 1;
-    bool use_sliced = family != KRIPKE_KERNEL_SCALAR && plan.n_slots > 0 &&
-                      sliced_select(n, k, cls, plan.max_need, &fpu);
-    uint64_t ab = begin, ae = begin;          // aligned sub-range for the sliced kernel
-    if (use_sliced) {
-        ab = (begin + fpu - 1) / fpu * fpu;
-        ae = (begin + count) / fpu * fpu;
-        if (ae <= ab) { use_sliced = false; ab = ae = begin; }
-    }
-    if (family == KRIPKE_KERNEL_SLICED) {
-        if (!use_sliced || plan.n_unfit || ab != begin || ae != begin + count) return KRIPKE_EUNSUPPORTED;
-    }
-    if (use_sliced) {
-        ScanJob sj = job;
-        sj.frame_begin = ab; sj.frame_count = ae - ab;
-        SlicedPlan sp;
-        sp.ucode = plan.ucode; sp.slot_record = plan.slot_record;
-        sp.n_slots = plan.n_slots; sp.stride = plan.stride; sp.max_need = plan.max_need;
-        if ((e = launch_sliced(sj, sp, stream, &launches))) return cuda_fail(e);
-        h->last.kernel_family = 1;
-        if (plan.n_unfit && (e = launch_scalar(sj, plan.unfit, plan.n_unfit, reduce, stream, &launches)))
-            return cuda_fail(e);
-        ScanJob head = job, tail = job;
-        head.frame_count = ab - begin;
-        tail.frame_begin = ae; tail.frame_count = begin + count - ae;
-        if ((e = launch_scalar(head, nullptr, n_records, reduce, stream, &launches))) return cuda_fail(e);
-        if ((e = launch_scalar(tail, nullptr, n_records, reduce, stream, &launches))) return cuda_fail(e);
-    } else {
+    if (family == KRIPKE_KERNEL_SCALAR) {
         if ((e = launch_scalar(job, nullptr, n_records, reduce, stream, &launches))) return cuda_fail(e);
+    }
+    for (const GroupPlan &g : plan.groups) {
+        if (family == KRIPKE_KERNEL_SCALAR) break;
+        const DevicePlan &dp = g.dp;
+        uint32_t max_need = 0;
+        for (uint32_t d = 1; d <= (uint32_t)UC_DMAX; ++d)
+            if (dp.need_end[d] > dp.need_end[d - 1]) max_need = d;
+        uint64_t fpu = 1;
+        bool use_sliced = dp.n_slots > 0 && sliced_select(n, g.k_eff, cls, 1, &fpu);
+        uint64_t ab = begin, ae = begin;          // aligned sub-range for the sliced kernel
+        if (use_sliced) {
+            ab = (begin + fpu - 1) / fpu * fpu;
+            ae = (begin + count) / fpu * fpu;
+            if (ae <= ab) { use_sliced = false; ab = ae = begin; }
+        }
+        if (family == KRIPKE_KERNEL_SLICED) {
+            if ((dp.n_slots && !use_sliced) || dp.n_unfit || ab != begin || ae != begin + count ||
+                (dp.n_slots && !sliced_select(n, g.k_eff, cls, max_need, nullptr)))
+                return KRIPKE_EUNSUPPORTED;
+        }
+        if (use_sliced) {
+            ScanJob sj = job;                     // scalar launches on the sub-range (true k)
+            sj.frame_begin = ab; sj.frame_count = ae - ab;
+            ScanJob rj = sj;                      // the reduced scan: its own variable count
+            rj.k = g.k_eff;
+            h->last.kernel_family = 1;
+            // consecutive need classes that map to the same instantiation run as one launch
+            uint32_t d = 1;
+            while (d <= (uint32_t)UC_DMAX) {
+                uint32_t lo = dp.need_end[d - 1], hi = dp.need_end[d], top = d;
+                const uint32_t row = sliced_row(n, g.k_eff, cls, d);
+                while (top < (uint32_t)UC_DMAX && sliced_row(n, g.k_eff, cls, top + 1) == row) { ++top; hi = dp.need_end[top]; }
+                if (hi > lo) {
+                    if (row == UINT32_MAX) {       // no instantiation keeps this many slots: scalar kernel
+                        if ((e = launch_scalar(sj, dp.slot_record + lo, hi - lo, reduce, stream, &launches)))
+                            return cuda_fail(e);
+                    } else {
+                        SlicedPlan sp;
+                        sp.ucode = dp.ucode + (size_t)lo * dp.stride;
+                        sp.slot_record = dp.slot_record + lo;
+                        sp.n_slots = hi - lo; sp.stride = dp.stride; sp.max_need = top;
+                        sp.model_shift = (k - g.k_eff) * n;
+                        if ((e = launch_sliced(rj, sp, stream, &launches))) return cuda_fail(e);
+                    }
+                }
+                d = top + 1;
+            }
+            ScanJob head = job, tail = job;
+            head.frame_count = ab - begin;
+            tail.frame_begin = ae; tail.frame_count = begin + count - ae;
+            if ((e = launch_scalar(head, dp.slot_record, dp.n_slots, reduce, stream, &launches))) return cuda_fail(e);
+            if ((e = launch_scalar(tail, dp.slot_record, dp.n_slots, reduce, stream, &launches))) return cuda_fail(e);
+        } else if (dp.n_slots) {
+            if ((e = launch_scalar(job, dp.slot_record, dp.n_slots, reduce, stream, &launches))) return cuda_fail(e);
+        }
+        if (dp.n_unfit && (e = launch_scalar(job, dp.unfit, dp.n_unfit, reduce, stream, &launches)))
+            return cuda_fail(e);
     }
     if ((e = launch_finish(job, (flags & KRIPKE_ACCUMULATE) != 0, counts_out, witness_out, stream)))
         return cuda_fail(e);
     h->last.launches = launches + 1;
+    return KRIPKE_OK;
+}
+
+int build_scan_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
+                    uint32_t shapes, ScanPlan *out) {
+    out->release();
+    auto prog = [&](uint32_t f) { return &h->h_code[h->h_offsets[f]]; };
+    auto plen = [&](uint32_t f) { return h->h_offsets[f + 1] - h->h_offsets[f]; };
+    // group of every record: the least usable variable count that covers its support
+    std::vector<uint32_t> support(n_records), group(n_records);
+    for (uint32_t r = 0; r < n_records; ++r) {
+        uint32_t s = pairs ? (program_support(prog(pairs[2 * r]), plen(pairs[2 * r])) |
+                              program_support(prog(pairs[2 * r + 1]), plen(pairs[2 * r + 1])))
+                           : program_support(prog(r), plen(r));
+        support[r] = s;
+        uint32_t cnt = 0;
+        for (uint32_t i = 0; i < KRIPKE_MAX_VARS; ++i) cnt += (s >> i) & 1u;
+        uint32_t g = cnt;
+        while (g < k && !((shapes >> g) & 1u)) ++g;
+        group[r] = g;
+    }
+    for (uint32_t g = 0; g <= k; ++g) {
+        std::vector<uint32_t> recs;
+        for (uint32_t r = 0; r < n_records; ++r)
+            if (group[r] == g) recs.push_back(r);
+        if (recs.empty()) continue;
+        const uint32_t mode = sliced_lower_mode(n, g);
+        std::vector<Lowered> low(recs.size());
+        std::vector<bool> fits(recs.size());
+        for (size_t i = 0; i < recs.size(); ++i) {
+            const uint32_t r = recs[i];
+            uint8_t rename[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
+            uint8_t next = 0;
+            for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v)
+                if ((support[r] >> v) & 1u) rename[v] = next++;
+            if (g == k) for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v) rename[v] = (uint8_t)v;   // full sweep: as written
+            fits[i] = pairs ? lower_pair(prog(pairs[2 * r]), plen(pairs[2 * r]), prog(pairs[2 * r + 1]),
+                                         plen(pairs[2 * r + 1]), mode, rename, &low[i])
+                            : lower_single(prog(r), plen(r), mode, rename, &low[i]);
+        }
+        HostPlan hp;
+        build_plan(low, fits, &hp);
+        for (auto &x : hp.slot_record) x = recs[x];       // slot -> record index of the whole batch
+        for (auto &x : hp.unfit) x = recs[x];
+        GroupPlan gp;
+        gp.k_eff = g;
+        int rc = upload_plan(hp, &gp.dp);
+        if (rc) { gp.dp.release(); out->release(); return rc; }
+        out->groups.push_back(gp);
+    }
+    return KRIPKE_OK;
+}
+
+// The batch's plan for one shape (cached in the handle; synchronous upload on first use).
+int single_plan(kripke_programs *h, uint32_t n, uint32_t k, uint32_t shapes, const ScanPlan **out) {
+    const uint64_t key = ((uint64_t)n << 32) | shapes;
+    auto it = h->single.find(key);
+    if (it == h->single.end()) {
+        ScanPlan sp;
+        int rc = build_scan_plan(h, nullptr, h->n_formulas, n, k, shapes, &sp);
+        if (rc) return rc;
+        it = h->single.emplace(key, std::move(sp)).first;
+    }
+    *out = &it->second;
     return KRIPKE_OK;
 }
 
@@ -359,8 +477,8 @@ int kripke_eval_batch_range(const kripke_programs_t *programs, uint32_t n_worlds
                             void *stream) {
     if (!programs) return KRIPKE_EINVAL;
     kripke_programs *h = const_cast<kripke_programs *>(programs);
-    const DevicePlan *plan = nullptr;
-    int rc = single_plan(h, sliced_lower_mode(n_worlds, n_vars), &plan);
+    const ScanPlan *plan = nullptr;
+    int rc = single_plan(h, n_worlds, n_vars, reduced_shapes(n_worlds, n_vars, frame_class, flags), &plan);
     if (rc) return rc;
     return run_scan(h, *plan, nullptr, h->n_formulas, n_worlds, n_vars, frame_class, frame_begin,
                     frame_count, flags, counts_out, witness_out, stream);
@@ -384,19 +502,10 @@ int kripke_distinguish_pairs(const kripke_programs_t *programs, const uint32_t *
     kripke_programs *h = const_cast<kripke_programs *>(programs);
     for (uint32_t i = 0; i < 2 * n_pairs; ++i)
         if (pairs[i] >= h->n_formulas) return KRIPKE_EINVAL;
-    const uint32_t mode = sliced_lower_mode(n_worlds, n_vars);
-    std::vector<Lowered> low(n_pairs);
-    std::vector<bool> fits(n_pairs);
-    for (uint32_t j = 0; j < n_pairs; ++j) {
-        const uint32_t a = pairs[2 * j], b = pairs[2 * j + 1];
-        fits[j] = lower_pair(&h->h_code[h->h_offsets[a]], h->h_offsets[a + 1] - h->h_offsets[a],
-                             &h->h_code[h->h_offsets[b]], h->h_offsets[b + 1] - h->h_offsets[b], mode, &low[j]);
-    }
-    HostPlan hp;
-    build_plan(low, fits, &hp);
     // the previous call's plan may still be in use on another stream: wait before replacing it
     CU(cudaDeviceSynchronize());
-    int rc = upload_plan(hp, &h->pair);
+    int rc = build_scan_plan(h, pairs, n_pairs, n_worlds, n_vars,
+                             reduced_shapes(n_worlds, n_vars, frame_class, flags), &h->pair);
     if (rc) return rc;
     if (n_pairs > h->pairs_cap) {
         cudaFree(h->d_pairs);
@@ -555,8 +664,8 @@ int kripke_debug_lower(const uint8_t *code_a, uint32_t len_a, const uint8_t *cod
     if (rc) return rc;
     Lowered low;
     if (leaf_mode > 3) return KRIPKE_EINVAL;
-    const bool fits = code_b ? lower_pair(code_a, len_a, code_b, len_b, leaf_mode, &low)
-                             : lower_single(code_a, len_a, leaf_mode, &low);
+    const bool fits = code_b ? lower_pair(code_a, len_a, code_b, len_b, leaf_mode, nullptr, &low)
+                             : lower_single(code_a, len_a, leaf_mode, nullptr, &low);
     if (need_out) *need_out = (uint32_t)low.need;
     if (!fits) return KRIPKE_EUNSUPPORTED;
     if (low.ucode.size() > cap) return KRIPKE_EINVAL;

@@ -18,9 +18,12 @@ struct Lowered {
 };
 int validate_programs(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas, uint32_t n_vars,
                       uint32_t *max_stack_out);
-bool lower_single(const uint8_t *code, uint32_t len, uint32_t mode, Lowered *out);
+// Variables a program still mentions after constant folding (bit i = p_i).
+uint32_t program_support(const uint8_t *code, uint32_t len);
+// rename: variable index -> index in the reduced valuation (null = identity).
+bool lower_single(const uint8_t *code, uint32_t len, uint32_t mode, const uint8_t *rename, Lowered *out);
 bool lower_pair(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b, uint32_t mode,
-                Lowered *out);
+                const uint8_t *rename, Lowered *out);
 
 // ---- device-side job description (kernels) -----------------------------------------------------
 // Accumulators per output record, owned by the programs handle, zeroed at the start of a call.
@@ -56,11 +59,14 @@ struct SlicedPlan {
     uint32_t n_slots;
     uint32_t stride;              // micro-ops per slot (even, >= longest program + 1)
     uint32_t max_need;            // most register-stack slots any slot needs
+    uint32_t model_shift;         // refuting models are counted x 2^model_shift (unused variables)
 };
 
 // Is there a sliced instantiation for this shape and class that keeps `need` stack slots?  If so
 // *frames_per_unit is the alignment frame ranges must have for it.
 bool sliced_select(uint32_t n, uint32_t k, uint32_t cls, uint32_t need, uint64_t *frames_per_unit);
+// Index of the instantiation `sliced_select` would pick (UINT32_MAX = none).
+uint32_t sliced_row(uint32_t n, uint32_t k, uint32_t cls, uint32_t need);
 // LOWER_LEAF_* flags of the derived leaves the instantiations for this shape provide (0 = no shape).
 uint32_t sliced_lower_mode(uint32_t n, uint32_t k);
 // Enqueue the sliced scan; returns a cudaError_t as int and the number of kernel launches.

@@ -32,6 +32,7 @@ struct Leaf {
 
 struct Lowerer {
     uint32_t mode = 0;               // LOWER_LEAF_* flags
+    uint8_t rename[KRIPKE_MAX_VARS] = {0, 1, 2, 3};   // variable index -> index in the reduced valuation
     std::vector<Node> nodes;
     std::vector<uint16_t> out;
     uint32_t n_modal = 0, n_bool = 0;
@@ -81,7 +82,7 @@ struct Lowerer {
             if (c == KRIPKE_OP_TOP) st.push_back(add(N_CONST, 1, -1, -1));
             else if (c == KRIPKE_OP_BOT) st.push_back(add(N_CONST, 0, -1, -1));
             else if (c >= KRIPKE_OP_VAR0 && c < KRIPKE_OP_VAR0 + KRIPKE_MAX_VARS)
-                st.push_back(add(N_VAR, (uint8_t)(c - KRIPKE_OP_VAR0), -1, -1));
+                st.push_back(add(N_VAR, rename[c - KRIPKE_OP_VAR0], -1, -1));
             else if (is_unary(c)) {
                 int x = st.back(); st.pop_back();
                 st.push_back(c == KRIPKE_OP_NOT ? mk_not(x) : mk_modal(c == KRIPKE_OP_BOX ? N_BOX : N_DIA, x));
@@ -92,6 +93,16 @@ struct Lowerer {
             }
         }
         return st.back();
+    }
+
+    // Variables the folded tree still mentions (bit i = p_i, after renaming).
+    uint32_t support(int i) const {
+        const Node &nd = nodes[i];
+        if (nd.kind == N_VAR) return 1u << nd.value;
+        uint32_t s = 0;
+        if (nd.a >= 0) s |= support(nd.a);
+        if (nd.b >= 0) s |= support(nd.b);
+        return s;
     }
 
     // Is the subtree an atom or a derived leaf of the target kernel?
@@ -241,9 +252,15 @@ int validate_programs(const uint8_t *code, const uint32_t *offsets, uint32_t n_f
     return KRIPKE_OK;
 }
 
-bool lower_single(const uint8_t *code, uint32_t len, uint32_t mode, Lowered *out) {
+uint32_t program_support(const uint8_t *code, uint32_t len) {
+    Lowerer lw;
+    return lw.support(lw.build(code, len));
+}
+
+bool lower_single(const uint8_t *code, uint32_t len, uint32_t mode, const uint8_t *rename, Lowered *out) {
     Lowerer lw;
     lw.mode = mode;
+    if (rename) std::copy(rename, rename + KRIPKE_MAX_VARS, lw.rename);
     int root = lw.build(code, len);
     out->need = std::max(1, lw.need(root));
     if (out->need > UC_DMAX) return false;
@@ -256,9 +273,10 @@ bool lower_single(const uint8_t *code, uint32_t len, uint32_t mode, Lowered *out
 }
 
 bool lower_pair(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b, uint32_t mode,
-                Lowered *out) {
+                const uint8_t *rename, Lowered *out) {
     Lowerer lw;
     lw.mode = mode;
+    if (rename) std::copy(rename, rename + KRIPKE_MAX_VARS, lw.rename);
     int ra = lw.build(code_a, len_a);
     int rb = lw.build(code_b, len_b);
     int na = std::max(1, lw.need(ra)), nb = std::max(1, lw.need(rb));

@@ -53,6 +53,7 @@ struct SlicedParams {
     uint32_t n_chunks;
     uint32_t tiles_per_item;        // tiles of TPB (threads per block) units per work item
     uint32_t n_ranges;              // work items = n_ranges * n_chunks
+    uint32_t model_shift;           // models count x 2^model_shift: variables the programs do not mention
     Accum *accum;
 };
 
@@ -73,7 +74,7 @@ struct SlicedCfg {
     // words of the thread); group-per-unit: the dead-end leaf only, one copy per word (M x N)
     static constexpr int LEAF_WORDS = FRAME_PER_UNIT ? LEAF_COUNT * N : M * N;
     static constexpr uint32_t LOWER_MODE = LOWER_LEAF_DEAD | (P_LEAF ? LOWER_LEAF_P : 0u);
-    static_assert(N >= 1 && N <= 6 && K >= 0 && K <= 4 && DMAX >= 2 && DMAX <= UC_DMAX, "shape");
+    static_assert(N >= 1 && N <= 6 && K >= 0 && K <= 4 && DMAX >= 1 && DMAX <= UC_DMAX, "shape");
     static_assert(N * N + KN >= LOW, "too few models for one group");
 };
 
@@ -258,10 +259,11 @@ struct SlicedThread {
             uint32_t x = (F == 0) ? 0xFFFFFFFFu : 0u;
 #pragma unroll
             for (int w = 0; w < N; ++w) {
+                constexpr int d1 = DMAX > 1 ? 1 : 0;      // pairs always need two slots
                 if (F == 0) x &= D[0][m][w];
                 else if (F == 1) x |= D[0][m][w];
-                else if (F == 2) x |= D[0][m][w] ^ D[1][m][w];
-                else x |= ~(D[0][m][w] ^ D[1][m][w]);
+                else if (F == 2) x |= D[0][m][w] ^ D[d1][m][w];
+                else x |= ~(D[0][m][w] ^ D[d1][m][w]);
             }
             r[m] = (F == 0) ? ~x : x;
         }
@@ -346,8 +348,8 @@ struct SlicedThread {
 #undef KRIPKE_CASE3
             case UC_FIN_ALL: fin<0>(r); return;
             case UC_FIN_ANY: fin<1>(r); return;
-            case UC_FIN_XOR: fin<2>(r); return;
-            default: fin<3>(r); return;    // UC_FIN_XNOR
+            case UC_FIN_XOR: if (DMAX > 1) fin<2>(r); return;
+            default: if (DMAX > 1) fin<3>(r); return;    // UC_FIN_XNOR
             }
         }
     }
@@ -475,7 +477,7 @@ __global__ void __launch_bounds__(TPB, MINB) scan_sliced_kernel(SlicedParams p) 
         for (uint32_t i = threadIdx.x; i < nslots; i += SLICED_THREADS) {
             if (s_best[i] != 0xFFFFFFFFu) {
                 Accum *a = p.accum + p.slot_record[slot0 + i];
-                atomicAdd(&a->models, s_models[i]);
+                atomicAdd(&a->models, s_models[i] << p.model_shift);
                 atomicAdd(&a->frames, (unsigned long long)s_frames[i]);
                 atomicMin(&a->best, (unsigned long long)(u0 + s_best[i]) << C::UNIT_FRAME_BITS);
             }
@@ -513,6 +515,7 @@ int launch_sliced_inst(const ScanJob &job, const SlicedPlan &plan, void *stream,
     p.unit_count = job.frame_count / frames_per_unit;
     p.ucode = plan.ucode; p.slot_record = plan.slot_record;
     p.n_slots = plan.n_slots; p.stride = plan.stride;
+    p.model_shift = plan.model_shift;
     p.accum = job.accum;
     if (p.unit_count == 0 || p.n_slots == 0) return 0;
 

@@ -9,8 +9,8 @@ typedef int (*sliced_launch_fn)(const ScanJob &, const SlicedPlan &, void *, uin
 #define SHAPES(X) \
     X(3, 0, 2, 4) X(4, 0, 2, 4) X(5, 0, 2, 2) X(5, 0, 2, 4) X(6, 0, 2, 2) \
     X(6, 0, 2, 4) X(4, 1, 2, 4) X(5, 1, 2, 4) X(3, 2, 2, 4) X(4, 2, 3, 2) \
-    X(4, 2, 2, 4) X(5, 2, 3, 2) X(5, 2, 2, 3) X(5, 2, 2, 4) X(6, 2, 2, 3) \
-    X(4, 3, 2, 4) X(5, 3, 3, 2) X(5, 3, 2, 3) X(5, 3, 2, 4)
+    X(4, 2, 2, 4) X(5, 2, 4, 1) X(5, 2, 3, 2) X(5, 2, 2, 3) X(5, 2, 2, 4) \
+    X(6, 2, 2, 3) X(4, 3, 2, 4) X(5, 3, 3, 2) X(5, 3, 2, 3) X(5, 3, 2, 4)
 
 #define DECL(N, K, MB, D) \
     int launch_sliced_##N##_##K##_m##MB##_d##D(const ScanJob &, const SlicedPlan &, void *, uint32_t *);
@@ -46,6 +46,11 @@ bool sliced_select(uint32_t n, uint32_t k, uint32_t cls, uint32_t need, uint64_t
     return true;
 }
 
+uint32_t sliced_row(uint32_t n, uint32_t k, uint32_t cls, uint32_t need) {
+    const Row *r = find(n, k, cls, need);
+    return r ? (uint32_t)(r - kRows) : UINT32_MAX;
+}
+
 uint32_t sliced_lower_mode(uint32_t n, uint32_t k) {
     for (const Row &r : kRows)
         if (r.n == n && r.k == k)
@@ -54,6 +59,8 @@ uint32_t sliced_lower_mode(uint32_t n, uint32_t k) {
 }
 
 int launch_sliced(const ScanJob &job, const SlicedPlan &plan, void *stream, uint32_t *launches) {
+    // group-per-unit shapes need the range aligned to the unit of the row selected for need 1; every
+    // row of one (n, k) uses the same unit size
     const Row *r = find(job.n, job.k, job.cls, plan.max_need);
     if (!r) return 801;   // cudaErrorNotSupported
     return r->fn(job, plan, stream, launches);

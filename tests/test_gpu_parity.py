@@ -432,3 +432,27 @@ def test_c5_pairs_separation_sizes(kb, vol):
             assert O.check_pair_witness(a, b, 6, 0, K, int(wit6[i, 0]), 0, int(wit6[i, 1] >> np.uint64(32))), names[j]
     # Lemma 2: alpha_3 / alpha_4 need eight worlds, so they survive the complete six-world scan
     assert by_name["([]<>)^3T/([]<>)^4T"][0] == 0
+
+
+def test_variable_support_reduction_is_exact(kb, vol):
+    """Default scans sweep only the variables a program mentions and scale the model count
+    (PAPER.md:93 k_b; R8); KRIPKE_FULL_SWEEP evaluates every valuation.  Same results."""
+    progs = W.corpus_c2(1500)
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 2)
+    for n, cls, a, cnt in ((5, K, 777, 4000), (5, T, 10, 3000), (4, K, 0, 1 << 16), (4, S4, 0, 355), (3, K, 0, 512)):
+        red = run(kb, progs, n, 2, cls, a, cnt, handle=h)
+        executed_red = h.last_run_info().executed_models
+        full = run(kb, progs, n, 2, cls, a, cnt, flags=kb.FULL_SWEEP, handle=h)
+        executed_full = h.last_run_info().executed_models
+        same(red, full, f"support reduction n={n} cls={cls}")
+        assert executed_full == len(progs) * cnt << (2 * n) and executed_red <= executed_full
+    want = vol.census(code, offs, 4, 2, K)
+    same(run(kb, progs, 4, 2, K, handle=h), want, "reduced vs oracle")
+    # three variables: formulas over {p, r} only, {q} only, ...
+    c4 = W.corpus_c4(300)
+    sub = [c for c in c4 if not (b"\x10" in c and b"\x11" in c and b"\x12" in c)][:60] + c4[:20]
+    sc, so = W.pack_programs(sub)
+    want = vol.census(sc, so, 4, 3, K, 100, 64)
+    same(run(kb, sub, 4, 3, K, 100, 64), want, "k=3 reduced")
+    same(run(kb, sub, 4, 3, K, 100, 64, flags=kb.FULL_SWEEP), want, "k=3 full")
