@@ -1,6 +1,8 @@
 // sliced_dispatch.cpp - shape table of the bit-sliced kernel instantiations (scan_sliced_inst.cu).
 #include "internal.h"
 
+#include <cstdlib>
+
 namespace kripke {
 
 typedef int (*sliced_launch_fn)(const ScanJob &, const SlicedPlan &, void *, uint32_t *);
@@ -9,7 +11,7 @@ typedef int (*sliced_launch_fn)(const ScanJob &, const SlicedPlan &, void *, uin
 #define SHAPES(X) \
     X(3, 0, 2, 4) X(4, 0, 2, 4) X(5, 0, 2, 2) X(5, 0, 2, 4) X(6, 0, 2, 2) \
     X(6, 0, 2, 4) X(4, 1, 2, 4) X(5, 1, 2, 4) X(3, 2, 2, 4) X(4, 2, 3, 2) \
-    X(4, 2, 2, 4) X(5, 2, 4, 1) X(5, 2, 3, 2) X(5, 2, 2, 3) X(5, 2, 2, 4) \
+    X(4, 2, 2, 4) X(5, 2, 4, 1) X(5, 2, 3, 1) X(5, 2, 3, 2) X(5, 2, 2, 3) X(5, 2, 2, 4) \
     X(6, 2, 2, 3) X(4, 3, 2, 4) X(5, 3, 3, 2) X(5, 3, 2, 3) X(5, 3, 2, 4)
 
 #define DECL(N, K, MB, D) \
@@ -29,8 +31,11 @@ bool frame_per_unit(const Row &r) { return r.k * r.n >= 5 + r.mb; }
 // the most words per thread.
 const Row *find(uint32_t n, uint32_t k, uint32_t cls, uint32_t need) {
     const Row *best = nullptr;
+    static const char *cap_env = std::getenv("KRIPKE_MB_CAP");        // tuning aid: cap words per thread
+    const uint32_t mb_cap = cap_env ? (uint32_t)std::atoi(cap_env) : 99u;
     for (const Row &r : kRows) {
         if (r.n != n || r.k != k || r.dmax < need) continue;
+        if (r.mb > mb_cap && frame_per_unit(r)) continue;
         // group-per-unit shapes enumerate frames from the model index: class K only
         if (!frame_per_unit(r) && cls != KRIPKE_CLASS_K) continue;
         if (!best || r.dmax < best->dmax || (r.dmax == best->dmax && r.mb > best->mb)) best = &r;
