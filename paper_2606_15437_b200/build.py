@@ -29,7 +29,9 @@ UNITS = [
     ("sliced_dispatch", "sliced_dispatch.cpp", []),
     ("scan_scalar", "scan_scalar.cu", []),
     ("calibrate", "calibrate.cu", []),
-] + [(f"scan_sliced_inst{g}", "scan_sliced_inst.cu", [f"-DKRIPKE_INST_GROUP={g}"]) for g in range(4)]
+    ("wf_dispatch", "wf_dispatch.cpp", []),
+] + [(f"scan_sliced_inst{g}", "scan_sliced_inst.cu", [f"-DKRIPKE_INST_GROUP={g}"]) for g in range(4)] \
+  + [(f"scan_wf_inst{g}", "scan_wf_inst.cu", [f"-DKRIPKE_WF_INST={g}"]) for g in range(5)]
 
 
 def _headers_mtime() -> float:

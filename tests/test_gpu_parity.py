@@ -165,6 +165,38 @@ def test_n5_closed_forms_full_range(kb):
     assert int(run(kb, [progs[3]], 5, 2, S5)["models"][0]) == 0 and int(run(kb, [progs[3]], 5, 2, S4)["models"][0]) > 0
 
 
+def test_warp_frame_kernel_windows_live(kb, vol):
+    """The warp-frame kernel (class K and T at n=5; every variable-count group) against the oracle
+    run live on windows that hold whole scan units of each group (8 / 256 / 8,192 frames) plus ragged
+    ends, and against the bit-sliced kernel on the whole corpus."""
+    progs = W.corpus_c2()[::12] + [W.to_postfix(t) for t in W.named_axioms().values()]
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 2)
+    for cls, begin, count in ((K, 8192 * 122 - 5, 8500), (T, 8192 * 50 - 5, 8500), (K, (1 << 25) - 8192, 8192)):
+        want = vol.census(code, offs, 5, 2, cls, begin, count)
+        got = run(kb, progs, 5, 2, cls, begin, count, flags=kb.KERNEL_WARPFRAME, handle=h)
+        info = h.last_run_info()
+        assert info.kernel_family == 2 and info.wf_programs > 0.9 * len(progs)
+        same(got, want, f"warp-frame cls={cls} [{begin},+{count})")
+        certify(progs, got, 5, 2, cls, idx=range(0, len(progs), 9))
+        same(run(kb, progs, 5, 2, cls, begin, count, handle=h), want, "auto")
+        assert h.last_run_info().kernel_family == 1
+    allp = W.corpus_c2()
+    ha = kb.Programs(*W.pack_programs(allp), 2)
+    for cls, begin, count in ((K, 3 << 20, 1 << 15), (T, 1 << 19, 1 << 14)):
+        a = run(kb, allp, 5, 2, cls, begin, count, flags=kb.KERNEL_WARPFRAME, handle=ha)
+        assert ha.last_run_info().kernel_family == 2
+        b = run(kb, allp, 5, 2, cls, begin, count, flags=kb.KERNEL_SLICED | kb.FULL_SWEEP, handle=ha)
+        assert ha.last_run_info().kernel_family == 1
+        same(a, b, f"warp-frame vs bit-sliced cls={cls}")
+    # a class without an instantiation cannot be forced
+    import torch
+    c = torch.zeros((len(progs), 2), dtype=torch.int64, device="cuda")
+    w = torch.zeros((len(progs), 2), dtype=torch.int64, device="cuda")
+    rc = kb.load().kripke_eval_batch_range(h._h, 5, 2, S4, 0, 64, kb.KERNEL_WARPFRAME, c.data_ptr(), w.data_ptr(), None)
+    assert rc == kb.EUNSUPPORTED
+
+
 def test_c4_three_variables_ranges_golden(kb):
     g = gold("c4_ranges.npz")
     progs = W.corpus_c4()
