@@ -253,19 +253,27 @@ struct SlicedThread {
 #pragma unroll
             for (int w = 0; w < N; ++w) D[dd][m][w] = bool_fn<F>(D[dd][m][w], D[d1][m][w]);
     }
-    template <int F> __device__ __forceinline__ void fin(uint32_t (&r)[M]) const {
+    // FIN, kind = 0 ALL, 1 ANY, 2 XOR, 3 XNOR (ucode.h): r[m] = OR_w (D0[w] ^ [pair] D1[w] ^ pol) with
+    // pol = all-ones for ALL / XNOR - one warp-uniform formula, no dispatch.
+    __device__ __forceinline__ void fin(uint32_t kind, uint32_t (&r)[M]) const {
+        const uint32_t pol = ((kind ^ (kind >> 1)) & 1u) ? 0u : 0xFFFFFFFFu;
+        if (DMAX > 1 && kind >= 2u) {
+            constexpr int d1 = DMAX > 1 ? 1 : 0;
+#pragma unroll
+            for (int m = 0; m < M; ++m) {
+                uint32_t x = 0u;
+#pragma unroll
+                for (int w = 0; w < N; ++w) x |= D[0][m][w] ^ D[d1][m][w] ^ pol;
+                r[m] = x;
+            }
+            return;
+        }
 #pragma unroll
         for (int m = 0; m < M; ++m) {
-            uint32_t x = (F == 0) ? 0xFFFFFFFFu : 0u;
+            uint32_t x = 0u;
 #pragma unroll
-            for (int w = 0; w < N; ++w) {
-                constexpr int d1 = DMAX > 1 ? 1 : 0;      // pairs always need two slots
-                if (F == 0) x &= D[0][m][w];
-                else if (F == 1) x |= D[0][m][w];
-                else if (F == 2) x |= D[0][m][w] ^ D[d1][m][w];
-                else x |= ~(D[0][m][w] ^ D[d1][m][w]);
-            }
-            r[m] = (F == 0) ? ~x : x;
+            for (int w = 0; w < N; ++w) x |= D[0][m][w] ^ pol;
+            r[m] = x;
         }
     }
 
@@ -273,15 +281,19 @@ struct SlicedThread {
     __device__ __forceinline__ void run(const uint16_t *__restrict__ uc, uint32_t (&r)[M]) {
         uint32_t pc = 0;
         uint32_t nxt = uc[0];
+        uint32_t op;
         for (;;) {
-            const uint32_t op = nxt & 0xFFu, arg = nxt >> 8;
+            op = nxt & 0xFFu;
+            const uint32_t arg = nxt >> 8;
+            if (op >= (uint32_t)UC_FIN_ALL && op <= (uint32_t)UC_FIN_XNOR) break;          // FIN
             nxt = uc[++pc];          // prefetch (the slot's stride leaves an entry after FIN)
             switch (op) {
 #define KRIPKE_CASE4(base, call) \
     case (base) + 0: call(0); break; case (base) + 1: call(1); break; \
     case (base) + 2: call(2); break; case (base) + 3: call(3); break;
 #define KRIPKE_CASE3(base, call) \
-    case (base) + 0: call(0); break; case (base) + 1: call(1); break; case (base) + 2: call(2); break;
+    case (base) + 0: call(0); break; case (base) + 1: call(1); break; \
+    case (base) + 2: call(2); break;
 #define LV0(d) load_var<d>(0)
 #define LV1(d) load_var<d>(1)
 #define LV2(d) load_var<d>(2)
@@ -346,12 +358,10 @@ struct SlicedThread {
 #undef LZ
 #undef KRIPKE_CASE4
 #undef KRIPKE_CASE3
-            case UC_FIN_ALL: fin<0>(r); return;
-            case UC_FIN_ANY: fin<1>(r); return;
-            case UC_FIN_XOR: if (DMAX > 1) fin<2>(r); return;
-            default: if (DMAX > 1) fin<3>(r); return;    // UC_FIN_XNOR
+            default: break;
             }
         }
+        fin(op - (uint32_t)UC_FIN_ALL, r);
     }
 };
 
