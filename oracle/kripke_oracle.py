@@ -208,6 +208,59 @@ def distinguish(code_a, code_b, n, k, cls=CLASS_K, frame_begin=0, frame_count=No
 
 
 # ---------------------------------------------------------------------------------------------
+# explicit frame lists (PAPER.md:183-185 stress templates, :192 synthesized relations)
+# ---------------------------------------------------------------------------------------------
+def relation_from_matrix(n: int, mat):
+    """R from an n x n 0/1 adjacency matrix: mat[w][u] != 0 iff w -> u."""
+    return {(w, u) for w in range(n) for u in range(n) if mat[w][u]}
+
+
+def census_relations(code, n, k, mats):
+    """One formula over an explicit list of frames (adjacency matrices, any n) and all 2^(k*n)
+    valuations.  Same outputs as `census`, the witness frame being the POSITION j in the list:
+    (refuting_models, refuting_frames, (j, v, w))."""
+    phi = parse_postfix(code)
+    everything = list(range(n))
+    models = nframes = 0
+    witness = (NO_WITNESS, 0, 0)
+    for j, mat in enumerate(mats):
+        R = relation_from_matrix(n, mat)
+        hit = False
+        for v in range(1 << (k * n)):
+            V = valuation_from_index(n, k, v)
+            ts = truth_set(n, R, V, phi)
+            if ts != everything:
+                models += 1
+                hit = True
+                if witness[0] == NO_WITNESS:
+                    witness = (j, v, min(w for w in everything if w not in ts))
+        nframes += hit
+    return models, nframes, witness
+
+
+def distinguish_relations(code_a, code_b, n, k, mats):
+    """Pair path over an explicit list of frames; witness = (position, v, least
+    disagreement world)."""
+    phi = parse_postfix(code_a)
+    psi = parse_postfix(code_b)
+    models = nframes = 0
+    witness = (NO_WITNESS, 0, 0)
+    for j, mat in enumerate(mats):
+        R = relation_from_matrix(n, mat)
+        hit = False
+        for v in range(1 << (k * n)):
+            V = valuation_from_index(n, k, v)
+            D = [w for w in range(n) if sat(n, R, V, w, phi) != sat(n, R, V, w, psi)]
+            if D:
+                models += 1
+                hit = True
+                if witness[0] == NO_WITNESS:
+                    witness = (j, v, min(D))
+        nframes += hit
+    return models, nframes, witness
+
+
+# ---------------------------------------------------------------------------------------------
 # certificates (PAPER.md:129-135) and least refuting size (PAPER.md:137)
 # ---------------------------------------------------------------------------------------------
 def check_certificate(code, n, succ, val_masks, w, cls) -> bool:

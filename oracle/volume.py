@@ -51,6 +51,10 @@ def _load():
         lib.kov_census_list.argtypes = [u8p, u32p, ctypes.c_uint32, u32p, ctypes.c_uint32,
                                         ctypes.c_int, ctypes.c_int, u64p, u64p, ctypes.c_uint64,
                                         u64p, u64p, u64p, u32p, u32p, ctypes.c_int]
+        lib.kov_census_relations.restype = ctypes.c_int
+        lib.kov_census_relations.argtypes = [u8p, u32p, ctypes.c_uint32, u32p, ctypes.c_uint32,
+                                             ctypes.c_int, ctypes.c_int, u8p, ctypes.c_uint64,
+                                             u64p, u64p, u64p, u32p, u32p, ctypes.c_int]
         lib.kov_max_threads.restype = ctypes.c_int
         lib.kov_orbits.restype = ctypes.c_int64
         lib.kov_orbits.argtypes = [ctypes.c_int, u64p, u64p, ctypes.c_uint64]
@@ -139,6 +143,36 @@ def census_list(code, offsets, n, k, frames, weights=None, pairs=None, threads=0
         _p(res["wit_w"], ctypes.c_uint32), threads)
     if rc:
         raise ValueError("kov_census_list failed (malformed program or bad argument)")
+    return res
+
+
+def census_relations(code, offsets, n, k, rel, pairs=None, threads=0):
+    """Census of every program (or pair) over explicit frames rel[F, n, n] (uint8 adjacency matrices,
+    n <= 16) and all 2^(k*n) valuations.  Same dict as census_list; wit_f is the POSITION in rel."""
+    code = np.ascontiguousarray(code, dtype=np.uint8)
+    offsets = np.ascontiguousarray(offsets, dtype=np.uint32)
+    rel = np.ascontiguousarray(rel, dtype=np.uint8)
+    assert rel.ndim == 3 and rel.shape[1] == n and rel.shape[2] == n
+    B = len(offsets) - 1
+    P = 0
+    if pairs is not None:
+        pairs = np.ascontiguousarray(pairs, dtype=np.uint32).reshape(-1)
+        P = len(pairs) // 2
+        assert pairs.max(initial=0) < B
+    Q = P if pairs is not None else B
+    res = {"models": np.zeros(Q, np.uint64), "frames": np.zeros(Q, np.uint64),
+           "wit_f": np.zeros(Q, np.uint64), "wit_v": np.zeros(Q, np.uint32),
+           "wit_w": np.zeros(Q, np.uint32)}
+    if len(code) == 0:
+        code = np.zeros(1, np.uint8)
+    rc = _load().kov_census_relations(
+        _p(code, ctypes.c_uint8), _p(offsets, ctypes.c_uint32), B, _p(pairs, ctypes.c_uint32), P, n, k,
+        _p(rel if len(rel) else np.zeros((1, n, n), np.uint8), ctypes.c_uint8), len(rel),
+        _p(res["models"], ctypes.c_uint64), _p(res["frames"], ctypes.c_uint64),
+        _p(res["wit_f"], ctypes.c_uint64), _p(res["wit_v"], ctypes.c_uint32),
+        _p(res["wit_w"], ctypes.c_uint32), threads)
+    if rc:
+        raise ValueError("kov_census_relations failed (malformed program or bad argument)")
     return res
 
 

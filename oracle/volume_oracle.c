@@ -434,3 +434,129 @@ int64_t kov_orbits(int n, uint64_t *reps, uint64_t *sizes, uint64_t cap) {
     free(is_rep); free(perms);
     return (int64_t)count;
 }
+
+/* ---- explicit frame lists, up to 16 worlds (PAPER.md:183-185 templates, :192 synthesized relations) ----
+ * The same definitions once more, with the relation given as an n x n byte matrix per frame instead
+ * of an index, and arrays sized for 16 worlds.  rel[(j*n + w)*n + u] != 0 iff frame j has w -> u. */
+#define BIGN 16
+
+static int eval_program_big(const u8 *code, uint32_t len, int n, const u8 *R /* n*n */,
+                            u8 V[MAXVARS][BIGN], u8 out[BIGN]) {
+    u8 st[MAXDEPTH][BIGN];
+    int sp = 0;
+    for (uint32_t pc = 0; pc < len; ++pc) {
+        u8 c = code[pc];
+        if (c == OP_TOP || c == OP_BOT || (c >= OP_VAR0 && c < OP_VAR0 + MAXVARS)) {
+            if (sp >= MAXDEPTH) return -1;
+            for (int w = 0; w < n; ++w)
+                st[sp][w] = (c == OP_TOP) ? 1 : (c == OP_BOT) ? 0 : V[c - OP_VAR0][w];
+            ++sp;
+        } else if (c == OP_NOT) {
+            if (sp < 1) return -1;
+            for (int w = 0; w < n; ++w) st[sp - 1][w] = !st[sp - 1][w];
+        } else if (c == OP_BOX || c == OP_DIA) {
+            if (sp < 1) return -1;
+            u8 r[BIGN];
+            for (int w = 0; w < n; ++w) {
+                int all = 1, some = 0;            /* box: every successor; dia: some successor */
+                for (int u = 0; u < n; ++u)
+                    if (R[w * n + u]) {
+                        if (st[sp - 1][u]) some = 1; else all = 0;
+                    }
+                r[w] = (u8)((c == OP_BOX) ? all : some);
+            }
+            memcpy(st[sp - 1], r, (size_t)n);
+        } else if (c == OP_AND || c == OP_OR || c == OP_IMP) {
+            if (sp < 2) return -1;
+            for (int w = 0; w < n; ++w) {
+                int x = st[sp - 2][w], y = st[sp - 1][w];
+                st[sp - 2][w] = (u8)((c == OP_AND) ? (x && y) : (c == OP_OR) ? (x || y) : (!x || y));
+            }
+            --sp;
+        } else {
+            return -1;
+        }
+    }
+    if (sp != 1) return -1;
+    memcpy(out, st[0], (size_t)n);
+    return 0;
+}
+
+/* Census of B formulas (or P pairs) over the explicit frames rel[0..nframes) and all 2^(k*n)
+ * valuations.  Outputs as kov_census_list; the witness frame is the POSITION in the list. */
+int kov_census_relations(const u8 *code, const uint32_t *offs, uint32_t B,
+                         const uint32_t *pairs, uint32_t P, int n, int k,
+                         const u8 *rel, uint64_t nframes,
+                         uint64_t *models_out, uint64_t *frames_out,
+                         uint64_t *wit_f, uint32_t *wit_v, uint32_t *wit_w, int nthreads) {
+    if (n < 1 || n > BIGN || k < 0 || k > MAXVARS || k * n > 24) return -1;
+    const uint32_t Q = pairs ? P : B;
+    const uint64_t nval = 1ull << (k * n);
+    int bad = 0;
+#ifdef _OPENMP
+    if (nthreads <= 0) nthreads = omp_get_max_threads();
+#else
+    nthreads = 1;
+#endif
+    uint64_t *acc_m = calloc((size_t)nthreads * Q, sizeof(uint64_t));
+    uint64_t *acc_f = calloc((size_t)nthreads * Q, sizeof(uint64_t));
+    first_t *first = malloc((size_t)nthreads * Q * sizeof(first_t));
+    if (!acc_m || !acc_f || !first) return -1;
+    for (size_t i = 0; i < (size_t)nthreads * Q; ++i) first[i].pos = NO_WITNESS;
+
+#pragma omp parallel num_threads(nthreads)
+    {
+#ifdef _OPENMP
+        int tid = omp_get_thread_num();
+#else
+        int tid = 0;
+#endif
+        uint64_t *am = acc_m + (size_t)tid * Q, *af = acc_f + (size_t)tid * Q;
+        first_t *fi = first + (size_t)tid * Q;
+#pragma omp for schedule(dynamic, 4)
+        for (uint64_t pos = 0; pos < nframes; ++pos) {
+            const u8 *R = rel + (size_t)pos * n * n;
+            for (uint32_t q = 0; q < Q; ++q) {
+                uint32_t a = pairs ? pairs[2 * q] : q, b = pairs ? pairs[2 * q + 1] : q;
+                int hit = 0;
+                for (uint64_t v = 0; v < nval; ++v) {
+                    u8 V[MAXVARS][BIGN], ta[BIGN], tb[BIGN];
+                    for (int i = 0; i < k; ++i)
+                        for (int w = 0; w < n; ++w) V[i][w] = (u8)((v >> (i * n + w)) & 1u);
+                    int fail_world = -1;
+                    if (eval_program_big(code + offs[a], offs[a + 1] - offs[a], n, R, V, ta)) bad = 1;
+                    if (pairs) {
+                        if (eval_program_big(code + offs[b], offs[b + 1] - offs[b], n, R, V, tb)) bad = 1;
+                        for (int w = 0; w < n; ++w)
+                            if ((ta[w] != 0) != (tb[w] != 0)) { fail_world = w; break; }
+                    } else {
+                        for (int w = 0; w < n; ++w)
+                            if (!ta[w]) { fail_world = w; break; }
+                    }
+                    if (fail_world >= 0) {
+                        am[q] += 1;
+                        hit = 1;
+                        if (pos < fi[q].pos) { fi[q].pos = pos; fi[q].v = v; fi[q].w = (uint32_t)fail_world; }
+                    }
+                }
+                if (hit) af[q] += 1;
+            }
+        }
+    }
+    for (uint32_t q = 0; q < Q; ++q) {
+        uint64_t m = 0, fr = 0;
+        first_t best; best.pos = NO_WITNESS; best.v = 0; best.w = 0;
+        for (int t = 0; t < nthreads; ++t) {
+            m += acc_m[(size_t)t * Q + q];
+            fr += acc_f[(size_t)t * Q + q];
+            if (first[(size_t)t * Q + q].pos < best.pos) best = first[(size_t)t * Q + q];
+        }
+        models_out[q] = m;
+        frames_out[q] = fr;
+        wit_f[q] = best.pos;
+        wit_v[q] = (uint32_t)best.v;
+        wit_w[q] = best.w;
+    }
+    free(acc_m); free(acc_f); free(first);
+    return bad ? -1 : 0;
+}
