@@ -65,6 +65,9 @@ enum { KRIPKE_CLASS_K = 0, KRIPKE_CLASS_T = 1, KRIPKE_CLASS_S4 = 2, KRIPKE_CLASS
 #define KRIPKE_MAX_STACK 16u        /* postfix stack slots a program may need               */
 #define KRIPKE_MAX_PROGRAM_LEN 64u  /* opcodes per program                                   */
 #define KRIPKE_MAX_MODEL_BITS 61u   /* n*n + n_vars*n must not exceed this                   */
+#define KRIPKE_LIST_MAX_WORLDS 16u  /* frame-list mode: worlds per explicit frame ("16
+                                       successor slots")                                     */
+#define KRIPKE_LIST_MAX_VAL_BITS 20u/* frame-list mode: n_vars*n must not exceed this       */
 
 /* flags of the *_range calls */
 enum {
@@ -178,6 +181,29 @@ int kripke_minimal_refutation(const kripke_programs_t *programs, uint32_t n_vars
 int kripke_pairs_separation(const kripke_programs_t *programs, const uint32_t *pairs, uint32_t n_pairs,
                             uint32_t n_vars, uint32_t n_max, uint64_t chunk_frames,
                             uint32_t *size_out, kripke_witness_t *witness_out, void *stream);
+
+/* Frame-list mode (the pairs that survive the exhaustive prefix are "challenged on paths,
+ * reverse paths, looped paths, and forked paths of six to ten worlds" / templates "at each size from
+ * six through sixteen"; P:192 and Table 2: synthesized relations).  The frames are given, not
+ * enumerated: succ is a DEVICE array of n_frames * n_worlds 16-bit successor masks, succ[j*n + w]
+ * bit u = edge w -> u of frame j (bits >= n_worlds must be 0), 1 <= n_worlds <= 16,
+ * n_vars * n_worlds <= KRIPKE_LIST_MAX_VAL_BITS.  Every program of the batch is evaluated on every
+ * listed frame and every valuation; outputs as kripke_eval_batch, with witness.frame =
+ * index_base + (position j of the first refuting frame in the list).  flags: KRIPKE_ACCUMULATE
+ * (chunked lists: pass each chunk with its index_base), KRIPKE_KERNEL_SCALAR (thread = frame, one
+ * model per iteration: cross-check / ablation).  counts_out / witness_out: DEVICE, n_formulas. */
+int kripke_eval_frames(const kripke_programs_t *programs, uint32_t n_worlds, uint32_t n_vars,
+                       const uint16_t *succ, uint64_t n_frames, uint64_t index_base, uint32_t flags,
+                       kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream);
+
+/* The pair path over a frame list: pairs is a HOST array of 2*n_pairs program indices;
+ * a frame distinguishes pair j under a valuation iff the two truth sets differ; world = least
+ * disagreement world.  counts_out / witness_out: DEVICE, n_pairs entries. */
+int kripke_distinguish_pairs_frames(const kripke_programs_t *programs, const uint32_t *pairs,
+                                    uint32_t n_pairs, uint32_t n_worlds, uint32_t n_vars,
+                                    const uint16_t *succ, uint64_t n_frames, uint64_t index_base,
+                                    uint32_t flags, kripke_count_t *counts_out,
+                                    kripke_witness_t *witness_out, void *stream);
 
 /* End-to-end convenience with HOST buffers only: create + eval over the full class + copy the
  * results back + destroy, synchronously (this is what bench.py's "e2e" figure times). */

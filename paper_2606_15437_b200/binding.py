@@ -32,6 +32,7 @@ EXPORTS = [
     "kripke_distinguish_pairs", "kripke_eval_batch_host", "kripke_last_run_info",
     "kripke_calibrate_int32", "kripke_debug_lower", "kripke_witness_to_keys", "kripke_keys_to_witness",
     "kripke_minimal_refutation", "kripke_pairs_separation", "kripke_debug_lower_wf",
+    "kripke_eval_frames", "kripke_distinguish_pairs_frames",
 ]
 
 
@@ -84,6 +85,8 @@ def load():
     lib.kripke_keys_to_witness.argtypes = [vp, u32, u32, u32, vp, vp]
     lib.kripke_debug_lower.argtypes = [u8p, u32, u8p, u32, u32, u32, u8p, u32, ctypes.POINTER(u32)]
     lib.kripke_debug_lower_wf.argtypes = [u8p, u32, u32, u8p, u32]
+    lib.kripke_eval_frames.argtypes = [vp, u32, u32, vp, u64, u64, u32, vp, vp, vp]
+    lib.kripke_distinguish_pairs_frames.argtypes = [vp, u32p, u32, u32, u32, vp, u64, u64, u32, vp, vp, vp]
     for name in EXPORTS:
         if name not in ("kripke_version",):
             getattr(lib, name).restype = ctypes.c_int
@@ -208,6 +211,40 @@ def distinguish_pairs(programs: Programs, pairs, n_worlds: int, n_vars: int, fra
                                            frame_class, frame_begin, frame_count, flags,
                                            counts_out.data_ptr(), witness_out.data_ptr(),
                                            _stream(stream)), "kripke_distinguish_pairs")
+    return counts_out, witness_out
+
+
+def _succ(succ, n_worlds: int):
+    """succ: CUDA tensor of successor masks, int16 (bit pattern of uint16) or uint16, F*n entries."""
+    import torch
+    assert succ.is_cuda and succ.is_contiguous() and succ.element_size() == 2
+    assert succ.numel() % n_worlds == 0
+    return succ.numel() // n_worlds
+
+
+def eval_frames(programs: Programs, n_worlds: int, n_vars: int, succ, index_base: int = 0, flags: int = 0,
+                counts_out=None, witness_out=None, stream=None):
+    """kripke_eval_frames: every program on every listed frame (succ: CUDA tensor of F*n 16-bit
+    successor masks) and every valuation.  witness.frame = index_base + list position."""
+    n_frames = _succ(succ, n_worlds)
+    counts_out, witness_out = _outputs(programs.n_formulas, counts_out, witness_out)
+    _check(load().kripke_eval_frames(programs._h, n_worlds, n_vars, succ.data_ptr(), n_frames, index_base,
+                                     flags, counts_out.data_ptr(), witness_out.data_ptr(), _stream(stream)),
+           "kripke_eval_frames")
+    return counts_out, witness_out
+
+
+def distinguish_pairs_frames(programs: Programs, pairs, n_worlds: int, n_vars: int, succ,
+                             index_base: int = 0, flags: int = 0, counts_out=None, witness_out=None,
+                             stream=None):
+    pairs = np.ascontiguousarray(pairs, dtype=np.uint32).reshape(-1)
+    n_pairs = len(pairs) // 2
+    n_frames = _succ(succ, n_worlds)
+    counts_out, witness_out = _outputs(n_pairs, counts_out, witness_out)
+    _check(load().kripke_distinguish_pairs_frames(programs._h, pairs.ctypes.data, n_pairs, n_worlds, n_vars,
+                                                  succ.data_ptr(), n_frames, index_base, flags,
+                                                  counts_out.data_ptr(), witness_out.data_ptr(),
+                                                  _stream(stream)), "kripke_distinguish_pairs_frames")
     return counts_out, witness_out
 
 

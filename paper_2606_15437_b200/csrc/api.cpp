@@ -222,6 +222,9 @@ struct kripke_programs {
     uint32_t *d_offsets = nullptr;
     std::map<uint64_t, ScanPlan> single;     // one record per formula; cached per (n, usable reduced shapes)
     ScanPlan pair;                     // rebuilt by each kripke_distinguish_pairs call
+    DevicePlan list_single;            // frame-list mode: every formula lowered without derived leaves
+    bool list_single_built = false;
+    DevicePlan list_pair;              // rebuilt by each kripke_distinguish_pairs_frames call
     uint32_t *d_pairs = nullptr;
     uint32_t pairs_cap = 0;
     Accum *d_accum = nullptr;
@@ -513,9 +516,108 @@ int single_plan(kripke_programs *h, uint32_t n, uint32_t k, uint32_t shapes, con
     return KRIPKE_OK;
 }
 
+// ---- frame-list mode ----------------------------------------------------------------------------
+// Lowers the records for scan_frames.cu: no derived leaves (the frames are data, nothing is
+// thread-uniform), variables as written.
+int build_list_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, DevicePlan *out) {
+    auto prog = [&](uint32_t f) { return &h->h_code[h->h_offsets[f]]; };
+    auto plen = [&](uint32_t f) { return h->h_offsets[f + 1] - h->h_offsets[f]; };
+    const uint8_t rename[KRIPKE_MAX_VARS] = {0, 1, 2, 3};
+    std::vector<Lowered> low(n_records);
+    std::vector<bool> fits(n_records);
+    for (uint32_t r = 0; r < n_records; ++r)
+        fits[r] = pairs ? lower_pair(prog(pairs[2 * r]), plen(pairs[2 * r]), prog(pairs[2 * r + 1]),
+                                     plen(pairs[2 * r + 1]), 0u, rename, &low[r])
+                        : lower_single(prog(r), plen(r), 0u, rename, &low[r]);
+    HostPlan hp;
+    build_plan(low, fits, &hp);
+    return upload_plan(hp, out);
+}
+
+int run_frames(kripke_programs *h, const DevicePlan &dp, const uint32_t *d_pairs, uint32_t n_records,
+               uint32_t n, uint32_t k, const uint16_t *succ, uint64_t n_frames, uint64_t index_base,
+               uint32_t flags, kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream) {
+    if (n < 1 || n > KRIPKE_LIST_MAX_WORLDS || k != h->n_vars) return KRIPKE_EINVAL;
+    if (k * n > KRIPKE_LIST_MAX_VAL_BITS) return KRIPKE_EUNSUPPORTED;
+    if (flags & ~(KRIPKE_ACCUMULATE | KRIPKE_KERNEL_MASK)) return KRIPKE_EINVAL;
+    const uint32_t family = flags & KRIPKE_KERNEL_MASK;
+    if (family == KRIPKE_KERNEL_WARPFRAME) return KRIPKE_EUNSUPPORTED;
+    if (n_frames && !succ) return KRIPKE_EINVAL;
+    if (n_frames > (1ull << 40)) return KRIPKE_EUNSUPPORTED;
+    if (n_records && (!counts_out || !witness_out)) return KRIPKE_EINVAL;
+    if (family == KRIPKE_KERNEL_SLICED && dp.n_unfit) return KRIPKE_EUNSUPPORTED;
+    h->last = kripke_run_info_t{};
+    h->last.models_per_program = n_frames << (k * n);
+    h->last.executed_models = (uint64_t)n_records * h->last.models_per_program;
+    h->last.sliced_logic_ops_per_word = dp.n_modal * n * n + dp.n_bool * n + (uint64_t)dp.n_slots * (n + 1);
+    h->last.logic_instr_per_frame = (double)h->last.sliced_logic_ops_per_word * (double)(1ull << (k * n)) / 32.0;
+    h->last.dense_logic_instr_per_frame = h->last.logic_instr_per_frame;
+    h->last.kernel_family = family == KRIPKE_KERNEL_SCALAR ? 0 : 1;
+    if (n_records == 0) return KRIPKE_OK;
+    int rc = ensure_accum(h, n_records);
+    if (rc) return rc;
+    FramesJob job;
+    job.n = n; job.k = k; job.succ = succ; job.n_frames = n_frames; job.index_base = index_base;
+    job.code = h->d_code; job.offsets = h->d_offsets; job.pairs = d_pairs;
+    job.n_records = n_records; job.accum = h->d_accum;
+    int e = launch_init(job.accum, n_records, stream);
+    if (e) return cuda_fail(e);
+    uint32_t launches = 1;
+    if (family == KRIPKE_KERNEL_SCALAR) {
+        if ((e = launch_frames_scalar(job, nullptr, n_records, stream, &launches))) return cuda_fail(e);
+    } else {
+        SlicedPlan sp;
+        sp.ucode = dp.ucode; sp.slot_record = dp.slot_record; sp.n_slots = dp.n_slots;
+        sp.stride = dp.stride; sp.max_need = UC_DMAX; sp.model_shift = 0;
+        if ((e = launch_frames(job, sp, stream, &launches))) return cuda_fail(e);
+        if (dp.n_unfit && (e = launch_frames_scalar(job, dp.unfit, dp.n_unfit, stream, &launches))) return cuda_fail(e);
+    }
+    if ((e = launch_frames_finish(job, (flags & KRIPKE_ACCUMULATE) != 0, counts_out, witness_out, stream)))
+        return cuda_fail(e);
+    h->last.launches = launches + 1;
+    return KRIPKE_OK;
+}
+
 }  // namespace
 
 extern "C" {
+
+int kripke_eval_frames(const kripke_programs_t *programs, uint32_t n_worlds, uint32_t n_vars,
+                       const uint16_t *succ, uint64_t n_frames, uint64_t index_base, uint32_t flags,
+                       kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream) {
+    if (!programs) return KRIPKE_EINVAL;
+    kripke_programs *h = const_cast<kripke_programs *>(programs);
+    if (!h->list_single_built) {
+        int rc = build_list_plan(h, nullptr, h->n_formulas, &h->list_single);
+        if (rc) return rc;
+        h->list_single_built = true;
+    }
+    return run_frames(h, h->list_single, nullptr, h->n_formulas, n_worlds, n_vars, succ, n_frames, index_base,
+                      flags, counts_out, witness_out, stream);
+}
+
+int kripke_distinguish_pairs_frames(const kripke_programs_t *programs, const uint32_t *pairs,
+                                    uint32_t n_pairs, uint32_t n_worlds, uint32_t n_vars,
+                                    const uint16_t *succ, uint64_t n_frames, uint64_t index_base,
+                                    uint32_t flags, kripke_count_t *counts_out,
+                                    kripke_witness_t *witness_out, void *stream) {
+    if (!programs || (n_pairs && !pairs)) return KRIPKE_EINVAL;
+    kripke_programs *h = const_cast<kripke_programs *>(programs);
+    for (uint32_t i = 0; i < 2 * n_pairs; ++i)
+        if (pairs[i] >= h->n_formulas) return KRIPKE_EINVAL;
+    CU(cudaDeviceSynchronize());      // the previous call's plan may still be in use
+    int rc = build_list_plan(h, pairs, n_pairs, &h->list_pair);
+    if (rc) return rc;
+    if (n_pairs > h->pairs_cap) {
+        cudaFree(h->d_pairs);
+        h->d_pairs = nullptr; h->pairs_cap = 0;
+        CU(cudaMalloc((void **)&h->d_pairs, (size_t)2 * n_pairs * sizeof(uint32_t)));
+        h->pairs_cap = n_pairs;
+    }
+    if (n_pairs) CU(cudaMemcpy(h->d_pairs, pairs, (size_t)2 * n_pairs * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    return run_frames(h, h->list_pair, h->d_pairs, n_pairs, n_worlds, n_vars, succ, n_frames, index_base, flags,
+                      counts_out, witness_out, stream);
+}
 
 const char *kripke_version(void) { return "kripke-b200 0.1 (sm_100a)"; }
 
@@ -559,6 +661,7 @@ int kripke_programs_destroy(kripke_programs_t *h) {
     cudaDeviceSynchronize();
     for (auto &kv : h->single) kv.second.release();
     h->pair.release();
+    h->list_single.release(); h->list_pair.release();
     cudaFree(h->d_code); cudaFree(h->d_offsets); cudaFree(h->d_pairs); cudaFree(h->d_accum);
     cudaFree(h->d_tmp_counts); cudaFree(h->d_tmp_wit);
     delete h;

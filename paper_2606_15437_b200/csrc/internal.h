@@ -107,6 +107,26 @@ int launch_wf(const ScanJob &job, const WfPlan &plan, void *stream, uint32_t *la
 // per frame of the class for one program, averaged over the class.
 double wf_cost_per_frame(uint32_t n, uint32_t k, uint32_t cls, const WfOpCounts &c);
 
+// ---- frame-list mode (scan_frames.cu) ----------------------------------------------------------
+struct FramesJob {
+    uint32_t n, k;
+    const uint16_t *succ;         // device: n_frames * n successor masks
+    uint64_t n_frames;
+    uint64_t index_base;          // added to the list position in witness.frame
+    const uint8_t *code;          // device (raw postfix form: scalar kernel, witness completion)
+    const uint32_t *offsets;
+    const uint32_t *pairs;        // device, 2 * n_records, or null
+    uint32_t n_records;
+    Accum *accum;
+};
+// Bit-sliced scan of the lowered slots over the list (32 frames per word); n <= 16.
+int launch_frames(const FramesJob &job, const SlicedPlan &plan, void *stream, uint32_t *launches);
+// Scalar scan (thread = frame) of the listed records (device list, or null = all).
+int launch_frames_scalar(const FramesJob &job, const uint32_t *records, uint32_t n_list, void *stream,
+                         uint32_t *launches);
+int launch_frames_finish(const FramesJob &job, bool accumulate, kripke_count_t *counts_out,
+                         kripke_witness_t *witness_out, void *stream);
+
 // Zero the accumulators; finish: turn accumulators into counts / witnesses (handles ACCUMULATE).
 int launch_init(Accum *accum, uint32_t n_records, void *stream);
 int launch_finish(const ScanJob &job, bool accumulate, kripke_count_t *counts_out,
