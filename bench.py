@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py - formula-model evaluations/s of the n=5 census layer (BASELINE.json configs[2]).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c3|c3_small]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c3|c3_small|c4|frames]
 
 One step = one pass of the whole hot path (DESIGN.md steps H1-H6, H8's class loop) over the
 5,624-formula seeded corpus on every labelled frame of five worlds in K, T, S4 and S5 and every
@@ -366,13 +366,107 @@ def run_c4(args):
     }))
 
 
+def run_frames(args):
+    """--workload frames: frame-list mode (Table 2).  Per size n the
+    pair path is timed on a seeded list of 2^20 explicit frames (workloads/frames.py stress_list):
+    constant pairs (the 36 named pairs of PAPER.md:179/190 plus seeded ones, one valuation) at every
+    size, one-variable pairs (2^n valuations) through n = 12.  Reports pair-frame
+    tests/s, valuation-frame evaluations/s (2 formulas per pair), the kernel's logic-instruction rate
+    against the ALU peak, its shared-memory operand rate and HBM bytes, the scalar (thread = frame)
+    kernel on the same list, and the oracle on a bounded sample."""
+    import torch
+    from paper_2606_15437_b200 import binding as kb
+    from workloads import frames as F
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    kb.load()
+    n_frames = 1 << 20
+    progs0, pairs0, _ = W.pairs_c5(count=220)
+    pairs0 = np.asarray(pairs0, np.uint32)
+    rng = W.SplitMix64(15437007)
+    progs1 = [W.to_postfix(W.gen_formula(rng, 9, 9, "pTF")) for _ in range(256)]
+    pairs1 = np.arange(256, dtype=np.uint32).reshape(-1, 2)
+    peak = SM_COUNT * INT_LANES_PER_SM * 1.965e9
+    reps = max(1, args.steps)
+
+    def timed(fn):
+        for _ in range(max(1, min(args.warmup, 3))):
+            fn()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b) * 1e-3)
+        return float(np.median(ts))
+
+    clock = ClockSampler(0)
+    clock.start()
+    rows = {}
+    total_tests = total_evals = total_time = 0.0
+    for n in (6, 8, 10, 12, 14, 16):
+        rel = F.stress_list(n, n_frames)
+        succ = torch.from_numpy(F.succ_masks(rel).view(np.int16).reshape(-1).copy()).cuda()
+        row = {}
+        for k, progs, pairs in ((0, progs0, pairs0), (1, progs1, pairs1)):
+            if k * n > 12:
+                continue
+            h = kb.Programs(*W.pack_programs(progs), k)
+            P = len(pairs)
+            c = torch.zeros((P, 2), dtype=torch.int64, device="cuda")
+            w = torch.zeros((P, 2), dtype=torch.int64, device="cuda")
+            t = timed(lambda: kb.distinguish_pairs_frames(h, pairs, n, k, succ, 0, 0, c, w))
+            info = h.last_run_info()
+            tests = P * n_frames
+            evals = 2 * tests * (1 << (k * n))
+            logic = info.logic_instr_per_frame * n_frames
+            sub = 1 << 16
+            ts = timed(lambda: kb.distinguish_pairs_frames(h, pairs, n, k, succ[:sub * n].contiguous(), 0,
+                                                           kb.KERNEL_SCALAR, c, w))
+            row[f"k{k}"] = {"pairs": P, "seconds": t, "pair_frame_tests_per_s": tests / t,
+                            "evaluations_per_s": evals / t, "logic_instr_per_s": logic / t,
+                            "frac_of_alu_peak": logic / t / peak,
+                            "scalar_kernel_evaluations_per_s": 2 * P * sub * (1 << (k * n)) / ts,
+                            "hbm_bytes_frames": 2 * n * n_frames}
+            total_tests += tests; total_evals += evals; total_time += t
+            h.destroy()
+        rows[str(n)] = row
+        del succ
+    clocks = clock.result()
+    # the oracle on a bounded sample of the same workload (n = 8, one-variable pairs)
+    from oracle import volume as V
+    V.build()
+    n = 8
+    rel = F.stress_list(n, 2048)
+    code, offs = W.pack_programs(progs1)
+    t0 = time.perf_counter()
+    V.census_relations(code, offs, n, 1, rel, pairs=pairs1)
+    dt = time.perf_counter() - t0
+    cpu = 2 * len(pairs1) * len(rel) * (1 << n) / dt
+    print(json.dumps({
+        "metric": "valuation-frame evaluations/sec on explicit frame lists (n = 6..16)",
+        "value": total_evals / total_time, "unit": "evaluations/s", "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": total_time * 1e3, "higher_is_better": True, "scaling": "strong",
+        "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": "frame-list mode (PAPER.md:183-192, Table 2): 2^20 seeded explicit frames per size "
+                               "n in {6,8,10,12,14,16} (templates, Erdos-Renyi, edge-flip, dead-end, back-edge); "
+                               f"{len(pairs0)} constant pairs at every size, {len(pairs1)} one-variable pairs through n = 12",
+                   "pair_frame_tests_per_s": total_tests / total_time,
+                   "context": "paper, H100: 586,365,732 pair-frame tests / 94.68e9 evaluations in 53.0 s of GPU "
+                              "evaluation (Table 2) = 1.79e9 evaluations/s"},
+        "clocks": clocks, "per_size": rows,
+        "cpu_baseline": {"value": cpu, "unit": "evaluations/s", "cores": V.max_threads(), "kind": "oracle",
+                         "sample": f"n=8, 2,048 frames x 256 valuations x {len(pairs1)} one-variable pairs ({dt:.1f} s)"},
+    }))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c3", "c3_small", "c4"])
+    ap.add_argument("--workload", default="c3", choices=["c3", "c3_small", "c4", "frames"])
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--ref-frames", type=int, default=256)
     args = ap.parse_args()
@@ -380,6 +474,8 @@ def main():
         run_reference(args)
     elif args.workload == "c4":
         run_c4(args)
+    elif args.workload == "frames":
+        run_frames(args)
     else:
         run_ours(args)
 

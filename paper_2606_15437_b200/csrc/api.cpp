@@ -568,7 +568,9 @@ int run_frames(kripke_programs *h, const DevicePlan &dp, const uint32_t *d_pairs
     } else {
         SlicedPlan sp;
         sp.ucode = dp.ucode; sp.slot_record = dp.slot_record; sp.n_slots = dp.n_slots;
-        sp.stride = dp.stride; sp.max_need = UC_DMAX; sp.model_shift = 0;
+        sp.stride = dp.stride; sp.max_need = 1; sp.model_shift = 0;
+        for (uint32_t d = 1; d <= (uint32_t)UC_DMAX; ++d)
+            if (dp.need_end[d] > dp.need_end[d - 1]) sp.max_need = d;
         if ((e = launch_frames(job, sp, stream, &launches))) return cuda_fail(e);
         if (dp.n_unfit && (e = launch_frames_scalar(job, dp.unfit, dp.n_unfit, stream, &launches))) return cuda_fail(e);
     }

@@ -1,23 +1,5 @@
-// scan_frames.cu - frame-list mode: the fused evaluator over EXPLICIT frames of up to 16 worlds
-// (survivors of the exhaustive prefix are "challenged on paths, reverse paths,
-// looped paths, and forked paths of six to ten worlds" / "39 ... templates at each size from six
-// through sixteen"; Table 2: synthesized relations, 8,995,007 of them).
-//
-// Here frames are data (n successor masks each, 2n bytes), so the layout is the transpose of the
-// census kernel's: a 32-bit word carries one truth bit for 32 consecutive FRAMES of the list, a
-// truth set is N words, and the valuation is block-uniform (atoms are all-0 / all-1 words).  Lemma
-// 1 on 32 frames at once is the same N*N three-input logic instructions as in scan_sliced.cuh,
-//     box: R[w] = AND_u ( T[u] | ~E[w][u] )        dia: R[w] = OR_u ( T[u] & E[w][u] )
-// with E[w][u] = the word of edge bits w->u of the thread's 32 frames.  A block reads its tile of
-// TPB*32 frames from HBM once (coalesced 16-bit masks), transposes it on chip with warp ballots
-// into a shared-memory table E[w*N+u][thread], and then runs every program of its chunk and every
-// valuation against that table: HBM traffic is 2n bytes per frame per program chunk, the inner
-// loop reads one shared-memory word per logic instruction.
-//
-// Programs are the same lowered micro-ops as the census kernel's (ucode.h, lowered without derived
-// leaves).  The top of the register stack lives in registers A[N]; deeper slots are spilled to a
-// per-thread shared-memory column when a load pushes (the lowering is stack-disciplined: a load
-// into slot d happens exactly when slot d-1 is the top).
+// scan_frames.cu - frame-list mode: dispatch over the bit-sliced instantiations
+// (scan_frames.cuh, scan_frames_inst.cu), the scalar kernel and the witness-completion kernel.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -27,201 +9,16 @@
 
 namespace kripke {
 
+// scan_frames_inst.cu: launch_frames_<N>_v<VB>
+#define FR_DECL(N) \
+    int launch_frames_##N##_v1(const FramesJob &, const SlicedPlan &, void *, uint32_t *); \
+    int launch_frames_##N##_v2(const FramesJob &, const SlicedPlan &, void *, uint32_t *); \
+    int launch_frames_##N##_v4(const FramesJob &, const SlicedPlan &, void *, uint32_t *);
+FR_DECL(1) FR_DECL(2) FR_DECL(3) FR_DECL(4) FR_DECL(5) FR_DECL(6) FR_DECL(7) FR_DECL(8)
+FR_DECL(9) FR_DECL(10) FR_DECL(11) FR_DECL(12) FR_DECL(13) FR_DECL(14) FR_DECL(15) FR_DECL(16)
+#undef FR_DECL
+
 namespace {
-
-constexpr int FR_TPB = 128;                     // threads per block = groups of 32 frames per tile
-constexpr int FR_SPILL = UC_DMAX - 1;           // stack slots below the top
-
-struct FramesParams {
-    const uint16_t *succ;          // n_frames * N masks
-    uint64_t n_frames;
-    uint32_t k;
-    const uint16_t *ucode;
-    const uint32_t *slot_record;
-    uint32_t n_slots, stride;
-    uint32_t chunk, n_chunks;      // slots per work item
-    uint32_t n_tiles;              // tiles of FR_TPB * 32 frames
-    Accum *accum;
-};
-
-template <int F> __device__ __forceinline__ uint32_t bfn(uint32_t a, uint32_t b) {
-    return (F == BF_AND) ? (a & b) : (F == BF_OR) ? (a | b) : (F == BF_ANDN) ? (a & ~b) : (~a & b);
-}
-__device__ __forceinline__ uint32_t bfn_rt(uint32_t f, uint32_t a, uint32_t b) {
-    return (f == BF_AND) ? (a & b) : (f == BF_OR) ? (a | b) : (f == BF_ANDN) ? (a & ~b) : (~a & b);
-}
-
-template <int N>
-struct FramesThread {
-    uint32_t A[N];                 // top of the stack
-    const uint32_t *E;             // this thread's column of the edge table: E[(w*N+u)*FR_TPB]
-    uint32_t *S;                   // this thread's spill column: S[(d*N+w)*FR_TPB]
-
-    __device__ __forceinline__ void push(uint32_t d) {          // a load into slot d > 0 pushes
-        if (d == 0) return;
-#pragma unroll
-        for (int w = 0; w < N; ++w) S[((d - 1) * N + w) * FR_TPB] = A[w];
-    }
-    __device__ __forceinline__ void box() {
-        uint32_t r[N];
-#pragma unroll
-        for (int w = 0; w < N; ++w) {
-            uint32_t acc = 0xFFFFFFFFu;
-#pragma unroll
-            for (int u = 0; u < N; ++u) acc &= (A[u] | ~E[(w * N + u) * FR_TPB]);
-            r[w] = acc;
-        }
-#pragma unroll
-        for (int w = 0; w < N; ++w) A[w] = r[w];
-    }
-    __device__ __forceinline__ void dia() {
-        uint32_t r[N];
-#pragma unroll
-        for (int w = 0; w < N; ++w) {
-            uint32_t acc = 0u;
-#pragma unroll
-            for (int u = 0; u < N; ++u) acc |= (A[u] & E[(w * N + u) * FR_TPB]);
-            r[w] = acc;
-        }
-#pragma unroll
-        for (int w = 0; w < N; ++w) A[w] = r[w];
-    }
-
-    // One lowered program on the thread's 32 frames under valuation v; returns the word of frames
-    // that refute the formula / distinguish the pair.
-    __device__ __forceinline__ uint32_t run(const uint16_t *__restrict__ uc, uint32_t v) {
-        uint32_t pc = 0, nxt = uc[0], op;
-        for (;;) {
-            op = nxt & 0xFFu;
-            if (op >= (uint32_t)UC_FIN_ALL && op <= (uint32_t)UC_FIN_XNOR) break;
-            nxt = uc[++pc];
-            if (op < (uint32_t)UC_BOOLV) {                       // LOADV + i*4 + d
-                const uint32_t i = op >> 2;
-                push(op & 3u);
-#pragma unroll
-                for (int w = 0; w < N; ++w) A[w] = 0u - ((v >> (i * N + w)) & 1u);
-            } else if (op < (uint32_t)UC_LOADL) {                // BOOLV + (f*4 + i)*4 + d
-                const uint32_t x = op - UC_BOOLV, i = (x >> 2) & 3u, f = x >> 4;
-#pragma unroll
-                for (int w = 0; w < N; ++w) A[w] = bfn_rt(f, A[w], 0u - ((v >> (i * N + w)) & 1u));
-            } else if (op >= (uint32_t)UC_BOOL && op < (uint32_t)UC_BOX) {   // BOOL + f*4 + d
-                const uint32_t x = op - UC_BOOL, d = x & 3u, f = x >> 2;
-#pragma unroll
-                for (int w = 0; w < N; ++w) A[w] = bfn_rt(f, S[(d * N + w) * FR_TPB], A[w]);
-            } else if (op >= (uint32_t)UC_BOX && op < (uint32_t)UC_DIA) {
-                box();
-            } else if (op >= (uint32_t)UC_DIA && op < (uint32_t)UC_FIN_ALL) {
-                dia();
-            } else if (op >= (uint32_t)UC_LOADZ) {               // LOADZ + d
-                push(op - UC_LOADZ);
-#pragma unroll
-                for (int w = 0; w < N; ++w) A[w] = 0u;
-            }
-            // UC_LOADL / UC_BOOLL are never emitted: the programs are lowered without derived leaves
-        }
-        const uint32_t kind = op - UC_FIN_ALL;
-        const uint32_t pol = ((kind ^ (kind >> 1)) & 1u) ? 0u : 0xFFFFFFFFu;
-        uint32_t x = 0u;
-        if (kind >= 2u) {
-#pragma unroll
-            for (int w = 0; w < N; ++w) x |= S[w * FR_TPB] ^ A[w] ^ pol;
-        } else {
-#pragma unroll
-            for (int w = 0; w < N; ++w) x |= A[w] ^ pol;
-        }
-        return x;
-    }
-};
-
-template <int N>
-__global__ void __launch_bounds__(FR_TPB) scan_frames_kernel(FramesParams p) {
-    extern __shared__ __align__(16) unsigned char smem[];
-    // [E: N*N x TPB][spill: FR_SPILL*N x TPB][valid: TPB][models u64 x chunk][frames u32][best u32][ucode]
-    uint32_t *s_E = reinterpret_cast<uint32_t *>(smem);
-    uint32_t *s_S = s_E + N * N * FR_TPB;
-    uint32_t *s_valid = s_S + FR_SPILL * N * FR_TPB;
-    unsigned long long *s_models = reinterpret_cast<unsigned long long *>(s_valid + FR_TPB);
-    uint32_t *s_frames = reinterpret_cast<uint32_t *>(s_models + p.chunk);
-    uint32_t *s_best = s_frames + p.chunk;
-    uint16_t *s_ucode = reinterpret_cast<uint16_t *>(s_best + p.chunk);
-
-    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const uint32_t n_items = p.n_tiles * p.n_chunks;
-    const uint32_t nval = 1u << (p.k * N);
-    FramesThread<N> T;
-    T.E = s_E + threadIdx.x;
-    T.S = s_S + threadIdx.x;
-
-    for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
-        const uint32_t chunk_id = item % p.n_chunks, tile = item / p.n_chunks;
-        const uint32_t slot0 = chunk_id * p.chunk;
-        const uint32_t nslots = min(p.chunk, p.n_slots - slot0);
-        const uint64_t frame0 = (uint64_t)tile * (FR_TPB * 32);
-
-        __syncthreads();
-        for (uint32_t i = threadIdx.x; i < nslots; i += FR_TPB) {
-            s_models[i] = 0ull; s_frames[i] = 0u; s_best[i] = 0xFFFFFFFFu;
-        }
-        {
-            const uint32_t words = nslots * (p.stride / 2);
-            const uint32_t *src = reinterpret_cast<const uint32_t *>(p.ucode + (size_t)slot0 * p.stride);
-            uint32_t *dst = reinterpret_cast<uint32_t *>(s_ucode);
-            for (uint32_t i = threadIdx.x; i < words; i += FR_TPB) dst[i] = src[i];
-        }
-        // the tile's frames -> bit-sliced edge table: warp `warp` transposes the groups of its own
-        // 32 threads, one group (32 frames, one per lane) at a time
-        for (uint32_t gi = 0; gi < 32; ++gi) {
-            const uint32_t t = warp * 32 + gi;
-            const uint64_t j = frame0 + (uint64_t)t * 32 + lane;
-            const bool valid = j < p.n_frames;
-            uint32_t m[N];
-#pragma unroll
-            for (int w = 0; w < N; ++w) m[w] = valid ? (uint32_t)__ldg(p.succ + j * N + w) : 0u;
-            const uint32_t vm = __ballot_sync(0xFFFFFFFFu, valid);
-            if (lane == 0) s_valid[t] = vm;
-#pragma unroll
-            for (int w = 0; w < N; ++w)
-#pragma unroll
-                for (int u = 0; u < N; ++u) {
-                    const uint32_t word = __ballot_sync(0xFFFFFFFFu, (m[w] >> u) & 1u);
-                    if (lane == (uint32_t)((w * N + u) & 31)) s_E[(w * N + u) * FR_TPB + t] = word;
-                }
-        }
-        __syncthreads();
-
-        const uint32_t vmask = s_valid[threadIdx.x];
-        const bool warp_live = __ballot_sync(0xFFFFFFFFu, vmask != 0u) != 0u;   // else: whole warp past the end
-        for (uint32_t s = 0; warp_live && s < nslots; ++s) {
-            const uint16_t *uc = s_ucode + s * p.stride;
-            uint32_t cnt = 0, any = 0;
-            for (uint32_t v = 0; v < nval; ++v) {
-                const uint32_t r = T.run(uc, v) & vmask;
-                cnt += __popc(r);
-                any |= r;
-            }
-            const uint32_t bal = __ballot_sync(0xFFFFFFFFu, any != 0u);
-            if (bal) {
-                const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, cnt);
-                const uint32_t ftot = __reduce_add_sync(0xFFFFFFFFu, (uint32_t)__popc(any));
-                const uint32_t first = __shfl_sync(0xFFFFFFFFu, any, __ffs(bal) - 1);
-                if (lane == 0) {
-                    atomicAdd(&s_models[s], (unsigned long long)tot);
-                    atomicAdd(&s_frames[s], ftot);
-                    atomicMin(&s_best[s], (warp * 32 + (uint32_t)(__ffs(bal) - 1)) * 32 + (uint32_t)(__ffs(first) - 1));
-                }
-            }
-        }
-        __syncthreads();
-        for (uint32_t i = threadIdx.x; i < nslots; i += FR_TPB) {
-            if (s_best[i] != 0xFFFFFFFFu) {
-                Accum *a = p.accum + p.slot_record[slot0 + i];
-                atomicAdd(&a->models, s_models[i]);
-                atomicAdd(&a->frames, (unsigned long long)s_frames[i]);
-                atomicMin(&a->best, frame0 + s_best[i]);
-            }
-        }
-    }
-}
 
 // Scalar form (the paper's own layout, Algorithm 1: thread = frame, one model per iteration on
 // n-bit masks): records whose programs need more register-stack slots than the lowering keeps, the
@@ -348,60 +145,23 @@ __global__ void __launch_bounds__(128) finish_frames_kernel(FramesFinishParams p
     }
 }
 
-template <int N>
-int launch_frames_n(const FramesJob &job, const SlicedPlan &plan, void *stream, uint32_t *launches) {
-    static int sm_count = 0;
-    static size_t smem_max = 0;
-    auto kern = scan_frames_kernel<N>;
-    const size_t fixed = ((size_t)N * N + (size_t)FR_SPILL * N + 1) * FR_TPB * sizeof(uint32_t);
-    const size_t per_slot = 16 + 2 * (size_t)plan.stride;
-    if (!sm_count) {
-        int dev = 0, optin = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e != cudaSuccess) return (int)e;
-        e = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess) return (int)e;
-        e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-        if (e != cudaSuccess) return (int)e;
-        smem_max = std::min<size_t>((size_t)optin, fixed + 32 * 1024 + 16);
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
-        if (e != cudaSuccess) return (int)e;
-    }
-    FramesParams p;
-    p.succ = job.succ; p.n_frames = job.n_frames; p.k = job.k;
-    p.ucode = plan.ucode; p.slot_record = plan.slot_record;
-    p.n_slots = plan.n_slots; p.stride = plan.stride;
-    p.accum = job.accum;
-    if (p.n_frames == 0 || p.n_slots == 0) return 0;
-    const uint64_t tiles = (p.n_frames + FR_TPB * 32 - 1) / (FR_TPB * 32);
-    if (tiles > 0x7FFFFFFFull / 4096) return 801;                  // cudaErrorNotSupported
-    p.n_tiles = (uint32_t)tiles;
-    const uint32_t chunk_cap = (uint32_t)std::max<size_t>(1, std::min<size_t>(2048, (smem_max - fixed - 16) / per_slot));
-    // enough work items to fill the grid (two resident blocks per SM at most), each as large as allowed
-    const uint64_t want_items = (uint64_t)sm_count * 4;
-    uint64_t want_chunks = (want_items + tiles - 1) / tiles;
-    uint32_t chunk = (uint32_t)std::max<uint64_t>(1, (p.n_slots + want_chunks - 1) / want_chunks);
-    chunk = std::min(std::min(chunk, chunk_cap), p.n_slots);
-    p.chunk = chunk;
-    p.n_chunks = (p.n_slots + chunk - 1) / chunk;
-    const uint64_t items = tiles * p.n_chunks;
-    const uint32_t grid = (uint32_t)std::min<uint64_t>(items, (uint64_t)sm_count * 2);
-    const size_t smem = fixed + (size_t)chunk * per_slot + 16;
-    kern<<<grid, FR_TPB, smem, (cudaStream_t)stream>>>(p);
-    if (launches) ++*launches;
-    return (int)cudaGetLastError();
-}
-
 }  // namespace
 
+// Valuations per pass: 4 for n <= 9 (registers and spill columns still leave several resident
+// blocks), else 2, else 1 (variable-free programs have a single valuation).
 int launch_frames(const FramesJob &job, const SlicedPlan &plan, void *stream, uint32_t *launches) {
+    const uint32_t bits = job.k * job.n;
+    const int vb = (bits >= 2 && job.n <= 9) ? 4 : (bits >= 1 ? 2 : 1);
     switch (job.n) {
-#define FR_CASE(N) case N: return launch_frames_n<N>(job, plan, stream, launches);
+#define FR_CASE(N) \
+    case N: return vb == 4 ? launch_frames_##N##_v4(job, plan, stream, launches) \
+                 : vb == 2 ? launch_frames_##N##_v2(job, plan, stream, launches) \
+                           : launch_frames_##N##_v1(job, plan, stream, launches);
         FR_CASE(1) FR_CASE(2) FR_CASE(3) FR_CASE(4) FR_CASE(5) FR_CASE(6) FR_CASE(7) FR_CASE(8)
         FR_CASE(9) FR_CASE(10) FR_CASE(11) FR_CASE(12) FR_CASE(13) FR_CASE(14) FR_CASE(15) FR_CASE(16)
 #undef FR_CASE
     }
-    return 801;
+    return 801;   // cudaErrorNotSupported
 }
 
 int launch_frames_scalar(const FramesJob &job, const uint32_t *records, uint32_t n_list, void *stream,
