@@ -14,8 +14,8 @@
 // Work decomposition.  A work item is (tile of 32 x 32 = 1,024 consecutive frames) x (chunk of
 // programs).  The block reads the tile's masks from HBM once (2n bytes per frame), transposes them
 // on chip with warp ballots into a shared-memory edge table E[w*N+u][lane] (N*N*128 bytes: 32 KB
-// at n = 16), and its four warps then take the chunk's programs round-robin, every warp against
-// the same table: lane = group of 32 frames, so the table reads are conflict-free and the table is
+// at n = 16), and its four warps then take the chunk's programs from a shared work counter, every
+// warp against the same table: lane = group of 32 frames, so the table reads are conflict-free and the table is
 // shared by all warps (small footprint -> several resident blocks per SM).  One shared-memory word
 // feeds VB logic instructions: a pass evaluates VB consecutive valuations (VB = 4 or 2 when the
 // programs have variables), whose atoms differ only in compile-time bits.
@@ -174,10 +174,11 @@ struct FramesThread {
 template <int N, int VB>
 __global__ void __launch_bounds__(FR_TPB) scan_frames_kernel(FramesParams p) {
     extern __shared__ __align__(16) unsigned char smem[];
-    // [E: N*N x 32][valid: 32][spill: spill_slots*N*VB x TPB][ucode]
+    // [E: N*N x 32][valid: 32][next: 4][spill: spill_slots*N*VB x TPB][ucode]
     uint32_t *s_E = reinterpret_cast<uint32_t *>(smem);
     uint32_t *s_valid = s_E + N * N * 32;
-    uint32_t *s_S = s_valid + 32;
+    uint32_t *s_next = s_valid + 32;                    // work counter of the item (one word, padded to 4)
+    uint32_t *s_S = s_next + 4;
     uint16_t *s_ucode = reinterpret_cast<uint16_t *>(s_S + p.spill_slots * N * VB * FR_TPB);
 
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -209,6 +210,7 @@ __global__ void __launch_bounds__(FR_TPB) scan_frames_kernel(FramesParams p) {
             for (int w = 0; w < N; ++w) m[w] = valid ? (uint32_t)__ldg(p.succ + j * N + w) : 0u;
             const uint32_t vm = __ballot_sync(0xFFFFFFFFu, valid);
             if (lane == 0) s_valid[t] = vm;
+            if (threadIdx.x == 0) *s_next = 0u;
 #pragma unroll
             for (int w = 0; w < N; ++w)
 #pragma unroll
@@ -220,7 +222,12 @@ __global__ void __launch_bounds__(FR_TPB) scan_frames_kernel(FramesParams p) {
         __syncthreads();
 
         const uint32_t vmask = s_valid[lane];
-        for (uint32_t s = warp; s < nslots; s += FR_WARPS) {
+        // the chunk's programs go to whichever warp is free next (programs differ in length)
+        for (;;) {
+            uint32_t s = 0;
+            if (lane == 0) s = atomicAdd(s_next, 1u);
+            s = __shfl_sync(0xFFFFFFFFu, s, 0);
+            if (s >= nslots) break;
             const uint16_t *uc = s_ucode + s * p.stride;
             uint32_t cnt = 0, any = 0;
             for (uint32_t v0 = 0; v0 < nval; v0 += VB) {
@@ -255,13 +262,13 @@ int launch_frames_inst(const FramesJob &job, const SlicedPlan &plan, void *strea
     static int sm_count = 0, blocks_per_sm[FR_SPILL + 1] = {0, 0, 0, 0};
     auto kern = scan_frames_kernel<N, VB>;
     const uint32_t spill_slots = std::min<uint32_t>(FR_SPILL, plan.max_need > 0 ? plan.max_need - 1 : 0);
-    const size_t fixed = ((size_t)N * N * 32 + 32 + (size_t)spill_slots * N * VB * FR_TPB) * sizeof(uint32_t);
+    const size_t fixed = ((size_t)N * N * 32 + 36 + (size_t)spill_slots * N * VB * FR_TPB) * sizeof(uint32_t);
     const size_t slot_budget = 8 * 1024;
     if (!sm_count) {
         int dev = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return (int)e;
-        const size_t most = ((size_t)N * N * 32 + 32 + (size_t)FR_SPILL * N * VB * FR_TPB) * sizeof(uint32_t);
+        const size_t most = ((size_t)N * N * 32 + 36 + (size_t)FR_SPILL * N * VB * FR_TPB) * sizeof(uint32_t);
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(most + slot_budget));
         if (e != cudaSuccess) return (int)e;
         e = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
