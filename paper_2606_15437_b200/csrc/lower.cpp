@@ -365,6 +365,42 @@ uint32_t program_support(const uint8_t *code, uint32_t len) {
     return lw.support(lw.build(code, len));
 }
 
+// LOWER_FUSE: a load followed by a modal operator on the same slot becomes one fused micro-op.
+// LOWER_FUSE_BOOL also fuses a load into a Boolean operator with a leaf (measured slower on the
+// census corpus, so the kernels' lowering mode leaves it off).
+static void fuse_loads(std::vector<uint16_t> &uc, bool fuse_bool) {
+    std::vector<uint16_t> out;
+    out.reserve(uc.size());
+    auto swap_fn = [](uint32_t f) { return f == BF_ANDN ? (uint32_t)BF_NAND : f == BF_NAND ? (uint32_t)BF_ANDN : f; };
+    for (size_t i = 0; i < uc.size(); ++i) {
+        const uint32_t op = uc[i] & 0xFFu, arg = uc[i] >> 8;
+        if (i + 1 < uc.size()) {
+            const uint32_t op2 = uc[i + 1] & 0xFFu, arg2 = uc[i + 1] >> 8;
+            if (op < UC_BOOLV) {                                        // LOADV i, d
+                const uint32_t iv = op >> 2, d = op & 3u;
+                if (d == 0 && op2 == UC_BOX + d) { out.push_back((uint16_t)(UC_BOXV0 + iv)); ++i; continue; }
+                if (d == 0 && op2 == UC_DIA + d) { out.push_back((uint16_t)(UC_DIAV0 + iv)); ++i; continue; }
+                if (fuse_bool && op2 >= UC_BOOLL && op2 < UC_BOOL && ((op2 - UC_BOOLL) & 3u) == d) {   // f(p_i, leaf)
+                    const uint32_t f = (op2 - UC_BOOLL) >> 2;
+                    out.push_back((uint16_t)((UC_BOOLVL + f * 4 + d) | ((arg2 | (iv << 4)) << 8)));
+                    ++i; continue;
+                }
+            } else if (op >= UC_LOADL && op < UC_BOOLL) {               // LOADL leaf, d
+                const uint32_t d = op - UC_LOADL;
+                if (op2 == UC_BOX + d) { out.push_back((uint16_t)((UC_BOXL + d) | (arg << 8))); ++i; continue; }
+                if (op2 == UC_DIA + d) { out.push_back((uint16_t)((UC_DIAL + d) | (arg << 8))); ++i; continue; }
+                if (fuse_bool && op2 >= UC_BOOLV && op2 < UC_LOADL && ((op2 - UC_BOOLV) & 3u) == d) {  // f(leaf, p_i) = f'(p_i, leaf)
+                    const uint32_t y = op2 - UC_BOOLV, iv = (y >> 2) & 3u, f = swap_fn(y >> 4);
+                    out.push_back((uint16_t)((UC_BOOLVL + f * 4 + d) | ((arg | (iv << 4)) << 8)));
+                    ++i; continue;
+                }
+            }
+        }
+        out.push_back(uc[i]);
+    }
+    uc.swap(out);
+}
+
 bool lower_single(const uint8_t *code, uint32_t len, uint32_t mode, const uint8_t *rename, Lowered *out) {
     Lowerer lw;
     lw.mode = mode;
@@ -374,6 +410,7 @@ bool lower_single(const uint8_t *code, uint32_t len, uint32_t mode, const uint8_
     if (out->need > UC_DMAX) return false;
     int p = lw.emit(root, 0);
     lw.op(p ? UC_FIN_ANY : UC_FIN_ALL);
+    if (mode & LOWER_FUSE) fuse_loads(lw.out, (mode & LOWER_FUSE_BOOL) != 0);
     out->ucode = std::move(lw.out);
     out->n_modal = lw.n_modal;
     out->n_bool = lw.n_bool;
@@ -395,6 +432,7 @@ bool lower_pair(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, ui
     int pa = lw.emit(ra, 0);
     int pb = lw.emit(rb, 1);
     lw.op(pa == pb ? UC_FIN_XOR : UC_FIN_XNOR);
+    if (mode & LOWER_FUSE) fuse_loads(lw.out, (mode & LOWER_FUSE_BOOL) != 0);
     out->ucode = std::move(lw.out);
     out->n_modal = lw.n_modal;
     out->n_bool = lw.n_bool;

@@ -245,6 +245,77 @@ struct SlicedThread {
             for (int w = 0; w < N; ++w) D[dd][m][w] = r[w];
         }
     }
+    // ---- fused forms (ucode.h, LOWER_FUSE): the operand is read where it lives ----------------------
+    // D[0] <- box / dia p_I: the compile-time bits of the atom fold into the logic, and since the
+    // source is not D[0] the result needs no staging copy
+    template <int I, bool BOX> __device__ __forceinline__ void modal_var0() {
+        if (I >= C::K || (C::P_LEAF && I == 0)) return;
+#pragma unroll
+        for (int m = 0; m < M; ++m)
+#pragma unroll
+            for (int w = 0; w < N; ++w) {
+                uint32_t acc = BOX ? 0xFFFFFFFFu : 0u;
+#pragma unroll
+                for (int u = 0; u < N; ++u) {
+                    if (BOX) acc &= (atom(I, m, u) | ~edge(m, w, u));
+                    else acc |= (atom(I, m, u) & edge(m, w, u));
+                }
+                D[0][m][w] = acc;
+            }
+    }
+    // D[d] <- box / dia leaf; with one frame per thread the leaf and the edge masks are the same for
+    // all M words, so the N results are computed once
+    template <int d, bool BOX> __device__ __forceinline__ void modal_leaf(uint32_t l) {
+        if (d >= DMAX) return;
+        constexpr int dd = d < DMAX ? d : 0;
+        if (C::FRAME_PER_UNIT) {
+            uint32_t v[N], r[N];
+#pragma unroll
+            for (int u = 0; u < N; ++u) v[u] = leaf_word(l, 0, u);
+#pragma unroll
+            for (int w = 0; w < N; ++w) {
+                uint32_t acc = BOX ? 0xFFFFFFFFu : 0u;
+#pragma unroll
+                for (int u = 0; u < N; ++u) {
+                    if (BOX) acc &= (v[u] | ~edge(0, w, u));
+                    else acc |= (v[u] & edge(0, w, u));
+                }
+                r[w] = acc;
+            }
+#pragma unroll
+            for (int m = 0; m < M; ++m)
+#pragma unroll
+                for (int w = 0; w < N; ++w) D[dd][m][w] = r[w];
+        } else {
+#pragma unroll
+            for (int m = 0; m < M; ++m)
+#pragma unroll
+                for (int w = 0; w < N; ++w) {
+                    uint32_t acc = BOX ? 0xFFFFFFFFu : 0u;
+#pragma unroll
+                    for (int u = 0; u < N; ++u) {
+                        if (BOX) acc &= (leaf_word(l, m, u) | ~edge(m, w, u));
+                        else acc |= (leaf_word(l, m, u) & edge(m, w, u));
+                    }
+                    D[dd][m][w] = acc;
+                }
+        }
+    }
+    // D[d] <- F(p_i, leaf), arg = leaf | i << 4
+    template <int d, int F> __device__ __forceinline__ void bool_var_leaf(uint32_t arg) {
+        if (d >= DMAX) return;
+        constexpr int dd = d < DMAX ? d : 0;
+        const uint32_t l = arg & 15u, iv = arg >> 4;
+#pragma unroll
+        for (int i = 0; i < C::K; ++i) {
+            if ((C::P_LEAF && i == 0) || iv != (uint32_t)i) continue;
+#pragma unroll
+            for (int m = 0; m < M; ++m)
+#pragma unroll
+                for (int w = 0; w < N; ++w)
+                    D[dd][m][w] = bool_fn<F>(atom(i, m, w), leaf_word(l, C::FRAME_PER_UNIT ? 0 : m, w));
+        }
+    }
     template <int d, int F> __device__ __forceinline__ void boolean() {
         if (d + 1 >= DMAX) return;
         constexpr int dd = d + 1 < DMAX ? d : 0, d1 = d + 1 < DMAX ? d + 1 : 1;
@@ -287,10 +358,10 @@ struct SlicedThread {
             const uint32_t arg = nxt >> 8;
             if (op >= (uint32_t)UC_FIN_ALL && op <= (uint32_t)UC_FIN_XNOR) break;          // FIN
             nxt = uc[++pc];          // prefetch (the slot's stride leaves an entry after FIN)
-            switch (op) {
 #define KRIPKE_CASE4(base, call) \
     case (base) + 0: call(0); break; case (base) + 1: call(1); break; \
     case (base) + 2: call(2); break; case (base) + 3: call(3); break;
+            switch (op) {
 #define KRIPKE_CASE3(base, call) \
     case (base) + 0: call(0); break; case (base) + 1: call(1); break; \
     case (base) + 2: call(2); break;
@@ -339,6 +410,25 @@ struct SlicedThread {
                 KRIPKE_CASE4(UC_BOX, BOXD)
                 KRIPKE_CASE4(UC_DIA, DIAD)
                 KRIPKE_CASE4(UC_LOADZ, LZ)
+                case UC_BOXV0 + 0: modal_var0<0, true>(); break;  case UC_BOXV0 + 1: modal_var0<1, true>(); break;
+                case UC_BOXV0 + 2: modal_var0<2, true>(); break;  case UC_BOXV0 + 3: modal_var0<3, true>(); break;
+                case UC_DIAV0 + 0: modal_var0<0, false>(); break; case UC_DIAV0 + 1: modal_var0<1, false>(); break;
+                case UC_DIAV0 + 2: modal_var0<2, false>(); break; case UC_DIAV0 + 3: modal_var0<3, false>(); break;
+#define BXL(d) modal_leaf<d, true>(arg)
+#define DXL(d) modal_leaf<d, false>(arg)
+#define BVL0(d) bool_var_leaf<d, 0>(arg)
+#define BVL1(d) bool_var_leaf<d, 1>(arg)
+#define BVL2(d) bool_var_leaf<d, 2>(arg)
+#define BVL3(d) bool_var_leaf<d, 3>(arg)
+                KRIPKE_CASE4(UC_BOXL, BXL) KRIPKE_CASE4(UC_DIAL, DXL)
+                KRIPKE_CASE4(UC_BOOLVL + 0, BVL0) KRIPKE_CASE4(UC_BOOLVL + 4, BVL1)
+                KRIPKE_CASE4(UC_BOOLVL + 8, BVL2) KRIPKE_CASE4(UC_BOOLVL + 12, BVL3)
+#undef BXL
+#undef DXL
+#undef BVL0
+#undef BVL1
+#undef BVL2
+#undef BVL3
 #undef LV0
 #undef LV1
 #undef LV2

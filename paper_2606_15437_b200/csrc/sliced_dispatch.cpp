@@ -57,9 +57,12 @@ uint32_t sliced_row(uint32_t n, uint32_t k, uint32_t cls, uint32_t need) {
 }
 
 uint32_t sliced_lower_mode(uint32_t n, uint32_t k) {
+    // tuning aid / test hook: KRIPKE_FUSE_BOOL=1 also fuses loads into Boolean operators (UC_BOOLVL)
+    static const char *fb_env = std::getenv("KRIPKE_FUSE_BOOL");
+    const uint32_t fuse = LOWER_FUSE | ((fb_env && std::atoi(fb_env)) ? (uint32_t)LOWER_FUSE_BOOL : 0u);
     for (const Row &r : kRows)
         if (r.n == n && r.k == k)
-            return LOWER_LEAF_DEAD | ((frame_per_unit(r) && k >= 1 && n <= 5) ? LOWER_LEAF_P : 0u);
+            return fuse | LOWER_LEAF_DEAD | ((frame_per_unit(r) && k >= 1 && n <= 5) ? LOWER_LEAF_P : 0u);
     return 0;
 }
 

@@ -12,6 +12,9 @@
 //   * modal operators applied to a constant or to the in-word variable p_0: box F ("dead end"),
 //     dia T, box p_0, dia p_0 (and their negations) depend on the frame only, so the kernel computes
 //     them once per scan unit as "derived leaves" and every program reads them like atoms.
+//   * loads that feed the next operator directly (LOWER_FUSE): "load q; box" becomes one micro-op
+//     that reads q where it lives - one dispatch and one register copy fewer, and the compile-time
+//     bits of q fold into the logic;
 // The last micro-op is one of the FIN ops and produces, per 32-model word, the mask of models that
 // refute the formula (or distinguish the pair).
 #pragma once
@@ -27,7 +30,10 @@ enum : uint8_t { LEAF_P = 0, LEAF_DEAD = 1, LEAF_BOXP = 2, LEAF_DIAP = 3, LEAF_C
 // lowering modes (which derived leaves the target kernel instantiation provides)
 enum : uint32_t {
     LOWER_LEAF_DEAD = 1u << 0,   // box F / dia T as a leaf
-    LOWER_LEAF_P = 1u << 1       // p_0, box p_0, dia p_0 as leaves (p_0 lies inside the 32-model word)
+    LOWER_LEAF_P = 1u << 1,      // p_0, box p_0, dia p_0 as leaves (p_0 lies inside the 32-model word)
+    LOWER_FUSE = 1u << 2,        // fold a load into the modal operator that follows it (fused ops below)
+    LOWER_FUSE_BOOL = 1u << 3    // also into a Boolean operator with a leaf (UC_BOOLVL); measured slower on
+                                 // the census corpus, so no kernel asks for it by default
 };
 
 // Boolean functions of (slot value a, operand b); the lowering picks one by the two polarities
@@ -45,7 +51,13 @@ enum : uint8_t {
     UC_FIN_ANY = 125, // refuted =   D0[0] | ... | D0[n-1]       truth set = ~D0
     UC_FIN_XOR = 126, // differ  = OR_w (D0[w] ^ D1[w])          pair, equal polarities
     UC_FIN_XNOR = 127,// differ  = OR_w ~(D0[w] ^ D1[w])         pair, opposite polarities
-    UC_LOADZ = 128    // + d                : D[d] <- all-false
+    UC_LOADZ = 128,   // + d                : D[d] <- all-false
+    // fused forms (LOWER_FUSE): the operand is read where it lives instead of being loaded first
+    UC_BOXV0 = 132,   // + i                : D[0] <- box p_i
+    UC_DIAV0 = 136,   // + i                : D[0] <- dia p_i
+    UC_BOXL = 140,    // + d   (arg = leaf) : D[d] <- box leaf
+    UC_DIAL = 144,    // + d   (arg = leaf) : D[d] <- dia leaf
+    UC_BOOLVL = 148   // + f*4 + d (arg = leaf | i << 4) : D[d] <- f(p_i, leaf)   (LOWER_FUSE_BOOL)
 };
 
 }  // namespace kripke

@@ -488,3 +488,31 @@ def test_variable_support_reduction_is_exact(kb, vol):
     want = vol.census(sc, so, 4, 3, K, 100, 64)
     same(run(kb, sub, 4, 3, K, 100, 64), want, "k=3 reduced")
     same(run(kb, sub, 4, 3, K, 100, 64, flags=kb.FULL_SWEEP), want, "k=3 full")
+
+
+def test_fused_boolean_lowering_in_a_subprocess(vol):
+    """The UC_BOOLVL micro-op (a load fused into a Boolean operator) is off by default because it
+    measured slower; KRIPKE_FUSE_BOOL=1 turns it on.  Same C1 / C2-sample parity with it on."""
+    import subprocess
+    import sys
+    script = r'''
+import numpy as np
+import workloads as W
+from oracle import volume as V
+from paper_2606_15437_b200 import binding as kb
+V.build()
+for progs, n, k, count in ((W.corpus_c1(), 3, 2, 512), (W.corpus_c2()[:600], 5, 2, 4096)):
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, k)
+    for cls in (0, 1):
+        cnt = min(count, kb.class_size(n, cls))
+        got = kb.unpack(*kb.eval_batch_range(h, n, k, cls, 0, cnt))
+        want = V.census(code, offs, n, k, cls, 0, cnt)
+        for key in ("models", "frames", "wit_f", "wit_v", "wit_w"):
+            assert (np.asarray(got[key]).astype(np.uint64) == np.asarray(want[key]).astype(np.uint64)).all(), (n, cls, key)
+print("fused-bool parity ok")
+'''
+    env = dict(os.environ, KRIPKE_FUSE_BOOL="1")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    res = subprocess.run([sys.executable, "-c", script], cwd=root, env=env, capture_output=True, text=True, timeout=900)
+    assert res.returncode == 0 and "fused-bool parity ok" in res.stdout, res.stdout + res.stderr
