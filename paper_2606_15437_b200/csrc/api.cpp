@@ -445,9 +445,16 @@ int build_scan_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_
             for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v)
                 if ((support[r] >> v) & 1u) rename[v] = next++;
             if (g == k) for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v) rename[v] = (uint8_t)v;   // full sweep: as written
-            fits[i] = pairs ? lower_pair(prog(pairs[2 * r]), plen(pairs[2 * r]), prog(pairs[2 * r + 1]),
-                                         plen(pairs[2 * r + 1]), mode, rename, &low[i])
-                            : lower_single(prog(r), plen(r), mode, rename, &low[i]);
+            auto lower = [&](uint32_t m) {
+                return pairs ? lower_pair(prog(pairs[2 * r]), plen(pairs[2 * r]), prog(pairs[2 * r + 1]),
+                                          plen(pairs[2 * r + 1]), m, rename, &low[i])
+                             : lower_single(prog(r), plen(r), m, rename, &low[i]);
+            };
+            fits[i] = lower(mode);
+            if (fits[i] && (mode & LOWER_FUSE) && !sliced_fuses(n, g, (uint32_t)low[i].need)) {
+                low[i] = Lowered();
+                fits[i] = lower(mode & ~(uint32_t)(LOWER_FUSE | LOWER_FUSE_BOOL));
+            }
         }
         HostPlan hp;
         build_plan(low, fits, &hp);

@@ -77,6 +77,8 @@ bool sliced_select(uint32_t n, uint32_t k, uint32_t cls, uint32_t need, uint64_t
 uint32_t sliced_row(uint32_t n, uint32_t k, uint32_t cls, uint32_t need);
 // LOWER_LEAF_* flags of the derived leaves the instantiations for this shape provide (0 = no shape).
 uint32_t sliced_lower_mode(uint32_t n, uint32_t k);
+// Should programs of this need class be lowered with LOWER_FUSE?
+bool sliced_fuses(uint32_t n, uint32_t k, uint32_t need);
 // Enqueue the sliced scan; returns a cudaError_t as int and the number of kernel launches.
 int launch_sliced(const ScanJob &job, const SlicedPlan &plan, void *stream, uint32_t *launches);
 // Enqueue the scalar (Algorithm 1) scan over the records listed in `records` (device, or null = all).

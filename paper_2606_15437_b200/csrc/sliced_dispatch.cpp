@@ -66,6 +66,13 @@ uint32_t sliced_lower_mode(uint32_t n, uint32_t k) {
     return 0;
 }
 
+// Fused micro-ops (LOWER_FUSE) pay off on the one-slot instantiations only: programs
+// whose need class runs on a kernel with more slots are lowered without them.
+bool sliced_fuses(uint32_t n, uint32_t k, uint32_t need) {
+    const Row *r = find(n, k, KRIPKE_CLASS_K, need);
+    return r && r->dmax == 1;
+}
+
 int launch_sliced(const ScanJob &job, const SlicedPlan &plan, void *stream, uint32_t *launches) {
     // group-per-unit shapes need the range aligned to the unit of the row selected for need 1; every
     // row of one (n, k) uses the same unit size
