@@ -205,6 +205,40 @@ int kripke_distinguish_pairs_frames(const kripke_programs_t *programs, const uin
                                     uint32_t flags, kripke_count_t *counts_out,
                                     kripke_witness_t *witness_out, void *stream);
 
+/* Correspondence recovery (Table 9 at P:366-376): "per-formula valid-frame bitmaps ...
+ * matched against a first-order condition library".  A bitmap has one bit per class frame of the
+ * range [frame_begin, frame_begin + frame_count): bit (j % 32) of word (j / 32) is frame
+ * frame_begin + j in class order; words = ceil(frame_count / 32); bits past the range are 0.
+ *
+ * kripke_validity_bitmap: bit = 1 iff the formula is VALID on the frame (no valuation of the n_vars
+ *   variables and no world falsify it).  bitmap_out: DEVICE, n_formulas * words uint32,
+ *   formula-major.  (The complement of what refuting_frames counts, per frame.)
+ * kripke_condition_bitmap: bit = 1 iff the frame satisfies the first-order condition.  bitmap_out:
+ *   DEVICE, words uint32.
+ * kripke_match_bitmaps: match_out[r] = least l with bitmaps[r] == library[l] word for word, or
+ *   UINT32_MAX.  bitmaps: DEVICE n_records * words; library: DEVICE n_library * words; match_out:
+ *   DEVICE n_records. */
+enum {
+    KRIPKE_COND_REFLEXIVE = 0,            /* T:  box p -> p                                       */
+    KRIPKE_COND_TRANSITIVE = 1,           /* 4:  box p -> box box p                               */
+    KRIPKE_COND_SYMMETRIC = 2,            /* B:  p -> box dia p                                   */
+    KRIPKE_COND_SERIAL = 3,               /* D:  box p -> dia p                                   */
+    KRIPKE_COND_EUCLIDEAN = 4,            /* 5:  dia p -> box dia p                               */
+    KRIPKE_COND_PARTIALLY_FUNCTIONAL = 5, /* CD: dia p -> box p                                   */
+    KRIPKE_COND_DENSE = 6,                /* C4: box box p -> box p                               */
+    KRIPKE_COND_CONFLUENT = 7,            /* G:  dia box p -> box dia p                           */
+    KRIPKE_COND_COUNT = 8
+};
+int kripke_validity_bitmap(const kripke_programs_t *programs, uint32_t n_worlds, uint32_t n_vars,
+                           uint32_t frame_class, uint64_t frame_begin, uint64_t frame_count,
+                           uint32_t *bitmap_out, void *stream);
+int kripke_condition_bitmap(uint32_t n_worlds, uint32_t condition, uint32_t frame_class,
+                            uint64_t frame_begin, uint64_t frame_count, uint32_t *bitmap_out,
+                            void *stream);
+int kripke_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words,
+                         const uint32_t *library, uint32_t n_library, uint32_t *match_out,
+                         void *stream);
+
 /* End-to-end convenience with HOST buffers only: create + eval over the full class + copy the
  * results back + destroy, synchronously (this is what bench.py's "e2e" figure times). */
 int kripke_eval_batch_host(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,

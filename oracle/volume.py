@@ -55,6 +55,9 @@ def _load():
         lib.kov_census_relations.argtypes = [u8p, u32p, ctypes.c_uint32, u32p, ctypes.c_uint32,
                                              ctypes.c_int, ctypes.c_int, u8p, ctypes.c_uint64,
                                              u64p, u64p, u64p, u32p, u32p, ctypes.c_int]
+        lib.kov_validity_list.restype = ctypes.c_int
+        lib.kov_validity_list.argtypes = [u8p, u32p, ctypes.c_uint32, ctypes.c_int, ctypes.c_int, u64p,
+                                          ctypes.c_uint64, u8p, ctypes.c_int]
         lib.kov_max_threads.restype = ctypes.c_int
         lib.kov_orbits.restype = ctypes.c_int64
         lib.kov_orbits.argtypes = [ctypes.c_int, u64p, u64p, ctypes.c_uint64]
@@ -190,6 +193,32 @@ def census(code, offsets, n, k, cls=CLASS_K, frame_begin=0, frame_count=None, pa
             frame_count = len(allf) - frame_begin
         frames = allf[frame_begin:frame_begin + frame_count]
     return census_list(code, offsets, n, k, frames, None, pairs, threads)
+
+
+def validity(code, offsets, n, k, cls=CLASS_K, frame_begin=0, frame_count=None, threads=0):
+    """uint8 array [B, frame_count]: 1 iff formula b is valid on the class frame frame_begin + i
+    (class order = ascending f): no valuation and no world falsify it."""
+    code = np.ascontiguousarray(code, dtype=np.uint8)
+    offsets = np.ascontiguousarray(offsets, dtype=np.uint32)
+    if cls == CLASS_K:
+        total = 1 << (n * n)
+        if frame_count is None:
+            frame_count = total - frame_begin
+        frames = np.arange(frame_begin, frame_begin + frame_count, dtype=np.uint64)
+    else:
+        allf = class_frames(n, cls)
+        if frame_count is None:
+            frame_count = len(allf) - frame_begin
+        frames = np.ascontiguousarray(allf[frame_begin:frame_begin + frame_count], dtype=np.uint64)
+    B = len(offsets) - 1
+    out = np.zeros((B, len(frames)), np.uint8)
+    if len(frames) == 0 or B == 0:
+        return out
+    rc = _load().kov_validity_list(_p(code, ctypes.c_uint8), _p(offsets, ctypes.c_uint32), B, n, k,
+                                   _p(frames, ctypes.c_uint64), len(frames), _p(out, ctypes.c_uint8), threads)
+    if rc:
+        raise ValueError("kov_validity_list failed")
+    return out
 
 
 def signatures(code, offsets, max_n: int, k: int):

@@ -560,3 +560,34 @@ int kov_census_relations(const u8 *code, const uint32_t *offs, uint32_t B,
     free(acc_m); free(acc_f); free(first);
     return bad ? -1 : 0;
 }
+
+/* ---- frame validity per frame ("valid on a frame"; PAPER.md:358-380 correspondence) ----
+ * out[b * nframes + i] = 1 iff formula b is valid on frame frames[i]: no valuation of the k variables
+ * and no world falsify it.  Same plain evaluation as kov_census_list. */
+int kov_validity_list(const u8 *code, const uint32_t *offs, uint32_t B, int n, int k,
+                      const uint64_t *frames, uint64_t nframes, u8 *out, int nthreads) {
+    if (n < 1 || n > MAXN || k < 0 || k > MAXVARS || k * n > 30) return -1;
+    const uint64_t nval = 1ull << (k * n);
+    int bad = 0;
+#ifdef _OPENMP
+    if (nthreads <= 0) nthreads = omp_get_max_threads();
+#else
+    nthreads = 1;
+#endif
+#pragma omp parallel for num_threads(nthreads) schedule(dynamic, 16)
+    for (uint64_t i = 0; i < nframes; ++i) {
+        u8 R[MAXN][MAXN], V[MAXVARS][MAXN], t[MAXN];
+        decode_frame(n, frames[i], R);
+        for (uint32_t b = 0; b < B; ++b) {
+            int valid = 1;
+            for (uint64_t v = 0; v < nval && valid; ++v) {
+                decode_valuation(n, k, v, V);
+                if (eval_program(code + offs[b], offs[b + 1] - offs[b], n, R, V, t)) bad = 1;
+                for (int w = 0; w < n; ++w)
+                    if (!t[w]) valid = 0;
+            }
+            out[(size_t)b * nframes + i] = (u8)valid;
+        }
+    }
+    return bad ? -1 : 0;
+}

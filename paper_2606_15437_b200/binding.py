@@ -33,6 +33,7 @@ EXPORTS = [
     "kripke_calibrate_int32", "kripke_debug_lower", "kripke_witness_to_keys", "kripke_keys_to_witness",
     "kripke_minimal_refutation", "kripke_pairs_separation", "kripke_debug_lower_wf",
     "kripke_eval_frames", "kripke_distinguish_pairs_frames",
+    "kripke_validity_bitmap", "kripke_condition_bitmap", "kripke_match_bitmaps",
 ]
 
 
@@ -85,6 +86,9 @@ def load():
     lib.kripke_keys_to_witness.argtypes = [vp, u32, u32, u32, vp, vp]
     lib.kripke_debug_lower.argtypes = [u8p, u32, u8p, u32, u32, u32, u8p, u32, ctypes.POINTER(u32)]
     lib.kripke_debug_lower_wf.argtypes = [u8p, u32, u32, u8p, u32]
+    lib.kripke_validity_bitmap.argtypes = [vp, u32, u32, u32, u64, u64, vp, vp]
+    lib.kripke_condition_bitmap.argtypes = [u32, u32, u32, u64, u64, vp, vp]
+    lib.kripke_match_bitmaps.argtypes = [vp, u32, u64, vp, u32, vp, vp]
     lib.kripke_eval_frames.argtypes = [vp, u32, u32, vp, u64, u64, u32, vp, vp, vp]
     lib.kripke_distinguish_pairs_frames.argtypes = [vp, u32p, u32, u32, u32, vp, u64, u64, u32, vp, vp, vp]
     for name in EXPORTS:
@@ -246,6 +250,57 @@ def distinguish_pairs_frames(programs: Programs, pairs, n_worlds: int, n_vars: i
                                                   counts_out.data_ptr(), witness_out.data_ptr(),
                                                   _stream(stream)), "kripke_distinguish_pairs_frames")
     return counts_out, witness_out
+
+
+COND = {"reflexive": 0, "transitive": 1, "symmetric": 2, "serial": 3, "euclidean": 4,
+        "partially_functional": 5, "dense": 6, "confluent": 7}
+
+
+def validity_bitmap(programs: Programs, n_worlds: int, n_vars: int, frame_class: int, frame_begin: int,
+                    frame_count: int, bitmap_out=None, stream=None):
+    """kripke_validity_bitmap.  Returns an int32 CUDA tensor (B, ceil(frame_count/32)) of bit words."""
+    import torch
+    words = (frame_count + 31) // 32
+    if bitmap_out is None:
+        bitmap_out = torch.zeros((programs.n_formulas, words), dtype=torch.int32, device="cuda")
+    assert bitmap_out.is_cuda and bitmap_out.is_contiguous() and bitmap_out.numel() >= programs.n_formulas * words
+    _check(load().kripke_validity_bitmap(programs._h, n_worlds, n_vars, frame_class, frame_begin, frame_count,
+                                         bitmap_out.data_ptr(), _stream(stream)), "kripke_validity_bitmap")
+    return bitmap_out
+
+
+def condition_bitmap(n_worlds: int, condition: int, frame_class: int, frame_begin: int, frame_count: int,
+                     bitmap_out=None, stream=None):
+    import torch
+    words = (frame_count + 31) // 32
+    if bitmap_out is None:
+        bitmap_out = torch.zeros((words,), dtype=torch.int32, device="cuda")
+    assert bitmap_out.is_cuda and bitmap_out.is_contiguous() and bitmap_out.numel() >= words
+    _check(load().kripke_condition_bitmap(n_worlds, condition, frame_class, frame_begin, frame_count,
+                                          bitmap_out.data_ptr(), _stream(stream)), "kripke_condition_bitmap")
+    return bitmap_out
+
+
+def match_bitmaps(bitmaps, library, match_out=None, stream=None):
+    """kripke_match_bitmaps: bitmaps (R, words), library (L, words) int32 CUDA tensors -> int32 (R,)
+    index of the first equal library row, -1 if none."""
+    import torch
+    assert bitmaps.is_cuda and library.is_cuda and bitmaps.is_contiguous() and library.is_contiguous()
+    n_records, words = bitmaps.shape
+    assert library.shape[1] == words
+    if match_out is None:
+        match_out = torch.empty((n_records,), dtype=torch.int32, device="cuda")
+    _check(load().kripke_match_bitmaps(bitmaps.data_ptr(), n_records, words, library.data_ptr(), library.shape[0],
+                                       match_out.data_ptr(), _stream(stream)), "kripke_match_bitmaps")
+    return match_out
+
+
+def bits_to_bool(bitmap, count: int):
+    """int32 bit words (..., words) (torch or numpy) -> numpy bool array (..., count)."""
+    a = bitmap.cpu().numpy() if hasattr(bitmap, "cpu") else np.asarray(bitmap)
+    a = np.ascontiguousarray(a).view(np.uint32)
+    bits = (a[..., :, None] >> np.arange(32, dtype=np.uint32)) & 1
+    return bits.reshape(a.shape[:-1] + (-1,))[..., :count].astype(bool)
 
 
 def minimal_refutation(programs: Programs, n_vars: int, frame_class: int, n_max: int,

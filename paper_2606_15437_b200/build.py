@@ -30,6 +30,7 @@ UNITS = [
     ("scan_scalar", "scan_scalar.cu", []),
     ("calibrate", "calibrate.cu", []),
     ("scan_frames", "scan_frames.cu", []),
+    ("bitmaps", "bitmaps.cu", []),
     ("wf_dispatch", "wf_dispatch.cpp", []),
 ] + [(f"scan_sliced_inst{g}", "scan_sliced_inst.cu", [f"-DKRIPKE_INST_GROUP={g}"]) for g in range(4)] \
   + [(f"scan_wf_inst{g}", "scan_wf_inst.cu", [f"-DKRIPKE_WF_INST={g}"]) for g in range(5)] \

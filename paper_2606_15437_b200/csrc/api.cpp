@@ -591,6 +591,52 @@ int run_frames(kripke_programs *h, const DevicePlan &dp, const uint32_t *d_pairs
 
 extern "C" {
 
+int kripke_validity_bitmap(const kripke_programs_t *programs, uint32_t n_worlds, uint32_t n_vars,
+                           uint32_t frame_class, uint64_t frame_begin, uint64_t frame_count,
+                           uint32_t *bitmap_out, void *stream) {
+    if (!programs) return KRIPKE_EINVAL;
+    const kripke_programs *h = programs;
+    if (n_worlds < 1 || n_worlds > KRIPKE_MAX_WORLDS || n_vars != h->n_vars || frame_class > KRIPKE_CLASS_S5)
+        return KRIPKE_EINVAL;
+    if (n_worlds * n_worlds + n_vars * n_worlds > KRIPKE_MAX_MODEL_BITS) return KRIPKE_EUNSUPPORTED;
+    uint64_t csize = 0;
+    int rc = class_size(n_worlds, frame_class, &csize);
+    if (rc) return rc;
+    if (frame_begin > csize || frame_count > csize - frame_begin) return KRIPKE_EINVAL;
+    if (frame_count && h->n_formulas && !bitmap_out) return KRIPKE_EINVAL;
+    ScanJob job;
+    job.n = n_worlds; job.k = n_vars; job.cls = frame_class;
+    job.frame_begin = frame_begin; job.frame_count = frame_count;
+    if ((rc = class_table_device(n_worlds, frame_class, &job.class_table))) return rc;
+    job.code = h->d_code; job.offsets = h->d_offsets; job.n_formulas = h->n_formulas;
+    job.pairs = nullptr; job.n_records = h->n_formulas; job.accum = nullptr;
+    int e = launch_validity_bitmap(job, bitmap_out, stream);
+    return e ? cuda_fail(e) : KRIPKE_OK;
+}
+
+int kripke_condition_bitmap(uint32_t n_worlds, uint32_t condition, uint32_t frame_class, uint64_t frame_begin,
+                            uint64_t frame_count, uint32_t *bitmap_out, void *stream) {
+    if (n_worlds < 1 || n_worlds > KRIPKE_MAX_WORLDS || condition >= KRIPKE_COND_COUNT || frame_class > KRIPKE_CLASS_S5)
+        return KRIPKE_EINVAL;
+    uint64_t csize = 0;
+    int rc = class_size(n_worlds, frame_class, &csize);
+    if (rc) return rc;
+    if (frame_begin > csize || frame_count > csize - frame_begin) return KRIPKE_EINVAL;
+    if (frame_count && !bitmap_out) return KRIPKE_EINVAL;
+    const uint64_t *table = nullptr;
+    if ((rc = class_table_device(n_worlds, frame_class, &table))) return rc;
+    int e = launch_condition_bitmap(n_worlds, condition, frame_class, table, frame_begin, frame_count, bitmap_out, stream);
+    return e ? cuda_fail(e) : KRIPKE_OK;
+}
+
+int kripke_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words, const uint32_t *library,
+                         uint32_t n_library, uint32_t *match_out, void *stream) {
+    if (n_records && (!match_out || (words && !bitmaps))) return KRIPKE_EINVAL;
+    if (n_library && words && !library) return KRIPKE_EINVAL;
+    int e = launch_match_bitmaps(bitmaps, n_records, words, library, n_library, match_out, stream);
+    return e ? cuda_fail(e) : KRIPKE_OK;
+}
+
 int kripke_eval_frames(const kripke_programs_t *programs, uint32_t n_worlds, uint32_t n_vars,
                        const uint16_t *succ, uint64_t n_frames, uint64_t index_base, uint32_t flags,
                        kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream) {

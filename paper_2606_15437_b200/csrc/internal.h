@@ -129,6 +129,13 @@ int launch_frames_scalar(const FramesJob &job, const uint32_t *records, uint32_t
 int launch_frames_finish(const FramesJob &job, bool accumulate, kripke_count_t *counts_out,
                          kripke_witness_t *witness_out, void *stream);
 
+// ---- correspondence recovery (bitmaps.cu) ------------------------------------------------------
+int launch_validity_bitmap(const ScanJob &job, uint32_t *bitmap_out, void *stream);
+int launch_condition_bitmap(uint32_t n, uint32_t cond, uint32_t cls, const uint64_t *class_table, uint64_t begin,
+                            uint64_t count, uint32_t *bitmap_out, void *stream);
+int launch_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words, const uint32_t *library,
+                         uint32_t n_library, uint32_t *match_out, void *stream);
+
 // Zero the accumulators; finish: turn accumulators into counts / witnesses (handles ACCUMULATE).
 int launch_init(Accum *accum, uint32_t n_records, void *stream);
 int launch_finish(const ScanJob &job, bool accumulate, kripke_count_t *counts_out,

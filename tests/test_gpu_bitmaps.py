@@ -1,0 +1,103 @@
+"""Parity of the correspondence-recovery path (kripke_validity_bitmap, kripke_condition_bitmap,
+kripke_match_bitmaps; Table 9 at P:366-376) with the oracle: bit-exact bitmaps.
+"""
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+K, T, S4, S5 = 0, 1, 2, 3
+AX = {name: W.to_postfix(t) for name, t in W.named_axioms().items()}
+PAIRS = [("T", "reflexive"), ("4", "transitive"), ("B", "symmetric"), ("D", "serial"), ("5", "euclidean"),
+         ("CD", "partially_functional"), ("C4", "dense"), ("G", "confluent")]
+
+
+@pytest.fixture(scope="module")
+def kb():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    from paper_2606_15437_b200 import binding
+    binding.load()
+    return binding
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4])
+def test_condition_bitmaps_equal_the_oracle(kb, vol, n):
+    total = 1 << (n * n)
+    for name, cid in kb.COND.items():
+        got = kb.bits_to_bool(kb.condition_bitmap(n, cid, K, 0, total), total)
+        assert (got == vol.condition_bitmap(n, name).astype(bool)).all(), name
+    # a class range with a ragged tail: reflexive frames, positions [5, 5 + count)
+    tf = vol.class_frames(n, T)
+    if len(tf) > 8:
+        count = len(tf) - 7
+        got = kb.bits_to_bool(kb.condition_bitmap(n, kb.COND["transitive"], T, 5, count), count)
+        want = vol.condition_bitmap(n, "transitive").astype(bool)[tf[5:5 + count].astype(np.int64)]
+        assert (got == want).all()
+
+
+def test_n5_condition_counts(kb, vol):
+    """Closed forms at n = 5: reflexive 2^20, symmetric 2^15, serial 31^5, partially
+    functional 6^5, transitive 154,303 (OEIS A006905); the rest against the oracle's count."""
+    total = 1 << 25
+    want = {"reflexive": 1 << 20, "symmetric": 1 << 15, "serial": 31 ** 5, "partially_functional": 6 ** 5,
+            "transitive": 154303}
+    for name, cid in kb.COND.items():
+        bm = kb.condition_bitmap(5, cid, K, 0, total).cpu().numpy().view(np.uint32)
+        cnt = int(np.unpackbits(bm.view(np.uint8)).sum())
+        assert cnt == want.get(name, vol.count_condition(5, name)), name
+
+
+@pytest.mark.parametrize("n,cls", [(3, K), (4, K), (4, T), (4, S4), (4, S5), (2, K)])
+def test_validity_bitmaps_equal_the_oracle(kb, vol, n, cls):
+    progs = W.corpus_c2(300) + [AX[a] for a, _ in PAIRS] + [AX["K"], AX["M"]]
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 2)
+    size = kb.class_size(n, cls)
+    for begin, count in ((0, size), (3, max(0, size - 10))):
+        if count <= 0:
+            continue
+        got = kb.bits_to_bool(kb.validity_bitmap(h, n, 2, cls, begin, count), count)
+        want = vol.validity(code, offs, n, 2, cls, begin, count).astype(bool)
+        assert got.shape == want.shape and (got == want).all(), (n, cls, begin)
+    # consistency with the census: valid frames = class size - refuting_frames
+    full = kb.bits_to_bool(kb.validity_bitmap(h, n, 2, cls, 0, size), size)
+    cen = kb.unpack(*kb.eval_batch_range(h, n, 2, cls, 0, size))
+    assert (full.sum(axis=1) == size - cen["frames"].astype(np.int64)).all()
+
+
+def test_table9_is_recovered_on_the_gpu(kb, vol):
+    """Table 9: every Sahlqvist axiom's validity bitmap over all 65,536 four-world frames matches its
+    own first-order correspondent in the library and no other; McKinsey's M matches none;
+    K, p -> p match nothing in the library of proper conditions; corpus formulas that match a
+    condition are re-checked against the oracle's bitmap of that condition."""
+    import torch
+    n, total = 4, 1 << 16
+    names = list(kb.COND)
+    lib = torch.stack([kb.condition_bitmap(n, kb.COND[c], K, 0, total) for c in names])
+    progs = [AX[a] for a, _ in PAIRS] + [AX["M"], AX["K"], W.to_postfix(W.parse("p -> p"))] + W.corpus_c2(400)
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 2)
+    bm = kb.validity_bitmap(h, n, 2, K, 0, total)
+    match = kb.match_bitmaps(bm, lib).cpu().numpy()
+    for i, (_, cond) in enumerate(PAIRS):
+        assert match[i] == names.index(cond)
+    assert match[8] == -1 and match[9] == -1 and match[10] == -1
+    val = vol.validity(code, offs, n, 2)
+    for b in np.nonzero(match >= 0)[0]:
+        assert (val[b] == vol.condition_bitmap(n, names[match[b]])).all(), b
+    for b in np.nonzero(match < 0)[0][:50]:
+        assert not any((val[b] == vol.condition_bitmap(n, c)).all() for c in names), b
+
+
+def test_bitmap_argument_errors(kb):
+    h = kb.Programs(*W.pack_programs([AX["T"]]), 1)
+    with pytest.raises(kb.KripkeError) as e:
+        kb.validity_bitmap(h, 4, 1, K, 1 << 16, 1)
+    assert e.value.status == kb.EINVAL
+    with pytest.raises(kb.KripkeError) as e:
+        kb.condition_bitmap(4, 8, K, 0, 16)
+    assert e.value.status == kb.EINVAL
+    assert kb.validity_bitmap(h, 4, 1, K, 0, 0).numel() == 0

@@ -332,3 +332,25 @@ def test_c_filter_consistency(vol):
         viaC = vol.census(code, offs, 3, 2, cls)
         for key in viaK:
             assert (viaK[key] == viaC[key]).all()
+
+
+@pytest.mark.parametrize("n", [2, 3, 4])
+def test_c_validity_bitmaps_are_the_correspondents(vol, n):
+    """Table 9 per frame: the validity bitmap of each Sahlqvist axiom over all K frames
+    equals the bitmap of its first-order correspondent; K, p -> p and T are valid everywhere, F and
+    p & ~p nowhere; validity = 'refuting_frames does not count this frame' of the census."""
+    names = ["T", "4", "B", "D", "5", "CD", "C4", "G"]
+    conds = ["reflexive", "transitive", "symmetric", "serial", "euclidean", "partially_functional", "dense",
+             "confluent"]
+    progs = [AX[a] for a in names] + [AX["K"], prog("p -> p"), prog("T"), prog("F"), prog("p & ~p")]
+    code, offs = W.pack_programs(progs)
+    val = vol.validity(code, offs, n, 2)
+    assert val.shape == (len(progs), 1 << (n * n))
+    for i, c in enumerate(conds):
+        assert (val[i] == vol.condition_bitmap(n, c)).all(), names[i]
+    assert val[8].all() and val[9].all() and val[10].all() and not val[11].any() and not val[12].any()
+    res = vol.census(code, offs, n, 2)
+    assert [int(x) for x in res["frames"]] == [int((1 << (n * n)) - v.sum()) for v in val]
+    # class order: the T-class bitmap is the K bitmap restricted to the reflexive frames
+    tf = vol.class_frames(n, T)
+    assert (vol.validity(code, offs, n, 2, T) == val[:, tf.astype(np.int64)]).all()
