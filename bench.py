@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py - formula-model evaluations/s of the n=5 census layer (BASELINE.json configs[2]).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c3|c3_small|c4|frames]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c3|c3_small|c4|frames|correspond]
 
 One step = one pass of the whole hot path (DESIGN.md steps H1-H6, H8's class loop) over the
 5,624-formula seeded corpus on every labelled frame of five worlds in K, T, S4 and S5 and every
@@ -464,13 +464,100 @@ def run_frames(args):
     }))
 
 
+def run_correspond(args):
+    """--workload correspond: correspondence recovery: validity
+    bitmaps of the whole 5,624-formula corpus over every K frame of 1..4 worlds, matched against the
+    library of eight first-order conditions (equal extensions at every size, Proposition 6); every
+    match is re-confirmed over all 2^25 five-world frames.  Reports the matched / constant / unmatched
+    split (paper, its own corpus: 220 / 2,798 / 2,606) and formula-frame validity tests per second."""
+    import torch
+    from paper_2606_15437_b200 import binding as kb
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    kb.load()
+    progs = W.corpus_c2()
+    B = len(progs)
+    h = kb.Programs(*W.pack_programs(progs), N_VARS)
+    names = list(kb.COND)
+    sizes = (1, 2, 3, 4)
+
+    def scan():
+        bms, libs = [], []
+        for n in sizes:
+            total = 1 << (n * n)
+            bms.append(kb.validity_bitmap(h, n, N_VARS, 0, 0, total))
+            libs.append(torch.stack([kb.condition_bitmap(n, kb.COND[c], 0, 0, total) for c in names]))
+        bm, lib = torch.cat(bms, dim=1).contiguous(), torch.cat(libs, dim=1).contiguous()
+        return bm, lib, kb.match_bitmaps(bm, lib)
+
+    for _ in range(max(1, min(args.warmup, 2))):
+        scan()
+    torch.cuda.synchronize()
+    clock = ClockSampler(0)
+    clock.start()
+    ts = []
+    for _ in range(max(1, args.steps)):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); bm, lib, match = scan(); b.record(); torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b) * 1e-3)
+    t = float(np.median(ts))
+    match = match.cpu().numpy()
+    bits = bm.cpu().numpy().view(np.uint32)
+    frames_total = sum(1 << (n * n) for n in sizes)
+    ones = np.unpackbits(bits.view(np.uint8), axis=1).sum(axis=1)
+    constant = (ones == 0) | (ones == frames_total)
+    matched = (match >= 0) & ~constant
+    # re-confirmation over all 2^25 five-world frames (P:380), on the bit-sliced kernels: Val_5(phi) = Ext_5(X)
+    # iff phi is refuted on no frame of Ext_5(X) (frame-list scan of the condition's own extension) and
+    # the census counts as many valid frames as |Ext_5(X)|
+    idx = np.nonzero(matched)[0]
+    t5, confirmed, ext5 = 0.0, 0, {}
+    if len(idx):
+        total5 = 1 << 25
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        h5 = kb.Programs(*W.pack_programs([progs[i] for i in idx]), N_VARS)
+        cen = kb.unpack(*kb.eval_batch(h5, 5, N_VARS, 0))
+        for j, cname in enumerate(names):
+            sel = np.nonzero(match[idx] == j)[0]
+            if len(sel) == 0:
+                continue
+            cb = kb.condition_bitmap(5, kb.COND[cname], 0, 0, total5)
+            _, n_set = kb.frames_from_bitmap(5, 0, 0, total5, cb, 0)
+            succ, _ = kb.frames_from_bitmap(5, 0, 0, total5, cb, n_set)
+            hj = kb.Programs(*W.pack_programs([progs[idx[i]] for i in sel]), N_VARS)
+            on_ext = kb.unpack(*kb.eval_frames(hj, 5, N_VARS, succ))
+            ok = (on_ext["frames"] == 0) & (cen["frames"][sel] == np.uint64(total5 - n_set))
+            confirmed += int(ok.sum())
+            ext5[cname] = n_set
+            hj.destroy()
+        b.record(); torch.cuda.synchronize()
+        t5 = a.elapsed_time(b) * 1e-3
+    clocks = clock.result()
+    print(json.dumps({
+        "metric": "formula-frame validity tests/sec (correspondence recovery, n <= 4)",
+        "value": B * frames_total / t, "unit": "formula-frames/s", "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "strong",
+        "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": f"correspondence recovery (PAPER.md:358-380): {B} seeded formulas x all K frames of "
+                               f"1..4 worlds ({frames_total} frames) x 8 first-order conditions",
+                   "split": {"matched": int(matched.sum()), "constant_extension": int(constant.sum()),
+                             "unmatched": int(B - matched.sum() - constant.sum())},
+                   "matched_by_condition": {names[j]: int((match[matched] == j).sum()) for j in range(len(names))},
+                   "reconfirmed_at_n5": {"formulas": int(len(idx)), "confirmed": confirmed, "seconds": t5,
+                                         "frames": 1 << 25, "extension_sizes": ext5},
+                   "context": "paper, its own 5,624-formula corpus: 220 matched / 2,798 constant / 2,606 unmatched"},
+        "clocks": clocks,
+    }))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c3", "c3_small", "c4", "frames"])
+    ap.add_argument("--workload", default="c3", choices=["c3", "c3_small", "c4", "frames", "correspond"])
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--ref-frames", type=int, default=256)
     args = ap.parse_args()
@@ -480,6 +567,8 @@ def main():
         run_c4(args)
     elif args.workload == "frames":
         run_frames(args)
+    elif args.workload == "correspond":
+        run_correspond(args)
     else:
         run_ours(args)
 

@@ -238,6 +238,14 @@ int kripke_condition_bitmap(uint32_t n_worlds, uint32_t condition, uint32_t fram
 int kripke_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words,
                          const uint32_t *library, uint32_t n_library, uint32_t *match_out,
                          void *stream);
+/* The frames whose bit is set in a bitmap, written as successor masks in the format of the frame-list
+ * calls (so a recovered condition can be re-confirmed on its own extension with kripke_eval_frames:
+ * "each re-confirmed over all 33,554,432 five-world frames").  succ_out: DEVICE, capacity *
+ * n_worlds uint16; *count_out (DEVICE uint64) = number of set bits; the first min(count, capacity)
+ * frames found are written, in unspecified order. */
+int kripke_frames_from_bitmap(uint32_t n_worlds, uint32_t frame_class, uint64_t frame_begin,
+                              uint64_t frame_count, const uint32_t *bitmap, uint16_t *succ_out,
+                              uint64_t capacity, uint64_t *count_out, void *stream);
 
 /* End-to-end convenience with HOST buffers only: create + eval over the full class + copy the
  * results back + destroy, synchronously (this is what bench.py's "e2e" figure times). */

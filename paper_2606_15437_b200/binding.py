@@ -33,7 +33,7 @@ EXPORTS = [
     "kripke_calibrate_int32", "kripke_debug_lower", "kripke_witness_to_keys", "kripke_keys_to_witness",
     "kripke_minimal_refutation", "kripke_pairs_separation", "kripke_debug_lower_wf",
     "kripke_eval_frames", "kripke_distinguish_pairs_frames",
-    "kripke_validity_bitmap", "kripke_condition_bitmap", "kripke_match_bitmaps",
+    "kripke_validity_bitmap", "kripke_condition_bitmap", "kripke_match_bitmaps", "kripke_frames_from_bitmap",
 ]
 
 
@@ -89,6 +89,7 @@ def load():
     lib.kripke_validity_bitmap.argtypes = [vp, u32, u32, u32, u64, u64, vp, vp]
     lib.kripke_condition_bitmap.argtypes = [u32, u32, u32, u64, u64, vp, vp]
     lib.kripke_match_bitmaps.argtypes = [vp, u32, u64, vp, u32, vp, vp]
+    lib.kripke_frames_from_bitmap.argtypes = [u32, u32, u64, u64, vp, vp, u64, vp, vp]
     lib.kripke_eval_frames.argtypes = [vp, u32, u32, vp, u64, u64, u32, vp, vp, vp]
     lib.kripke_distinguish_pairs_frames.argtypes = [vp, u32p, u32, u32, u32, vp, u64, u64, u32, vp, vp, vp]
     for name in EXPORTS:
@@ -293,6 +294,20 @@ def match_bitmaps(bitmaps, library, match_out=None, stream=None):
     _check(load().kripke_match_bitmaps(bitmaps.data_ptr(), n_records, words, library.data_ptr(), library.shape[0],
                                        match_out.data_ptr(), _stream(stream)), "kripke_match_bitmaps")
     return match_out
+
+
+def frames_from_bitmap(n_worlds: int, frame_class: int, frame_begin: int, frame_count: int, bitmap, capacity: int,
+                       stream=None):
+    """kripke_frames_from_bitmap.  Returns (succ int16 CUDA tensor of capacity*n masks, number of set bits);
+    synchronises to read the count."""
+    import torch
+    succ = torch.zeros((max(1, capacity) * n_worlds,), dtype=torch.int16, device="cuda")
+    count = torch.zeros((1,), dtype=torch.int64, device="cuda")
+    _check(load().kripke_frames_from_bitmap(n_worlds, frame_class, frame_begin, frame_count, bitmap.data_ptr(),
+                                            succ.data_ptr(), capacity, count.data_ptr(), _stream(stream)),
+           "kripke_frames_from_bitmap")
+    n_set = int(count.item())
+    return succ[:min(n_set, capacity) * n_worlds], n_set
 
 
 def bits_to_bool(bitmap, count: int):

@@ -629,6 +629,22 @@ int kripke_condition_bitmap(uint32_t n_worlds, uint32_t condition, uint32_t fram
     return e ? cuda_fail(e) : KRIPKE_OK;
 }
 
+int kripke_frames_from_bitmap(uint32_t n_worlds, uint32_t frame_class, uint64_t frame_begin, uint64_t frame_count,
+                              const uint32_t *bitmap, uint16_t *succ_out, uint64_t capacity, uint64_t *count_out,
+                              void *stream) {
+    if (n_worlds < 1 || n_worlds > KRIPKE_MAX_WORLDS || frame_class > KRIPKE_CLASS_S5 || !count_out) return KRIPKE_EINVAL;
+    uint64_t csize = 0;
+    int rc = class_size(n_worlds, frame_class, &csize);
+    if (rc) return rc;
+    if (frame_begin > csize || frame_count > csize - frame_begin) return KRIPKE_EINVAL;
+    if (frame_count && (!bitmap || (capacity && !succ_out))) return KRIPKE_EINVAL;
+    const uint64_t *table = nullptr;
+    if ((rc = class_table_device(n_worlds, frame_class, &table))) return rc;
+    int e = launch_frames_from_bitmap(n_worlds, frame_class, table, frame_begin, frame_count, bitmap, succ_out,
+                                      capacity, count_out, stream);
+    return e ? cuda_fail(e) : KRIPKE_OK;
+}
+
 int kripke_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words, const uint32_t *library,
                          uint32_t n_library, uint32_t *match_out, void *stream) {
     if (n_records && (!match_out || (words && !bitmaps))) return KRIPKE_EINVAL;

@@ -135,6 +135,27 @@ __global__ void __launch_bounds__(128) match_bitmaps_kernel(const uint32_t *bitm
     if (lane == 0) match_out[rec] = found;
 }
 
+// Frames whose bit is set -> successor masks (input format of the frame-list calls).  Warp-aggregated
+// append: the order inside a warp is kept, the order of warps is not.
+__global__ void __launch_bounds__(128) frames_from_bitmap_kernel(ConditionParams p, uint16_t *succ_out,
+                                                                 unsigned long long capacity,
+                                                                 unsigned long long *count_out) {
+    const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t lane = threadIdx.x & 31u;
+    const bool set = j < p.frame_count && ((p.bitmap[j >> 5] >> (j & 31u)) & 1u);
+    const uint32_t bal = __ballot_sync(0xFFFFFFFFu, set);
+    if (bal == 0u) return;
+    unsigned long long base = 0;
+    if (lane == 0) base = atomicAdd(count_out, (unsigned long long)__popc(bal));
+    base = __shfl_sync(0xFFFFFFFFu, base, 0);
+    if (!set) return;
+    const unsigned long long at = base + (unsigned long long)__popc(bal & ((1u << lane) - 1u));
+    if (at >= capacity) return;
+    uint32_t succ[KRIPKE_MAX_WORLDS];
+    decode_rows(p.n, class_frame(p.n, p.cls, p.class_table, p.frame_begin + j), succ);
+    for (uint32_t w = 0; w < p.n; ++w) succ_out[at * p.n + w] = (uint16_t)succ[w];
+}
+
 }  // namespace
 
 int launch_validity_bitmap(const ScanJob &job, uint32_t *bitmap_out, void *stream) {
@@ -161,6 +182,22 @@ int launch_condition_bitmap(uint32_t n, uint32_t cond, uint32_t cls, const uint6
     const uint64_t bx = (count + 127) / 128;
     if (bx > 0x7FFFFFFFull) return 801;
     condition_bitmap_kernel<<<(uint32_t)bx, 128, 0, (cudaStream_t)stream>>>(p);
+    return (int)cudaGetLastError();
+}
+
+int launch_frames_from_bitmap(uint32_t n, uint32_t cls, const uint64_t *class_table, uint64_t begin, uint64_t count,
+                              const uint32_t *bitmap, uint16_t *succ_out, uint64_t capacity, uint64_t *count_out,
+                              void *stream) {
+    cudaError_t e = cudaMemsetAsync(count_out, 0, sizeof(uint64_t), (cudaStream_t)stream);
+    if (e != cudaSuccess) return (int)e;
+    if (count == 0) return 0;
+    ConditionParams p;
+    p.n = n; p.cond = 0; p.cls = cls; p.class_table = class_table;
+    p.frame_begin = begin; p.frame_count = count; p.bitmap = const_cast<uint32_t *>(bitmap);
+    const uint64_t bx = (count + 127) / 128;
+    if (bx > 0x7FFFFFFFull) return 801;
+    frames_from_bitmap_kernel<<<(uint32_t)bx, 128, 0, (cudaStream_t)stream>>>(
+        p, succ_out, (unsigned long long)capacity, reinterpret_cast<unsigned long long *>(count_out));
     return (int)cudaGetLastError();
 }
 

@@ -133,6 +133,9 @@ int launch_frames_finish(const FramesJob &job, bool accumulate, kripke_count_t *
 int launch_validity_bitmap(const ScanJob &job, uint32_t *bitmap_out, void *stream);
 int launch_condition_bitmap(uint32_t n, uint32_t cond, uint32_t cls, const uint64_t *class_table, uint64_t begin,
                             uint64_t count, uint32_t *bitmap_out, void *stream);
+int launch_frames_from_bitmap(uint32_t n, uint32_t cls, const uint64_t *class_table, uint64_t begin, uint64_t count,
+                              const uint32_t *bitmap, uint16_t *succ_out, uint64_t capacity, uint64_t *count_out,
+                              void *stream);
 int launch_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words, const uint32_t *library,
                          uint32_t n_library, uint32_t *match_out, void *stream);
 

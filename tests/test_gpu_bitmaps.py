@@ -101,3 +101,40 @@ def test_bitmap_argument_errors(kb):
         kb.condition_bitmap(4, 8, K, 0, 16)
     assert e.value.status == kb.EINVAL
     assert kb.validity_bitmap(h, 4, 1, K, 0, 0).numel() == 0
+
+
+@pytest.mark.parametrize("n,cond", [(4, "transitive"), (4, "confluent"), (3, "serial"), (5, "partially_functional")])
+def test_frames_from_bitmap_is_the_extension(kb, vol, n, cond):
+    """The compacted list holds exactly the frames whose bit is set (as successor masks, any order)."""
+    total = 1 << (n * n)
+    bm = kb.condition_bitmap(n, kb.COND[cond], K, 0, total)
+    _, n_set = kb.frames_from_bitmap(n, K, 0, total, bm, 0)
+    assert n_set == vol.count_condition(n, cond)
+    succ, n2 = kb.frames_from_bitmap(n, K, 0, total, bm, n_set)
+    assert n2 == n_set
+    rows = succ.cpu().numpy().view(np.uint16).reshape(-1, n).astype(np.uint64)
+    f = sum(rows[:, w] << np.uint64(w * n) for w in range(n))
+    if n <= 4:
+        want = np.nonzero(vol.condition_bitmap(n, cond))[0].astype(np.uint64)
+    else:
+        want = np.nonzero(kb.bits_to_bool(bm, total))[0].astype(np.uint64)
+    assert (np.sort(f) == want).all()
+    # a capacity smaller than the extension: only `capacity` frames are written, all of them members
+    part, n3 = kb.frames_from_bitmap(n, K, 0, total, bm, 5)
+    assert n3 == n_set and part.numel() == min(5, n_set) * n
+
+
+def test_recovered_condition_reconfirmed_on_its_extension(kb, vol):
+    """P:380 "each re-confirmed over all 33,554,432 five-world frames", composed from the bit-sliced
+    kernels: T is refuted on no reflexive five-world frame (frame-list scan of the extension) and the
+    census counts 2^25 - 2^20 refuting frames; 4 likewise on the 154,303 transitive frames."""
+    total = 1 << 25
+    for ax, cond, size in (("T", "reflexive", 1 << 20), ("4", "transitive", 154303)):
+        bm = kb.condition_bitmap(5, kb.COND[cond], K, 0, total)
+        succ, n_set = kb.frames_from_bitmap(5, K, 0, total, bm, size)
+        assert n_set == size
+        h = kb.Programs(*W.pack_programs([AX[ax], AX["B"]]), 1)
+        on_ext = kb.unpack(*kb.eval_frames(h, 5, 1, succ))
+        assert int(on_ext["frames"][0]) == 0 and int(on_ext["frames"][1]) > 0      # B fails on some of them
+        cen = kb.unpack(*kb.eval_batch(h, 5, 1, K))
+        assert int(cen["frames"][0]) == total - size
