@@ -247,11 +247,14 @@ int ensure_accum(kripke_programs *h, uint32_t n) {
 }
 
 // Which reduced shapes (n, g), g < k, the sliced kernel can run for this class: bit g.
+// Bit 31 says "class other than K": such scans can only use the frame-per-unit instantiations, whose
+// lowering mode differs (sliced_lower_mode), so their plans are built and cached separately.
+constexpr uint32_t SHAPES_NOT_K = 1u << 31;
 uint32_t reduced_shapes(uint32_t n, uint32_t k, uint32_t cls, uint32_t flags) {
-    uint32_t mask = 0;
-    if ((flags & KRIPKE_FULL_SWEEP) || (flags & KRIPKE_KERNEL_MASK) == KRIPKE_KERNEL_SCALAR) return 0;
-    if (n < 1 || n > KRIPKE_MAX_WORLDS || k > KRIPKE_MAX_VARS) return 0;
-    if (!sliced_select(n, k, cls, 1, nullptr)) return 0;
+    uint32_t mask = cls != KRIPKE_CLASS_K ? SHAPES_NOT_K : 0u;
+    if ((flags & KRIPKE_FULL_SWEEP) || (flags & KRIPKE_KERNEL_MASK) == KRIPKE_KERNEL_SCALAR) return mask;
+    if (n < 1 || n > KRIPKE_MAX_WORLDS || k > KRIPKE_MAX_VARS) return mask;
+    if (!sliced_select(n, k, cls, 1, nullptr)) return mask;
     for (uint32_t g = 0; g < k; ++g)
         if (sliced_select(n, g, cls, 1, nullptr)) mask |= 1u << g;
     return mask;
@@ -435,7 +438,7 @@ int build_scan_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_
         for (uint32_t r = 0; r < n_records; ++r)
             if (group[r] == g) recs.push_back(r);
         if (recs.empty()) continue;
-        const uint32_t mode = sliced_lower_mode(n, g);
+        const uint32_t mode = sliced_lower_mode(n, g, (shapes & SHAPES_NOT_K) ? KRIPKE_CLASS_T : KRIPKE_CLASS_K);
         std::vector<Lowered> low(recs.size());
         std::vector<bool> fits(recs.size());
         for (size_t i = 0; i < recs.size(); ++i) {

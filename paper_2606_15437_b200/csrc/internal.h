@@ -75,8 +75,9 @@ struct SlicedPlan {
 bool sliced_select(uint32_t n, uint32_t k, uint32_t cls, uint32_t need, uint64_t *frames_per_unit);
 // Index of the instantiation `sliced_select` would pick (UINT32_MAX = none).
 uint32_t sliced_row(uint32_t n, uint32_t k, uint32_t cls, uint32_t need);
-// LOWER_LEAF_* flags of the derived leaves the instantiations for this shape provide (0 = no shape).
-uint32_t sliced_lower_mode(uint32_t n, uint32_t k);
+// LOWER_* flags for the instantiations this shape and class run on (0 = no shape): classes other than K
+// can only use the frame-per-unit rows, whose derived leaves differ from the group-per-unit rows'.
+uint32_t sliced_lower_mode(uint32_t n, uint32_t k, uint32_t cls);
 // Should programs of this need class be lowered with LOWER_FUSE?
 bool sliced_fuses(uint32_t n, uint32_t k, uint32_t need);
 // Enqueue the sliced scan; returns a cudaError_t as int and the number of kernel launches.

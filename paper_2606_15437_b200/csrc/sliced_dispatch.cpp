@@ -10,7 +10,7 @@ typedef int (*sliced_launch_fn)(const ScanJob &, const SlicedPlan &, void *, uin
 // X(n, k, MB, DMAX)
 #define SHAPES(X) \
     X(3, 0, 2, 4) X(4, 0, 2, 4) X(5, 0, 2, 2) X(5, 0, 2, 4) X(6, 0, 2, 2) \
-    X(6, 0, 2, 4) X(4, 1, 2, 4) X(5, 1, 2, 4) X(3, 2, 2, 4) X(4, 2, 3, 2) \
+    X(6, 0, 2, 4) X(4, 1, 2, 4) X(5, 1, 2, 4) X(5, 1, 0, 4) X(3, 2, 2, 4) X(4, 2, 3, 2) \
     X(4, 2, 2, 4) X(5, 2, 4, 1) X(5, 2, 3, 1) X(5, 2, 3, 2) X(5, 2, 2, 3) X(5, 2, 2, 4) \
     X(6, 2, 2, 3) X(4, 3, 2, 4) X(5, 3, 3, 2) X(5, 3, 2, 3) X(5, 3, 2, 4)
 
@@ -56,14 +56,14 @@ uint32_t sliced_row(uint32_t n, uint32_t k, uint32_t cls, uint32_t need) {
     return r ? (uint32_t)(r - kRows) : UINT32_MAX;
 }
 
-uint32_t sliced_lower_mode(uint32_t n, uint32_t k) {
+uint32_t sliced_lower_mode(uint32_t n, uint32_t k, uint32_t cls) {
     // tuning aid / test hook: KRIPKE_FUSE_BOOL=1 also fuses loads into Boolean operators (UC_BOOLVL)
     static const char *fb_env = std::getenv("KRIPKE_FUSE_BOOL");
     const uint32_t fuse = LOWER_FUSE | ((fb_env && std::atoi(fb_env)) ? (uint32_t)LOWER_FUSE_BOOL : 0u);
-    for (const Row &r : kRows)
-        if (r.n == n && r.k == k)
-            return fuse | LOWER_LEAF_DEAD | ((frame_per_unit(r) && k >= 1 && n <= 5) ? LOWER_LEAF_P : 0u);
-    return 0;
+    // every row of one (n, k) that a class can use has the same layout kind (see SHAPES above)
+    const Row *r = find(n, k, cls, 1);
+    if (!r) return 0;
+    return fuse | LOWER_LEAF_DEAD | ((frame_per_unit(*r) && k >= 1 && n <= 5) ? LOWER_LEAF_P : 0u);
 }
 
 // Fused micro-ops (LOWER_FUSE) pay off on the one-slot instantiations only: programs
