@@ -337,6 +337,12 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *d_pairs, 
         bool use_sliced = dp.n_slots > 0 && sliced_select(n, k_eff, cls, 1, &fpu);
         uint64_t ab = begin, ae = begin;          // aligned sub-range for the sliced kernel
         if (use_sliced) {
+            // the need classes may run on instantiations with different unit sizes (powers of two):
+            // align the range to the largest one in use
+            for (uint32_t d = 2; d <= (uint32_t)UC_DMAX; ++d) {
+                uint64_t f2 = 1;
+                if (dp.need_end[d] > dp.need_end[d - 1] && sliced_select(n, k_eff, cls, d, &f2)) fpu = std::max(fpu, f2);
+            }
             ab = (begin + fpu - 1) / fpu * fpu;
             ae = (begin + count) / fpu * fpu;
             if (ae <= ab) { use_sliced = false; ab = ae = begin; }

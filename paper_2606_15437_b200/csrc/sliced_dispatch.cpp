@@ -10,7 +10,7 @@ typedef int (*sliced_launch_fn)(const ScanJob &, const SlicedPlan &, void *, uin
 // X(n, k, MB, DMAX)
 #define SHAPES(X) \
     X(3, 0, 2, 4) X(4, 0, 2, 4) X(5, 0, 2, 2) X(5, 0, 2, 4) X(6, 0, 2, 2) \
-    X(6, 0, 2, 4) X(4, 1, 2, 4) X(5, 1, 2, 4) X(5, 1, 0, 4) X(3, 2, 2, 4) X(4, 2, 3, 2) \
+    X(6, 0, 2, 4) X(4, 1, 2, 4) X(5, 1, 2, 4) X(5, 1, 4, 1) X(5, 1, 0, 4) X(3, 2, 2, 4) X(4, 2, 3, 2) \
     X(4, 2, 2, 4) X(5, 2, 4, 1) X(5, 2, 3, 1) X(5, 2, 3, 2) X(5, 2, 2, 3) X(5, 2, 2, 4) \
     X(6, 2, 2, 3) X(4, 3, 2, 4) X(5, 3, 3, 2) X(5, 3, 2, 3) X(5, 3, 2, 4)
 
@@ -74,8 +74,8 @@ bool sliced_fuses(uint32_t n, uint32_t k, uint32_t need) {
 }
 
 int launch_sliced(const ScanJob &job, const SlicedPlan &plan, void *stream, uint32_t *launches) {
-    // group-per-unit shapes need the range aligned to the unit of the row selected for need 1; every
-    // row of one (n, k) uses the same unit size
+    // group-per-unit shapes need the range aligned to the unit of the row (the caller aligns to the
+    // largest unit of the rows it uses)
     const Row *r = find(job.n, job.k, job.cls, plan.max_need);
     if (!r) return 801;   // cudaErrorNotSupported
     return r->fn(job, plan, stream, launches);
