@@ -502,8 +502,10 @@ __global__ void __launch_bounds__(TPB, MINB) scan_sliced_kernel(SlicedParams p) 
     T.leaf = s_leaf + threadIdx.x;
 
     for (uint32_t item = blockIdx.x; item < n_items; item += gridDim.x) {
-        const uint32_t chunk_id = item % p.n_chunks;
+        // (range, chunk) <- item, rotated by the range so that a block's stride through the items does
+        // not keep handing it the same program chunk (chunks differ in cost)
         const uint32_t range_id = item / p.n_chunks;
+        const uint32_t chunk_id = (item % p.n_chunks + range_id) % p.n_chunks;
         const uint32_t slot0 = chunk_id * p.chunk;
         const uint32_t nslots = min(p.chunk, p.n_slots - slot0);
         const uint64_t u0 = p.unit_begin + (uint64_t)range_id * units_per_item;

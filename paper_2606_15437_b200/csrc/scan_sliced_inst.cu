@@ -21,7 +21,7 @@ INST(3, 0, 2, 4, 256, 2) INST(4, 0, 2, 4, 256, 2) INST(5, 0, 2, 2, 128, 4) INST(
 #elif KRIPKE_INST_GROUP == 1
 INST(4, 1, 2, 4, 256, 2) INST(5, 1, 2, 4, 128, 3) INST(5, 1, 4, 1, 128, 3) INST(5, 1, 0, 4, 128, 4) INST(3, 2, 2, 4, 256, 2) INST(4, 2, 3, 2, 128, 3) INST(4, 2, 2, 4, 128, 3)
 #elif KRIPKE_INST_GROUP == 2
-INST(5, 2, 4, 1, 128, 3) INST(5, 2, 3, 1, 128, 4) INST(5, 2, 3, 2, 128, 3) INST(5, 2, 2, 3, 128, 3) INST(5, 2, 2, 4, 128, 2) INST(6, 2, 2, 3, 128, 2)
+INST(5, 2, 4, 1, 128, 3) INST(5, 2, 3, 1, 128, 4) INST(5, 2, 3, 2, 128, 3) INST(5, 2, 4, 2, 128, 2) INST(5, 2, 2, 3, 128, 3) INST(5, 2, 2, 4, 128, 2) INST(6, 2, 2, 3, 128, 2)
 #elif KRIPKE_INST_GROUP == 3
 INST(4, 3, 2, 4, 128, 2) INST(5, 3, 3, 2, 128, 2) INST(5, 3, 2, 3, 128, 2) INST(5, 3, 2, 4, 128, 2)
 #endif

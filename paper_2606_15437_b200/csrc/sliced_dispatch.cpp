@@ -11,7 +11,7 @@ typedef int (*sliced_launch_fn)(const ScanJob &, const SlicedPlan &, void *, uin
 #define SHAPES(X) \
     X(3, 0, 2, 4) X(4, 0, 2, 4) X(5, 0, 2, 2) X(5, 0, 2, 4) X(6, 0, 2, 2) \
     X(6, 0, 2, 4) X(4, 1, 2, 4) X(5, 1, 2, 4) X(5, 1, 4, 1) X(5, 1, 0, 4) X(3, 2, 2, 4) X(4, 2, 3, 2) \
-    X(4, 2, 2, 4) X(5, 2, 4, 1) X(5, 2, 3, 1) X(5, 2, 3, 2) X(5, 2, 2, 3) X(5, 2, 2, 4) \
+    X(4, 2, 2, 4) X(5, 2, 4, 1) X(5, 2, 3, 1) X(5, 2, 3, 2) X(5, 2, 4, 2) X(5, 2, 2, 3) X(5, 2, 2, 4) \
     X(6, 2, 2, 3) X(4, 3, 2, 4) X(5, 3, 3, 2) X(5, 3, 2, 3) X(5, 3, 2, 4)
 
 #define DECL(N, K, MB, D) \
