@@ -261,6 +261,9 @@ def run_ours(args):
                 "executed_evaluations_per_step": executed[0] // args.steps,
                 "valuation_sweep": "per-formula variable support (PAPER.md:93 k_b), counts scaled; "
                                    "KRIPKE_FULL_SWEEP evaluates every valuation",
+                "program_sharing": "formulas whose lowered programs are identical (alpha-equivalent or equal after "
+                                   "constant folding) are scanned once and share counts; executed_evaluations_per_step "
+                                   "counts what ran; KRIPKE_NO_SHARING scans every formula itself",
                 "parallelism": f"frame-range shard x{world}",
                 "l2": "flushed between iterations (256 MiB fill); the kernels read < 100 KB of input",
             },
@@ -277,8 +280,8 @@ def run_ours(args):
                 "peak_source": "derived: 148 SMs x 4 x 16 ALU lanes/clk x 1.965 GHz (DESIGN.md)",
                 "peak_measured_calibration": {k: v / 1e12 for k, v in cal.items()},
                 "frac_of_measured_lop3": achieved / (cal["lop3"] / 1e12),
-                "algorithmic_ops": "executed 3-input logic instr of the lowered programs: sum_b (modal*n^2 + "
-                                   "bool*n + n+1) x 2^(k_b*n)/32 per frame (k_b = variables formula b mentions)",
+                "algorithmic_ops": "3-input logic instr of the lowered programs that ran: sum over distinct lowered "
+                                   "programs b (modal*n^2 + bool*n + n+1) x 2^(k_b*n)/32 per frame (k_b = variables b mentions)",
             },
             "cpu_baseline": {"value": cpu_rate, "unit": "evaluations/s", "cores": cores, "kind": "oracle",
                              "sample": f"first {args.ref_frames} K-frames of n=5 x 1024 valuations x {B} formulas "

@@ -78,6 +78,12 @@ enum {
                                          valuations of the variables it mentions - the paper's
                                          per-formula k_b, P:93 - and its model count scaled; results
                                          are identical either way)                                 */
+    KRIPKE_NO_SHARING = 1u << 2,      /* scan every program itself (default: programs of one call whose
+                                         lowered forms are identical - equal after constant folding and
+                                         the renaming of the variables they mention - are scanned once
+                                         and the others receive the same counts and first refuting
+                                         frame; the witness valuation and world are computed per
+                                         formula; results are identical either way)                */
     KRIPKE_KERNEL_AUTO = 0u << 4,     /* bit-sliced kernel where it applies, else the scalar one  */
     KRIPKE_KERNEL_SCALAR = 1u << 4,   /* force the scalar kernel (Algorithm 1 restated, one model
                                          per thread iteration): baseline / ablation / cross-check */

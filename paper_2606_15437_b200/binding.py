@@ -19,6 +19,7 @@ OK, EINVAL, EPROGRAM, EUNSUPPORTED, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 CLASS_K, CLASS_T, CLASS_S4, CLASS_S5 = 0, 1, 2, 3
 ACCUMULATE = 1 << 0
 FULL_SWEEP = 1 << 1
+NO_SHARING = 1 << 2
 KERNEL_AUTO, KERNEL_SCALAR, KERNEL_SLICED, KERNEL_WARPFRAME = 0 << 4, 1 << 4, 2 << 4, 3 << 4
 REDUCE_BLOCK, REDUCE_WARP, REDUCE_THREAD = 0 << 8, 1 << 8, 2 << 8
 NO_WITNESS = (1 << 64) - 1

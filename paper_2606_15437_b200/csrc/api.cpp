@@ -108,10 +108,12 @@ struct GroupPlan {
     DevicePlan rest;                  // the records the warp-frame kernel cannot take
     WfPlan wf;                        // the records it can (host micro-ops; they travel as kernel parameters)
     uint32_t *d_wf_records = nullptr; // device: record index per warp-frame program
+    uint32_t *d_alias = nullptr;      // device: (record, representative) pairs - records whose lowered program
+    uint32_t n_alias = 0;             // equals the representative's are not scanned, they copy its accumulators
     void release() {
         dp.release(); rest.release();
-        cudaFree(d_wf_records);
-        d_wf_records = nullptr;
+        cudaFree(d_wf_records); cudaFree(d_alias);
+        d_wf_records = nullptr; d_alias = nullptr; n_alias = 0;
         wf = WfPlan();
     }
 };
@@ -250,8 +252,9 @@ int ensure_accum(kripke_programs *h, uint32_t n) {
 // Bit 31 says "class other than K": such scans can only use the frame-per-unit instantiations, whose
 // lowering mode differs (sliced_lower_mode), so their plans are built and cached separately.
 constexpr uint32_t SHAPES_NOT_K = 1u << 31;
+constexpr uint32_t SHAPES_NO_SHARING = 1u << 30;      // KRIPKE_NO_SHARING: scan every record itself
 uint32_t reduced_shapes(uint32_t n, uint32_t k, uint32_t cls, uint32_t flags) {
-    uint32_t mask = cls != KRIPKE_CLASS_K ? SHAPES_NOT_K : 0u;
+    uint32_t mask = (cls != KRIPKE_CLASS_K ? SHAPES_NOT_K : 0u) | ((flags & KRIPKE_NO_SHARING) ? SHAPES_NO_SHARING : 0u);
     if ((flags & KRIPKE_FULL_SWEEP) || (flags & KRIPKE_KERNEL_MASK) == KRIPKE_KERNEL_SCALAR) return mask;
     if (n < 1 || n > KRIPKE_MAX_WORLDS || k > KRIPKE_MAX_VARS) return mask;
     if (!sliced_select(n, k, cls, 1, nullptr)) return mask;
@@ -271,7 +274,7 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *d_pairs, 
              kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream) {
     if (n < 1 || n > KRIPKE_MAX_WORLDS || k != h->n_vars || cls > KRIPKE_CLASS_S5) return KRIPKE_EINVAL;
     if (n * n + k * n > KRIPKE_MAX_MODEL_BITS) return KRIPKE_EUNSUPPORTED;
-    if (flags & ~(KRIPKE_ACCUMULATE | KRIPKE_FULL_SWEEP | KRIPKE_KERNEL_MASK | KRIPKE_REDUCE_MASK)) return KRIPKE_EINVAL;
+    if (flags & ~(KRIPKE_ACCUMULATE | KRIPKE_FULL_SWEEP | KRIPKE_NO_SHARING | KRIPKE_KERNEL_MASK | KRIPKE_REDUCE_MASK)) return KRIPKE_EINVAL;
     const uint32_t family = flags & KRIPKE_KERNEL_MASK, reduce = (flags & KRIPKE_REDUCE_MASK) >> 8;
     if (reduce > 2) return KRIPKE_EINVAL;
     if (n_records && (!counts_out || !witness_out)) return KRIPKE_EINVAL;
@@ -415,6 +418,14 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *d_pairs, 
             if ((rc = run_sliced_or_scalar(g.dp, g.k_eff))) return rc;
         }
     }
+    // records that share a representative's lowered program take its accumulators (the scalar family
+    // scanned every record itself)
+    if (family != KRIPKE_KERNEL_SCALAR)
+        for (const GroupPlan &g : plan.groups)
+            if (g.n_alias) {
+                if ((e = launch_alias_accum(job.accum, g.d_alias, g.n_alias, stream))) return cuda_fail(e);
+                ++launches;
+            }
     if ((e = launch_finish(job, (flags & KRIPKE_ACCUMULATE) != 0, counts_out, witness_out, stream)))
         return cuda_fail(e);
     h->last.launches = launches + 1;
@@ -465,6 +476,27 @@ int build_scan_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_
                 fits[i] = lower(mode & ~(uint32_t)(LOWER_FUSE | LOWER_FUSE_BOOL));
             }
         }
+        // Records of the group whose lowered programs are identical (alpha-equivalent after the variable
+        // renaming, or equal after constant folding) are scanned once: the first is the representative,
+        // the others receive a copy of its accumulators before the finish step (DESIGN.md 5.1 "Sharing").
+        std::vector<uint32_t> alias;
+        if (!(shapes & SHAPES_NO_SHARING)) {
+            std::map<std::vector<uint16_t>, uint32_t> seen;
+            std::vector<uint32_t> recs2;
+            std::vector<Lowered> low2;
+            std::vector<bool> fits2;
+            for (size_t i = 0; i < recs.size(); ++i) {
+                if (fits[i]) {
+                    auto it = seen.find(low[i].ucode);
+                    if (it != seen.end()) { alias.push_back(recs[i]); alias.push_back(it->second); continue; }
+                    seen.emplace(low[i].ucode, recs[i]);
+                }
+                recs2.push_back(recs[i]);
+                low2.push_back(std::move(low[i]));
+                fits2.push_back(fits[i]);
+            }
+            recs.swap(recs2); low.swap(low2); fits.swap(fits2);
+        }
         HostPlan hp;
         build_plan(low, fits, &hp);
         for (auto &x : hp.slot_record) x = recs[x];       // slot -> record index of the whole batch
@@ -472,7 +504,9 @@ int build_scan_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_
         GroupPlan gp;
         gp.k_eff = g;
         int rc = upload_plan(hp, &gp.dp);
+        if (!rc) rc = upload(&gp.d_alias, alias);
         if (rc) { gp.release(); out->release(); return rc; }
+        gp.n_alias = (uint32_t)(alias.size() / 2);
         // warp-frame kernel (single formulas, shapes it is instantiated for): the programs it can
         // take are lowered to its typed micro-ops, the others keep a bit-sliced plan of their own
         if (!pairs && (wf_select(n, g, KRIPKE_CLASS_K, nullptr) || wf_select(n, g, KRIPKE_CLASS_T, nullptr))) {

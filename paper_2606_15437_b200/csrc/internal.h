@@ -142,6 +142,8 @@ int launch_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t w
 
 // Zero the accumulators; finish: turn accumulators into counts / witnesses (handles ACCUMULATE).
 int launch_init(Accum *accum, uint32_t n_records, void *stream);
+// accum[pairs[2i]] = accum[pairs[2i+1]] for i < n (records sharing a representative's program).
+int launch_alias_accum(Accum *accum, const uint32_t *pairs, uint32_t n, void *stream);
 int launch_finish(const ScanJob &job, bool accumulate, kripke_count_t *counts_out,
                   kripke_witness_t *witness_out, void *stream);
 // Size record of step H8.

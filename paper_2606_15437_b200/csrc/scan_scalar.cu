@@ -295,6 +295,17 @@ int launch_scalar(const ScanJob &job, const uint32_t *records, uint32_t n_list, 
     return 0;
 }
 
+__global__ void alias_accum_kernel(Accum *accum, const uint32_t *pairs, uint32_t n) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) accum[pairs[2 * i]] = accum[pairs[2 * i + 1]];
+}
+
+int launch_alias_accum(Accum *accum, const uint32_t *pairs, uint32_t n, void *stream) {
+    if (n == 0) return 0;
+    alias_accum_kernel<<<(n + 255) / 256, 256, 0, (cudaStream_t)stream>>>(accum, pairs, n);
+    return (int)cudaGetLastError();
+}
+
 int launch_init(Accum *accum, uint32_t n_records, void *stream) {
     if (n_records == 0) return 0;
     init_accum_kernel<<<(n_records + 255) / 256, 256, 0, (cudaStream_t)stream>>>(accum, n_records);

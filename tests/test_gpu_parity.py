@@ -174,9 +174,10 @@ def test_warp_frame_kernel_windows_live(kb, vol):
     h = kb.Programs(code, offs, 2)
     for cls, begin, count in ((K, 8192 * 122 - 5, 8500), (T, 8192 * 50 - 5, 8500), (K, (1 << 25) - 8192, 8192)):
         want = vol.census(code, offs, 5, 2, cls, begin, count)
-        got = run(kb, progs, 5, 2, cls, begin, count, flags=kb.KERNEL_WARPFRAME, handle=h)
+        got = run(kb, progs, 5, 2, cls, begin, count, flags=kb.KERNEL_WARPFRAME | kb.NO_SHARING, handle=h)
         info = h.last_run_info()
         assert info.kernel_family == 2 and info.wf_programs > 0.9 * len(progs)
+        same(run(kb, progs, 5, 2, cls, begin, count, flags=kb.KERNEL_WARPFRAME, handle=h), got, "warp-frame, shared")
         same(got, want, f"warp-frame cls={cls} [{begin},+{count})")
         certify(progs, got, 5, 2, cls, idx=range(0, len(progs), 9))
         same(run(kb, progs, 5, 2, cls, begin, count, handle=h), want, "auto")
@@ -475,9 +476,10 @@ def test_variable_support_reduction_is_exact(kb, vol):
     for n, cls, a, cnt in ((5, K, 777, 4000), (5, T, 10, 3000), (4, K, 0, 1 << 16), (4, S4, 0, 355), (3, K, 0, 512)):
         red = run(kb, progs, n, 2, cls, a, cnt, handle=h)
         executed_red = h.last_run_info().executed_models
-        full = run(kb, progs, n, 2, cls, a, cnt, flags=kb.FULL_SWEEP, handle=h)
+        full = run(kb, progs, n, 2, cls, a, cnt, flags=kb.FULL_SWEEP | kb.NO_SHARING, handle=h)
         executed_full = h.last_run_info().executed_models
         same(red, full, f"support reduction n={n} cls={cls}")
+        same(run(kb, progs, n, 2, cls, a, cnt, flags=kb.FULL_SWEEP, handle=h), full, "full sweep, shared")
         assert executed_full == len(progs) * cnt << (2 * n) and executed_red <= executed_full
     want = vol.census(code, offs, 4, 2, K)
     same(run(kb, progs, 4, 2, K, handle=h), want, "reduced vs oracle")
@@ -516,3 +518,28 @@ print("fused-bool parity ok")
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     res = subprocess.run([sys.executable, "-c", script], cwd=root, env=env, capture_output=True, text=True, timeout=900)
     assert res.returncode == 0 and "fused-bool parity ok" in res.stdout, res.stdout + res.stderr
+
+
+def test_program_sharing_is_exact(kb, vol):
+    """Formulas whose lowered programs coincide (alpha-equivalent, or equal after constant folding) are
+    scanned once by default; KRIPKE_NO_SHARING scans each itself.  Same records either way, equal to
+    the oracle, witnesses per formula (the valuation of '[]q -> q' sets q bits, not p bits)."""
+    texts = ["[]p -> p", "[]q -> q", "([]p -> p) & T", "F | ([]q -> q)", "<>p & q", "<>q & p", "<>p & q",
+             "[](p -> q) -> ([]p -> []q)", "[](q -> p) -> ([]q -> []p)", "~~[]<>p", "[]<>p", "[]<>q"]
+    progs = [W.to_postfix(W.parse(t)) for t in texts] + W.corpus_c2(500)
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 2)
+    for n, cls, begin, count in ((4, K, 0, 1 << 16), (4, T, 0, 1 << 12), (5, K, (1 << 22) + 64, 4096), (5, T, 128, 2048)):
+        shared = kb.unpack(*kb.eval_batch_range(h, n, 2, cls, begin, count))
+        ex_shared = h.last_run_info().executed_models
+        own = kb.unpack(*kb.eval_batch_range(h, n, 2, cls, begin, count, kb.NO_SHARING))
+        ex_own = h.last_run_info().executed_models
+        same(shared, own, f"sharing n={n} cls={cls}")
+        assert ex_shared < ex_own
+        want = vol.census(code, offs, n, 2, cls, begin, count)
+        same(shared, want, f"sharing vs oracle n={n} cls={cls}")
+    # chunked accumulation composes with sharing
+    c = w = None
+    for a, b in ((0, 1000), (1000, 4096)):
+        c, w = kb.eval_batch_range(h, 4, 2, T, a, b - a, kb.ACCUMULATE if a else 0, c, w)
+    same(kb.unpack(c, w), vol.census(code, offs, 4, 2, T, 0, 4096), "sharing + accumulate")
