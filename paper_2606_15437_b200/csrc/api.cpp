@@ -470,10 +470,39 @@ int build_scan_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_
                                           plen(pairs[2 * r + 1]), m, rename, &low[i])
                              : lower_single(prog(r), plen(r), m, rename, &low[i]);
             };
-            fits[i] = lower(mode);
-            if (fits[i] && (mode & LOWER_FUSE) && !sliced_fuses(n, g, (uint32_t)low[i].need)) {
-                low[i] = Lowered();
-                fits[i] = lower(mode & ~(uint32_t)(LOWER_FUSE | LOWER_FUSE_BOOL));
+            auto lower_for_kernel = [&]() {
+                bool ok = lower(mode);
+                if (ok && (mode & LOWER_FUSE) && !sliced_fuses(n, g, (uint32_t)low[i].need)) {
+                    low[i] = Lowered();
+                    ok = lower(mode & ~(uint32_t)(LOWER_FUSE | LOWER_FUSE_BOOL));
+                }
+                return ok;
+            };
+            fits[i] = lower_for_kernel();
+            // Counts and the least refuting frame do not depend on which variable plays which role (a
+            // permutation of the variables permutes the valuations of every frame), so with sharing on
+            // the cheapest - then lexicographically least - of the permuted lowerings is taken: more
+            // programs coincide, and the in-word variable p_0 lands where it saves most.
+            if (g >= 2 && !(shapes & SHAPES_NO_SHARING)) {
+                uint8_t perm[KRIPKE_MAX_VARS] = {0, 1, 2, 3}, base[KRIPKE_MAX_VARS];
+                std::copy(rename, rename + KRIPKE_MAX_VARS, base);
+                auto cost = [&](const Lowered &l) { return (uint64_t)l.n_modal * n * n + (uint64_t)l.n_bool * n; };
+                Lowered best = low[i];
+                bool best_ok = fits[i];
+                while (std::next_permutation(perm, perm + g)) {
+                    for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v) rename[v] = base[v] < g ? perm[base[v]] : base[v];
+                    low[i] = Lowered();
+                    const bool ok = lower_for_kernel();
+                    if (!ok) continue;
+                    if (!best_ok || cost(low[i]) < cost(best) ||
+                        (cost(low[i]) == cost(best) && (low[i].need < best.need ||
+                                                        (low[i].need == best.need && low[i].ucode < best.ucode)))) {
+                        best = low[i];
+                        best_ok = true;
+                    }
+                }
+                low[i] = best;
+                fits[i] = best_ok;
             }
         }
         // Records of the group whose lowered programs are identical (alpha-equivalent after the variable
