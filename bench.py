@@ -30,7 +30,7 @@ import workloads as W  # noqa: E402
 
 CLASSES = (("K", 0), ("T", 1), ("S4", 2), ("S5", 3))
 N_WORLDS, N_VARS = 5, 2
-NCU_TRAFFIC_BYTES = 4002304                  # class-K launch group, profiles/r1_v4_sliced_5_2_m16_full.md
+NCU_TRAFFIC_BYTES = 3067648                  # class-K launch group, profiles/r1_v5_sliced_5_2_m16_full.md
 SM_COUNT, INT_LANES_PER_SM = 148, 64       # 4 sub-partitions x 16 lanes/clk on the ALU pipe (B300_MICROARCH.md)
 
 
@@ -275,7 +275,7 @@ def run_ours(args):
                 "achieved": achieved, "peak": peak, "unit": "T thread-instr/s", "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES if (args.workload == "c3" and world == 1) else None,
                 "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of the class-K kernels of one step, "
-                                  "ncu capture profiles/r1_v4_launches_c3.csv (bytes; algorithmic HBM bytes = 0)",
+                                  "ncu capture profiles/r1_v5_launches_c3.csv (bytes; algorithmic HBM bytes = 0)",
                 "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_per_step,
                 "peak_source": "derived: 148 SMs x 4 x 16 ALU lanes/clk x 1.965 GHz (DESIGN.md)",
                 "peak_measured_calibration": {k: v / 1e12 for k, v in cal.items()},
