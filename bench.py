@@ -242,6 +242,25 @@ def run_ours(args):
         e2e = {"value": evals_per_step / float(np.mean(times)), "unit": "evaluations/s",
                "h2d_bytes_per_step": int(4 * (code.nbytes + offs.nbytes)), "d2h_bytes_per_step": int(4 * 32 * B)}
 
+    # ablation, one pass each after the timed region: every formula scanned itself (KRIPKE_NO_SHARING), and
+    # additionally over all 2^(n_vars*n) valuations (KRIPKE_FULL_SWEEP): the same records, no work shared
+    ablation = None
+    if rank == 0 and world == 1 and args.workload == "c3" and args.e2e_steps > 0:
+        ablation = {}
+        for name, fl in (("no_sharing", kb.NO_SHARING), ("no_sharing_full_sweep", kb.NO_SHARING | kb.FULL_SWEEP)):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ex = 0
+            for timed in (False, True):
+                torch.cuda.synchronize()
+                a.record()
+                for cname, cls in CLASSES:
+                    kb.eval_batch_range(h, N_WORLDS, N_VARS, cls, 0, sizes[cname], fl, counts[cname], wits[cname])
+                    ex += h.last_run_info().executed_models if timed else 0
+                b.record()
+                torch.cuda.synchronize()
+            ms = a.elapsed_time(b)
+            ablation[name] = {"ms_per_step": ms, "value": evals_per_step / (ms * 1e-3), "executed_evaluations_per_step": ex}
+
     if rank == 0:
         k_instr = k_info["instr_per_frame"] * k_info["frames"]    # executed 3-input logic thread-instructions
         achieved = k_instr / (k_ms * 1e-3) / 1e12
@@ -283,6 +302,7 @@ def run_ours(args):
                 "algorithmic_ops": "3-input logic instr of the lowered programs that ran: sum over distinct lowered "
                                    "programs b (modal*n^2 + bool*n + n+1) x 2^(k_b*n)/32 per frame (k_b = variables b mentions)",
             },
+            "ablation": ablation,
             "cpu_baseline": {"value": cpu_rate, "unit": "evaluations/s", "cores": cores, "kind": "oracle",
                              "sample": f"first {args.ref_frames} K-frames of n=5 x 1024 valuations x {B} formulas "
                                        f"({cpu_evals:.3g} evaluations, {cpu_dt:.1f} s)"},
