@@ -302,7 +302,9 @@ int kripke_keys_to_witness(const uint64_t *keys, uint32_t n_records, uint32_t n_
 /* Diagnostic (pure host, no CUDA): lowers one program - or the pair (a, b) if code_b != NULL - to
  * the bit-sliced kernel's 16-bit micro-ops (csrc/ucode.h: low byte op, high byte argument) and
  * copies them to ucode_out (capacity cap entries).  leaf_mode: bit 0 = "box F / dia T is a leaf",
- * bit 1 = "p_0, box p_0, dia p_0 are leaves" (what the kernel instantiation for a shape provides).
+ * bit 1 = "p_0, box p_0, dia p_0 are leaves" (what the kernel instantiation for a shape provides),
+ * bit 2 = "fuse a load into the modal operator that follows it", bit 3 = "and into a Boolean operator
+ * with a leaf".
  * Returns the number of micro-ops, or a negative kripke_status (KRIPKE_EUNSUPPORTED if the program
  * needs more register-stack slots than the kernel has; *need_out is set in both cases). */
 int kripke_debug_lower(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b,

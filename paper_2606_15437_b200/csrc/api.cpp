@@ -1003,7 +1003,7 @@ int kripke_debug_lower(const uint8_t *code_a, uint32_t len_a, const uint8_t *cod
     if (rc == KRIPKE_OK && code_b) rc = validate_programs(code_b, offs_b, 1, n_vars, nullptr);
     if (rc) return rc;
     Lowered low;
-    if (leaf_mode > 3) return KRIPKE_EINVAL;
+    if (leaf_mode > (LOWER_LEAF_DEAD | LOWER_LEAF_P | LOWER_FUSE | LOWER_FUSE_BOOL)) return KRIPKE_EINVAL;
     const bool fits = code_b ? lower_pair(code_a, len_a, code_b, len_b, leaf_mode, nullptr, &low)
                              : lower_single(code_a, len_a, leaf_mode, nullptr, &low);
     if (need_out) *need_out = (uint32_t)low.need;

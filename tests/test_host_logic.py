@@ -118,6 +118,17 @@ def _run_ucode(uc, n, succ, vals):
             return (~(D[0] ^ D[1]) & full) != 0
         elif 128 <= op < 132:
             D[op - 128] = 0
+        elif 132 <= op < 136:                        # fused forms (csrc/ucode.h, LOWER_FUSE)
+            D[0] = box(vals[op - 132])
+        elif 136 <= op < 140:
+            D[0] = dia(vals[op - 136])
+        elif 140 <= op < 144:
+            D[op - 140] = box(leaves[arg])
+        elif 144 <= op < 148:
+            D[op - 144] = dia(leaves[arg])
+        elif 148 <= op < 164:                        # LOWER_FUSE_BOOL
+            f, d = divmod(op - 148, 4)
+            D[d] = fn[f](vals[arg >> 4], leaves[arg & 15])
         else:
             raise AssertionError(f"bad micro-op {op}")
     raise AssertionError("no FIN op")
@@ -134,21 +145,25 @@ def _models(rng, n, k, count):
     return out
 
 
-@pytest.mark.parametrize("mode", [0, 1, 3])
+@pytest.mark.parametrize("mode", [0, 1, 3, 4 | 1, 4 | 3, 8 | 4 | 3])
 def test_lowering_matches_oracle_truth(vol, mode):
     """Refuted-or-not of the lowered program == truth set != W from the oracle, on random models,
     for every leaf mode the kernel instantiations use."""
     rng = W.SplitMix64(2024 + mode)
     sets = [(W.corpus_c1(300), 2), (W.corpus_c2(600)[300:], 2), (W.corpus_c4(300), 3)]
-    if mode != 3:
+    if not mode & 2:
         sets.append((W.pairs_c5(100)[0], 0))
     for progs, k in sets:
         for c in progs:
             uc, need = kb.debug_lower(c, None, k, mode)
             assert 1 <= need <= 4 and uc[-1][0] in (124, 125)
-            if mode == 3:
+            if mode & 2:
                 assert all(op >= 4 and not (16 <= op < 80 and ((op - 16) // 4) % 4 == 0) for op, _ in uc), \
                     "p_0 must be read through the leaf table in this mode"
+            if mode & 4:       # a load never stays in front of a modal operator on the same slot
+                for (o1, _), (o2, _) in zip(uc, uc[1:]):
+                    assert not (80 <= o1 < 84 and o2 in (116 + o1 - 80, 120 + o1 - 80))
+                    assert not (o1 < 16 and o1 % 4 == 0 and o2 in (116, 120))
             for n in (3, 5):
                 for f, v, succ, vals in _models(rng, n, k, 5):
                     want = vol.truth(c, n, f, k, v) != [1] * n
