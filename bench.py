@@ -79,6 +79,15 @@ class ClockSampler(threading.Thread):
                 pass
             self.stop_flag.wait(0.2)
 
+    def energy_mj(self):
+        """NVML total energy counter of the device in millijoules, or None."""
+        if self.nv is None:
+            return None
+        try:
+            return int(self.nv.nvmlDeviceGetTotalEnergyConsumption(self.h))
+        except Exception:
+            return None
+
     def result(self):
         self.stop_flag.set()
         if self.nv is None or not self.samples:
@@ -205,12 +214,14 @@ def run_ours(args):
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     evk = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
+    e_before = sampler.energy_mj()
     ev0.record()
     for i in range(args.steps):
         step(evk[i])
         flush.fill_(i & 0xFF)            # L2 flush between iterations (inputs are < 100 KB anyway)
     ev1.record()
     barrier()
+    e_after = sampler.energy_mj()
     ms_total = ev0.elapsed_time(ev1)
     clocks = sampler.result()
     k_ms = float(np.mean([a.elapsed_time(b) for a, b in evk]))
@@ -303,6 +314,11 @@ def run_ours(args):
                                    "programs b (modal*n^2 + bool*n + n+1) x 2^(k_b*n)/32 per frame (k_b = variables b mentions)",
             },
             "ablation": ablation,
+            # P:262 reports 10.53 nJ per evaluation on the H100: the same figure from NVML's energy counter
+            "energy": None if (e_before is None or e_after is None or world > 1) else {
+                "joules_per_step": (e_after - e_before) * 1e-3 / args.steps,
+                "nj_per_evaluation": (e_after - e_before) * 1e-3 / args.steps / evals_per_step * 1e9,
+                "source": "nvmlDeviceGetTotalEnergyConsumption around the timed region (whole board)"},
             "cpu_baseline": {"value": cpu_rate, "unit": "evaluations/s", "cores": cores, "kind": "oracle",
                              "sample": f"first {args.ref_frames} K-frames of n=5 x 1024 valuations x {B} formulas "
                                        f"({cpu_evals:.3g} evaluations, {cpu_dt:.1f} s)"},

@@ -138,3 +138,30 @@ def test_recovered_condition_reconfirmed_on_its_extension(kb, vol):
         assert int(on_ext["frames"][0]) == 0 and int(on_ext["frames"][1]) > 0      # B fails on some of them
         cen = kb.unpack(*kb.eval_batch(h, 5, 1, K))
         assert int(cen["frames"][0]) == total - size
+
+
+def test_k4_as_a_scan_class_by_composition(kb, vol):
+    """Other frame classes (K4 = transitive frames, Table 4; serial, Euclidean, ...) need no kernel of
+    their own: the condition's extension becomes a frame list and the frame-list scan runs on it.  K4 at
+    n = 4: counts equal the oracle's census over the 3,994 transitive frames; the reported position maps
+    back to a transitive frame that refutes."""
+    n = 4
+    total = 1 << (n * n)
+    progs = W.corpus_c2(200) + [AX["4"], AX["T"], AX["K"]]
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 2)
+    bm = kb.condition_bitmap(n, kb.COND["transitive"], K, 0, total)
+    succ, n_set = kb.frames_from_bitmap(n, K, 0, total, bm, 3994)
+    assert n_set == 3994
+    got = kb.unpack(*kb.eval_frames(h, n, 2, succ))
+    frames = np.nonzero(vol.condition_bitmap(n, "transitive"))[0].astype(np.uint64)
+    want = vol.census_list(code, offs, n, 2, frames)
+    assert (got["models"] == want["models"]).all() and (got["frames"] == want["frames"]).all()
+    assert int(got["frames"][200]) == 0 and int(got["frames"][201]) > 0 and int(got["models"][202]) == 0
+    rows = succ.cpu().numpy().view(np.uint16).reshape(-1, n).astype(np.uint64)
+    b = 201                                           # T is refuted on the non-reflexive transitive frames
+    j = int(got["wit_f"][b])
+    f = int(sum(int(rows[j, w]) << (w * n) for w in range(n)))
+    assert f in set(int(x) for x in frames)
+    from oracle import kripke_oracle as O
+    assert O.check_witness(progs[b], n, 2, K, f, int(got["wit_v"][b]), int(got["wit_w"][b]))
