@@ -253,6 +253,20 @@ int kripke_frames_from_bitmap(uint32_t n_worlds, uint32_t frame_class, uint64_t 
                               uint64_t frame_count, const uint32_t *bitmap, uint16_t *succ_out,
                               uint64_t capacity, uint64_t *count_out, void *stream);
 
+/* Failure densities - the atlas matrix ("D_ij = the fraction of valuation-world pairs on which
+ * formula i fails on ... frame j"; "Atlas-3 concatenates density panels for all frames through
+ * three worlds. Atlas-4 and Atlas-5 append stratified panels of 2,048 four-world and 4,096 five-world
+ * frames").  counts_out[b * F + j] = #{(v, w) : world w is outside the truth set of formula b under
+ * valuation v on frame j}, F = number of frames; D = count / (2^(n_vars*n) * n).  DEVICE uint32,
+ * formula-major.  Frames: a class range (n <= 6) or an explicit list of successor masks (n <= 16, the
+ * format of kripke_eval_frames).  n_vars * n_worlds <= KRIPKE_LIST_MAX_VAL_BITS. */
+int kripke_failure_density(const kripke_programs_t *programs, uint32_t n_worlds, uint32_t n_vars,
+                           uint32_t frame_class, uint64_t frame_begin, uint64_t frame_count,
+                           uint32_t *counts_out, void *stream);
+int kripke_failure_density_frames(const kripke_programs_t *programs, uint32_t n_worlds, uint32_t n_vars,
+                                  const uint16_t *succ, uint64_t n_frames, uint32_t *counts_out,
+                                  void *stream);
+
 /* End-to-end convenience with HOST buffers only: create + eval over the full class + copy the
  * results back + destroy, synchronously (this is what bench.py's "e2e" figure times). */
 int kripke_eval_batch_host(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,

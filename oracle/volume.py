@@ -58,6 +58,12 @@ def _load():
         lib.kov_validity_list.restype = ctypes.c_int
         lib.kov_validity_list.argtypes = [u8p, u32p, ctypes.c_uint32, ctypes.c_int, ctypes.c_int, u64p,
                                           ctypes.c_uint64, u8p, ctypes.c_int]
+        lib.kov_failure_counts.restype = ctypes.c_int
+        lib.kov_failure_counts.argtypes = [u8p, u32p, ctypes.c_uint32, ctypes.c_int, ctypes.c_int, u64p,
+                                           ctypes.c_uint64, u32p, ctypes.c_int]
+        lib.kov_failure_counts_relations.restype = ctypes.c_int
+        lib.kov_failure_counts_relations.argtypes = [u8p, u32p, ctypes.c_uint32, ctypes.c_int, ctypes.c_int, u8p,
+                                                     ctypes.c_uint64, u32p, ctypes.c_int]
         lib.kov_max_threads.restype = ctypes.c_int
         lib.kov_orbits.restype = ctypes.c_int64
         lib.kov_orbits.argtypes = [ctypes.c_int, u64p, u64p, ctypes.c_uint64]
@@ -218,6 +224,41 @@ def validity(code, offsets, n, k, cls=CLASS_K, frame_begin=0, frame_count=None, 
                                    _p(frames, ctypes.c_uint64), len(frames), _p(out, ctypes.c_uint8), threads)
     if rc:
         raise ValueError("kov_validity_list failed")
+    return out
+
+
+def failure_counts(code, offsets, n, k, cls=CLASS_K, frame_begin=0, frame_count=None, rel=None, threads=0):
+    """uint32 array [B, frames]: the number of (valuation, world) pairs at which formula b fails on each
+    frame (PAPER.md:270; density = count / (2^(k*n) * n)).  Frames: the class range, or - if `rel` is
+    given - the explicit relations rel[F, n, n] (n <= 16)."""
+    code = np.ascontiguousarray(code, dtype=np.uint8)
+    offsets = np.ascontiguousarray(offsets, dtype=np.uint32)
+    B = len(offsets) - 1
+    if rel is not None:
+        rel = np.ascontiguousarray(rel, dtype=np.uint8)
+        out = np.zeros((B, len(rel)), np.uint32)
+        if len(rel) and B:
+            rc = _load().kov_failure_counts_relations(_p(code, ctypes.c_uint8), _p(offsets, ctypes.c_uint32), B, n, k,
+                                                      _p(rel, ctypes.c_uint8), len(rel), _p(out, ctypes.c_uint32), threads)
+            if rc:
+                raise ValueError("kov_failure_counts_relations failed")
+        return out
+    if cls == CLASS_K:
+        total = 1 << (n * n)
+        if frame_count is None:
+            frame_count = total - frame_begin
+        frames = np.arange(frame_begin, frame_begin + frame_count, dtype=np.uint64)
+    else:
+        allf = class_frames(n, cls)
+        if frame_count is None:
+            frame_count = len(allf) - frame_begin
+        frames = np.ascontiguousarray(allf[frame_begin:frame_begin + frame_count], dtype=np.uint64)
+    out = np.zeros((B, len(frames)), np.uint32)
+    if len(frames) and B:
+        rc = _load().kov_failure_counts(_p(code, ctypes.c_uint8), _p(offsets, ctypes.c_uint32), B, n, k,
+                                        _p(frames, ctypes.c_uint64), len(frames), _p(out, ctypes.c_uint32), threads)
+        if rc:
+            raise ValueError("kov_failure_counts failed")
     return out
 
 

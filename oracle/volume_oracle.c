@@ -591,3 +591,62 @@ int kov_validity_list(const u8 *code, const uint32_t *offs, uint32_t B, int n, i
     }
     return bad ? -1 : 0;
 }
+
+/* ---- failure densities ("D_ij = the fraction of valuation-world pairs on which formula i
+ * fails on frame j") ----  out[b * nframes + j] = #{(v, w) : world w is outside the truth set of formula b
+ * under valuation v on frame j}; the density is that count divided by 2^(k*n) * n. */
+int kov_failure_counts(const u8 *code, const uint32_t *offs, uint32_t B, int n, int k,
+                       const uint64_t *frames, uint64_t nframes, uint32_t *out, int nthreads) {
+    if (n < 1 || n > MAXN || k < 0 || k > MAXVARS || k * n > 24) return -1;
+    const uint64_t nval = 1ull << (k * n);
+    int bad = 0;
+#ifdef _OPENMP
+    if (nthreads <= 0) nthreads = omp_get_max_threads();
+#else
+    nthreads = 1;
+#endif
+#pragma omp parallel for num_threads(nthreads) schedule(dynamic, 16)
+    for (uint64_t j = 0; j < nframes; ++j) {
+        u8 R[MAXN][MAXN], V[MAXVARS][MAXN], t[MAXN];
+        decode_frame(n, frames[j], R);
+        for (uint32_t b = 0; b < B; ++b) {
+            uint32_t cnt = 0;
+            for (uint64_t v = 0; v < nval; ++v) {
+                decode_valuation(n, k, v, V);
+                if (eval_program(code + offs[b], offs[b + 1] - offs[b], n, R, V, t)) bad = 1;
+                for (int w = 0; w < n; ++w) cnt += !t[w];
+            }
+            out[(size_t)b * nframes + j] = cnt;
+        }
+    }
+    return bad ? -1 : 0;
+}
+
+/* The same over explicit relations rel[nframes][n][n] (n <= 16). */
+int kov_failure_counts_relations(const u8 *code, const uint32_t *offs, uint32_t B, int n, int k,
+                                 const u8 *rel, uint64_t nframes, uint32_t *out, int nthreads) {
+    if (n < 1 || n > BIGN || k < 0 || k > MAXVARS || k * n > 24) return -1;
+    const uint64_t nval = 1ull << (k * n);
+    int bad = 0;
+#ifdef _OPENMP
+    if (nthreads <= 0) nthreads = omp_get_max_threads();
+#else
+    nthreads = 1;
+#endif
+#pragma omp parallel for num_threads(nthreads) schedule(dynamic, 16)
+    for (uint64_t j = 0; j < nframes; ++j) {
+        const u8 *R = rel + (size_t)j * n * n;
+        for (uint32_t b = 0; b < B; ++b) {
+            uint32_t cnt = 0;
+            for (uint64_t v = 0; v < nval; ++v) {
+                u8 V[MAXVARS][BIGN], t[BIGN];
+                for (int i = 0; i < k; ++i)
+                    for (int w = 0; w < n; ++w) V[i][w] = (u8)((v >> (i * n + w)) & 1u);
+                if (eval_program_big(code + offs[b], offs[b + 1] - offs[b], n, R, V, t)) bad = 1;
+                for (int w = 0; w < n; ++w) cnt += !t[w];
+            }
+            out[(size_t)b * nframes + j] = cnt;
+        }
+    }
+    return bad ? -1 : 0;
+}

@@ -35,6 +35,7 @@ EXPORTS = [
     "kripke_minimal_refutation", "kripke_pairs_separation", "kripke_debug_lower_wf",
     "kripke_eval_frames", "kripke_distinguish_pairs_frames",
     "kripke_validity_bitmap", "kripke_condition_bitmap", "kripke_match_bitmaps", "kripke_frames_from_bitmap",
+    "kripke_failure_density", "kripke_failure_density_frames",
 ]
 
 
@@ -90,6 +91,8 @@ def load():
     lib.kripke_validity_bitmap.argtypes = [vp, u32, u32, u32, u64, u64, vp, vp]
     lib.kripke_condition_bitmap.argtypes = [u32, u32, u32, u64, u64, vp, vp]
     lib.kripke_match_bitmaps.argtypes = [vp, u32, u64, vp, u32, vp, vp]
+    lib.kripke_failure_density.argtypes = [vp, u32, u32, u32, u64, u64, vp, vp]
+    lib.kripke_failure_density_frames.argtypes = [vp, u32, u32, vp, u64, vp, vp]
     lib.kripke_frames_from_bitmap.argtypes = [u32, u32, u64, u64, vp, vp, u64, vp, vp]
     lib.kripke_eval_frames.argtypes = [vp, u32, u32, vp, u64, u64, u32, vp, vp, vp]
     lib.kripke_distinguish_pairs_frames.argtypes = [vp, u32p, u32, u32, u32, vp, u64, u64, u32, vp, vp, vp]
@@ -309,6 +312,31 @@ def frames_from_bitmap(n_worlds: int, frame_class: int, frame_begin: int, frame_
            "kripke_frames_from_bitmap")
     n_set = int(count.item())
     return succ[:min(n_set, capacity) * n_worlds], n_set
+
+
+def failure_density(programs: Programs, n_worlds: int, n_vars: int, frame_class: int, frame_begin: int,
+                    frame_count: int, counts_out=None, stream=None):
+    """kripke_failure_density.  Returns an int32 CUDA tensor (B, frame_count) of failing (valuation, world)
+    pair counts."""
+    import torch
+    if counts_out is None:
+        counts_out = torch.zeros((programs.n_formulas, frame_count), dtype=torch.int32, device="cuda")
+    assert counts_out.is_cuda and counts_out.is_contiguous() and counts_out.numel() >= programs.n_formulas * frame_count
+    _check(load().kripke_failure_density(programs._h, n_worlds, n_vars, frame_class, frame_begin, frame_count,
+                                         counts_out.data_ptr(), _stream(stream)), "kripke_failure_density")
+    return counts_out
+
+
+def failure_density_frames(programs: Programs, n_worlds: int, n_vars: int, succ, counts_out=None, stream=None):
+    import torch
+    n_frames = _succ(succ, n_worlds)
+    if counts_out is None:
+        counts_out = torch.zeros((programs.n_formulas, n_frames), dtype=torch.int32, device="cuda")
+    assert counts_out.is_cuda and counts_out.is_contiguous() and counts_out.numel() >= programs.n_formulas * n_frames
+    _check(load().kripke_failure_density_frames(programs._h, n_worlds, n_vars, succ.data_ptr(), n_frames,
+                                                counts_out.data_ptr(), _stream(stream)),
+           "kripke_failure_density_frames")
+    return counts_out
 
 
 def bits_to_bool(bitmap, count: int):

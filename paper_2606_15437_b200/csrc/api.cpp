@@ -701,6 +701,45 @@ int kripke_condition_bitmap(uint32_t n_worlds, uint32_t condition, uint32_t fram
     return e ? cuda_fail(e) : KRIPKE_OK;
 }
 
+int kripke_failure_density(const kripke_programs_t *programs, uint32_t n_worlds, uint32_t n_vars,
+                           uint32_t frame_class, uint64_t frame_begin, uint64_t frame_count,
+                           uint32_t *counts_out, void *stream) {
+    if (!programs) return KRIPKE_EINVAL;
+    const kripke_programs *h = programs;
+    if (n_worlds < 1 || n_worlds > KRIPKE_MAX_WORLDS || n_vars != h->n_vars || frame_class > KRIPKE_CLASS_S5)
+        return KRIPKE_EINVAL;
+    if (n_vars * n_worlds > KRIPKE_LIST_MAX_VAL_BITS) return KRIPKE_EUNSUPPORTED;
+    uint64_t csize = 0;
+    int rc = class_size(n_worlds, frame_class, &csize);
+    if (rc) return rc;
+    if (frame_begin > csize || frame_count > csize - frame_begin) return KRIPKE_EINVAL;
+    if (frame_count && h->n_formulas && !counts_out) return KRIPKE_EINVAL;
+    ScanJob job;
+    job.n = n_worlds; job.k = n_vars; job.cls = frame_class;
+    job.frame_begin = frame_begin; job.frame_count = frame_count;
+    if ((rc = class_table_device(n_worlds, frame_class, &job.class_table))) return rc;
+    job.code = h->d_code; job.offsets = h->d_offsets; job.n_formulas = h->n_formulas;
+    job.pairs = nullptr; job.n_records = h->n_formulas; job.accum = nullptr;
+    int e = launch_failure_density(job, nullptr, counts_out, stream);
+    return e ? cuda_fail(e) : KRIPKE_OK;
+}
+
+int kripke_failure_density_frames(const kripke_programs_t *programs, uint32_t n_worlds, uint32_t n_vars,
+                                  const uint16_t *succ, uint64_t n_frames, uint32_t *counts_out, void *stream) {
+    if (!programs) return KRIPKE_EINVAL;
+    const kripke_programs *h = programs;
+    if (n_worlds < 1 || n_worlds > KRIPKE_LIST_MAX_WORLDS || n_vars != h->n_vars) return KRIPKE_EINVAL;
+    if (n_vars * n_worlds > KRIPKE_LIST_MAX_VAL_BITS) return KRIPKE_EUNSUPPORTED;
+    if (n_frames && (!succ || (h->n_formulas && !counts_out))) return KRIPKE_EINVAL;
+    ScanJob job;
+    job.n = n_worlds; job.k = n_vars; job.cls = KRIPKE_CLASS_K;
+    job.frame_begin = 0; job.frame_count = n_frames; job.class_table = nullptr;
+    job.code = h->d_code; job.offsets = h->d_offsets; job.n_formulas = h->n_formulas;
+    job.pairs = nullptr; job.n_records = h->n_formulas; job.accum = nullptr;
+    int e = launch_failure_density(job, succ, counts_out, stream);
+    return e ? cuda_fail(e) : KRIPKE_OK;
+}
+
 int kripke_frames_from_bitmap(uint32_t n_worlds, uint32_t frame_class, uint64_t frame_begin, uint64_t frame_count,
                               const uint32_t *bitmap, uint16_t *succ_out, uint64_t capacity, uint64_t *count_out,
                               void *stream) {

@@ -135,6 +135,45 @@ __global__ void __launch_bounds__(128) match_bitmaps_kernel(const uint32_t *bitm
     if (lane == 0) match_out[rec] = found;
 }
 
+// Failure densities (the atlas matrix): thread = frame, every valuation evaluated with the
+// scalar recurrence, count of worlds outside the truth set; blockIdx.y strides the formulas; the store
+// counts[b * frames + j] is coalesced over the frames of a warp.  Frames come from the class enumerator
+// or, if `succ_list` is set, from an explicit list (n <= 16).
+struct DensityParams {
+    uint32_t n, k, cls;
+    const uint64_t *class_table;
+    const uint16_t *succ_list;
+    uint64_t frame_begin, frame_count;
+    const uint8_t *code;
+    const uint32_t *offsets;
+    uint32_t n_formulas;
+    uint32_t *counts;
+};
+
+__global__ void __launch_bounds__(128) failure_density_kernel(DensityParams p) {
+    const uint64_t j = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= p.frame_count) return;
+    const uint32_t full = (p.n >= 32 ? 0xFFFFFFFFu : (1u << p.n) - 1u);
+    const uint64_t nval = 1ull << (p.k * p.n);
+    uint32_t succ[KRIPKE_LIST_MAX_WORLDS];
+    if (p.succ_list) {
+        for (uint32_t w = 0; w < p.n; ++w) succ[w] = p.succ_list[j * p.n + w];
+    } else {
+        decode_rows(p.n, class_frame(p.n, p.cls, p.class_table, p.frame_begin + j), succ);
+    }
+    for (uint32_t b = blockIdx.y; b < p.n_formulas; b += gridDim.y) {
+        const uint8_t *c = p.code + p.offsets[b];
+        const uint32_t len = p.offsets[b + 1] - p.offsets[b];
+        uint32_t cnt = 0;
+        for (uint64_t v = 0; v < nval; ++v) {
+            uint32_t val[KRIPKE_MAX_VARS];
+            for (uint32_t i = 0; i < KRIPKE_MAX_VARS; ++i) val[i] = (uint32_t)(v >> (i * p.n)) & full;
+            cnt += __popc(full & ~eval_postfix_scalar(c, len, p.n, succ, val, full));
+        }
+        p.counts[(uint64_t)b * p.frame_count + j] = cnt;
+    }
+}
+
 // Frames whose bit is set -> successor masks (input format of the frame-list calls).  Warp-aggregated
 // append: the order inside a warp is kept, the order of warps is not.
 __global__ void __launch_bounds__(128) frames_from_bitmap_kernel(ConditionParams p, uint16_t *succ_out,
@@ -198,6 +237,20 @@ int launch_frames_from_bitmap(uint32_t n, uint32_t cls, const uint64_t *class_ta
     if (bx > 0x7FFFFFFFull) return 801;
     frames_from_bitmap_kernel<<<(uint32_t)bx, 128, 0, (cudaStream_t)stream>>>(
         p, succ_out, (unsigned long long)capacity, reinterpret_cast<unsigned long long *>(count_out));
+    return (int)cudaGetLastError();
+}
+
+int launch_failure_density(const ScanJob &job, const uint16_t *succ_list, uint32_t *counts_out, void *stream) {
+    if (job.frame_count == 0 || job.n_formulas == 0) return 0;
+    DensityParams p;
+    p.n = job.n; p.k = job.k; p.cls = job.cls; p.class_table = job.class_table; p.succ_list = succ_list;
+    p.frame_begin = job.frame_begin; p.frame_count = job.frame_count;
+    p.code = job.code; p.offsets = job.offsets; p.n_formulas = job.n_formulas; p.counts = counts_out;
+    const uint64_t bx = (job.frame_count + 127) / 128;
+    if (bx > 0x7FFFFFFFull) return 801;
+    const uint32_t by = (uint32_t)std::min<uint64_t>(std::min<uint64_t>(job.n_formulas, 65535),
+                                                     std::max<uint64_t>(1, (148ull * 32 + bx - 1) / bx));
+    failure_density_kernel<<<dim3((uint32_t)bx, by), 128, 0, (cudaStream_t)stream>>>(p);
     return (int)cudaGetLastError();
 }
 

@@ -137,6 +137,8 @@ int launch_condition_bitmap(uint32_t n, uint32_t cond, uint32_t cls, const uint6
 int launch_frames_from_bitmap(uint32_t n, uint32_t cls, const uint64_t *class_table, uint64_t begin, uint64_t count,
                               const uint32_t *bitmap, uint16_t *succ_out, uint64_t capacity, uint64_t *count_out,
                               void *stream);
+// Failure densities: frames of job's class range, or of succ_list (job.frame_count masks rows) if not null.
+int launch_failure_density(const ScanJob &job, const uint16_t *succ_list, uint32_t *counts_out, void *stream);
 int launch_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words, const uint32_t *library,
                          uint32_t n_library, uint32_t *match_out, void *stream);
 

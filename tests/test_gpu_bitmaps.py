@@ -165,3 +165,32 @@ def test_k4_as_a_scan_class_by_composition(kb, vol):
     assert f in set(int(x) for x in frames)
     from oracle import kripke_oracle as O
     assert O.check_witness(progs[b], n, 2, K, f, int(got["wit_v"][b]), int(got["wit_w"][b]))
+
+
+def test_failure_density_panels_equal_the_oracle(kb, vol):
+    """The atlas matrix: Atlas-3 = every K frame of 1..3 worlds; panels of explicit four- and
+    five-world frames; a class range with a ragged size.  Counts of failing (valuation, world) pairs,
+    bit-exact against the oracle."""
+    import torch
+    from workloads import frames as F
+    progs = W.corpus_c2(250) + [AX[a] for a, _ in PAIRS]
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 2)
+    for n in (1, 2, 3):
+        total = 1 << (n * n)
+        got = kb.failure_density(h, n, 2, K, 0, total).cpu().numpy().view(np.uint32)
+        assert (got == vol.failure_counts(code, offs, n, 2)).all(), n
+    for n, count in ((4, 2048), (5, 1000), (8, 70)):
+        rel = F.stress_list(n, count)
+        k = 2 if n <= 5 else 1
+        pr = progs if k == 2 else [W.to_postfix(W.parse(t)) for t in ("[]p -> p", "<>[]p", "[]<>[]p | p", "F")]
+        c2, o2 = W.pack_programs(pr)
+        hh = kb.Programs(c2, o2, k)
+        succ = torch.from_numpy(F.succ_masks(rel).view(np.int16).reshape(-1).copy()).cuda()
+        got = kb.failure_density_frames(hh, n, k, succ).cpu().numpy().view(np.uint32)
+        assert (got == vol.failure_counts(c2, o2, n, k, rel=rel)).all(), n
+    got = kb.failure_density(h, 4, 2, S4, 3, 300).cpu().numpy().view(np.uint32)
+    assert (got == vol.failure_counts(code, offs, 4, 2, S4, 3, 300)).all()
+    # zero density <=> valid frame (the validity bitmap of the same range)
+    val = kb.bits_to_bool(kb.validity_bitmap(h, 4, 2, S4, 3, 300), 300)
+    assert ((got == 0) == val).all()

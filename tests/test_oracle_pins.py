@@ -354,3 +354,29 @@ def test_c_validity_bitmaps_are_the_correspondents(vol, n):
     # class order: the T-class bitmap is the K bitmap restricted to the reflexive frames
     tf = vol.class_frames(n, T)
     assert (vol.validity(code, offs, n, 2, T) == val[:, tf.astype(np.int64)]).all()
+
+
+def test_c_failure_counts_closed_forms_and_consistency(vol):
+    """D_ij counts the (valuation, world) pairs where formula i fails on frame j.  Closed forms: F
+    fails everywhere (n * 2^(kn)), T nowhere, p at half of the pairs; []F fails exactly at the worlds that
+    have a successor (P:215), under every valuation; a count is 0 iff the frame is valid for the formula;
+    the set-based oracle agrees pair by pair on two worlds; explicit relations = indexed frames."""
+    n, k = 3, 2
+    texts = ["F", "T", "p", "[]F", "[]p -> p", "p -> []<>p", "<>q & []p"]
+    progs = [prog(t) for t in texts]
+    code, offs = W.pack_programs(progs)
+    cnt = vol.failure_counts(code, offs, n, k)
+    pairs = n << (k * n)
+    assert (cnt[0] == pairs).all() and (cnt[1] == 0).all() and (cnt[2] == pairs // 2).all()
+    outdeg = np.array([sum(1 for w in range(n) if (f >> (w * n)) & 7) for f in range(1 << (n * n))])
+    assert (cnt[3] == outdeg << (k * n)).all()
+    assert ((cnt == 0) == vol.validity(code, offs, n, k).astype(bool)).all()
+    for f in (0, 5, 17, 300, 511):
+        R = O.relation_from_index(n, f)
+        for b, c in enumerate(progs):
+            phi = O.parse_postfix(c)
+            want = sum(1 for v in range(1 << (k * n)) for w in range(n)
+                       if not O.sat(n, R, O.valuation_from_index(n, k, v), w, phi))
+            assert int(cnt[b, f]) == want
+    rel = np.array([[[(f >> (w * n + u)) & 1 for u in range(n)] for w in range(n)] for f in range(1 << (n * n))], np.uint8)
+    assert (vol.failure_counts(code, offs, n, k, rel=rel) == cnt).all()
