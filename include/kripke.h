@@ -84,17 +84,16 @@ enum {
                                          and the others receive the same counts and first refuting
                                          frame; the witness valuation and world are computed per
                                          formula; results are identical either way)                */
-    KRIPKE_KERNEL_AUTO = 0u << 4,     /* bit-sliced kernel where it applies, else the scalar one  */
+    KRIPKE_KERNEL_AUTO = 0u << 4,     /* compiled bit-sliced kernels where the emitter covers the shape,
+                                         else the interpreted bit-sliced kernel, else the scalar one */
     KRIPKE_KERNEL_SCALAR = 1u << 4,   /* force the scalar kernel (Algorithm 1 restated, one model
                                          per thread iteration): baseline / ablation / cross-check */
-    KRIPKE_KERNEL_SLICED = 2u << 4,   /* force the bit-sliced kernel (never the warp-frame one);
-                                         KRIPKE_EUNSUPPORTED if the shape or a program does not fit */
-    KRIPKE_KERNEL_WARPFRAME = 3u << 4,/* experimental warp-frame kernel (warp-uniform frames as control
-                                         flow, values typed by modal depth) for every
-                                         program and frame it can take, the rest runs as in AUTO.
-                                         KRIPKE_EUNSUPPORTED if there is no instantiation for the shape
-                                         and class.  Exact, but slower than the bit-sliced kernel today,
-                                         so AUTO never picks it                                        */
+    KRIPKE_KERNEL_SLICED = 2u << 4,   /* force the interpreted bit-sliced kernel (micro-op dispatch, no
+                                         run-time compilation); KRIPKE_EUNSUPPORTED if the shape or a
+                                         program does not fit                                      */
+    KRIPKE_KERNEL_JIT = 3u << 4,      /* force the compiled bit-sliced kernels (see "Compiled scans"
+                                         below); KRIPKE_EUNSUPPORTED if the shape, class or range is
+                                         outside what the emitter covers                           */
     KRIPKE_KERNEL_MASK = 3u << 4,
     KRIPKE_REDUCE_BLOCK = 0u << 8,    /* scalar kernel only: one atomic pair per (block, formula),
                                          the paper's revised reduction                     */
@@ -277,8 +276,8 @@ int kripke_eval_batch_host(const uint8_t *code, const uint32_t *offsets, uint32_
  * after the call returns). */
 typedef struct {
     uint32_t launches;                    /* kernel launches enqueued                                  */
-    uint32_t kernel_family;               /* which family ran the bulk: 0 scalar, 1 bit-sliced,
-                                             2 warp-frame                                              */
+    uint32_t kernel_family;               /* which family ran the bulk: 0 scalar, 1 interpreted bit-sliced,
+                                             2 compiled bit-sliced                                     */
     uint64_t sliced_logic_ops_per_word;   /* 3-input logic instructions per 32-model word the lowered
                                              programs need, summed over the batch                      */
     uint64_t models_per_program;          /* definitional: (frames in range) * 2^(n_vars*n)            */
@@ -287,7 +286,7 @@ typedef struct {
     double logic_instr_per_frame;         /* 3-input logic thread-instructions the sliced kernel executes
                                              per frame of the range, summed over programs: the
                                              "algorithmic ops" of DESIGN.md's roofline                 */
-    uint32_t wf_programs;                 /* records the warp-frame kernel evaluated                    */
+    uint32_t jit_programs;                /* distinct programs the compiled kernels evaluated          */
     uint32_t reserved;
     double dense_logic_instr_per_frame;   /* the same programs costed as the bit-sliced kernel would run
                                              them (n^2 per modal operator, every word of every frame):
@@ -317,19 +316,12 @@ int kripke_keys_to_witness(const uint64_t *keys, uint32_t n_records, uint32_t n_
  * the bit-sliced kernel's 16-bit micro-ops (csrc/ucode.h: low byte op, high byte argument) and
  * copies them to ucode_out (capacity cap entries).  leaf_mode: bit 0 = "box F / dia T is a leaf",
  * bit 1 = "p_0, box p_0, dia p_0 are leaves" (what the kernel instantiation for a shape provides),
- * bit 2 = "fuse a load into the modal operator that follows it", bit 3 = "and into a Boolean operator
- * with a leaf".
+ * bit 2 = "fuse a load into the modal operator that follows it".
  * Returns the number of micro-ops, or a negative kripke_status (KRIPKE_EUNSUPPORTED if the program
  * needs more register-stack slots than the kernel has; *need_out is set in both cases). */
 int kripke_debug_lower(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b,
                        uint32_t n_vars, uint32_t leaf_mode, uint16_t *ucode_out, uint32_t cap,
                        uint32_t *need_out);
-
-/* Diagnostic (pure host, no CUDA): lowers one program to the warp-frame kernel's typed micro-ops
- * (csrc/wf_ucode.h).  Returns the number of micro-ops, or KRIPKE_EUNSUPPORTED if the program needs
- * more typed registers than that kernel keeps (it then runs on the bit-sliced kernel). */
-int kripke_debug_lower_wf(const uint8_t *code, uint32_t len, uint32_t n_vars, uint16_t *ucode_out,
-                          uint32_t cap);
 
 #ifdef __cplusplus
 }

@@ -20,7 +20,7 @@ CLASS_K, CLASS_T, CLASS_S4, CLASS_S5 = 0, 1, 2, 3
 ACCUMULATE = 1 << 0
 FULL_SWEEP = 1 << 1
 NO_SHARING = 1 << 2
-KERNEL_AUTO, KERNEL_SCALAR, KERNEL_SLICED, KERNEL_WARPFRAME = 0 << 4, 1 << 4, 2 << 4, 3 << 4
+KERNEL_AUTO, KERNEL_SCALAR, KERNEL_SLICED, KERNEL_JIT = 0 << 4, 1 << 4, 2 << 4, 3 << 4
 REDUCE_BLOCK, REDUCE_WARP, REDUCE_THREAD = 0 << 8, 1 << 8, 2 << 8
 NO_WITNESS = (1 << 64) - 1
 
@@ -32,7 +32,7 @@ EXPORTS = [
     "kripke_programs_destroy", "kripke_class_size", "kripke_eval_batch", "kripke_eval_batch_range",
     "kripke_distinguish_pairs", "kripke_eval_batch_host", "kripke_last_run_info",
     "kripke_calibrate_int32", "kripke_debug_lower", "kripke_witness_to_keys", "kripke_keys_to_witness",
-    "kripke_minimal_refutation", "kripke_pairs_separation", "kripke_debug_lower_wf",
+    "kripke_minimal_refutation", "kripke_pairs_separation",
     "kripke_eval_frames", "kripke_distinguish_pairs_frames",
     "kripke_validity_bitmap", "kripke_condition_bitmap", "kripke_match_bitmaps", "kripke_frames_from_bitmap",
     "kripke_failure_density", "kripke_failure_density_frames",
@@ -51,7 +51,7 @@ class RunInfo(ctypes.Structure):
     _fields_ = [("launches", ctypes.c_uint32), ("kernel_family", ctypes.c_uint32),
                 ("sliced_logic_ops_per_word", ctypes.c_uint64), ("models_per_program", ctypes.c_uint64),
                 ("executed_models", ctypes.c_uint64), ("logic_instr_per_frame", ctypes.c_double),
-                ("wf_programs", ctypes.c_uint32), ("reserved", ctypes.c_uint32),
+                ("jit_programs", ctypes.c_uint32), ("reserved", ctypes.c_uint32),
                 ("dense_logic_instr_per_frame", ctypes.c_double)]
 
 
@@ -87,7 +87,6 @@ def load():
     lib.kripke_witness_to_keys.argtypes = [vp, u32, u32, u32, vp, vp]
     lib.kripke_keys_to_witness.argtypes = [vp, u32, u32, u32, vp, vp]
     lib.kripke_debug_lower.argtypes = [u8p, u32, u8p, u32, u32, u32, u8p, u32, ctypes.POINTER(u32)]
-    lib.kripke_debug_lower_wf.argtypes = [u8p, u32, u32, u8p, u32]
     lib.kripke_validity_bitmap.argtypes = [vp, u32, u32, u32, u64, u64, vp, vp]
     lib.kripke_condition_bitmap.argtypes = [u32, u32, u32, u64, u64, vp, vp]
     lib.kripke_match_bitmaps.argtypes = [vp, u32, u64, vp, u32, vp, vp]
@@ -431,17 +430,6 @@ def debug_lower(code_a: bytes, code_b: bytes | None, n_vars: int, leaf_mode: int
         raise KripkeError(rc, "kripke_debug_lower")
     return [(int(x) & 0xFF, int(x) >> 8) for x in out[:rc]], need.value
 
-
-def debug_lower_wf(code: bytes, n_vars: int):
-    """[(op, arg), ...] of the warp-frame lowering, or None if the program does not fit that kernel."""
-    a = np.frombuffer(bytes(code), np.uint8).copy()
-    out = np.zeros(256, np.uint16)
-    rc = load().kripke_debug_lower_wf(a.ctypes.data, len(a), n_vars, out.ctypes.data, len(out))
-    if rc == -3:
-        return None
-    if rc < 0:
-        raise KripkeError(rc, "kripke_debug_lower_wf")
-    return [(int(x) & 0xFF, int(x) >> 8) for x in out[:rc]]
 
 
 def unpack(counts, witness):

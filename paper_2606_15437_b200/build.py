@@ -31,9 +31,7 @@ UNITS = [
     ("calibrate", "calibrate.cu", []),
     ("scan_frames", "scan_frames.cu", []),
     ("bitmaps", "bitmaps.cu", []),
-    ("wf_dispatch", "wf_dispatch.cpp", []),
 ] + [(f"scan_sliced_inst{g}", "scan_sliced_inst.cu", [f"-DKRIPKE_INST_GROUP={g}"]) for g in range(4)] \
-  + [(f"scan_wf_inst{g}", "scan_wf_inst.cu", [f"-DKRIPKE_WF_INST={g}"]) for g in range(5)] \
   + [(f"scan_frames_inst{g}", "scan_frames_inst.cu", [f"-DKRIPKE_FR_GROUP={g}"]) for g in range(4)]
 
 

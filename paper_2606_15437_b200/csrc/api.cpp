@@ -105,16 +105,12 @@ int upload_plan(const HostPlan &hp, DevicePlan *dp) {
 struct GroupPlan {
     uint32_t k_eff = 0;
     DevicePlan dp;                    // every record of the group, for the bit-sliced / scalar kernels
-    DevicePlan rest;                  // the records the warp-frame kernel cannot take
-    WfPlan wf;                        // the records it can (host micro-ops; they travel as kernel parameters)
-    uint32_t *d_wf_records = nullptr; // device: record index per warp-frame program
     uint32_t *d_alias = nullptr;      // device: (record, representative) pairs - records whose lowered program
     uint32_t n_alias = 0;             // equals the representative's are not scanned, they copy its accumulators
     void release() {
-        dp.release(); rest.release();
-        cudaFree(d_wf_records); cudaFree(d_alias);
-        d_wf_records = nullptr; d_alias = nullptr; n_alias = 0;
-        wf = WfPlan();
+        dp.release();
+        cudaFree(d_alias);
+        d_alias = nullptr; n_alias = 0;
     }
 };
 struct ScanPlan {
@@ -284,32 +280,16 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *d_pairs, 
     if (begin > csize || count > csize - begin) return KRIPKE_EINVAL;
     h->last = kripke_run_info_t{};
     h->last.models_per_program = count << (k * n);
-    // opt-in only: measured slower than the bit-sliced kernel, so AUTO does not pick it
-    const bool wf_allowed = family == KRIPKE_KERNEL_WARPFRAME;
-    if (family == KRIPKE_KERNEL_WARPFRAME && !wf_select(n, k, cls, nullptr)) return KRIPKE_EUNSUPPORTED;
-    // which groups run (partly) on the warp-frame kernel, and on which aligned sub-range
-    struct WfUse { bool on; uint64_t ab, ae; };
-    std::vector<WfUse> wf_use(plan.groups.size(), WfUse{false, begin, begin});
     for (size_t gi = 0; gi < plan.groups.size(); ++gi) {
         const GroupPlan &g = plan.groups[gi];
-        uint64_t fpu = 1;
-        if (wf_allowed && g.wf.n_progs && wf_select(n, g.k_eff, cls, &fpu)) {
-            const uint64_t ab = (begin + fpu - 1) / fpu * fpu, ae = (begin + count) / fpu * fpu;
-            if (ae > ab) wf_use[gi] = WfUse{true, ab, ae};
-        }
         // bookkeeping for the roofline: instructions the kernels need per frame of the range
         const double words = (double)(1ull << (g.k_eff * n)) / 32.0;
         auto dense = [&](const DevicePlan &dp) {
             return (double)(dp.n_modal * n * n + dp.n_bool * n + (uint64_t)dp.n_slots * (n + 1)) * words;
         };
-        const DevicePlan &old_part = wf_use[gi].on ? g.rest : g.dp;
-        h->last.sliced_logic_ops_per_word += old_part.n_modal * n * n + old_part.n_bool * n + (uint64_t)old_part.n_slots * (n + 1);
-        h->last.logic_instr_per_frame += dense(old_part);
+        h->last.sliced_logic_ops_per_word += g.dp.n_modal * n * n + g.dp.n_bool * n + (uint64_t)g.dp.n_slots * (n + 1);
+        h->last.logic_instr_per_frame += dense(g.dp);
         h->last.dense_logic_instr_per_frame += dense(g.dp);
-        if (wf_use[gi].on) {
-            for (const WfOpCounts &c : g.wf.counts) h->last.logic_instr_per_frame += wf_cost_per_frame(n, g.k_eff, cls, c);
-            h->last.wf_programs += g.wf.n_progs;
-        }
         h->last.executed_models += (uint64_t)(g.dp.n_slots + g.dp.n_unfit) * (count << (g.k_eff * n));
     }
     if (n_records == 0) return KRIPKE_OK;
@@ -398,25 +378,7 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *d_pairs, 
     for (size_t gi = 0; gi < plan.groups.size(); ++gi) {
         if (family == KRIPKE_KERNEL_SCALAR) break;
         const GroupPlan &g = plan.groups[gi];
-        if (wf_use[gi].on) {
-            // warp-frame kernel on the unit-aligned part, scalar kernel on the ragged ends
-            ScanJob wj = job;
-            wj.k = g.k_eff;
-            wj.frame_begin = wf_use[gi].ab; wj.frame_count = wf_use[gi].ae - wf_use[gi].ab;
-            WfPlan wp = g.wf;
-            wp.prog_record = g.d_wf_records;
-            wp.model_shift = (k - g.k_eff) * n;
-            h->last.kernel_family = 2;
-            if ((e = launch_wf(wj, wp, stream, &launches))) return cuda_fail(e);
-            ScanJob head = job, tail = job;
-            head.frame_count = wf_use[gi].ab - begin;
-            tail.frame_begin = wf_use[gi].ae; tail.frame_count = begin + count - wf_use[gi].ae;
-            if ((e = launch_scalar(head, g.d_wf_records, g.wf.n_progs, reduce, stream, &launches))) return cuda_fail(e);
-            if ((e = launch_scalar(tail, g.d_wf_records, g.wf.n_progs, reduce, stream, &launches))) return cuda_fail(e);
-            if ((rc = run_sliced_or_scalar(g.rest, g.k_eff))) return rc;
-        } else {
-            if ((rc = run_sliced_or_scalar(g.dp, g.k_eff))) return rc;
-        }
+        if ((rc = run_sliced_or_scalar(g.dp, g.k_eff))) return rc;
     }
     // records that share a representative's lowered program take its accumulators (the scalar family
     // scanned every record itself)
@@ -474,7 +436,7 @@ int build_scan_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_
                 bool ok = lower(mode);
                 if (ok && (mode & LOWER_FUSE) && !sliced_fuses(n, g, (uint32_t)low[i].need)) {
                     low[i] = Lowered();
-                    ok = lower(mode & ~(uint32_t)(LOWER_FUSE | LOWER_FUSE_BOOL));
+                    ok = lower(mode & ~(uint32_t)LOWER_FUSE);
                 }
                 return ok;
             };
@@ -536,46 +498,6 @@ int build_scan_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_
         if (!rc) rc = upload(&gp.d_alias, alias);
         if (rc) { gp.release(); out->release(); return rc; }
         gp.n_alias = (uint32_t)(alias.size() / 2);
-        // warp-frame kernel (single formulas, shapes it is instantiated for): the programs it can
-        // take are lowered to its typed micro-ops, the others keep a bit-sliced plan of their own
-        if (!pairs && (wf_select(n, g, KRIPKE_CLASS_K, nullptr) || wf_select(n, g, KRIPKE_CLASS_T, nullptr))) {
-            std::vector<uint32_t> wf_records;
-            std::vector<Lowered> rest_low;
-            std::vector<bool> rest_fits;
-            std::vector<uint32_t> rest_recs;
-            gp.wf.prog_off.push_back(0);
-            for (size_t i = 0; i < recs.size(); ++i) {
-                const uint32_t r = recs[i];
-                uint8_t rename[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
-                uint8_t next = 0;
-                for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v)
-                    if ((support[r] >> v) & 1u) rename[v] = next++;
-                if (g == k) for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v) rename[v] = (uint8_t)v;
-                WfLowered wl;
-                if (lower_wf_single(prog(r), plen(r), rename, &wl) && wl.ucode.size() <= WF_MAX_UCODE) {
-                    gp.wf.ucode.insert(gp.wf.ucode.end(), wl.ucode.begin(), wl.ucode.end());
-                    gp.wf.prog_off.push_back((uint32_t)gp.wf.ucode.size());
-                    gp.wf.counts.push_back(wl.counts);
-                    wf_records.push_back(r);
-                } else {
-                    rest_low.push_back(low[i]);
-                    rest_fits.push_back(fits[i]);
-                    rest_recs.push_back(r);
-                }
-            }
-            gp.wf.n_progs = (uint32_t)wf_records.size();
-            gp.wf.prog_record = nullptr;
-            gp.wf.model_shift = 0;
-            HostPlan rp;
-            build_plan(rest_low, rest_fits, &rp);
-            for (auto &x : rp.slot_record) x = rest_recs[x];
-            for (auto &x : rp.unfit) x = rest_recs[x];
-            if ((rc = upload_plan(rp, &gp.rest)) || (rc = upload(&gp.d_wf_records, wf_records))) {
-                gp.release(); out->release(); return rc;
-            }
-        } else {
-            gp.wf.n_progs = 0;
-        }
         out->groups.push_back(gp);
     }
     return KRIPKE_OK;
@@ -620,7 +542,6 @@ int run_frames(kripke_programs *h, const DevicePlan &dp, const uint32_t *d_pairs
     if (k * n > KRIPKE_LIST_MAX_VAL_BITS) return KRIPKE_EUNSUPPORTED;
     if (flags & ~(KRIPKE_ACCUMULATE | KRIPKE_KERNEL_MASK)) return KRIPKE_EINVAL;
     const uint32_t family = flags & KRIPKE_KERNEL_MASK;
-    if (family == KRIPKE_KERNEL_WARPFRAME) return KRIPKE_EUNSUPPORTED;
     if (n_frames && !succ) return KRIPKE_EINVAL;
     if (n_frames > (1ull << 40)) return KRIPKE_EUNSUPPORTED;
     if (n_records && (!counts_out || !witness_out)) return KRIPKE_EINVAL;
@@ -1042,7 +963,7 @@ int kripke_debug_lower(const uint8_t *code_a, uint32_t len_a, const uint8_t *cod
     if (rc == KRIPKE_OK && code_b) rc = validate_programs(code_b, offs_b, 1, n_vars, nullptr);
     if (rc) return rc;
     Lowered low;
-    if (leaf_mode > (LOWER_LEAF_DEAD | LOWER_LEAF_P | LOWER_FUSE | LOWER_FUSE_BOOL)) return KRIPKE_EINVAL;
+    if (leaf_mode > (LOWER_LEAF_DEAD | LOWER_LEAF_P | LOWER_FUSE)) return KRIPKE_EINVAL;
     const bool fits = code_b ? lower_pair(code_a, len_a, code_b, len_b, leaf_mode, nullptr, &low)
                              : lower_single(code_a, len_a, leaf_mode, nullptr, &low);
     if (need_out) *need_out = (uint32_t)low.need;
@@ -1050,18 +971,6 @@ int kripke_debug_lower(const uint8_t *code_a, uint32_t len_a, const uint8_t *cod
     if (low.ucode.size() > cap) return KRIPKE_EINVAL;
     std::memcpy(ucode_out, low.ucode.data(), low.ucode.size() * sizeof(uint16_t));
     return (int)low.ucode.size();
-}
-
-int kripke_debug_lower_wf(const uint8_t *code, uint32_t len, uint32_t n_vars, uint16_t *ucode_out, uint32_t cap) {
-    if (!code || !ucode_out) return KRIPKE_EINVAL;
-    const uint32_t offs[2] = {0, len};
-    int rc = validate_programs(code, offs, 1, n_vars, nullptr);
-    if (rc) return rc;
-    WfLowered wl;
-    if (!lower_wf_single(code, len, nullptr, &wl)) return KRIPKE_EUNSUPPORTED;
-    if (wl.ucode.size() > cap) return KRIPKE_EINVAL;
-    std::memcpy(ucode_out, wl.ucode.data(), wl.ucode.size() * sizeof(uint16_t));
-    return (int)wl.ucode.size();
 }
 
 int kripke_calibrate_int32(uint32_t variant, double *thread_instr_per_s_out, double *elapsed_ms_out,

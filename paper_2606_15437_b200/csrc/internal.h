@@ -6,7 +6,6 @@
 
 #include "../../include/kripke.h"
 #include "ucode.h"
-#include "wf_ucode.h"
 
 namespace kripke {
 
@@ -25,13 +24,6 @@ uint32_t program_support(const uint8_t *code, uint32_t len);
 bool lower_single(const uint8_t *code, uint32_t len, uint32_t mode, const uint8_t *rename, Lowered *out);
 bool lower_pair(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b, uint32_t mode,
                 const uint8_t *rename, Lowered *out);
-
-// Warp-frame lowering (wf_ucode.h); false if the program needs registers the kernel does not have.
-struct WfLowered {
-    std::vector<uint16_t> ucode;  // typed micro-ops, FIN last
-    WfOpCounts counts;
-};
-bool lower_wf_single(const uint8_t *code, uint32_t len, const uint8_t *rename, WfLowered *out);
 
 // ---- device-side job description (kernels) -----------------------------------------------------
 // Accumulators per output record, owned by the programs handle, zeroed at the start of a call.
@@ -85,31 +77,6 @@ int launch_sliced(const ScanJob &job, const SlicedPlan &plan, void *stream, uint
 // Enqueue the scalar (Algorithm 1) scan over the records listed in `records` (device, or null = all).
 int launch_scalar(const ScanJob &job, const uint32_t *records, uint32_t n_list, uint32_t reduce_mode,
                   void *stream, uint32_t *launches);
-// ---- warp-frame kernel (scan_wf_inst.cu) -------------------------------------------------------
-// Host copy of the lowered programs of one variable-count group that fit the warp-frame kernel.
-struct WfPlan {
-    std::vector<uint16_t> ucode;       // concatenated micro-ops
-    std::vector<uint32_t> prog_off;    // n_progs + 1 offsets into ucode
-    std::vector<WfOpCounts> counts;    // per program
-    const uint32_t *prog_record = nullptr;   // device: record index per program
-    uint32_t n_progs = 0;
-    uint32_t model_shift = 0;          // refuting models are counted x 2^model_shift
-};
-// One instantiation of the warp-frame kernel (scan_wf_inst.cu defines kWfRow0..; wf_dispatch.cpp lists them).
-struct WfRow {
-    uint32_t n, k, cls;
-    uint64_t frames_per_unit;
-    int (*launch)(const ScanJob &, const WfPlan &, void *, uint32_t *);
-    double (*cost)(const WfOpCounts &);
-};
-// Is there a warp-frame instantiation for (n, k, class)?  *frames_per_unit: range alignment needed.
-bool wf_select(uint32_t n, uint32_t k, uint32_t cls, uint64_t *frames_per_unit);
-// Enqueue the warp-frame scan of job's range (aligned to frames_per_unit); cudaError_t as int.
-int launch_wf(const ScanJob &job, const WfPlan &plan, void *stream, uint32_t *launches);
-// Logic instructions (3-input logic + popc + add; no moves, no dispatch) the warp-frame kernel needs
-// per frame of the class for one program, averaged over the class.
-double wf_cost_per_frame(uint32_t n, uint32_t k, uint32_t cls, const WfOpCounts &c);
-
 // ---- frame-list mode (scan_frames.cu) ----------------------------------------------------------
 struct FramesJob {
     uint32_t n, k;

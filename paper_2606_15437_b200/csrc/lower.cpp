@@ -220,114 +220,6 @@ struct Lowerer {
         }
         }
     }
-
-    // ---- warp-frame lowering (wf_ucode.h): values typed by modal depth --------------------------
-    struct WVal { int type, loc, pol; bool ok; };
-    struct WAtom { bool is; uint8_t arg; int pol; };
-    WfOpCounts wc;
-
-    int mdepth(int i) const {
-        const Node &nd = nodes[i];
-        switch (nd.kind) {
-        case N_CONST: case N_VAR: return 0;
-        case N_NOT: return mdepth(nd.a);
-        case N_BOX: case N_DIA: return 1 + mdepth(nd.a);
-        default: return std::max(mdepth(nd.a), mdepth(nd.b));
-        }
-    }
-    int wtype(int i) const { return std::min(2, mdepth(i)); }
-    WAtom watom(int i) const {
-        int pol = 0;
-        while (nodes[i].kind == N_NOT) { pol ^= 1; i = nodes[i].a; }
-        if (nodes[i].kind == N_VAR) return WAtom{true, (uint8_t)(WF_ATOM_VAR0 + nodes[i].value), pol};
-        return WAtom{false, 0, 0};
-    }
-    static WVal wfail() { return WVal{0, 0, 0, false}; }
-    static int bool_fn_of(int a1, int a2) {
-        return (!a1 && !a2) ? BF_AND : (!a1 && a2) ? BF_ANDN : (a1 && !a2) ? BF_NAND : BF_OR;
-    }
-    void count_bool(int type) { ++(type == 0 ? wc.bool_s : type == 1 ? wc.bool_h : wc.bool_f); }
-
-    // Emits micro-ops leaving node i's value in typed registers.  ns / nh: S and H slots in use by
-    // pending operands; fbusy: F buffer held by a pending operand (-1: none).
-    WVal wf_emit(int i, int ns, int nh, int fbusy) {
-        int pol = 0;
-        while (nodes[i].kind == N_NOT) { pol ^= 1; i = nodes[i].a; }
-        const Node nd = nodes[i];
-        switch (nd.kind) {
-        case N_CONST: case N_VAR:
-            if (ns >= WF_S_SLOTS) return wfail();
-            op(WF_LOADA + ns, nd.kind == N_VAR ? (uint32_t)(WF_ATOM_VAR0 + nd.value) : (uint32_t)WF_ATOM_FALSE);
-            return WVal{0, ns, pol ^ (nd.kind == N_CONST ? (int)nd.value : 0), true};
-        case N_BOX: case N_DIA: {
-            const WVal v = wf_emit(nd.a, ns, nh, fbusy);
-            if (!v.ok) return v;
-            // box ~s = ~dia s ; dia ~s = ~box s
-            const int t = ((nd.kind == N_BOX) != (v.pol != 0)) ? 0 : 1;
-            if (v.type == 0) {
-                if (v.loc != 0 || nh >= WF_H_SLOTS) return wfail();
-                op(WF_S2H + t * 2 + nh);
-                ++wc.modal_s;
-                return WVal{1, nh, pol ^ v.pol, true};
-            }
-            ++wc.modal_hf;
-            if (v.type == 1) {
-                if (v.loc != 0 || fbusy >= 0) return wfail();
-                op(WF_H2F + t * 2 + 0);
-                return WVal{2, 0, pol ^ v.pol, true};
-            }
-            op(WF_MF + t * 2 + v.loc);
-            return WVal{2, 1 - v.loc, pol ^ v.pol, true};
-        }
-        default: break;
-        }
-        // binary connective as a conjunction of literals: and = x & y ; or = ~(~x & ~y) ; imp = ~(x & ~y)
-        const int negx = (nd.kind == N_OR), negy = (nd.kind != N_AND), flip = (nd.kind != N_AND);
-        const WAtom la = watom(nd.a), lb = watom(nd.b);
-        if (la.is || lb.is) {
-            const bool b_atom = lb.is;                   // both atoms: x is loaded, y is the operand
-            const WAtom at = b_atom ? lb : la;
-            const WVal v = wf_emit(b_atom ? nd.a : nd.b, ns, nh, fbusy);
-            if (!v.ok) return v;
-            const int a1 = v.pol ^ (b_atom ? negx : negy), a2 = at.pol ^ (b_atom ? negy : negx);
-            const int f = bool_fn_of(a1, a2);
-            if (v.type == 0) op(WF_BSA + f * 4 + v.loc, at.arg);
-            else if (v.type == 1) op(WF_BHA + f * 2 + v.loc, at.arg);
-            else op(WF_BFA + f * 2 + v.loc, at.arg);
-            count_bool(v.type);
-            return WVal{v.type, v.loc, pol ^ ((f == BF_OR) ? !flip : flip), true};
-        }
-        const int ta = wtype(nd.a), tb = wtype(nd.b);
-        const bool a_first = (ta != tb) ? (ta > tb) : (nodes[nd.a].need >= nodes[nd.b].need);
-        const WVal v1 = wf_emit(a_first ? nd.a : nd.b, ns, nh, fbusy);
-        if (!v1.ok) return v1;
-        const WVal v2 = wf_emit(a_first ? nd.b : nd.a, ns + (v1.type == 0), nh + (v1.type == 1),
-                                v1.type == 2 ? v1.loc : fbusy);
-        if (!v2.ok) return v2;
-        const int px = a_first ? v1.pol : v2.pol, py = a_first ? v2.pol : v1.pol;
-        const int ax = px ^ negx, ay = py ^ negy;
-        const int f = bool_fn_of(a_first ? ax : ay, a_first ? ay : ax);      // by register: v1, v2
-        if (v1.type == 0 && v2.type == 0) {
-            if (v2.loc != v1.loc + 1 || v1.loc > 2) return wfail();
-            op(WF_BSS + f * 4 + v1.loc);
-        } else if (v1.type == 1 && v2.type == 0) {
-            if (v2.loc != 0) return wfail();
-            op(WF_BHS + f * 2 + v1.loc);
-        } else if (v1.type == 1 && v2.type == 1) {
-            if (v1.loc != 0 || v2.loc != 1) return wfail();
-            op(WF_BHH + f);
-        } else if (v1.type == 2 && v2.type == 0) {
-            if (v2.loc != 0) return wfail();
-            op(WF_BFS + f * 2 + v1.loc);
-        } else if (v1.type == 2 && v2.type == 1) {
-            if (v2.loc != 0) return wfail();
-            op(WF_BFH + f * 2 + v1.loc);
-        } else {
-            return wfail();                          // two live F values (or an ordering slip)
-        }
-        count_bool(v1.type);
-        return WVal{v1.type, v1.loc, pol ^ ((f == BF_OR) ? !flip : flip), true};
-    }
 };
 
 }  // namespace
@@ -366,34 +258,21 @@ uint32_t program_support(const uint8_t *code, uint32_t len) {
 }
 
 // LOWER_FUSE: a load followed by a modal operator on the same slot becomes one fused micro-op.
-// LOWER_FUSE_BOOL also fuses a load into a Boolean operator with a leaf (measured slower on the
-// census corpus, so the kernels' lowering mode leaves it off).
-static void fuse_loads(std::vector<uint16_t> &uc, bool fuse_bool) {
+static void fuse_loads(std::vector<uint16_t> &uc) {
     std::vector<uint16_t> out;
     out.reserve(uc.size());
-    auto swap_fn = [](uint32_t f) { return f == BF_ANDN ? (uint32_t)BF_NAND : f == BF_NAND ? (uint32_t)BF_ANDN : f; };
     for (size_t i = 0; i < uc.size(); ++i) {
         const uint32_t op = uc[i] & 0xFFu, arg = uc[i] >> 8;
         if (i + 1 < uc.size()) {
-            const uint32_t op2 = uc[i + 1] & 0xFFu, arg2 = uc[i + 1] >> 8;
+            const uint32_t op2 = uc[i + 1] & 0xFFu;
             if (op < UC_BOOLV) {                                        // LOADV i, d
                 const uint32_t iv = op >> 2, d = op & 3u;
                 if (d == 0 && op2 == UC_BOX + d) { out.push_back((uint16_t)(UC_BOXV0 + iv)); ++i; continue; }
                 if (d == 0 && op2 == UC_DIA + d) { out.push_back((uint16_t)(UC_DIAV0 + iv)); ++i; continue; }
-                if (fuse_bool && op2 >= UC_BOOLL && op2 < UC_BOOL && ((op2 - UC_BOOLL) & 3u) == d) {   // f(p_i, leaf)
-                    const uint32_t f = (op2 - UC_BOOLL) >> 2;
-                    out.push_back((uint16_t)((UC_BOOLVL + f * 4 + d) | ((arg2 | (iv << 4)) << 8)));
-                    ++i; continue;
-                }
             } else if (op >= UC_LOADL && op < UC_BOOLL) {               // LOADL leaf, d
                 const uint32_t d = op - UC_LOADL;
                 if (op2 == UC_BOX + d) { out.push_back((uint16_t)((UC_BOXL + d) | (arg << 8))); ++i; continue; }
                 if (op2 == UC_DIA + d) { out.push_back((uint16_t)((UC_DIAL + d) | (arg << 8))); ++i; continue; }
-                if (fuse_bool && op2 >= UC_BOOLV && op2 < UC_LOADL && ((op2 - UC_BOOLV) & 3u) == d) {  // f(leaf, p_i) = f'(p_i, leaf)
-                    const uint32_t y = op2 - UC_BOOLV, iv = (y >> 2) & 3u, f = swap_fn(y >> 4);
-                    out.push_back((uint16_t)((UC_BOOLVL + f * 4 + d) | ((arg | (iv << 4)) << 8)));
-                    ++i; continue;
-                }
             }
         }
         out.push_back(uc[i]);
@@ -410,7 +289,7 @@ bool lower_single(const uint8_t *code, uint32_t len, uint32_t mode, const uint8_
     if (out->need > UC_DMAX) return false;
     int p = lw.emit(root, 0);
     lw.op(p ? UC_FIN_ANY : UC_FIN_ALL);
-    if (mode & LOWER_FUSE) fuse_loads(lw.out, (mode & LOWER_FUSE_BOOL) != 0);
+    if (mode & LOWER_FUSE) fuse_loads(lw.out);
     out->ucode = std::move(lw.out);
     out->n_modal = lw.n_modal;
     out->n_bool = lw.n_bool;
@@ -432,27 +311,10 @@ bool lower_pair(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, ui
     int pa = lw.emit(ra, 0);
     int pb = lw.emit(rb, 1);
     lw.op(pa == pb ? UC_FIN_XOR : UC_FIN_XNOR);
-    if (mode & LOWER_FUSE) fuse_loads(lw.out, (mode & LOWER_FUSE_BOOL) != 0);
+    if (mode & LOWER_FUSE) fuse_loads(lw.out);
     out->ucode = std::move(lw.out);
     out->n_modal = lw.n_modal;
     out->n_bool = lw.n_bool;
-    return true;
-}
-
-bool lower_wf_single(const uint8_t *code, uint32_t len, const uint8_t *rename, WfLowered *out) {
-    Lowerer lw;
-    lw.mode = 0;
-    if (rename) std::copy(rename, rename + KRIPKE_MAX_VARS, lw.rename);
-    const int root = lw.build(code, len);
-    lw.need(root);                               // Sethi-Ullman numbers break ties between equal types
-    const Lowerer::WVal v = lw.wf_emit(root, 0, 0, -1);
-    if (!v.ok || v.loc > 1 || (v.type != 2 && v.loc != 0)) return false;
-    if (v.type == 0) lw.op(WF_FIN_S + v.pol);
-    else if (v.type == 1) lw.op(WF_FIN_H + v.pol);
-    else lw.op(WF_FIN_F + v.pol * 2 + v.loc);
-    lw.wc.fin_type = (uint32_t)v.type;
-    out->ucode = std::move(lw.out);
-    out->counts = lw.wc;
     return true;
 }
 

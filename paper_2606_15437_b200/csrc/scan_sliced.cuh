@@ -301,21 +301,6 @@ struct SlicedThread {
                 }
         }
     }
-    // D[d] <- F(p_i, leaf), arg = leaf | i << 4
-    template <int d, int F> __device__ __forceinline__ void bool_var_leaf(uint32_t arg) {
-        if (d >= DMAX) return;
-        constexpr int dd = d < DMAX ? d : 0;
-        const uint32_t l = arg & 15u, iv = arg >> 4;
-#pragma unroll
-        for (int i = 0; i < C::K; ++i) {
-            if ((C::P_LEAF && i == 0) || iv != (uint32_t)i) continue;
-#pragma unroll
-            for (int m = 0; m < M; ++m)
-#pragma unroll
-                for (int w = 0; w < N; ++w)
-                    D[dd][m][w] = bool_fn<F>(atom(i, m, w), leaf_word(l, C::FRAME_PER_UNIT ? 0 : m, w));
-        }
-    }
     template <int d, int F> __device__ __forceinline__ void boolean() {
         if (d + 1 >= DMAX) return;
         constexpr int dd = d + 1 < DMAX ? d : 0, d1 = d + 1 < DMAX ? d + 1 : 1;
@@ -416,19 +401,9 @@ struct SlicedThread {
                 case UC_DIAV0 + 2: modal_var0<2, false>(); break; case UC_DIAV0 + 3: modal_var0<3, false>(); break;
 #define BXL(d) modal_leaf<d, true>(arg)
 #define DXL(d) modal_leaf<d, false>(arg)
-#define BVL0(d) bool_var_leaf<d, 0>(arg)
-#define BVL1(d) bool_var_leaf<d, 1>(arg)
-#define BVL2(d) bool_var_leaf<d, 2>(arg)
-#define BVL3(d) bool_var_leaf<d, 3>(arg)
                 KRIPKE_CASE4(UC_BOXL, BXL) KRIPKE_CASE4(UC_DIAL, DXL)
-                KRIPKE_CASE4(UC_BOOLVL + 0, BVL0) KRIPKE_CASE4(UC_BOOLVL + 4, BVL1)
-                KRIPKE_CASE4(UC_BOOLVL + 8, BVL2) KRIPKE_CASE4(UC_BOOLVL + 12, BVL3)
 #undef BXL
 #undef DXL
-#undef BVL0
-#undef BVL1
-#undef BVL2
-#undef BVL3
 #undef LV0
 #undef LV1
 #undef LV2

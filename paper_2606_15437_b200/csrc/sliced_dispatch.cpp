@@ -1,8 +1,6 @@
 // sliced_dispatch.cpp - shape table of the bit-sliced kernel instantiations (scan_sliced_inst.cu).
 #include "internal.h"
 
-#include <cstdlib>
-
 namespace kripke {
 
 typedef int (*sliced_launch_fn)(const ScanJob &, const SlicedPlan &, void *, uint32_t *);
@@ -31,11 +29,8 @@ bool frame_per_unit(const Row &r) { return r.k * r.n >= 5 + r.mb; }
 // the most words per thread.
 const Row *find(uint32_t n, uint32_t k, uint32_t cls, uint32_t need) {
     const Row *best = nullptr;
-    static const char *cap_env = std::getenv("KRIPKE_MB_CAP");        // tuning aid: cap words per thread
-    const uint32_t mb_cap = cap_env ? (uint32_t)std::atoi(cap_env) : 99u;
     for (const Row &r : kRows) {
         if (r.n != n || r.k != k || r.dmax < need) continue;
-        if (r.mb > mb_cap && frame_per_unit(r)) continue;
         // group-per-unit shapes enumerate frames from the model index: class K only
         if (!frame_per_unit(r) && cls != KRIPKE_CLASS_K) continue;
         if (!best || r.dmax < best->dmax || (r.dmax == best->dmax && r.mb > best->mb)) best = &r;
@@ -57,9 +52,7 @@ uint32_t sliced_row(uint32_t n, uint32_t k, uint32_t cls, uint32_t need) {
 }
 
 uint32_t sliced_lower_mode(uint32_t n, uint32_t k, uint32_t cls) {
-    // tuning aid / test hook: KRIPKE_FUSE_BOOL=1 also fuses loads into Boolean operators (UC_BOOLVL)
-    static const char *fb_env = std::getenv("KRIPKE_FUSE_BOOL");
-    const uint32_t fuse = LOWER_FUSE | ((fb_env && std::atoi(fb_env)) ? (uint32_t)LOWER_FUSE_BOOL : 0u);
+    const uint32_t fuse = LOWER_FUSE;
     // every row of one (n, k) that a class can use has the same layout kind (see SHAPES above)
     const Row *r = find(n, k, cls, 1);
     if (!r) return 0;

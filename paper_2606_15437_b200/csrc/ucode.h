@@ -31,9 +31,7 @@ enum : uint8_t { LEAF_P = 0, LEAF_DEAD = 1, LEAF_BOXP = 2, LEAF_DIAP = 3, LEAF_C
 enum : uint32_t {
     LOWER_LEAF_DEAD = 1u << 0,   // box F / dia T as a leaf
     LOWER_LEAF_P = 1u << 1,      // p_0, box p_0, dia p_0 as leaves (p_0 lies inside the 32-model word)
-    LOWER_FUSE = 1u << 2,        // fold a load into the modal operator that follows it (fused ops below)
-    LOWER_FUSE_BOOL = 1u << 3    // also into a Boolean operator with a leaf (UC_BOOLVL); measured slower on
-                                 // the census corpus, so no kernel asks for it by default
+    LOWER_FUSE = 1u << 2         // fold a load into the modal operator that follows it (fused ops below)
 };
 
 // Boolean functions of (slot value a, operand b); the lowering picks one by the two polarities
@@ -56,8 +54,7 @@ enum : uint8_t {
     UC_BOXV0 = 132,   // + i                : D[0] <- box p_i
     UC_DIAV0 = 136,   // + i                : D[0] <- dia p_i
     UC_BOXL = 140,    // + d   (arg = leaf) : D[d] <- box leaf
-    UC_DIAL = 144,    // + d   (arg = leaf) : D[d] <- dia leaf
-    UC_BOOLVL = 148   // + f*4 + d (arg = leaf | i << 4) : D[d] <- f(p_i, leaf)   (LOWER_FUSE_BOOL)
+    UC_DIAL = 144     // + d   (arg = leaf) : D[d] <- dia leaf
 };
 
 }  // namespace kripke

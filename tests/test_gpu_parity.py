@@ -165,39 +165,6 @@ def test_n5_closed_forms_full_range(kb):
     assert int(run(kb, [progs[3]], 5, 2, S5)["models"][0]) == 0 and int(run(kb, [progs[3]], 5, 2, S4)["models"][0]) > 0
 
 
-def test_warp_frame_kernel_windows_live(kb, vol):
-    """The warp-frame kernel (class K and T at n=5; every variable-count group) against the oracle
-    run live on windows that hold whole scan units of each group (8 / 256 / 8,192 frames) plus ragged
-    ends, and against the bit-sliced kernel on the whole corpus."""
-    progs = W.corpus_c2()[::12] + [W.to_postfix(t) for t in W.named_axioms().values()]
-    code, offs = W.pack_programs(progs)
-    h = kb.Programs(code, offs, 2)
-    for cls, begin, count in ((K, 8192 * 122 - 5, 8500), (T, 8192 * 50 - 5, 8500), (K, (1 << 25) - 8192, 8192)):
-        want = vol.census(code, offs, 5, 2, cls, begin, count)
-        got = run(kb, progs, 5, 2, cls, begin, count, flags=kb.KERNEL_WARPFRAME | kb.NO_SHARING, handle=h)
-        info = h.last_run_info()
-        assert info.kernel_family == 2 and info.wf_programs > 0.9 * len(progs)
-        same(run(kb, progs, 5, 2, cls, begin, count, flags=kb.KERNEL_WARPFRAME, handle=h), got, "warp-frame, shared")
-        same(got, want, f"warp-frame cls={cls} [{begin},+{count})")
-        certify(progs, got, 5, 2, cls, idx=range(0, len(progs), 9))
-        same(run(kb, progs, 5, 2, cls, begin, count, handle=h), want, "auto")
-        assert h.last_run_info().kernel_family == 1
-    allp = W.corpus_c2()
-    ha = kb.Programs(*W.pack_programs(allp), 2)
-    for cls, begin, count in ((K, 3 << 20, 1 << 15), (T, 1 << 19, 1 << 14)):
-        a = run(kb, allp, 5, 2, cls, begin, count, flags=kb.KERNEL_WARPFRAME, handle=ha)
-        assert ha.last_run_info().kernel_family == 2
-        b = run(kb, allp, 5, 2, cls, begin, count, flags=kb.KERNEL_SLICED | kb.FULL_SWEEP, handle=ha)
-        assert ha.last_run_info().kernel_family == 1
-        same(a, b, f"warp-frame vs bit-sliced cls={cls}")
-    # a class without an instantiation cannot be forced
-    import torch
-    c = torch.zeros((len(progs), 2), dtype=torch.int64, device="cuda")
-    w = torch.zeros((len(progs), 2), dtype=torch.int64, device="cuda")
-    rc = kb.load().kripke_eval_batch_range(h._h, 5, 2, S4, 0, 64, kb.KERNEL_WARPFRAME, c.data_ptr(), w.data_ptr(), None)
-    assert rc == kb.EUNSUPPORTED
-
-
 def test_c4_three_variables_ranges_golden(kb):
     g = gold("c4_ranges.npz")
     progs = W.corpus_c4()
@@ -490,34 +457,6 @@ def test_variable_support_reduction_is_exact(kb, vol):
     want = vol.census(sc, so, 4, 3, K, 100, 64)
     same(run(kb, sub, 4, 3, K, 100, 64), want, "k=3 reduced")
     same(run(kb, sub, 4, 3, K, 100, 64, flags=kb.FULL_SWEEP), want, "k=3 full")
-
-
-def test_fused_boolean_lowering_in_a_subprocess(vol):
-    """The UC_BOOLVL micro-op (a load fused into a Boolean operator) is off by default because it
-    measured slower; KRIPKE_FUSE_BOOL=1 turns it on.  Same C1 / C2-sample parity with it on."""
-    import subprocess
-    import sys
-    script = r'''
-import numpy as np
-import workloads as W
-from oracle import volume as V
-from paper_2606_15437_b200 import binding as kb
-V.build()
-for progs, n, k, count in ((W.corpus_c1(), 3, 2, 512), (W.corpus_c2()[:600], 5, 2, 4096)):
-    code, offs = W.pack_programs(progs)
-    h = kb.Programs(code, offs, k)
-    for cls in (0, 1):
-        cnt = min(count, kb.class_size(n, cls))
-        got = kb.unpack(*kb.eval_batch_range(h, n, k, cls, 0, cnt))
-        want = V.census(code, offs, n, k, cls, 0, cnt)
-        for key in ("models", "frames", "wit_f", "wit_v", "wit_w"):
-            assert (np.asarray(got[key]).astype(np.uint64) == np.asarray(want[key]).astype(np.uint64)).all(), (n, cls, key)
-print("fused-bool parity ok")
-'''
-    env = dict(os.environ, KRIPKE_FUSE_BOOL="1")
-    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    res = subprocess.run([sys.executable, "-c", script], cwd=root, env=env, capture_output=True, text=True, timeout=900)
-    assert res.returncode == 0 and "fused-bool parity ok" in res.stdout, res.stdout + res.stderr
 
 
 def test_program_sharing_is_exact(kb, vol):
