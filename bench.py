@@ -379,21 +379,35 @@ def run_c4(args):
     t_fused = timed(lambda: kb.eval_batch_range(h32, n, k, 0, begin, count, 0, c, w))
     out["fusion"] = {"formulas": 32, "frames": count, "separate_s": t_sep, "fused_s": t_fused,
                      "fused_speedup": t_sep / t_fused}
-    # C. atomic contention on the scalar kernel (the paper's layout), 2^12-frame range
-    begin, count = 1 << 24, 1 << 12
-    mixed = progs[:64]
-    adversarial = [W.to_postfix(("and", ("bot",), W.from_postfix(p))) for p in progs[:64]]   # every model refutes
+    # C. atomic contention on the scalar kernel (the paper's layout: thread = frame, one model per iteration),
+    # SURVEY 8(d) shape: 256 formulas x K-frames [2^24, 2^24 + 2^20), "mixed" = the batch of 256 as it is,
+    # "adversarial" = F & (each formula): every model refutes every formula.  One timed pass per
+    # mode (each pass is 8.8e12 evaluations on the scalar kernel).
+    begin, count = 1 << 24, args.c4_contention_frames
+    NB = 256
+    mixed = progs[:NB]
+    adversarial = [W.to_postfix(("and", ("bot",), W.from_postfix(p))) for p in progs[:NB]]   # every model refutes
+
+    def once(fn):
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); fn(); b.record(); torch.cuda.synchronize()
+        return a.elapsed_time(b) * 1e-3
+
     for name, batch in (("mixed", mixed), ("adversarial", adversarial)):
         h = kb.Programs(*W.pack_programs(batch), k)
-        c = torch.zeros((64, 2), dtype=torch.int64, device="cuda")
-        w = torch.zeros((64, 2), dtype=torch.int64, device="cuda")
-        res = {}
+        c = torch.zeros((NB, 2), dtype=torch.int64, device="cuda")
+        w = torch.zeros((NB, 2), dtype=torch.int64, device="cuda")
+        res = {"formulas": NB, "frames": count}
+        kb.eval_batch_range(h, n, k, 0, begin, 256, kb.KERNEL_SCALAR, c, w)          # warm-up (module load)
         for mname, mode in (("block", kb.REDUCE_BLOCK), ("warp", kb.REDUCE_WARP), ("thread", kb.REDUCE_THREAD)):
-            t = timed(lambda: kb.eval_batch_range(h, n, k, 0, begin, count, kb.KERNEL_SCALAR | mode, c, w))
-            res[mname] = {"seconds": t, "evaluations_per_s": 64 * count * nval / t}
+            t = once(lambda: kb.eval_batch_range(h, n, k, 0, begin, count, kb.KERNEL_SCALAR | kb.NO_SHARING |
+                                                 kb.FULL_SWEEP | mode, c, w))
+            res[mname] = {"seconds": t, "evaluations_per_s": NB * count * nval / t}
         res["block_vs_thread"] = res["thread"]["seconds"] / res["block"]["seconds"]
+        res["block_vs_warp"] = res["warp"]["seconds"] / res["block"]["seconds"]
         t = timed(lambda: kb.eval_batch_range(h, n, k, 0, begin, count, 0, c, w))
-        res["sliced"] = {"seconds": t, "evaluations_per_s": 64 * count * nval / t}
+        res["bit_sliced_default"] = {"seconds": t, "evaluations_per_s": NB * count * nval / t}
         out["contention"][name] = res
         h.destroy()
     clocks = clock.result()
@@ -599,6 +613,7 @@ def main():
     ap.add_argument("--workload", default="c3", choices=["c3", "c3_small", "c4", "frames", "correspond"])
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--ref-frames", type=int, default=256)
+    ap.add_argument("--c4-contention-frames", type=int, default=1 << 20)
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -84,6 +84,10 @@ enum {
                                          and the others receive the same counts and first refuting
                                          frame; the witness valuation and world are computed per
                                          formula; results are identical either way)                */
+    KRIPKE_NO_SUBTERM_SHARING = 1u << 3, /* compiled kernels only: identical programs are still scanned once,
+                                         but a subterm that occurs in several programs is evaluated in each
+                                         of them (default: the batch is one graph of distinct subterms and
+                                         each is evaluated once per 32-model word); ablation                 */
     KRIPKE_KERNEL_AUTO = 0u << 4,     /* compiled bit-sliced kernels where the emitter covers the shape,
                                          else the interpreted bit-sliced kernel, else the scalar one */
     KRIPKE_KERNEL_SCALAR = 1u << 4,   /* force the scalar kernel (Algorithm 1 restated, one model
@@ -278,21 +282,59 @@ typedef struct {
     uint32_t launches;                    /* kernel launches enqueued                                  */
     uint32_t kernel_family;               /* which family ran the bulk: 0 scalar, 1 interpreted bit-sliced,
                                              2 compiled bit-sliced                                     */
-    uint64_t sliced_logic_ops_per_word;   /* 3-input logic instructions per 32-model word the lowered
-                                             programs need, summed over the batch                      */
+    uint64_t sliced_logic_ops_per_word;   /* 3-input logic instructions per 32-model word that the scanned
+                                             programs need: compiled kernels - what the emitter generated
+                                             (each distinct subterm once); interpreted kernel - the lowered
+                                             programs' op formula                                        */
     uint64_t models_per_program;          /* definitional: (frames in range) * 2^(n_vars*n)            */
     uint64_t executed_models;             /* models actually evaluated, summed over programs (a program
                                              that mentions g variables is scanned on 2^(g*n) valuations) */
-    double logic_instr_per_frame;         /* 3-input logic thread-instructions the sliced kernel executes
-                                             per frame of the range, summed over programs: the
-                                             "algorithmic ops" of DESIGN.md's roofline                 */
+    double logic_instr_per_frame;         /* the same per frame of the range (x words per frame of each
+                                             variable-count group): EXECUTED logic thread-instructions   */
     uint32_t jit_programs;                /* distinct programs the compiled kernels evaluated          */
     uint32_t reserved;
-    double dense_logic_instr_per_frame;   /* the same programs costed as the bit-sliced kernel would run
-                                             them (n^2 per modal operator, every word of every frame):
-                                             SURVEY.md 8(d)'s "bit-sliced" figure, for comparison       */
+    double dense_logic_instr_per_frame;   /* = logic_instr_per_frame (kept for layout compatibility)   */
+    double algorithmic_logic_instr_per_frame; /* SURVEY.md 8(d)'s ALGORITHMIC count: every formula of the
+                                             batch as written, no sharing and no folding - (d n^2 + b n +
+                                             n + 1) logic instructions per 32-model word (d modal operators,
+                                             b binary connectives) x 2^(k_b n) / 32 words per frame, k_b = the
+                                             variables the formula mentions.  Work the method defines, not
+                                             work the kernels issue                                      */
+    double jit_compile_seconds;           /* host time the plan of this call spent in the emitter, NVRTC and
+                                             the module load when it was built (0 for interpreted plans)  */
 } kripke_run_info_t;
 int kripke_last_run_info(const kripke_programs_t *programs, kripke_run_info_t *info_out);
+
+/* Compiled scans.  A batch is known when it is staged, so by default the library turns
+ * it into straight-line sm_100a code: all programs of a call become one graph of distinct subterms
+ * (negation folded into the operands, or / imp / dia rewritten onto and / box, conjunctions flattened and
+ * sorted, variables in a canonical order), groups of at most max_programs_per_kernel programs that share
+ * subterms become one kernel each, generated as CUDA C, compiled with NVRTC for sm_100a the first time a
+ * (handle, n, class, flags) combination is scanned and cached per process by source text.  That first
+ * call therefore blocks for the compilation (kripke_run_info_t.jit_compile_seconds); later calls only
+ * enqueue.  Results are identical to the interpreted and scalar kernels (GPU tests).
+ * kripke_jit_configure: 1 <= max_programs_per_kernel <= 160 (default 64; more programs per kernel share
+ * more subterms and need more registers).  Affects plans built afterwards. */
+int kripke_jit_configure(uint32_t max_programs_per_kernel);
+
+/* Diagnostic (pure host: works without a CUDA device): the CUDA C source of compiled kernel kernel_index
+ * of the group of programs that mention group_vars variables, for the given batch (HOST code / offsets as
+ * in kripke_programs_create; pairs == NULL) or the listed pairs of it, as kripke_eval_batch_range / kripke_distinguish_pairs would build it for
+ * (n_worlds, frame_class, flags).  compile != 0 also compiles it with NVRTC to an sm_100a cubin
+ * (*cubin_bytes_out).  source_out (capacity cap, NUL-terminated, may be NULL), *n_kernels_out = kernels of the
+ * group, *logic_ops_per_word_out = 3-input logic instructions per 32-model word of this kernel.  Returns the
+ * source length or a negative kripke_status (KRIPKE_EUNSUPPORTED: no compiled layout for the shape). */
+int kripke_debug_jit_source(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas, uint32_t n_vars,
+                            const uint32_t *pairs, uint32_t n_pairs, uint32_t n_worlds, uint32_t frame_class, uint32_t flags, uint32_t group_vars,
+                            uint32_t kernel_index, int compile, char *source_out, uint64_t cap,
+                            uint32_t *n_kernels_out, uint64_t *logic_ops_per_word_out, uint64_t *cubin_bytes_out);
+
+/* Diagnostic (pure host): the truth set (n-bit mask) of one program on one model as the batch graph of the
+ * compiled scans computes it - after every rewrite (negation edges, and / box normal form, box
+ * distribution, canonical variable order).  succ: n_worlds successor masks; val: n_vars variable masks.
+ * Returns the number of graph nodes or a negative kripke_status. */
+int kripke_debug_dag_truth(const uint8_t *code, uint32_t len, uint32_t n_vars, uint32_t n_worlds,
+                           const uint32_t *succ, const uint32_t *val, uint32_t *truth_out);
 
 /* Integer-pipe calibration ("source-level uint32 XOR/AND/OR" re-done as an instruction
  * rate): runs a register-resident loop of independent 3-input logic instructions on every SM and

@@ -288,12 +288,3 @@ def check_pair_witness(code_a, code_b, n, k, cls, f, v, w) -> bool:
     if not in_class(n, R, cls):
         return False
     return sat(n, R, V, w, parse_postfix(code_a)) != sat(n, R, V, w, parse_postfix(code_b))
-
-
-def minimal_refutation_size(code, k, cls, max_n=3):
-    """Least n in 1..max_n with a refuting model in the class, else None ('no countermodel through
-    max_n worlds', PAPER.md:143 - never 'valid')."""
-    for n in range(1, max_n + 1):
-        if census(code, n, k, cls)[0] > 0:
-            return n
-    return None

@@ -308,24 +308,6 @@ int kov_census_list(const u8 *code, const uint32_t *offs, uint32_t B,
     return bad ? -1 : 0;
 }
 
-/* Class K convenience: frames [begin, begin+count) are their own indices; no list is built by the
- * caller.  (For T / S4 / S5 the caller passes kov_class_frames' list to kov_census_list.) */
-int kov_census_k_range(const u8 *code, const uint32_t *offs, uint32_t B,
-                       const uint32_t *pairs, uint32_t P, int n, int k,
-                       uint64_t begin, uint64_t count,
-                       uint64_t *models_out, uint64_t *frames_out,
-                       uint64_t *wit_f, uint32_t *wit_v, uint32_t *wit_w, int nthreads) {
-    if (n < 1 || n > MAXN) return -1;
-    if (begin + count > (1ull << (n * n))) return -1;
-    uint64_t *list = malloc((size_t)(count ? count : 1) * sizeof(uint64_t));
-    if (!list) return -1;
-    for (uint64_t i = 0; i < count; ++i) list[i] = begin + i;
-    int rc = kov_census_list(code, offs, B, pairs, P, n, k, list, NULL, count, models_out, frames_out,
-                             wit_f, wit_v, wit_w, nthreads);
-    free(list);
-    return rc;
-}
-
 int kov_max_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

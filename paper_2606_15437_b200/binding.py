@@ -20,6 +20,7 @@ CLASS_K, CLASS_T, CLASS_S4, CLASS_S5 = 0, 1, 2, 3
 ACCUMULATE = 1 << 0
 FULL_SWEEP = 1 << 1
 NO_SHARING = 1 << 2
+NO_SUBTERM_SHARING = 1 << 3
 KERNEL_AUTO, KERNEL_SCALAR, KERNEL_SLICED, KERNEL_JIT = 0 << 4, 1 << 4, 2 << 4, 3 << 4
 REDUCE_BLOCK, REDUCE_WARP, REDUCE_THREAD = 0 << 8, 1 << 8, 2 << 8
 NO_WITNESS = (1 << 64) - 1
@@ -36,6 +37,7 @@ EXPORTS = [
     "kripke_eval_frames", "kripke_distinguish_pairs_frames",
     "kripke_validity_bitmap", "kripke_condition_bitmap", "kripke_match_bitmaps", "kripke_frames_from_bitmap",
     "kripke_failure_density", "kripke_failure_density_frames",
+    "kripke_jit_configure", "kripke_debug_jit_source", "kripke_debug_dag_truth",
 ]
 
 
@@ -52,7 +54,9 @@ class RunInfo(ctypes.Structure):
                 ("sliced_logic_ops_per_word", ctypes.c_uint64), ("models_per_program", ctypes.c_uint64),
                 ("executed_models", ctypes.c_uint64), ("logic_instr_per_frame", ctypes.c_double),
                 ("jit_programs", ctypes.c_uint32), ("reserved", ctypes.c_uint32),
-                ("dense_logic_instr_per_frame", ctypes.c_double)]
+                ("dense_logic_instr_per_frame", ctypes.c_double),
+                ("algorithmic_logic_instr_per_frame", ctypes.c_double),
+                ("jit_compile_seconds", ctypes.c_double)]
 
 
 _lib = None
@@ -95,6 +99,10 @@ def load():
     lib.kripke_frames_from_bitmap.argtypes = [u32, u32, u64, u64, vp, vp, u64, vp, vp]
     lib.kripke_eval_frames.argtypes = [vp, u32, u32, vp, u64, u64, u32, vp, vp, vp]
     lib.kripke_distinguish_pairs_frames.argtypes = [vp, u32p, u32, u32, u32, vp, u64, u64, u32, vp, vp, vp]
+    lib.kripke_jit_configure.argtypes = [u32]
+    lib.kripke_debug_jit_source.argtypes = [u8p, u32p, u32, u32, u32p, u32, u32, u32, u32, u32, u32, ctypes.c_int, vp, u64,
+                                            ctypes.POINTER(u32), ctypes.POINTER(u64), ctypes.POINTER(u64)]
+    lib.kripke_debug_dag_truth.argtypes = [u8p, u32, u32, u32, u32p, u32p, ctypes.POINTER(u32)]
     for name in EXPORTS:
         if name not in ("kripke_version",):
             getattr(lib, name).restype = ctypes.c_int
@@ -430,6 +438,44 @@ def debug_lower(code_a: bytes, code_b: bytes | None, n_vars: int, leaf_mode: int
         raise KripkeError(rc, "kripke_debug_lower")
     return [(int(x) & 0xFF, int(x) >> 8) for x in out[:rc]], need.value
 
+
+
+def jit_configure(max_programs_per_kernel: int):
+    _check(load().kripke_jit_configure(max_programs_per_kernel), "kripke_jit_configure")
+
+
+def debug_jit_source(code, offsets, n_vars: int, n_worlds: int, frame_class: int, group_vars: int,
+                     kernel_index: int = 0, flags: int = 0, pairs=None, compile: bool = False):
+    """(source text, kernels in the group, logic ops per word of this kernel, cubin bytes) of one compiled
+    kernel; None if the emitter has no layout for the shape.  Pure host."""
+    code, offsets = _host(code, offsets)
+    cap = 1 << 22
+    buf = ctypes.create_string_buffer(cap)
+    nk, ops, cb = ctypes.c_uint32(0), ctypes.c_uint64(0), ctypes.c_uint64(0)
+    pa = None if pairs is None else np.ascontiguousarray(pairs, dtype=np.uint32).reshape(-1)
+    rc = load().kripke_debug_jit_source(code.ctypes.data, offsets.ctypes.data, len(offsets) - 1, n_vars,
+                                        None if pa is None else pa.ctypes.data,
+                                        0 if pa is None else len(pa) // 2, n_worlds, frame_class, flags, group_vars,
+                                        kernel_index, 1 if compile else 0, ctypes.cast(buf, ctypes.c_void_p), cap,
+                                        ctypes.byref(nk), ctypes.byref(ops), ctypes.byref(cb))
+    if rc == EUNSUPPORTED:
+        return None
+    if rc < 0:
+        raise KripkeError(rc, "kripke_debug_jit_source")
+    return buf.value.decode(), nk.value, ops.value, cb.value
+
+
+def debug_dag_truth(code: bytes, n_vars: int, n_worlds: int, succ, val) -> int:
+    """Truth set (bit mask) of one program on one model as the compiled scans' batch graph computes it."""
+    a = np.frombuffer(code, dtype=np.uint8)
+    s = np.ascontiguousarray(succ, dtype=np.uint32)
+    v = np.ascontiguousarray(list(val) + [0] * (4 - len(val)), dtype=np.uint32)
+    out = ctypes.c_uint32(0)
+    rc = load().kripke_debug_dag_truth(a.ctypes.data, len(a), n_vars, n_worlds, s.ctypes.data, v.ctypes.data,
+                                       ctypes.byref(out))
+    if rc < 0:
+        raise KripkeError(rc, "kripke_debug_dag_truth")
+    return out.value
 
 
 def unpack(counts, witness):

@@ -31,13 +31,16 @@ UNITS = [
     ("calibrate", "calibrate.cu", []),
     ("scan_frames", "scan_frames.cu", []),
     ("bitmaps", "bitmaps.cu", []),
+    ("jit_dag", "jit_dag.cpp", []),
+    ("jit_emit", "jit_emit.cpp", []),
+    ("jit_runtime", "jit_runtime.cpp", []),
 ] + [(f"scan_sliced_inst{g}", "scan_sliced_inst.cu", [f"-DKRIPKE_INST_GROUP={g}"]) for g in range(4)] \
   + [(f"scan_frames_inst{g}", "scan_frames_inst.cu", [f"-DKRIPKE_FR_GROUP={g}"]) for g in range(4)]
 
 
 def _headers_mtime() -> float:
     inc = os.path.join(os.path.dirname(HERE), "include", "kripke.h")
-    files = [inc] + [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh"))]
+    files = [inc] + [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh", ".inc"))]
     return max(os.path.getmtime(f) for f in files)
 
 
@@ -66,7 +69,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objs = [o for o, _ in results]
     if force or any(changed for _, changed in results) or not os.path.exists(LIB):
         tmp = LIB + f".{os.getpid()}.tmp"
-        cmd = [NVCC] + ARCH + ["-shared", "-o", tmp] + objs
+        cmd = [NVCC] + ARCH + ["-shared", "-o", tmp] + objs + ["-lnvrtc"]
         res = subprocess.run(cmd, capture_output=True, text=True)
         if res.returncode != 0:
             raise RuntimeError("link failed:\n" + res.stderr)

@@ -10,7 +10,11 @@
 #include <new>
 #include <tuple>
 
+#include <chrono>
+#include <string>
+
 #include "internal.h"
+#include "jit.h"
 
 using namespace kripke;
 
@@ -104,17 +108,21 @@ int upload_plan(const HostPlan &hp, DevicePlan *dp) {
 // per-formula k_b - and its model count is multiplied by 2^((k-g)*n) (reading R8).
 struct GroupPlan {
     uint32_t k_eff = 0;
-    DevicePlan dp;                    // every record of the group, for the bit-sliced / scalar kernels
+    DevicePlan dp;                    // every record of the group, for the interpreted bit-sliced / scalar kernels
+    bool use_jit = false;             // the group runs on compiled kernels (jit.h) instead of dp
+    JitGroupPlan jit;
     uint32_t *d_alias = nullptr;      // device: (record, representative) pairs - records whose lowered program
     uint32_t n_alias = 0;             // equals the representative's are not scanned, they copy its accumulators
     void release() {
         dp.release();
+        jit.release();
         cudaFree(d_alias);
         d_alias = nullptr; n_alias = 0;
     }
 };
 struct ScanPlan {
     std::vector<GroupPlan> groups;
+    double jit_compile_seconds = 0.0; // host time spent emitting + compiling + loading (0 if cached or interpreted)
     void release() {
         for (auto &g : groups) g.release();
         groups.clear();
@@ -218,8 +226,21 @@ struct kripke_programs {
     std::vector<uint32_t> h_offsets;
     uint8_t *d_code = nullptr;
     uint32_t *d_offsets = nullptr;
-    std::map<uint64_t, ScanPlan> single;     // one record per formula; cached per (n, usable reduced shapes)
-    ScanPlan pair;                     // rebuilt by each kripke_distinguish_pairs call
+    // per formula, from the postfix program as written: modal operators, binary connectives, variables
+    std::vector<uint32_t> f_modal, f_binary, f_vars;
+    std::map<uint64_t, ScanPlan> single;     // one record per formula; cached per (n, k, class, flags, engine)
+    struct PairPlan {                  // plans of kripke_distinguish_pairs, cached per pair list and shape
+        std::vector<uint32_t> pairs;
+        uint64_t key = 0;
+        ScanPlan plan;
+        uint32_t *d_pairs = nullptr;
+        uint64_t last_use = 0;
+    };
+    std::vector<PairPlan *> pair_plans;
+    uint64_t use_clock = 0;
+    cudaEvent_t done = nullptr;        // end of the last scan enqueued on this handle
+    void *last_stream = nullptr;
+    bool has_last = false;
     DevicePlan list_single;            // frame-list mode: every formula lowered without derived leaves
     bool list_single_built = false;
     DevicePlan list_pair;              // rebuilt by each kripke_distinguish_pairs_frames call
@@ -259,41 +280,100 @@ uint32_t reduced_shapes(uint32_t n, uint32_t k, uint32_t cls, uint32_t flags) {
     return mask;
 }
 
+// Engines of a scan plan.
+enum : uint32_t { ENGINE_INTERPRETED = 0, ENGINE_JIT = 1 };
+
+// Tunables of the compiled scans (kripke_jit_configure).
+uint32_t g_jit_max_programs = 64;
+
 // Lowers the records (formulas, or pairs if `pairs` != null) into one GroupPlan per variable count.
 int build_scan_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
                     uint32_t shapes, ScanPlan *out);
+int build_jit_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
+                   uint32_t cls, uint32_t flags, ScanPlan *out);
 
-// The common scan: zero accumulators, run every group on the sliced kernel where an instantiation
-// exists (aligned part of the range) and on the scalar kernel elsewhere, then finish.
-int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *d_pairs, uint32_t n_records,
-             uint32_t n, uint32_t k, uint32_t cls, uint64_t begin, uint64_t count, uint32_t flags,
-             kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream) {
+constexpr uint32_t SCAN_FLAGS = KRIPKE_ACCUMULATE | KRIPKE_FULL_SWEEP | KRIPKE_NO_SHARING | KRIPKE_NO_SUBTERM_SHARING |
+                                KRIPKE_KERNEL_MASK | KRIPKE_REDUCE_MASK;
+
+// Argument checks of every class scan - before any plan is built or cached.
+int check_scan_args(const kripke_programs *h, uint32_t n_records, uint32_t n, uint32_t k, uint32_t cls, uint64_t begin,
+                    uint64_t count, uint32_t flags, const void *counts_out, const void *witness_out) {
     if (n < 1 || n > KRIPKE_MAX_WORLDS || k != h->n_vars || cls > KRIPKE_CLASS_S5) return KRIPKE_EINVAL;
     if (n * n + k * n > KRIPKE_MAX_MODEL_BITS) return KRIPKE_EUNSUPPORTED;
-    if (flags & ~(KRIPKE_ACCUMULATE | KRIPKE_FULL_SWEEP | KRIPKE_NO_SHARING | KRIPKE_KERNEL_MASK | KRIPKE_REDUCE_MASK)) return KRIPKE_EINVAL;
-    const uint32_t family = flags & KRIPKE_KERNEL_MASK, reduce = (flags & KRIPKE_REDUCE_MASK) >> 8;
-    if (reduce > 2) return KRIPKE_EINVAL;
+    if (flags & ~SCAN_FLAGS) return KRIPKE_EINVAL;
+    if (((flags & KRIPKE_REDUCE_MASK) >> 8) > 2) return KRIPKE_EINVAL;
     if (n_records && (!counts_out || !witness_out)) return KRIPKE_EINVAL;
     uint64_t csize = 0;
     int rc = class_size(n, cls, &csize);
     if (rc) return rc;
     if (begin > csize || count > csize - begin) return KRIPKE_EINVAL;
+    return KRIPKE_OK;
+}
+
+// Which engine a scan with these flags uses: compiled kernels whenever the emitter has a layout for
+// the full shape (AUTO) or when forced; the interpreted kernels otherwise.
+int pick_engine(uint32_t n, uint32_t k, uint32_t cls, uint32_t flags, uint32_t *engine) {
+    const uint32_t family = flags & KRIPKE_KERNEL_MASK;
+    const bool can = jit_layout(n, k, cls, nullptr);
+    if (family == KRIPKE_KERNEL_JIT && !can) return KRIPKE_EUNSUPPORTED;
+    *engine = (can && (family == KRIPKE_KERNEL_JIT || family == KRIPKE_KERNEL_AUTO)) ? ENGINE_JIT : ENGINE_INTERPRETED;
+    return KRIPKE_OK;
+}
+
+// The common scan: zero accumulators, run every group on the compiled or interpreted bit-sliced kernels
+// where they apply (aligned part of the range) and on the scalar kernel elsewhere, then finish.
+int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *h_pairs, const uint32_t *d_pairs, uint32_t n_records,
+             uint32_t n, uint32_t k, uint32_t cls, uint64_t begin, uint64_t count, uint32_t flags,
+             kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream) {
+    int rc = check_scan_args(h, n_records, n, k, cls, begin, count, flags, counts_out, witness_out);
+    if (rc) return rc;
+    const uint32_t family = flags & KRIPKE_KERNEL_MASK, reduce = (flags & KRIPKE_REDUCE_MASK) >> 8;
     h->last = kripke_run_info_t{};
     h->last.models_per_program = count << (k * n);
+    h->last.jit_compile_seconds = plan.jit_compile_seconds;
+    // SURVEY 8(d)'s algorithmic operation count, per FORMULA of the batch as written (no sharing, no folding):
+    // (d n^2 + b n + n + 1) 3-input logic instructions per 32-model word, 2^(k_b n) / 32 words per frame
+    {
+        auto alg = [&](uint32_t f, uint32_t kb) {
+            return (double)(h->f_modal[f] * n * n + h->f_binary[f] * n) * (double)(1ull << (kb * n)) / 32.0;
+        };
+        auto nv = [](uint32_t m) { uint32_t c = 0; for (; m; m >>= 1) c += m & 1u; return c; };
+        for (uint32_t r = 0; r < n_records; ++r) {
+            if (h_pairs) {
+                const uint32_t fa = h_pairs[2 * r], fb = h_pairs[2 * r + 1], kb = nv(h->f_vars[fa] | h->f_vars[fb]);
+                h->last.algorithmic_logic_instr_per_frame += alg(fa, kb) + alg(fb, kb) + (double)(2 * n + 1) * (double)(1ull << (kb * n)) / 32.0;
+            } else {
+                const uint32_t kb = nv(h->f_vars[r]);
+                h->last.algorithmic_logic_instr_per_frame += alg(r, kb) + (double)(n + 1) * (double)(1ull << (kb * n)) / 32.0;
+            }
+        }
+    }
     for (size_t gi = 0; gi < plan.groups.size(); ++gi) {
         const GroupPlan &g = plan.groups[gi];
         // bookkeeping for the roofline: instructions the kernels need per frame of the range
         const double words = (double)(1ull << (g.k_eff * n)) / 32.0;
+        if (g.use_jit) {
+            h->last.sliced_logic_ops_per_word += g.jit.stats.logic_ops_per_word;
+            h->last.logic_instr_per_frame += (double)g.jit.stats.logic_ops_per_word * words;
+            h->last.executed_models += (uint64_t)g.jit.n_slots * (count << (g.k_eff * n));
+            h->last.jit_programs += g.jit.n_slots;
+            continue;
+        }
         auto dense = [&](const DevicePlan &dp) {
             return (double)(dp.n_modal * n * n + dp.n_bool * n + (uint64_t)dp.n_slots * (n + 1)) * words;
         };
         h->last.sliced_logic_ops_per_word += g.dp.n_modal * n * n + g.dp.n_bool * n + (uint64_t)g.dp.n_slots * (n + 1);
         h->last.logic_instr_per_frame += dense(g.dp);
-        h->last.dense_logic_instr_per_frame += dense(g.dp);
         h->last.executed_models += (uint64_t)(g.dp.n_slots + g.dp.n_unfit) * (count << (g.k_eff * n));
     }
+    h->last.dense_logic_instr_per_frame = h->last.logic_instr_per_frame;
     if (n_records == 0) return KRIPKE_OK;
 
+    // One scan at a time per handle (its accumulators are shared): a call on another stream waits for
+    // the previous call's work on the device, it never blocks the host.
+    if (!h->done) CU(cudaEventCreateWithFlags(&h->done, cudaEventDisableTiming));
+    if (h->has_last && h->last_stream != stream) CU(cudaStreamWaitEvent((cudaStream_t)stream, h->done, 0));
+    if (n_records > h->accum_cap && h->has_last) CU(cudaEventSynchronize(h->done));   // the buffer is about to be replaced
     if ((rc = ensure_accum(h, n_records))) return rc;
     ScanJob job;
     job.n = n; job.k = k; job.cls = cls;
@@ -378,7 +458,26 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *d_pairs, 
     for (size_t gi = 0; gi < plan.groups.size(); ++gi) {
         if (family == KRIPKE_KERNEL_SCALAR) break;
         const GroupPlan &g = plan.groups[gi];
-        if ((rc = run_sliced_or_scalar(g.dp, g.k_eff))) return rc;
+        if (!g.use_jit) {
+            if ((rc = run_sliced_or_scalar(g.dp, g.k_eff))) return rc;
+            continue;
+        }
+        // compiled kernels on the unit-aligned part of the range, scalar kernel on the ragged ends
+        const uint64_t fpu = 1ull << g.jit.lay.unit_frames_log2;
+        uint64_t ab = (begin + fpu - 1) / fpu * fpu, ae = (begin + count) / fpu * fpu;
+        if (ae <= ab) ab = ae = begin;
+        if (family == KRIPKE_KERNEL_JIT && (ab != begin || ae != begin + count)) return KRIPKE_EUNSUPPORTED;
+        if (ae > ab) {
+            ScanJob rj = job;
+            rj.k = g.k_eff; rj.frame_begin = ab; rj.frame_count = ae - ab;
+            h->last.kernel_family = 2;
+            if ((e = jit_launch_group(rj, g.jit, (k - g.k_eff) * n, stream, &launches))) return cuda_fail(e);
+        }
+        ScanJob head = job, tail = job;
+        head.frame_count = ab - begin;
+        tail.frame_begin = ae; tail.frame_count = begin + count - ae;
+        if ((e = launch_scalar(head, g.jit.d_slot_record, g.jit.n_slots, reduce, stream, &launches))) return cuda_fail(e);
+        if ((e = launch_scalar(tail, g.jit.d_slot_record, g.jit.n_slots, reduce, stream, &launches))) return cuda_fail(e);
     }
     // records that share a representative's lowered program take its accumulators (the scalar family
     // scanned every record itself)
@@ -391,6 +490,9 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *d_pairs, 
     if ((e = launch_finish(job, (flags & KRIPKE_ACCUMULATE) != 0, counts_out, witness_out, stream)))
         return cuda_fail(e);
     h->last.launches = launches + 1;
+    CU(cudaEventRecord(h->done, (cudaStream_t)stream));
+    h->last_stream = stream;
+    h->has_last = true;
     return KRIPKE_OK;
 }
 
@@ -503,17 +605,169 @@ int build_scan_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_
     return KRIPKE_OK;
 }
 
-// The batch's plan for one shape (cached in the handle; synchronous upload on first use).
-int single_plan(kripke_programs *h, uint32_t n, uint32_t k, uint32_t shapes, const ScanPlan **out) {
-    const uint64_t key = ((uint64_t)n << 32) | shapes;
+// ---- compiled scans (jit.h) -----------------------------------------------------------------------
+// The records of one variable-count group as roots of one graph.  Host only.
+struct JitGroupHost {
+    uint32_t g = 0;
+    Dag dag;
+    std::vector<JitRoot> roots;          // distinct roots = the programs that are scanned
+    std::vector<uint32_t> slot_record;   // representative record of each root
+    std::vector<uint32_t> alias;         // (record, representative) pairs
+};
+
+// Groups the records by the number of variables they mention (Algorithm 1's per-formula k_b; the
+// least g >= that count for which the emitter has a layout) and builds each group's graph.
+int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
+                      uint32_t cls, uint32_t flags, std::vector<JitGroupHost> *out) {
+    auto prog = [&](uint32_t f) { return &h->h_code[h->h_offsets[f]]; };
+    auto plen = [&](uint32_t f) { return h->h_offsets[f + 1] - h->h_offsets[f]; };
+    out->clear();
+    out->resize(k + 1);
+    for (uint32_t g = 0; g <= k; ++g) (*out)[g].g = g;
+    std::vector<Dag> probe(k + 1);       // unsalted graphs: which records are the same program
+    std::vector<std::map<std::pair<uint32_t, uint32_t>, uint32_t>> seen(k + 1);
+    for (uint32_t r = 0; r < n_records; ++r) {
+        const uint32_t fa = pairs ? pairs[2 * r] : r, fb = pairs ? pairs[2 * r + 1] : r;
+        // the variables the record's GRAPH mentions (the rewrites fold more than the syntax shows: x & ~x, box T)
+        uint32_t sup;
+        {
+            Dag sd;
+            sup = sd.support(sd.build(prog(fa), plen(fa), nullptr));
+            if (pairs) sup |= sd.support(sd.build(prog(fb), plen(fb), nullptr));
+        }
+        uint32_t cnt = 0;
+        for (uint32_t i = 0; i < KRIPKE_MAX_VARS; ++i) cnt += (sup >> i) & 1u;
+        uint32_t g = (flags & KRIPKE_FULL_SWEEP) ? k : cnt;
+        while (g < k && !jit_layout(n, g, cls, nullptr)) ++g;
+        if (!jit_layout(n, g, cls, nullptr)) return KRIPKE_EUNSUPPORTED;
+        JitGroupHost &G = (*out)[g];
+        uint8_t rename[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
+        if (flags & KRIPKE_NO_SHARING) {                 // variables in their own order, nothing shared
+            uint8_t next = 0;
+            for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v)
+                if ((sup >> v) & 1u) rename[v] = next++;
+        } else {
+            canonical_rename(prog(fa), plen(fa), pairs ? prog(fb) : nullptr, pairs ? plen(fb) : 0u, sup, rename);
+        }
+        if (!(flags & KRIPKE_NO_SHARING)) {
+            // records whose graphs coincide are scanned once (the pair path is symmetric in its two formulas)
+            uint32_t pa = probe[g].build(prog(fa), plen(fa), rename);
+            uint32_t pb = pairs ? probe[g].build(prog(fb), plen(fb), rename) : UINT32_MAX;
+            if (pairs && pb < pa) std::swap(pa, pb);
+            auto it = seen[g].find(std::make_pair(pa, pb));
+            if (it != seen[g].end()) { G.alias.push_back(r); G.alias.push_back(it->second); continue; }
+            seen[g].emplace(std::make_pair(pa, pb), r);
+        }
+        G.dag.salt = (flags & (KRIPKE_NO_SHARING | KRIPKE_NO_SUBTERM_SHARING)) ? r + 1 : 0u;
+        JitRoot root;
+        root.a = G.dag.build(prog(fa), plen(fa), rename);
+        root.b = pairs ? G.dag.build(prog(fb), plen(fb), rename) : UINT32_MAX;
+        G.roots.push_back(root);
+        G.slot_record.push_back(r);
+    }
+    return KRIPKE_OK;
+}
+
+int build_jit_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
+                   uint32_t cls, uint32_t flags, ScanPlan *out) {
+    out->release();
+    const auto t0 = std::chrono::steady_clock::now();
+    std::vector<JitGroupHost> groups;
+    int rc = jit_group_records(h, pairs, n_records, n, k, cls, flags, &groups);
+    if (rc) return rc;
+    for (JitGroupHost &G : groups) {
+        if (G.roots.empty() && G.alias.empty()) continue;
+        GroupPlan gp;
+        gp.k_eff = G.g;
+        gp.use_jit = true;
+        JitLayout lay;
+        jit_layout(n, G.g, cls, &lay);
+        std::string log;
+        rc = jit_build_group(G.dag, lay, G.roots, G.slot_record, g_jit_max_programs, &gp.jit, &log);
+        if (rc > 0) rc = cuda_fail(rc);
+        if (!rc) rc = upload(&gp.d_alias, G.alias);
+        if (rc) { gp.release(); out->release(); return rc; }
+        gp.n_alias = (uint32_t)(G.alias.size() / 2);
+        out->groups.push_back(gp);
+    }
+    out->jit_compile_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    return KRIPKE_OK;
+}
+
+uint64_t plan_key(uint32_t n, uint32_t k, uint32_t cls, uint32_t flags, uint32_t engine, uint32_t shapes) {
+    const uint32_t fl = flags & (KRIPKE_FULL_SWEEP | KRIPKE_NO_SHARING | KRIPKE_NO_SUBTERM_SHARING);
+    return (uint64_t)n | ((uint64_t)k << 4) | ((uint64_t)cls << 8) | ((uint64_t)engine << 12) | ((uint64_t)fl << 16) |
+           ((uint64_t)shapes << 32);
+}
+
+// Builds the plan of a record list with the engine the flags ask for.
+int build_any_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
+                   uint32_t cls, uint32_t flags, uint32_t engine, ScanPlan *out) {
+    if (engine == ENGINE_JIT) {
+        int rc = build_jit_plan(h, pairs, n_records, n, k, cls, flags, out);
+        // AUTO falls back to the interpreted kernels when a record has no compiled layout
+        if (rc != KRIPKE_EUNSUPPORTED || (flags & KRIPKE_KERNEL_MASK) == KRIPKE_KERNEL_JIT) return rc;
+    }
+    return build_scan_plan(h, pairs, n_records, n, k, reduced_shapes(n, k, cls, flags), out);
+}
+
+// The batch's plan for one shape (cached in the handle; synchronous on first use).
+int single_plan(kripke_programs *h, uint32_t n, uint32_t k, uint32_t cls, uint32_t flags, const ScanPlan **out) {
+    uint32_t engine = ENGINE_INTERPRETED;
+    int rc = pick_engine(n, k, cls, flags, &engine);
+    if (rc) return rc;
+    // the interpreted plans depend on the class only through the usable shapes
+    const uint64_t key = engine == ENGINE_JIT ? plan_key(n, k, cls, flags, engine, 0)
+                                              : plan_key(n, k, 0, flags & (KRIPKE_FULL_SWEEP | KRIPKE_NO_SHARING), engine,
+                                                         reduced_shapes(n, k, cls, flags));
     auto it = h->single.find(key);
     if (it == h->single.end()) {
         ScanPlan sp;
-        int rc = build_scan_plan(h, nullptr, h->n_formulas, n, k, shapes, &sp);
+        rc = build_any_plan(h, nullptr, h->n_formulas, n, k, cls, flags, engine, &sp);
         if (rc) return rc;
         it = h->single.emplace(key, std::move(sp)).first;
     }
     *out = &it->second;
+    return KRIPKE_OK;
+}
+
+// The plan of a pair list (cached in the handle: the size loop and repeated scans of one candidate set
+// lower and compile once).  At most 8 lists are kept; the least recently used one is dropped.
+int pair_plan(kripke_programs *h, const uint32_t *pairs, uint32_t n_pairs, uint32_t n, uint32_t k, uint32_t cls,
+              uint32_t flags, kripke_programs::PairPlan **out) {
+    uint32_t engine = ENGINE_INTERPRETED;
+    int rc = pick_engine(n, k, cls, flags, &engine);
+    if (rc) return rc;
+    const uint64_t key = engine == ENGINE_JIT ? plan_key(n, k, cls, flags, engine, 0)
+                                              : plan_key(n, k, 0, flags & (KRIPKE_FULL_SWEEP | KRIPKE_NO_SHARING), engine,
+                                                         reduced_shapes(n, k, cls, flags));
+    for (kripke_programs::PairPlan *pp : h->pair_plans)
+        if (pp->key == key && pp->pairs.size() == 2 * (size_t)n_pairs &&
+            std::equal(pp->pairs.begin(), pp->pairs.end(), pairs)) {
+            pp->last_use = ++h->use_clock;
+            *out = pp;
+            return KRIPKE_OK;
+        }
+    if (h->pair_plans.size() >= 8) {
+        size_t victim = 0;
+        for (size_t i = 1; i < h->pair_plans.size(); ++i)
+            if (h->pair_plans[i]->last_use < h->pair_plans[victim]->last_use) victim = i;
+        if (h->has_last) CU(cudaEventSynchronize(h->done));          // it may still be in use on the device
+        h->pair_plans[victim]->plan.release();
+        cudaFree(h->pair_plans[victim]->d_pairs);
+        delete h->pair_plans[victim];
+        h->pair_plans.erase(h->pair_plans.begin() + victim);
+    }
+    kripke_programs::PairPlan *pp = new (std::nothrow) kripke_programs::PairPlan();
+    if (!pp) return KRIPKE_ENOMEM;
+    pp->pairs.assign(pairs, pairs + 2 * (size_t)n_pairs);
+    pp->key = key;
+    pp->last_use = ++h->use_clock;
+    rc = build_any_plan(h, pairs, n_pairs, n, k, cls, flags, engine, &pp->plan);
+    if (!rc) rc = upload(&pp->d_pairs, pp->pairs);
+    if (rc) { pp->plan.release(); cudaFree(pp->d_pairs); delete pp; return rc; }
+    h->pair_plans.push_back(pp);
+    *out = pp;
     return KRIPKE_OK;
 }
 
@@ -554,6 +808,9 @@ int run_frames(kripke_programs *h, const DevicePlan &dp, const uint32_t *d_pairs
     h->last.dense_logic_instr_per_frame = h->last.logic_instr_per_frame;
     h->last.kernel_family = family == KRIPKE_KERNEL_SCALAR ? 0 : 1;
     if (n_records == 0) return KRIPKE_OK;
+    if (!h->done) CU(cudaEventCreateWithFlags(&h->done, cudaEventDisableTiming));
+    if (h->has_last && h->last_stream != stream) CU(cudaStreamWaitEvent((cudaStream_t)stream, h->done, 0));
+    if (n_records > h->accum_cap && h->has_last) CU(cudaEventSynchronize(h->done));
     int rc = ensure_accum(h, n_records);
     if (rc) return rc;
     FramesJob job;
@@ -577,6 +834,9 @@ int run_frames(kripke_programs *h, const DevicePlan &dp, const uint32_t *d_pairs
     if ((e = launch_frames_finish(job, (flags & KRIPKE_ACCUMULATE) != 0, counts_out, witness_out, stream)))
         return cuda_fail(e);
     h->last.launches = launches + 1;
+    CU(cudaEventRecord(h->done, (cudaStream_t)stream));
+    h->last_stream = stream;
+    h->has_last = true;
     return KRIPKE_OK;
 }
 
@@ -708,7 +968,7 @@ int kripke_distinguish_pairs_frames(const kripke_programs_t *programs, const uin
     kripke_programs *h = const_cast<kripke_programs *>(programs);
     for (uint32_t i = 0; i < 2 * n_pairs; ++i)
         if (pairs[i] >= h->n_formulas) return KRIPKE_EINVAL;
-    CU(cudaDeviceSynchronize());      // the previous call's plan may still be in use
+    if (h->has_last) CU(cudaEventSynchronize(h->done));   // the previous call's plan may still be in use
     int rc = build_list_plan(h, pairs, n_pairs, &h->list_pair);
     if (rc) return rc;
     if (n_pairs > h->pairs_cap) {
@@ -722,7 +982,7 @@ int kripke_distinguish_pairs_frames(const kripke_programs_t *programs, const uin
                       counts_out, witness_out, stream);
 }
 
-const char *kripke_version(void) { return "kripke-b200 0.1 (sm_100a)"; }
+const char *kripke_version(void) { return "kripke-b200 0.2 (sm_100a)"; }
 
 int kripke_last_cuda_error(void) { return g_last_cuda_error; }
 
@@ -750,6 +1010,14 @@ int kripke_programs_create(const uint8_t *code, const uint32_t *offsets, uint32_
     h->h_code.assign(code + offsets[0], code + offsets[n_formulas]);
     const uint32_t base = offsets[0];
     for (auto &o : h->h_offsets) o -= base;
+    h->f_modal.assign(n_formulas, 0); h->f_binary.assign(n_formulas, 0); h->f_vars.assign(n_formulas, 0);
+    for (uint32_t f = 0; f < n_formulas; ++f)
+        for (uint32_t i = h->h_offsets[f]; i < h->h_offsets[f + 1]; ++i) {
+            const uint8_t c = h->h_code[i];
+            if (c == KRIPKE_OP_BOX || c == KRIPKE_OP_DIA) ++h->f_modal[f];
+            else if (c >= KRIPKE_OP_AND) ++h->f_binary[f];
+            else if (c >= KRIPKE_OP_VAR0 && c < KRIPKE_OP_NOT) h->f_vars[f] |= 1u << (c - KRIPKE_OP_VAR0);
+        }
     if (h->h_code.empty()) h->h_code.push_back(0);
     if ((rc = upload(&h->d_code, h->h_code)) || (rc = upload(&h->d_offsets, h->h_offsets))) {
         kripke_programs_destroy(h);
@@ -763,7 +1031,8 @@ int kripke_programs_destroy(kripke_programs_t *h) {
     if (!h) return KRIPKE_OK;
     cudaDeviceSynchronize();
     for (auto &kv : h->single) kv.second.release();
-    h->pair.release();
+    for (kripke_programs::PairPlan *pp : h->pair_plans) { pp->plan.release(); cudaFree(pp->d_pairs); delete pp; }
+    if (h->done) cudaEventDestroy(h->done);
     h->list_single.release(); h->list_pair.release();
     cudaFree(h->d_code); cudaFree(h->d_offsets); cudaFree(h->d_pairs); cudaFree(h->d_accum);
     cudaFree(h->d_tmp_counts); cudaFree(h->d_tmp_wit);
@@ -777,10 +1046,13 @@ int kripke_eval_batch_range(const kripke_programs_t *programs, uint32_t n_worlds
                             void *stream) {
     if (!programs) return KRIPKE_EINVAL;
     kripke_programs *h = const_cast<kripke_programs *>(programs);
-    const ScanPlan *plan = nullptr;
-    int rc = single_plan(h, n_worlds, n_vars, reduced_shapes(n_worlds, n_vars, frame_class, flags), &plan);
+    // every argument is checked before a plan is built or cached
+    int rc = check_scan_args(h, h->n_formulas, n_worlds, n_vars, frame_class, frame_begin, frame_count, flags,
+                             counts_out, witness_out);
     if (rc) return rc;
-    return run_scan(h, *plan, nullptr, h->n_formulas, n_worlds, n_vars, frame_class, frame_begin,
+    const ScanPlan *plan = nullptr;
+    if ((rc = single_plan(h, n_worlds, n_vars, frame_class, flags, &plan))) return rc;
+    return run_scan(h, *plan, nullptr, nullptr, h->n_formulas, n_worlds, n_vars, frame_class, frame_begin,
                     frame_count, flags, counts_out, witness_out, stream);
 }
 
@@ -802,19 +1074,12 @@ int kripke_distinguish_pairs(const kripke_programs_t *programs, const uint32_t *
     kripke_programs *h = const_cast<kripke_programs *>(programs);
     for (uint32_t i = 0; i < 2 * n_pairs; ++i)
         if (pairs[i] >= h->n_formulas) return KRIPKE_EINVAL;
-    // the previous call's plan may still be in use on another stream: wait before replacing it
-    CU(cudaDeviceSynchronize());
-    int rc = build_scan_plan(h, pairs, n_pairs, n_worlds, n_vars,
-                             reduced_shapes(n_worlds, n_vars, frame_class, flags), &h->pair);
+    int rc = check_scan_args(h, n_pairs, n_worlds, n_vars, frame_class, frame_begin, frame_count, flags, counts_out,
+                             witness_out);
     if (rc) return rc;
-    if (n_pairs > h->pairs_cap) {
-        cudaFree(h->d_pairs);
-        h->d_pairs = nullptr; h->pairs_cap = 0;
-        CU(cudaMalloc((void **)&h->d_pairs, (size_t)2 * n_pairs * sizeof(uint32_t)));
-        h->pairs_cap = n_pairs;
-    }
-    if (n_pairs) CU(cudaMemcpy(h->d_pairs, pairs, (size_t)2 * n_pairs * sizeof(uint32_t), cudaMemcpyHostToDevice));
-    return run_scan(h, h->pair, h->d_pairs, n_pairs, n_worlds, n_vars, frame_class, frame_begin,
+    kripke_programs::PairPlan *pp = nullptr;
+    if ((rc = pair_plan(h, pairs, n_pairs, n_worlds, n_vars, frame_class, flags, &pp))) return rc;
+    return run_scan(h, pp->plan, pp->pairs.data(), pp->d_pairs, n_pairs, n_worlds, n_vars, frame_class, frame_begin,
                     frame_count, flags, counts_out, witness_out, stream);
 }
 
@@ -862,34 +1127,42 @@ int kripke_pairs_separation(const kripke_programs_t *programs, const uint32_t *p
     }
     std::vector<kripke_count_t> hc(n_pairs);
     std::vector<kripke_witness_t> hw(n_pairs);
-    std::vector<uint32_t> sub;
+    std::vector<uint32_t> sub, listed;               // the pair list of the current plan and the pairs it holds
     int rc = KRIPKE_OK;
     for (uint32_t n = 1; n <= n_max && rc == KRIPKE_OK && !active.empty(); ++n) {
         const uint64_t total = 1ull << (n * n);
+        listed.clear();
         for (uint64_t begin = 0; begin < total && rc == KRIPKE_OK && !active.empty(); begin += chunk_frames) {
             const uint64_t count = std::min<uint64_t>(chunk_frames, total - begin);
-            sub.resize(2 * active.size());
-            for (size_t a = 0; a < active.size(); ++a) {
-                sub[2 * a] = pairs[2 * active[a]];
-                sub[2 * a + 1] = pairs[2 * active[a] + 1];
+            // the records are lowered (and compiled) once per size; a new list is made only when at least half
+            // of the listed pairs have left the scan, so a long chunked size costs O(log P) plans
+            if (listed.empty() || 2 * active.size() <= listed.size()) {
+                listed = active;
+                sub.resize(2 * listed.size());
+                for (size_t a = 0; a < listed.size(); ++a) {
+                    sub[2 * a] = pairs[2 * listed[a]];
+                    sub[2 * a + 1] = pairs[2 * listed[a] + 1];
+                }
             }
-            rc = kripke_distinguish_pairs(h, sub.data(), (uint32_t)active.size(), n, n_vars, KRIPKE_CLASS_K, begin,
+            rc = kripke_distinguish_pairs(h, sub.data(), (uint32_t)listed.size(), n, n_vars, KRIPKE_CLASS_K, begin,
                                           count, 0, d_counts, d_wit, stream);
             if (rc) break;
-            cudaError_t e = cudaMemcpyAsync(hc.data(), d_counts, active.size() * sizeof(kripke_count_t),
+            cudaError_t e = cudaMemcpyAsync(hc.data(), d_counts, listed.size() * sizeof(kripke_count_t),
                                             cudaMemcpyDeviceToHost, (cudaStream_t)stream);
             if (e == cudaSuccess)
-                e = cudaMemcpyAsync(hw.data(), d_wit, active.size() * sizeof(kripke_witness_t),
+                e = cudaMemcpyAsync(hw.data(), d_wit, listed.size() * sizeof(kripke_witness_t),
                                     cudaMemcpyDeviceToHost, (cudaStream_t)stream);
             if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
             if (e != cudaSuccess) { rc = cuda_fail((int)e); break; }
             std::vector<uint32_t> still;
-            for (size_t a = 0; a < active.size(); ++a) {
+            for (size_t a = 0; a < listed.size(); ++a) {
+                const uint32_t j = listed[a];
+                if (size_out[j] != 0) continue;                       // separated in an earlier chunk
                 if (hc[a].refuting_models != 0) {
-                    size_out[active[a]] = n;
-                    witness_out[active[a]] = hw[a];
+                    size_out[j] = n;
+                    witness_out[j] = hw[a];
                 } else {
-                    still.push_back(active[a]);
+                    still.push_back(j);
                 }
             }
             active.swap(still);
@@ -971,6 +1244,82 @@ int kripke_debug_lower(const uint8_t *code_a, uint32_t len_a, const uint8_t *cod
     if (low.ucode.size() > cap) return KRIPKE_EINVAL;
     std::memcpy(ucode_out, low.ucode.data(), low.ucode.size() * sizeof(uint16_t));
     return (int)low.ucode.size();
+}
+
+int kripke_jit_configure(uint32_t max_programs_per_kernel) {
+    if (max_programs_per_kernel < 1 || max_programs_per_kernel > 160) return KRIPKE_EINVAL;
+    g_jit_max_programs = max_programs_per_kernel;
+    return KRIPKE_OK;
+}
+
+int kripke_debug_jit_source(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas, uint32_t n_vars,
+                            const uint32_t *pairs, uint32_t n_pairs,
+                            uint32_t n_worlds, uint32_t frame_class, uint32_t flags, uint32_t group_vars,
+                            uint32_t kernel_index, int compile, char *source_out, uint64_t cap,
+                            uint32_t *n_kernels_out, uint64_t *logic_ops_per_word_out, uint64_t *cubin_bytes_out) {
+    if (n_worlds < 1 || n_worlds > KRIPKE_MAX_WORLDS || frame_class > KRIPKE_CLASS_S5) return KRIPKE_EINVAL;
+    int rc0 = validate_programs(code, offsets, n_formulas, n_vars, nullptr);
+    if (rc0) return rc0;
+    kripke_programs tmp;                       // host fields only: nothing here touches a device
+    tmp.n_formulas = n_formulas; tmp.n_vars = n_vars;
+    tmp.h_offsets.assign(offsets, offsets + n_formulas + 1);
+    tmp.h_code.assign(code + offsets[0], code + offsets[n_formulas]);
+    for (auto &o : tmp.h_offsets) o -= offsets[0];
+    const kripke_programs *h = &tmp;
+    if (group_vars > h->n_vars) return KRIPKE_EINVAL;
+    for (uint32_t i = 0; pairs && i < 2 * n_pairs; ++i)
+        if (pairs[i] >= h->n_formulas) return KRIPKE_EINVAL;
+    std::vector<JitGroupHost> groups;
+    int rc = jit_group_records(h, pairs, pairs ? n_pairs : h->n_formulas, n_worlds, h->n_vars, frame_class, flags, &groups);
+    if (rc) return rc;
+    const JitGroupHost &G = groups[group_vars];
+    JitLayout lay;
+    if (!jit_layout(n_worlds, group_vars, frame_class, &lay)) return KRIPKE_EUNSUPPORTED;
+    const std::vector<std::vector<uint32_t>> parts = jit_partition(G.dag, G.roots, n_worlds, g_jit_max_programs);
+    if (n_kernels_out) *n_kernels_out = (uint32_t)parts.size();
+    if (logic_ops_per_word_out) *logic_ops_per_word_out = 0;
+    if (cubin_bytes_out) *cubin_bytes_out = 0;
+    if (kernel_index >= parts.size()) return parts.empty() ? KRIPKE_OK : KRIPKE_EINVAL;
+    std::vector<JitRoot> rs;
+    for (uint32_t r : parts[kernel_index]) rs.push_back(G.roots[r]);
+    JitEmitStats st;
+    const std::string src = jit_emit_kernel(G.dag, lay, rs, 128, 2, &st);
+    if (logic_ops_per_word_out) *logic_ops_per_word_out = st.logic_ops_per_word;
+    if (compile) {
+        std::string log;
+        size_t bytes = 0;
+        if ((rc = jit_compile_only(src, &log, &bytes))) return rc;
+        if (cubin_bytes_out) *cubin_bytes_out = bytes;
+    }
+    if (source_out && cap) {
+        const size_t m = std::min<size_t>(src.size(), (size_t)cap - 1);
+        std::memcpy(source_out, src.data(), m);
+        source_out[m] = 0;
+    }
+    return (int)std::min<size_t>(src.size(), 0x7FFFFFFF);
+}
+
+int kripke_debug_dag_truth(const uint8_t *code, uint32_t len, uint32_t n_vars, uint32_t n_worlds,
+                           const uint32_t *succ, const uint32_t *val, uint32_t *truth_out) {
+    if (!code || !succ || !truth_out || n_worlds < 1 || n_worlds > KRIPKE_MAX_WORLDS || (n_vars && !val)) return KRIPKE_EINVAL;
+    const uint32_t offs[2] = {0, len};
+    int rc = validate_programs(code, offs, 1, n_vars, nullptr);
+    if (rc) return rc;
+    // evaluated under the canonical variable order, with the valuation permuted the same way
+    uint8_t rename[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
+    uint32_t sup;
+    {
+        Dag sd;
+        sup = sd.support(sd.build(code, len, nullptr));
+    }
+    canonical_rename(code, len, nullptr, 0, sup, rename);
+    uint32_t pv[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
+    for (uint32_t v = 0; v < n_vars; ++v)
+        if ((sup >> v) & 1u) pv[rename[v]] = val[v];
+    Dag d;
+    const uint32_t root = d.build(code, len, rename);
+    *truth_out = d.eval(root, n_worlds, succ, pv);
+    return (int)d.nodes.size();
 }
 
 int kripke_calibrate_int32(uint32_t variant, double *thread_instr_per_s_out, double *elapsed_ms_out,

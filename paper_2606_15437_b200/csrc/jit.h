@@ -1,0 +1,128 @@
+// jit.h - compiled bit-sliced scans: the batch's programs become straight-line sm_100a code.
+//
+// The interpreted bit-sliced kernel (scan_sliced.cuh) spends a third of its issue slots on micro-op
+// dispatch and evaluates every program on its own.  A batch is known when it is staged, so this path
+// (1) turns the whole batch into ONE directed acyclic graph of distinct subterms (jit_dag.cpp:
+//     negation is an edge attribute, or / imp / dia are rewritten onto and / box, conjunctions are
+//     flattened and sorted, variables are renamed to a canonical order) - a subterm that occurs in
+//     many formulas is evaluated once per 32-model word;
+// (2) emits CUDA C for groups of programs (jit_emit.cpp): one kernel per group, a thread owns one
+//     scan unit, loops over its 32-model words, and every node of the group's graph is a handful of
+//     3-input logic instructions on named registers - no dispatch, no stack, no program memory;
+// (3) compiles the groups with NVRTC for sm_100a and loads them (jit_runtime.cpp), cached per
+//     process by source hash.
+// The semantics are those of scan_sliced.cuh (Lemma 1 applied to 32 models at once);
+// the reduction is the same warp -> block -> one global atomic triple per (block, program)
+// (PAPER.md:74); witnesses are completed by finish_kernel.
+#pragma once
+#include <stdint.h>
+
+#include <array>
+#include <map>
+#include <string>
+#include <vector>
+
+#include "internal.h"
+
+namespace kripke {
+
+// ---- the batch graph (jit_dag.cpp) ----------------------------------------------------------------
+// A literal is node * 2 + neg.  Node kinds: the constant "false", a variable, and(a, b), box(a).
+struct DagNode {
+    enum Kind : uint8_t { CONST0, VAR, AND, BOX } kind;
+    uint8_t var;            // VAR: index in the group's valuation
+    uint32_t a, b;          // operand literals (AND: a < b)
+    uint32_t salt;          // 0, or the owner record + 1 when subterm sharing is off
+};
+
+struct Dag {
+    std::vector<DagNode> nodes;
+    uint32_t lit_const(bool v);
+    uint32_t lit_var(uint32_t i);
+    uint32_t mk_and(uint32_t x, uint32_t y);
+    uint32_t mk_box(uint32_t x);
+    // Postfix program -> literal.  rename: variable index -> index in the group's valuation.
+    uint32_t build(const uint8_t *code, uint32_t len, const uint8_t *rename);
+    // Variables a literal's cone mentions (bit i).
+    uint32_t support(uint32_t lit) const;
+    // Truth set (n-bit mask) of a literal on one model: succ[w] successor masks, val[i] variable masks.
+    uint32_t eval(uint32_t lit, uint32_t n, const uint32_t *succ, const uint32_t *val) const;
+    uint32_t salt = 0;      // applied to new AND / BOX nodes
+    // Canonical text of a literal's cone (conjunctions flattened, operands sorted by text).
+    std::string text(uint32_t lit) const;
+  private:
+    uint32_t intern(const DagNode &nd);
+    void conjuncts(uint32_t lit, std::vector<uint32_t> *out) const;
+    std::map<std::array<uint32_t, 5>, uint32_t> index_;
+};
+
+// Canonical variable order of one program (or pair): the permutation of the variables it mentions
+// under which its graph has the least canonical text; alpha-equivalent programs get the same graph.
+// support_mask: variables mentioned; rename_out[v] = index in the reduced valuation (g = popcount).
+void canonical_rename(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b,
+                      uint32_t support_mask, uint8_t *rename_out);
+
+// ---- layout (jit_emit.cpp) ------------------------------------------------------------------------
+// Model index X = (class-order frame index << g*n) | v.  Bits 0..4 of X vary inside a word, the next
+// `inner` bits (valuation) and `outer` bits (frame) are the thread's word loop, the rest is the
+// thread's unit index; `split` = log2 threads per frame when a frame's valuations exceed the loop.
+struct JitLayout {
+    uint32_t n = 0, g = 0, cls = 0;
+    uint32_t kn = 0;               // g * n
+    uint32_t inner = 0, outer = 0, split = 0;
+    uint32_t unit_frames_log2 = 0; // frames per unit = 2^this (0 when a unit is one frame or part of it)
+    bool table = false;            // frames come from the class table (S4 / S5)
+};
+// Is there a compiled layout for (n, g, class)?  Fills *out.
+bool jit_layout(uint32_t n, uint32_t g, uint32_t cls, JitLayout *out);
+
+// One record of a group: a single formula (b == UINT32_MAX) or a pair.
+struct JitRoot {
+    uint32_t a, b;                 // literals
+};
+
+struct JitEmitStats {
+    uint64_t logic_ops_per_word = 0;   // 3-input logic instructions the emitted body needs per word
+    uint32_t n_box = 0, n_and = 0;     // graph nodes evaluated per word (summed over kernels)
+};
+
+// CUDA C source of one kernel `kripke_jit_scan` that evaluates roots[0..) on the layout.
+std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vector<JitRoot> &roots,
+                            uint32_t threads, uint32_t min_blocks, JitEmitStats *stats);
+
+// Partition of the roots into kernels of at most `max_roots` that share as many subterms as possible.
+std::vector<std::vector<uint32_t>> jit_partition(const Dag &dag, const std::vector<JitRoot> &roots,
+                                                 uint32_t n, uint32_t max_roots);
+
+// ---- runtime (jit_runtime.cpp) --------------------------------------------------------------------
+struct JitKernel {
+    void *kernel = nullptr;        // cudaKernel_t
+    uint32_t slot_base = 0;        // first slot (index into the group's slot_record)
+    uint32_t n_slots = 0;
+};
+
+struct JitGroupPlan {
+    JitLayout lay;
+    std::vector<JitKernel> kernels;
+    uint32_t *d_slot_record = nullptr;   // device: record per slot
+    uint32_t n_slots = 0;
+    uint32_t threads = 128;
+    JitEmitStats stats;
+    void release();
+};
+
+// Compiles (or fetches from the process cache) the kernels of one group.  Sources are compiled in
+// parallel host threads.  Returns 0, a negative kripke_status, or a positive cudaError_t;
+// *log_out receives the NVRTC log on a compile error.
+int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitRoot> &roots,
+                    const std::vector<uint32_t> &slot_record, uint32_t max_roots, JitGroupPlan *out,
+                    std::string *log_out);
+
+// Enqueues the group's kernels over the aligned class range of `job` (job.k = the group's g).
+int jit_launch_group(const ScanJob &job, const JitGroupPlan &plan, uint32_t model_shift, void *stream,
+                     uint32_t *launches);
+
+// Compiles one source to a cubin without loading it (tests on a box without a GPU): 0 or error.
+int jit_compile_only(const std::string &source, std::string *log_out, size_t *cubin_bytes);
+
+}  // namespace kripke

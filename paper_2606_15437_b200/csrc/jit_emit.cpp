@@ -1,0 +1,308 @@
+// jit_emit.cpp - layout selection, program grouping and CUDA C emission of the compiled scans (jit.h).
+// Pure host code, no CUDA.  What is emitted is documented at jit_emit_kernel below; the fixed part
+// of every kernel (parameters, reduction helpers) is jit_prelude.inc.
+#include "jit.h"
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <set>
+
+namespace kripke {
+
+namespace {
+
+const char *const kPrelude =
+#include "jit_prelude.inc"
+    ;
+
+constexpr uint32_t LOOP_BITS = 5;      // words per thread aimed at: 2^5 (amortises the unit set-up and the flush)
+constexpr uint32_t MAX_SPLIT = 5;      // threads per frame <= 32: the frame's threads sit in one warp
+
+std::string fmt(const char *f, ...) __attribute__((format(printf, 1, 2)));
+std::string fmt(const char *f, ...) {
+    char buf[256];
+    va_list ap;
+    va_start(ap, f);
+    vsnprintf(buf, sizeof(buf), f, ap);
+    va_end(ap);
+    return buf;
+}
+
+const char *lane_const(uint32_t pos) {
+    static const char *const k[5] = {"0xAAAAAAAAu", "0xCCCCCCCCu", "0xF0F0F0F0u", "0xFF00FF00u", "0xFFFF0000u"};
+    return k[pos];
+}
+
+// Where the value of bit `pos` of the model index X comes from in a thread, as a C expression that is
+// an all-0 / all-1 word (or the in-word lane pattern).
+struct BitSource {
+    const JitLayout &lay;
+    std::set<uint32_t> used_inner, used_outer, used_unit;
+    explicit BitSource(const JitLayout &l) : lay(l) {}
+    std::string word(uint32_t pos) {
+        if (pos < 5) return lane_const(pos);
+        pos -= 5;
+        if (pos < lay.inner) { used_inner.insert(pos); return fmt("mi%u", pos); }
+        pos -= lay.inner;
+        if (pos < lay.outer) { used_outer.insert(pos); return fmt("mo%u", pos); }
+        pos -= lay.outer;
+        used_unit.insert(pos);
+        return fmt("mu%u", pos);
+    }
+};
+
+struct Emitter {
+    const Dag &dag;
+    const JitLayout &lay;
+    BitSource bits;
+    std::set<uint32_t> used_table;          // table classes: edge positions read from the table entry
+    std::vector<char> done;
+    std::string body;
+    JitEmitStats stats;
+
+    Emitter(const Dag &d, const JitLayout &l) : dag(d), lay(l), bits(l), done(d.nodes.size(), 0) {}
+
+    // word of "p_i holds at world w"
+    std::string atom(uint32_t i, uint32_t w) { return bits.word(i * lay.n + w); }
+    // word of the edge w -> u; "" = the edge is always present (class T diagonal)
+    std::string edge(uint32_t w, uint32_t u) {
+        const uint32_t n = lay.n;
+        if (lay.table) { used_table.insert(w * n + u); return fmt("me%u", w * n + u); }
+        if (lay.cls == KRIPKE_CLASS_T) {
+            if (w == u) return "";
+            return bits.word(lay.kn + w * (n - 1) + (u < w ? u : u - 1));      // reflexive_deposit's compact index
+        }
+        return bits.word(lay.kn + w * n + u);
+    }
+    // C expression of literal `lit` at world w
+    std::string lit(uint32_t l, uint32_t w) {
+        const DagNode &nd = dag.nodes[l >> 1];
+        std::string s;
+        if (nd.kind == DagNode::CONST0) return (l & 1u) ? "0xFFFFFFFFu" : "0u";
+        if (nd.kind == DagNode::VAR) s = atom(nd.var, w);
+        else s = fmt("t%u_%u", l >> 1, w);
+        return (l & 1u) ? "~" + s : s;
+    }
+    void node(uint32_t id) {
+        if (done[id]) return;
+        done[id] = 1;
+        const DagNode &nd = dag.nodes[id];
+        const uint32_t n = lay.n;
+        if (nd.kind == DagNode::AND) {
+            node(nd.a >> 1);
+            node(nd.b >> 1);
+            for (uint32_t w = 0; w < n; ++w)
+                body += fmt("      const unsigned t%u_%u = ", id, w) + lit(nd.a, w) + " & " + lit(nd.b, w) + ";\n";
+            stats.logic_ops_per_word += n;
+            ++stats.n_and;
+        } else if (nd.kind == DagNode::BOX) {
+            node(nd.a >> 1);
+            // Lemma 1 on 32 models: R[w] = AND_u ( T[u] | ~E[w][u] )
+            for (uint32_t w = 0; w < n; ++w) {
+                std::string e;
+                uint32_t runtime_terms = 0, terms = 0;
+                for (uint32_t u = 0; u < n; ++u) {
+                    const std::string ew = edge(w, u), x = lit(nd.a, u);
+                    std::string term;
+                    if (ew.empty()) term = x;                                  // edge always present
+                    else { term = "(" + x + " | ~" + ew + ")"; ++runtime_terms; }
+                    e += (terms++ ? " & " : "") + term;
+                }
+                body += fmt("      const unsigned t%u_%u = ", id, w) + e + ";\n";
+                stats.logic_ops_per_word += std::max(1u, runtime_terms);
+            }
+            ++stats.n_box;
+        }
+    }
+};
+
+}  // namespace
+
+bool jit_layout(uint32_t n, uint32_t g, uint32_t cls, JitLayout *out) {
+    if (n < 1 || n > KRIPKE_MAX_WORLDS || g > KRIPKE_MAX_VARS || cls > KRIPKE_CLASS_S5) return false;
+    JitLayout l;
+    l.n = n; l.g = g; l.cls = cls; l.kn = g * n;
+    l.table = cls == KRIPKE_CLASS_S4 || cls == KRIPKE_CLASS_S5;
+    const uint32_t fb = l.table ? 0u : (cls == KRIPKE_CLASS_T ? n * n - n : n * n);   // frame bits inside X
+    if (l.kn >= 5) {
+        l.inner = std::min(l.kn - 5, LOOP_BITS);
+        l.split = l.kn - 5 - l.inner;
+        if (l.split > MAX_SPLIT) { l.inner += l.split - MAX_SPLIT; l.split = MAX_SPLIT; }
+        if (l.split == 0 && l.inner < LOOP_BITS) l.outer = std::min(LOOP_BITS - l.inner, fb);
+        l.unit_frames_log2 = l.outer;
+    } else {
+        if (l.table || l.kn + fb < 5) return false;       // lanes would have to hold table frames / too few models
+        l.outer = std::min(LOOP_BITS, l.kn + fb - 5);
+        l.unit_frames_log2 = 5 - l.kn + l.outer;
+    }
+    if (out) *out = l;
+    return true;
+}
+
+std::vector<std::vector<uint32_t>> jit_partition(const Dag &dag, const std::vector<JitRoot> &roots,
+                                                 uint32_t n, uint32_t max_roots) {
+    const size_t R = roots.size();
+    // cone of every root: its AND / BOX nodes, with the cost model of the emitter (box n*n, and n)
+    std::vector<std::vector<uint32_t>> cone(R);
+    std::vector<uint32_t> cost(dag.nodes.size(), 0);
+    for (size_t i = 0; i < dag.nodes.size(); ++i)
+        cost[i] = dag.nodes[i].kind == DagNode::BOX ? n * n : dag.nodes[i].kind == DagNode::AND ? n : 0;
+    {
+        std::vector<uint32_t> stamp(dag.nodes.size(), UINT32_MAX), stack;
+        for (size_t r = 0; r < R; ++r) {
+            stack.clear();
+            stack.push_back(roots[r].a >> 1);
+            if (roots[r].b != UINT32_MAX) stack.push_back(roots[r].b >> 1);
+            while (!stack.empty()) {
+                const uint32_t id = stack.back(); stack.pop_back();
+                if (stamp[id] == r) continue;
+                stamp[id] = (uint32_t)r;
+                const DagNode &nd = dag.nodes[id];
+                if (nd.kind == DagNode::AND) { cone[r].push_back(id); stack.push_back(nd.a >> 1); stack.push_back(nd.b >> 1); }
+                else if (nd.kind == DagNode::BOX) { cone[r].push_back(id); stack.push_back(nd.a >> 1); }
+            }
+        }
+    }
+    auto total = [&](size_t r) { uint32_t c = 0; for (uint32_t id : cone[r]) c += cost[id]; return c; };
+    std::vector<std::vector<uint32_t>> groups;
+    std::vector<char> left(R, 1), in_union(dag.nodes.size(), 0);
+    size_t n_left = R;
+    while (n_left) {
+        // seed: the most expensive root left; then repeatedly the root that adds the least new work
+        size_t seed = R;
+        uint32_t seed_cost = 0;
+        for (size_t r = 0; r < R; ++r)
+            if (left[r] && (seed == R || total(r) > seed_cost)) { seed = r; seed_cost = total(r); }
+        std::vector<uint32_t> members, touched;
+        auto take = [&](size_t r) {
+            left[r] = 0; --n_left;
+            members.push_back((uint32_t)r);
+            for (uint32_t id : cone[r]) if (!in_union[id]) { in_union[id] = 1; touched.push_back(id); }
+        };
+        take(seed);
+        while (members.size() < max_roots && n_left) {
+            size_t best = R;
+            uint32_t best_add = 0;
+            for (size_t r = 0; r < R; ++r) {
+                if (!left[r]) continue;
+                uint32_t add = 0;
+                for (uint32_t id : cone[r]) if (!in_union[id]) add += cost[id];
+                if (best == R || add < best_add) { best = r; best_add = add; if (add == 0) break; }
+            }
+            take(best);
+        }
+        for (uint32_t id : touched) in_union[id] = 0;
+        groups.push_back(std::move(members));
+    }
+    return groups;
+}
+
+// The emitted kernel.  A thread owns one scan unit u: the models X = (u << (5+inner+outer)) | (jo << (5+inner))
+// | (ji << 5) | lane.  Every bit of X is one atom bit "p_i at world w" or one edge bit "w -> u" (class K:
+// frame index bits; class T: the off-diagonal bits, the diagonal is constant; S4 / S5: the table entry), so
+// each becomes a word: the lane pattern (bits 0..4), a loop mask (mi*, mo*) or a unit mask (mu*, me*) -
+// steps H2 / H3 without any memory traffic.  The loop body evaluates the group's graph in topological
+// order on named registers (step H4) and, per program, the refuted-lane word r, c += popc(r) (step H5).
+// After the loops kj_flush reduces per warp and block (step H6).
+std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vector<JitRoot> &roots,
+                            uint32_t threads, uint32_t min_blocks, JitEmitStats *stats) {
+    Emitter em(dag, lay);
+    const uint32_t n = lay.n, G = (uint32_t)roots.size();
+    // how refuted FRAMES are counted
+    enum { F_MODELS, F_THREAD, F_WORD, F_ANY, F_FOLD } fmode;
+    if (lay.kn == 0) fmode = F_MODELS;                              // one valuation: frames = models
+    else if (lay.unit_frames_log2 == 0) fmode = F_THREAD;           // the unit lies inside one frame
+    else if (lay.kn < 5) fmode = F_FOLD;                            // several frames per word
+    else if (lay.inner == 0) fmode = F_WORD;                        // one word per frame
+    else fmode = F_ANY;                                             // 2^inner words per frame, several frames per unit
+
+    for (uint32_t r = 0; r < G; ++r) {
+        em.body += fmt("      // program %u\n", r);
+        em.node(roots[r].a >> 1);
+        std::string e;
+        if (roots[r].b == UINT32_MAX) {
+            // refuted lanes: the truth set is not all worlds
+            const bool neg = roots[r].a & 1u;
+            for (uint32_t w = 0; w < n; ++w) e += (w ? (neg ? " | " : " & ") : "") + em.lit(roots[r].a & ~1u, w);
+            e = neg ? e : "~(" + e + ")";
+            em.stats.logic_ops_per_word += (n + 1) / 2;
+        } else {
+            // distinguishing lanes: the two truth sets differ
+            em.node(roots[r].b >> 1);
+            for (uint32_t w = 0; w < n; ++w)
+                e += (w ? " | " : "") + ("(" + em.lit(roots[r].a, w) + " ^ " + em.lit(roots[r].b, w) + ")");
+            em.stats.logic_ops_per_word += n;
+        }
+        em.body += fmt("      { const unsigned r = ") + e + fmt("; c%u += __popc(r);", r);
+        if (fmode == F_WORD) em.body += fmt(" f%u += (r != 0u);", r);
+        else if (fmode == F_ANY) em.body += fmt(" a%u |= r;", r);
+        else if (fmode == F_FOLD) em.body += fmt(" f%u += kj_frames_in_word<%u>(r);", r, lay.kn);
+        em.body += " }\n";
+    }
+
+    std::string s = kPrelude;
+    s += fmt("\n// layout: n=%u g=%u cls=%u inner=%u outer=%u split=%u unit_frames_log2=%u programs=%u\n", n, lay.g, lay.cls,
+             lay.inner, lay.outer, lay.split, lay.unit_frames_log2, G);
+    s += fmt("extern \"C\" __global__ void __launch_bounds__(%u, %u) kripke_jit_scan(const KjParams p) {\n", threads, min_blocks);
+    s += fmt("  __shared__ unsigned s_models[%u], s_frames[%u], s_best[%u];\n", G, G, G);
+    s += "  const unsigned lane = threadIdx.x & 31u;\n";
+    s += "  for (unsigned item = blockIdx.x; item < p.n_items; item += gridDim.x) {\n";
+    s += "    const unsigned long long u0 = p.unit_begin + (unsigned long long)item * p.units_per_item;\n";
+    s += "    const unsigned long long rem = p.unit_begin + p.unit_count - u0;\n";
+    s += "    const unsigned item_units = rem < p.units_per_item ? (unsigned)rem : p.units_per_item;\n";
+    s += "    __syncthreads();\n";
+    s += fmt("    for (unsigned i = threadIdx.x; i < %uu; i += %uu) { s_models[i] = 0u; s_frames[i] = 0u; s_best[i] = 0xFFFFFFFFu; }\n", G, threads);
+    s += "    __syncthreads();\n";
+    s += fmt("    for (unsigned t0 = 0; t0 < item_units; t0 += %uu) {\n", threads);
+    s += "      const unsigned warp_rel = t0 + (threadIdx.x & ~31u);\n";
+    s += "      if (warp_rel >= item_units) continue;\n";
+    s += "      const unsigned rel = warp_rel + lane;\n";
+    s += "      const bool valid = rel < item_units;\n";
+    s += "      const unsigned long long unit = u0 + (valid ? rel : 0u);\n";
+    std::string decl_unit, decl_outer, decl_inner;
+    // (the mask declarations depend on what the body used: emitted after the body is known)
+    for (uint32_t b : em.bits.used_unit) decl_unit += fmt("      const unsigned mu%u = 0u - (unsigned)((unit >> %u) & 1ull);\n", b, b);
+    if (lay.table) {
+        decl_unit += fmt("      const unsigned long long frame = p.class_table[unit >> %u];\n", lay.split);
+        for (uint32_t e : em.used_table) decl_unit += fmt("      const unsigned me%u = 0u - (unsigned)((frame >> %u) & 1ull);\n", e, e);
+    }
+    for (uint32_t b : em.bits.used_outer) decl_outer += fmt("      const unsigned mo%u = 0u - ((jo >> %u) & 1u);\n", b, b);
+    for (uint32_t b : em.bits.used_inner) decl_inner += fmt("      const unsigned mi%u = 0u - ((ji >> %u) & 1u);\n", b, b);
+    s += decl_unit;
+    for (uint32_t r = 0; r < G; ++r) {
+        s += fmt("      unsigned c%u = 0u;", r);
+        if (fmode == F_WORD || fmode == F_ANY || fmode == F_FOLD) s += fmt(" unsigned f%u = 0u;", r);
+        s += "\n";
+    }
+    s += "#pragma unroll 1\n";
+    s += fmt("      for (unsigned jo = 0; jo < %uu; ++jo) {\n", 1u << lay.outer);
+    s += decl_outer;
+    if (fmode == F_ANY) for (uint32_t r = 0; r < G; ++r) s += fmt("      unsigned a%u = 0u;\n", r);
+    s += "#pragma unroll 1\n";
+    s += fmt("      for (unsigned ji = 0; ji < %uu; ++ji) {\n", 1u << lay.inner);
+    s += decl_inner;
+    s += em.body;
+    s += "      }\n";
+    if (fmode == F_ANY) for (uint32_t r = 0; r < G; ++r) s += fmt("      f%u += (a%u != 0u);\n", r, r);
+    s += "      }\n";
+    for (uint32_t r = 0; r < G; ++r) {
+        const char *fm = fmode == F_MODELS ? "0" : fmode == F_THREAD ? "1" : "2";
+        const std::string f = (fmode == F_MODELS || fmode == F_THREAD) ? "0u" : fmt("f%u", r);
+        s += fmt("      kj_flush<%u, %s>(%uu, c%u, ", lay.split, fm, r, r) + f + ", valid, warp_rel, lane, s_models, s_frames, s_best);\n";
+    }
+    s += "    }\n";
+    s += "    __syncthreads();\n";
+    s += fmt("    for (unsigned i = threadIdx.x; i < %uu; i += %uu)\n", G, threads);
+    s += "      if (s_best[i] != 0xFFFFFFFFu) {\n";
+    s += "        KjAccum *a = p.accum + p.slot_record[i];\n";
+    s += "        atomicAdd(&a->models, (unsigned long long)s_models[i] << p.model_shift);\n";
+    s += "        atomicAdd(&a->frames, (unsigned long long)s_frames[i]);\n";
+    s += fmt("        atomicMin(&a->best, ((u0 + s_best[i]) >> %u) << %u);\n", lay.split, lay.unit_frames_log2);
+    s += "      }\n";
+    s += "  }\n}\n";
+    if (stats) *stats = em.stats;
+    return s;
+}
+
+}  // namespace kripke

@@ -5,9 +5,13 @@
 parts (sizes are oracle evaluations; times are for the 8-core build box at ~0.1 G eval/s):
   c2          config 2: 5,624 formulas, n=4, classes K/T/S4/S5, full ranges      (1.0e11, ~15 min)
   n5_classes  config 3: same corpus, n=5, classes S4 and S5 in full             (4.0e10, ~6 min)
-  n5_ranges   config 3: 16 seeded ranges of 64 frames of K and of T at n=5       (1.2e10, ~2 min)
-  n5_orbit    config 3: full-range K counts at n=5 for 96 corpus formulas and the named axioms,
-              by the isomorphism-orbit route (291,968 representatives x orbit sizes)
+  n5_ranges   config 3: 16 seeded ranges of 2^10 frames of K and of T at n=5, every formula
+              (SURVEY 8(c) plan item 4; 1.9e11, ~25 min)
+  n5_orbit    config 3: full-range K counts at n=5 for 200 seeded NON-CONSTANT corpus formulas (at
+              least 100 of them over both variables) and the named axioms, by the isomorphism-orbit
+              route (291,968 representatives x orbit sizes; plan item 5)
+  n5_t_full   config 3: 120 seeded non-constant corpus formulas over ALL 2^20 reflexive frames at
+              n=5 (plan item 3; 1.3e11, ~15 min)
   c4_ranges   config 4: 2,048 three-variable formulas, n=5, 4 seeded ranges of 8 K-frames
   c5_counts   config 5: distinguishing-frame counts of every pair for n=1..5 (orbit route at
               n=5) and first witnesses for n<=4
@@ -74,16 +78,32 @@ def part_n5_classes(threads):
     save("n5_s4s5.npz", **out)
 
 
+def seeded_formulas(seed, want, min_two_var=0):
+    """Indices into corpus_c2(): `want` distinct non-constant formulas drawn by seed from the whole
+    corpus ('non-constant' = mentions a variable), at least min_two_var of them over both p and q."""
+    progs = W.corpus_c2()
+    rng = W.SplitMix64(seed)
+    two = [i for i, c in enumerate(progs) if b"\x10" in c and b"\x11" in c]
+    some = [i for i, c in enumerate(progs) if b"\x10" in c or b"\x11" in c]
+    picked = set()
+    while len(picked) < min_two_var:
+        picked.add(two[rng.below(len(two))])
+    while len(picked) < want:
+        picked.add(some[rng.below(len(some))])
+    return sorted(picked)
+
+
 def part_n5_ranges(threads):
     progs = W.corpus_c2()
     code, offs = W.pack_programs(progs)
-    out = {"corpus_sha256": np.array(sha(progs)), "width": np.array(64)}
+    width = 1 << 10
+    out = {"corpus_sha256": np.array(sha(progs)), "width": np.array(width)}
     for cname, total, seed in (("K", 1 << 25, 501), ("T", 1 << 20, 502)):
-        begins = seeded_ranges(seed, total, 64, 16)
+        begins = seeded_ranges(seed, total, width, 16)
         out[f"{cname}_begin"] = np.array(begins, np.uint64)
         acc = {}
         for b in begins:
-            r = V.census(code, offs, 5, 2, CLASSES[cname], b, 64, threads=threads)
+            r = V.census(code, offs, 5, 2, CLASSES[cname], b, width, threads=threads)
             for key, val in r.items():
                 acc.setdefault(key, []).append(val)
         for key, val in acc.items():
@@ -91,15 +111,28 @@ def part_n5_ranges(threads):
     save("n5_ranges.npz", **out)
 
 
+def part_n5_t_full(threads):
+    corpus = W.corpus_c2()
+    idx = seeded_formulas(503, 120, 60)
+    progs = [corpus[i] for i in idx]
+    code, offs = W.pack_programs(progs)
+    t = time.time()
+    r = V.census(code, offs, 5, 2, CLASSES["T"], threads=threads)
+    print("T full census %.1fs" % (time.time() - t))
+    save("n5_t_full.npz", corpus_sha256=np.array(sha(progs)), index=np.array(idx, np.uint32), **r)
+
+
 def part_n5_orbit(threads):
-    progs = W.corpus_c2()[:96] + [W.to_postfix(t) for t in W.named_axioms().values()]
+    corpus = W.corpus_c2()
+    idx = seeded_formulas(505, 200, 100)
+    progs = [corpus[i] for i in idx] + [W.to_postfix(t) for t in W.named_axioms().values()]
     code, offs = W.pack_programs(progs)
     reps, sizes = V.orbits(5)
     assert int(sizes.sum()) == 1 << 25
     t = time.time()
     r = V.census_list(code, offs, 5, 2, reps, weights=sizes, threads=threads)
     print("orbit census %.1fs" % (time.time() - t))
-    save("n5_orbit.npz", corpus_sha256=np.array(sha(progs)), n_corpus=np.array(96),
+    save("n5_orbit.npz", corpus_sha256=np.array(sha(progs)), index=np.array(idx, np.uint32),
          models=r["models"], frames=r["frames"])
 
 
@@ -132,7 +165,7 @@ def part_c5_counts(threads):
 
 
 PARTS = {"c2": part_c2, "n5_classes": part_n5_classes, "n5_ranges": part_n5_ranges,
-         "n5_orbit": part_n5_orbit, "c4_ranges": part_c4_ranges, "c5_counts": part_c5_counts}
+         "n5_orbit": part_n5_orbit, "n5_t_full": part_n5_t_full, "c4_ranges": part_c4_ranges, "c5_counts": part_c5_counts}
 
 if __name__ == "__main__":
     ap = argparse.ArgumentParser()

@@ -70,7 +70,7 @@ def test_c1_n3_all_classes_both_kernels(kb, vol):
     h = kb.Programs(code, offs, 2)
     for cls in (K, T, S4, S5):
         want = vol.census(code, offs, 3, 2, cls)
-        for flags in (kb.KERNEL_AUTO, kb.KERNEL_SCALAR):
+        for flags in (kb.KERNEL_AUTO, kb.KERNEL_SLICED if cls in (K, T) else kb.KERNEL_AUTO, kb.KERNEL_SCALAR):
             got = run(kb, progs, 3, 2, cls, flags=flags, handle=h)
             same(got, want, f"C1 cls={cls} flags={flags}")
         certify(progs, got, 3, 2, cls, idx=range(0, 1000, 7))
@@ -105,7 +105,7 @@ def test_c2_n4_all_classes_golden(kb):
     h = kb.Programs(*W.pack_programs(progs), 2)
     for cname, cls in CLS.items():
         want = {key: g[f"{cname}_{key}"] for key in KEYS}
-        for flags in (kb.KERNEL_AUTO, kb.KERNEL_SCALAR):
+        for flags in (kb.KERNEL_AUTO, kb.KERNEL_SLICED, kb.KERNEL_SCALAR):
             got = run(kb, progs, 4, 2, cls, flags=flags, handle=h)
             same(got, want, f"C2 {cname} flags={flags}")
         certify(progs, got, 4, 2, cls, idx=range(0, len(progs), 23))
@@ -122,7 +122,8 @@ def test_c3_n5_s4_s5_full_golden(kb):
 
 
 def test_c3_n5_sampled_ranges_golden(kb):
-    """16 seeded ranges of 64 consecutive K-frames and T-frames at n=5, every formula."""
+    """16 seeded ranges of 2^10 consecutive K-frames and T-frames at n=5, every formula (SURVEY 8(c)
+    plan item 4); the windows hold whole scan units of every variable-count group plus ragged ends."""
     g = gold("n5_ranges.npz")
     progs = W.corpus_c2()
     h = kb.Programs(*W.pack_programs(progs), 2)
@@ -134,13 +135,30 @@ def test_c3_n5_sampled_ranges_golden(kb):
 
 
 def test_c3_n5_full_K_counts_by_orbits(kb):
-    """Full-range n=5 class-K counts of 96 corpus formulas + the named axioms = the oracle's
-    isomorphism-orbit sum (291,968 representatives x orbit sizes)."""
+    """Full-range n=5 class-K counts of 200 seeded non-constant corpus formulas (>= 100 over both
+    variables) + the named axioms = the oracle's isomorphism-orbit sum (291,968 representatives x
+    orbit sizes; kov_orbits is pinned in tests/test_oracle_pins.py)."""
     g = gold("n5_orbit.npz")
-    progs = W.corpus_c2()[:96] + [W.to_postfix(t) for t in W.named_axioms().values()]
+    corpus = W.corpus_c2()
+    progs = [corpus[i] for i in g["index"]] + [W.to_postfix(t) for t in W.named_axioms().values()]
+    assert sum(1 for c in progs if b"\x10" in c and b"\x11" in c) >= 100
     got = run(kb, progs, 5, 2, K)
     same(got, g, "n=5 full K", keys=("models", "frames"))
     certify(progs, got, 5, 2, K)
+
+
+def test_c3_n5_full_T_counts_golden(kb):
+    """120 seeded non-constant corpus formulas over ALL 2^20 reflexive frames at n=5 (SURVEY 8(c) plan
+    item 3): counts and first witnesses equal the oracle's full class-T census."""
+    g = gold("n5_t_full.npz")
+    corpus = W.corpus_c2()
+    progs = [corpus[i] for i in g["index"]]
+    got = run(kb, progs, 5, 2, T)
+    same(got, g, "n=5 full T")
+    certify(progs, got, 5, 2, T)
+    # the same records as part of the whole batch (program sharing, chunking over the corpus)
+    allr = run(kb, corpus, 5, 2, T)
+    same({k: v[g["index"]] for k, v in allr.items()}, g, "n=5 full T, whole batch")
 
 
 def test_n5_closed_forms_full_range(kb):
@@ -197,7 +215,7 @@ def test_c3_n5_full_corpus_witnesses(kb, vol):
         pos = res["wit_f"][hit] if cls == K else np.searchsorted(frames, res["wit_f"][hit])
         unverified = 0
         for p in np.unique(pos):
-            if p >= 512:                       # cap the oracle's prefix scan
+            if p >= 4096:                      # cap the oracle's prefix scan (4,096 frames x 1,024 valuations)
                 unverified += int((pos == p).sum())
                 continue
             sel = hit[pos == p]
@@ -205,6 +223,8 @@ def test_c3_n5_full_corpus_witnesses(kb, vol):
             want = vol.census(sc, so, 5, 2, cls, 0, int(p) + 1)
             for key in ("wit_f", "wit_v", "wit_w"):
                 assert (want[key].astype(np.uint64) == res[key][sel].astype(np.uint64)).all(), (cname, int(p), key)
+        print(f"firstness {cname}: {len(hit) - unverified} of {len(hit)} witnesses verified by an oracle prefix "
+              f"scan, {unverified} beyond the cap (firstness unverified)")
         assert unverified <= 8, f"{cname}: {unverified} witnesses beyond the firstness cap"
 
 

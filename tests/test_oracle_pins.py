@@ -380,3 +380,87 @@ def test_c_failure_counts_closed_forms_and_consistency(vol):
             assert int(cnt[b, f]) == want
     rel = np.array([[[(f >> (w * n + u)) & 1 for u in range(n)] for w in range(n)] for f in range(1 << (n * n))], np.uint8)
     assert (vol.failure_counts(code, offs, n, k, rel=rel) == cnt).all()
+
+
+# ------------------------------------------------------------------------------------------
+# C. the isomorphism-orbit route (feeds tests/golden/n5_orbit.npz and c5_counts.npz:n5_frames)
+# ------------------------------------------------------------------------------------------
+def _relabel(n, pi, f):
+    """Image of the K-index f under the world permutation pi (written a second time, in Python)."""
+    g = 0
+    for w in range(n):
+        for u in range(n):
+            if (f >> (w * n + u)) & 1:
+                g |= 1 << (pi[w] * n + pi[u])
+    return g
+
+
+def _burnside_orbits(n):
+    """Number of isomorphism classes of digraphs with loops on n labelled points by Burnside's lemma:
+    (1/n!) sum over permutations of 2^(cycles of the induced permutation of the n*n ordered pairs)."""
+    total = 0
+    for pi in itertools.permutations(range(n)):
+        seen, cycles = set(), 0
+        for start in itertools.product(range(n), repeat=2):
+            if start in seen:
+                continue
+            cycles += 1
+            x = start
+            while x not in seen:
+                seen.add(x)
+                x = (pi[x[0]], pi[x[1]])
+        total += 2 ** cycles
+    fact = 1
+    for i in range(2, n + 1):
+        fact *= i
+    assert total % fact == 0
+    return total // fact
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5])
+def test_c_orbits_counts_sizes_and_representatives(vol, n):
+    """kov_orbits: the number of orbits is OEIS A000595 (2, 10, 104, 3,044, 291,968 - SURVEY 8(c)
+    'relabelling invariance') and equals Burnside's count computed here; the sizes sum to 2^(n*n);
+    every representative is the least member of its orbit and its size is the number of distinct
+    relabellings (all orbits for n <= 3, a seeded sample for n = 4, 5); representatives ascend."""
+    reps, sizes = vol.orbits(n)
+    assert len(reps) == [2, 10, 104, 3044, 291968][n - 1] == _burnside_orbits(n)
+    assert int(sizes.sum()) == 1 << (n * n)
+    assert (np.diff(reps.astype(np.int64)) > 0).all()
+    perms = list(itertools.permutations(range(n)))
+    rng = W.SplitMix64(9100 + n)
+    idx = range(len(reps)) if n <= 3 else sorted({rng.below(len(reps)) for _ in range(150)} | {0, len(reps) - 1})
+    for i in idx:
+        images = {_relabel(n, pi, int(reps[i])) for pi in perms}
+        assert min(images) == int(reps[i]) and len(images) == int(sizes[i]), (n, i)
+    # every frame belongs to exactly one listed orbit (n <= 3: all frames; n = 4, 5: seeded frames)
+    repset = set(int(r) for r in reps)
+    frames = range(1 << (n * n)) if n <= 3 else [rng.below(1 << (n * n)) for _ in range(300)]
+    for f in frames:
+        assert min(_relabel(n, pi, f) for pi in perms) in repset
+
+
+def test_c_orbit_weighted_census_equals_direct_census(vol):
+    """Relabelling invariance (P:123 scans labelled frames; the orbit route is the oracle's exact
+    shortcut): class-K counts from one representative per orbit weighted by the orbit size equal the
+    direct census over all labelled frames - all of C1 at n=3, 240 seeded C2 formulas at n=4 (only
+    among non-constant ones), and the C5 pair counts at n=3, 4."""
+    for progs, n in ((W.corpus_c1(), 3), (None, 4)):
+        if progs is None:
+            c2 = [c for c in W.corpus_c2() if (b"\x10" in c or b"\x11" in c)]
+            rng = W.SplitMix64(9200)
+            progs = [c2[i] for i in sorted({rng.below(len(c2)) for _ in range(260)})][:240]
+        code, offs = W.pack_programs(progs)
+        reps, sizes = vol.orbits(n)
+        w = vol.census_list(code, offs, n, 2, reps, weights=sizes)
+        d = vol.census(code, offs, n, 2, K)
+        assert (w["models"] == d["models"]).all() and (w["frames"] == d["frames"]).all()
+        assert d["models"].max() > 0 and (d["models"] != d["models"][0]).any()
+    pprogs, pairs, _ = W.pairs_c5(300)
+    code, offs = W.pack_programs(pprogs)
+    pairs = np.array(pairs, np.uint32)
+    for n in (3, 4):
+        reps, sizes = vol.orbits(n)
+        w = vol.census_list(code, offs, n, 0, reps, weights=sizes, pairs=pairs)
+        d = vol.census(code, offs, n, 0, K, pairs=pairs)
+        assert (w["frames"] == d["frames"]).all() and (w["models"] == d["models"]).all()
