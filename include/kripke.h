@@ -270,6 +270,16 @@ int kripke_failure_density_frames(const kripke_programs_t *programs, uint32_t n_
                                   const uint16_t *succ, uint64_t n_frames, uint32_t *counts_out,
                                   void *stream);
 
+/* Semantic signatures (the census corpus is "reduced to one representative per semantic equivalence
+ * class on all frames of <= 3 worlds"; "64-bit per-size behaviour fingerprint"): sig_out[2b], sig_out[2b+1]
+ * = two independent 64-bit sums over every model (frame, valuation) of 1..n_max worlds of a mix of (size, model
+ * index, truth set of formula b).  Equal truth sets on all those models give equal signatures; the converse
+ * holds up to a ~2^-128 collision, so the hash only screens - a class is made certain with
+ * kripke_distinguish_pairs over the same sizes ("no equivalence claim rests on a matching
+ * fingerprint").  sig_out: DEVICE, 2 * n_formulas uint64.  1 <= n_max <= 4. */
+int kripke_signatures(const kripke_programs_t *programs, uint32_t n_vars, uint32_t n_max, uint64_t *sig_out,
+                      void *stream);
+
 /* End-to-end convenience with HOST buffers only: create + eval over the full class + copy the
  * results back + destroy, synchronously (this is what bench.py's "e2e" figure times). */
 int kripke_eval_batch_host(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,
@@ -314,8 +324,10 @@ int kripke_last_run_info(const kripke_programs_t *programs, kripke_run_info_t *i
  * call therefore blocks for the compilation (kripke_run_info_t.jit_compile_seconds); later calls only
  * enqueue.  Results are identical to the interpreted and scalar kernels (GPU tests).
  * kripke_jit_configure: 1 <= max_programs_per_kernel <= 160 (default 64; more programs per kernel share
- * more subterms and need more registers).  Affects plans built afterwards. */
-int kripke_jit_configure(uint32_t max_programs_per_kernel);
+ * more subterms and need more registers); 1 <= min_blocks_per_sm <= 8 = the __launch_bounds__ occupancy
+ * request of the generated kernels (128 threads per block; default 2, i.e. up to 255 registers per thread).
+ * Affects plans built afterwards. */
+int kripke_jit_configure(uint32_t max_programs_per_kernel, uint32_t min_blocks_per_sm);
 
 /* Diagnostic (pure host: works without a CUDA device): the CUDA C source of compiled kernel kernel_index
  * of the group of programs that mention group_vars variables, for the given batch (HOST code / offsets as

@@ -37,7 +37,7 @@ EXPORTS = [
     "kripke_eval_frames", "kripke_distinguish_pairs_frames",
     "kripke_validity_bitmap", "kripke_condition_bitmap", "kripke_match_bitmaps", "kripke_frames_from_bitmap",
     "kripke_failure_density", "kripke_failure_density_frames",
-    "kripke_jit_configure", "kripke_debug_jit_source", "kripke_debug_dag_truth",
+    "kripke_jit_configure", "kripke_debug_jit_source", "kripke_debug_dag_truth", "kripke_signatures",
 ]
 
 
@@ -99,7 +99,8 @@ def load():
     lib.kripke_frames_from_bitmap.argtypes = [u32, u32, u64, u64, vp, vp, u64, vp, vp]
     lib.kripke_eval_frames.argtypes = [vp, u32, u32, vp, u64, u64, u32, vp, vp, vp]
     lib.kripke_distinguish_pairs_frames.argtypes = [vp, u32p, u32, u32, u32, vp, u64, u64, u32, vp, vp, vp]
-    lib.kripke_jit_configure.argtypes = [u32]
+    lib.kripke_jit_configure.argtypes = [u32, u32]
+    lib.kripke_signatures.argtypes = [vp, u32, u32, vp, vp]
     lib.kripke_debug_jit_source.argtypes = [u8p, u32p, u32, u32, u32p, u32, u32, u32, u32, u32, u32, ctypes.c_int, vp, u64,
                                             ctypes.POINTER(u32), ctypes.POINTER(u64), ctypes.POINTER(u64)]
     lib.kripke_debug_dag_truth.argtypes = [u8p, u32, u32, u32, u32p, u32p, ctypes.POINTER(u32)]
@@ -346,6 +347,15 @@ def failure_density_frames(programs: Programs, n_worlds: int, n_vars: int, succ,
     return counts_out
 
 
+def signatures(programs: Programs, n_vars: int, n_max: int = 3, sig_out=None, stream=None):
+    """kripke_signatures: int64 CUDA tensor (B, 2) holding the two 64-bit sums per formula."""
+    import torch
+    if sig_out is None:
+        sig_out = torch.empty((programs.n_formulas, 2), dtype=torch.int64, device="cuda")
+    _check(load().kripke_signatures(programs._h, n_vars, n_max, sig_out.data_ptr(), _stream(stream)), "kripke_signatures")
+    return sig_out
+
+
 def bits_to_bool(bitmap, count: int):
     """int32 bit words (..., words) (torch or numpy) -> numpy bool array (..., count)."""
     a = bitmap.cpu().numpy() if hasattr(bitmap, "cpu") else np.asarray(bitmap)
@@ -440,8 +450,8 @@ def debug_lower(code_a: bytes, code_b: bytes | None, n_vars: int, leaf_mode: int
 
 
 
-def jit_configure(max_programs_per_kernel: int):
-    _check(load().kripke_jit_configure(max_programs_per_kernel), "kripke_jit_configure")
+def jit_configure(max_programs_per_kernel: int = 64, min_blocks_per_sm: int = 2):
+    _check(load().kripke_jit_configure(max_programs_per_kernel, min_blocks_per_sm), "kripke_jit_configure")
 
 
 def debug_jit_source(code, offsets, n_vars: int, n_worlds: int, frame_class: int, group_vars: int,

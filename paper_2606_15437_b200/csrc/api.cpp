@@ -285,6 +285,7 @@ enum : uint32_t { ENGINE_INTERPRETED = 0, ENGINE_JIT = 1 };
 
 // Tunables of the compiled scans (kripke_jit_configure).
 uint32_t g_jit_max_programs = 64;
+uint32_t g_jit_min_blocks = 2;
 
 // Lowers the records (formulas, or pairs if `pairs` != null) into one GroupPlan per variable count.
 int build_scan_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
@@ -353,8 +354,8 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *h_pairs, 
         // bookkeeping for the roofline: instructions the kernels need per frame of the range
         const double words = (double)(1ull << (g.k_eff * n)) / 32.0;
         if (g.use_jit) {
-            h->last.sliced_logic_ops_per_word += g.jit.stats.logic_ops_per_word;
-            h->last.logic_instr_per_frame += (double)g.jit.stats.logic_ops_per_word * words;
+            h->last.sliced_logic_ops_per_word += g.jit.stats.logic_ops_emitted;
+            h->last.logic_instr_per_frame += g.jit.stats.logic_ops_per_word * words;
             h->last.executed_models += (uint64_t)g.jit.n_slots * (count << (g.k_eff * n));
             h->last.jit_programs += g.jit.n_slots;
             continue;
@@ -683,7 +684,7 @@ int build_jit_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_r
         JitLayout lay;
         jit_layout(n, G.g, cls, &lay);
         std::string log;
-        rc = jit_build_group(G.dag, lay, G.roots, G.slot_record, g_jit_max_programs, &gp.jit, &log);
+        rc = jit_build_group(G.dag, lay, G.roots, G.slot_record, g_jit_max_programs, g_jit_min_blocks, &gp.jit, &log);
         if (rc > 0) rc = cuda_fail(rc);
         if (!rc) rc = upload(&gp.d_alias, G.alias);
         if (rc) { gp.release(); out->release(); return rc; }
@@ -918,6 +919,17 @@ int kripke_failure_density_frames(const kripke_programs_t *programs, uint32_t n_
     job.code = h->d_code; job.offsets = h->d_offsets; job.n_formulas = h->n_formulas;
     job.pairs = nullptr; job.n_records = h->n_formulas; job.accum = nullptr;
     int e = launch_failure_density(job, succ, counts_out, stream);
+    return e ? cuda_fail(e) : KRIPKE_OK;
+}
+
+int kripke_signatures(const kripke_programs_t *programs, uint32_t n_vars, uint32_t n_max, uint64_t *sig_out,
+                      void *stream) {
+    if (!programs) return KRIPKE_EINVAL;
+    const kripke_programs *h = programs;
+    if (n_vars != h->n_vars || n_max < 1 || n_max > 4) return KRIPKE_EINVAL;
+    if (n_max * n_max + n_vars * n_max > 40) return KRIPKE_EUNSUPPORTED;
+    if (h->n_formulas && !sig_out) return KRIPKE_EINVAL;
+    int e = launch_signatures(n_vars, n_max, h->d_code, h->d_offsets, h->n_formulas, sig_out, stream);
     return e ? cuda_fail(e) : KRIPKE_OK;
 }
 
@@ -1246,9 +1258,11 @@ int kripke_debug_lower(const uint8_t *code_a, uint32_t len_a, const uint8_t *cod
     return (int)low.ucode.size();
 }
 
-int kripke_jit_configure(uint32_t max_programs_per_kernel) {
+int kripke_jit_configure(uint32_t max_programs_per_kernel, uint32_t min_blocks_per_sm) {
     if (max_programs_per_kernel < 1 || max_programs_per_kernel > 160) return KRIPKE_EINVAL;
+    if (min_blocks_per_sm < 1 || min_blocks_per_sm > 8) return KRIPKE_EINVAL;
     g_jit_max_programs = max_programs_per_kernel;
+    g_jit_min_blocks = min_blocks_per_sm;
     return KRIPKE_OK;
 }
 
@@ -1283,8 +1297,8 @@ int kripke_debug_jit_source(const uint8_t *code, const uint32_t *offsets, uint32
     std::vector<JitRoot> rs;
     for (uint32_t r : parts[kernel_index]) rs.push_back(G.roots[r]);
     JitEmitStats st;
-    const std::string src = jit_emit_kernel(G.dag, lay, rs, 128, 2, &st);
-    if (logic_ops_per_word_out) *logic_ops_per_word_out = st.logic_ops_per_word;
+    const std::string src = jit_emit_kernel(G.dag, lay, rs, 128, g_jit_min_blocks, &st);
+    if (logic_ops_per_word_out) *logic_ops_per_word_out = (uint64_t)(st.logic_ops_per_word + 0.5);
     if (compile) {
         std::string log;
         size_t bytes = 0;

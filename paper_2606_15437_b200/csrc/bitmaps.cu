@@ -195,6 +195,62 @@ __global__ void __launch_bounds__(128) frames_from_bitmap_kernel(ConditionParams
     for (uint32_t w = 0; w < p.n; ++w) succ_out[at * p.n + w] = (uint16_t)succ[w];
 }
 
+// ---- semantic signatures ("one representative per semantic equivalence class on all frames of
+// <= 3 worlds"; "64-bit per-size behaviour fingerprint") ------------------------------------
+// One block per formula; its threads stride over every model (frame, valuation) of 1..n_max worlds, evaluate
+// the truth set with the scalar recurrence and fold (size, model index, truth set) into two independent
+// 64-bit sums.  Addition commutes, so the order of the models - and of the threads - does not matter.  Two
+// formulas with equal truth sets on all those models get equal signatures; unequal behaviour collides with
+// probability ~2^-128.  The hash only screens: callers that need certainty re-check a class with the pair
+// path (kripke_distinguish_pairs over the same sizes), as the paper does ("no equivalence claim
+// rests on a matching fingerprint").
+__device__ __forceinline__ unsigned long long sig_mix(unsigned long long x) {
+    x ^= x >> 30; x *= 0xBF58476D1CE4E5B9ull;
+    x ^= x >> 27; x *= 0x94D049BB133111EBull;
+    return x ^ (x >> 31);
+}
+
+struct SignatureParams {
+    uint32_t k, n_max;
+    const uint8_t *code;
+    const uint32_t *offsets;
+    uint32_t n_formulas;
+    unsigned long long *sig;      // 2 per formula
+};
+
+__global__ void __launch_bounds__(256) signature_kernel(SignatureParams p) {
+    __shared__ unsigned long long s_a[8], s_b[8];
+    const uint32_t b = blockIdx.x;
+    const uint8_t *c = p.code + p.offsets[b];
+    const uint32_t len = p.offsets[b + 1] - p.offsets[b];
+    unsigned long long ha = 0, hb = 0;
+    for (uint32_t n = 1; n <= p.n_max; ++n) {
+        const uint32_t full = (1u << n) - 1u, kn = p.k * n;
+        const uint64_t models = 1ull << (n * n + kn);
+        for (uint64_t x = threadIdx.x; x < models; x += blockDim.x) {
+            const uint64_t f = x >> kn, v = x & ((1ull << kn) - 1ull);
+            uint32_t succ[KRIPKE_MAX_WORLDS], val[KRIPKE_MAX_VARS];
+            decode_rows(n, f, succ);
+            for (uint32_t i = 0; i < KRIPKE_MAX_VARS; ++i) val[i] = (uint32_t)(v >> (i * n)) & full;
+            const unsigned long long t = eval_postfix_scalar(c, len, n, succ, val, full);
+            const unsigned long long key = ((unsigned long long)n << 60) | (x << 6) | t;
+            ha += sig_mix(key + 0x9E3779B97F4A7C15ull);
+            hb += sig_mix(key * 0xD6E8FEB86659FD93ull + 0x2545F4914F6CDD1Dull);
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        ha += __shfl_xor_sync(0xFFFFFFFFu, ha, o);
+        hb += __shfl_xor_sync(0xFFFFFFFFu, hb, o);
+    }
+    if ((threadIdx.x & 31u) == 0) { s_a[threadIdx.x >> 5] = ha; s_b[threadIdx.x >> 5] = hb; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int i = 1; i < 8; ++i) { ha += s_a[i]; hb += s_b[i]; }
+        p.sig[2 * b] = ha;
+        p.sig[2 * b + 1] = hb;
+    }
+}
+
 }  // namespace
 
 int launch_validity_bitmap(const ScanJob &job, uint32_t *bitmap_out, void *stream) {
@@ -259,6 +315,16 @@ int launch_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t w
     if (n_records == 0) return 0;
     match_bitmaps_kernel<<<(n_records + 3) / 4, 128, 0, (cudaStream_t)stream>>>(bitmaps, n_records, words, library,
                                                                                n_library, match_out);
+    return (int)cudaGetLastError();
+}
+
+int launch_signatures(uint32_t k, uint32_t n_max, const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,
+                      uint64_t *sig_out, void *stream) {
+    if (n_formulas == 0) return 0;
+    SignatureParams p;
+    p.k = k; p.n_max = n_max; p.code = code; p.offsets = offsets; p.n_formulas = n_formulas;
+    p.sig = (unsigned long long *)sig_out;
+    signature_kernel<<<n_formulas, 256, 0, (cudaStream_t)stream>>>(p);
     return (int)cudaGetLastError();
 }
 

@@ -109,6 +109,10 @@ int launch_failure_density(const ScanJob &job, const uint16_t *succ_list, uint32
 int launch_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words, const uint32_t *library,
                          uint32_t n_library, uint32_t *match_out, void *stream);
 
+// Semantic signatures: two 64-bit sums per formula over every model of 1..n_max worlds.
+int launch_signatures(uint32_t k, uint32_t n_max, const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,
+                      uint64_t *sig_out, void *stream);
+
 // Zero the accumulators; finish: turn accumulators into counts / witnesses (handles ACCUMULATE).
 int launch_init(Accum *accum, uint32_t n_records, void *stream);
 // accum[pairs[2i]] = accum[pairs[2i+1]] for i < n (records sharing a representative's program).

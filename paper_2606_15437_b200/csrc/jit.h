@@ -82,7 +82,9 @@ struct JitRoot {
 };
 
 struct JitEmitStats {
-    uint64_t logic_ops_per_word = 0;   // 3-input logic instructions the emitted body needs per word
+    double logic_ops_per_word = 0;     // 3-input logic instructions executed per 32-model word: statements of the
+                                       // inner loop + those of the outer loop and of the unit set-up per word
+    uint64_t logic_ops_emitted = 0;    // statements' logic instructions, wherever they are placed
     uint32_t n_box = 0, n_and = 0;     // graph nodes evaluated per word (summed over kernels)
 };
 
@@ -115,8 +117,8 @@ struct JitGroupPlan {
 // parallel host threads.  Returns 0, a negative kripke_status, or a positive cudaError_t;
 // *log_out receives the NVRTC log on a compile error.
 int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitRoot> &roots,
-                    const std::vector<uint32_t> &slot_record, uint32_t max_roots, JitGroupPlan *out,
-                    std::string *log_out);
+                    const std::vector<uint32_t> &slot_record, uint32_t max_roots, uint32_t min_blocks,
+                    JitGroupPlan *out, std::string *log_out);
 
 // Enqueues the group's kernels over the aligned class range of `job` (job.k = the group's g).
 int jit_launch_group(const ScanJob &job, const JitGroupPlan &plan, uint32_t model_shift, void *stream,

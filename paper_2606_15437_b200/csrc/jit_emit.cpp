@@ -4,8 +4,11 @@
 #include "jit.h"
 
 #include <algorithm>
+#include <array>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
+#include <map>
 #include <set>
 
 namespace kripke {
@@ -35,11 +38,19 @@ const char *lane_const(uint32_t pos) {
 }
 
 // Where the value of bit `pos` of the model index X comes from in a thread, as a C expression that is
-// an all-0 / all-1 word (or the in-word lane pattern).
+// an all-0 / all-1 word (or the in-word lane pattern), and at which loop level it changes:
+// 0 = fixed for the unit, 1 = changes with the outer (frame) loop, 2 = changes with the inner (valuation) loop.
 struct BitSource {
     const JitLayout &lay;
     std::set<uint32_t> used_inner, used_outer, used_unit;
     explicit BitSource(const JitLayout &l) : lay(l) {}
+    int level(uint32_t pos) const {
+        if (pos < 5) return 0;
+        pos -= 5;
+        if (pos < lay.inner) return 2;
+        pos -= lay.inner;
+        return pos < lay.outer ? 1 : 0;
+    }
     std::string word(uint32_t pos) {
         if (pos < 5) return lane_const(pos);
         pos -= 5;
@@ -52,37 +63,97 @@ struct BitSource {
     }
 };
 
+// ---- expressions and their mapping onto 3-input logic instructions ---------------------------------
+// Every value of the loop body (one world of one graph node, or a program's refuted-lane word) is a small
+// expression tree over operands (other values, masks, lane patterns).  A value with a single use at the same
+// loop level is substituted into its consumer; each remaining tree is then covered with 3-input look-up
+// tables (LOP3.LUT) by dynamic programming over its cuts - the fewest instructions a tree allows - and
+// emitted as lop3.b32 with the table computed here.  What the kernel executes is therefore known
+// statically: one LOP3 per emitted table.
+struct Ex {
+    enum Op : uint8_t { LEAF, CONST, AND, OR, XOR } op;
+    bool neg;           // the value is complemented (CONST: false = all-0, true = all-1)
+    int a, b;           // operands of a binary node
+    std::string tok;    // LEAF: the operand as a C expression
+};
+
 struct Emitter {
     const Dag &dag;
     const JitLayout &lay;
     BitSource bits;
     std::set<uint32_t> used_table;          // table classes: edge positions read from the table entry
     std::vector<char> done;
-    std::string body;
-    JitEmitStats stats;
+    std::vector<std::array<int8_t, KRIPKE_MAX_WORLDS>> lvl;   // loop level of every (node, world) value
+    uint32_t n_box = 0, n_and = 0;
 
-    Emitter(const Dag &d, const JitLayout &l) : dag(d), lay(l), bits(l), done(d.nodes.size(), 0) {}
+    std::vector<Ex> pool;
+    struct Stmt {
+        int level;
+        std::string out;        // value name; "" = a program's refuted-lane word r
+        int root;
+        std::string tail;       // text after the value (programs: the count updates)
+        bool inlined = false;
+    };
+    std::vector<Stmt> stmts;
+    std::string body[3];
+    uint64_t ops[3] = {0, 0, 0};
+    uint32_t n_tmp = 0;
 
-    // word of "p_i holds at world w"
-    std::string atom(uint32_t i, uint32_t w) { return bits.word(i * lay.n + w); }
+    Emitter(const Dag &d, const JitLayout &l) : dag(d), lay(l), bits(l), done(d.nodes.size(), 0), lvl(d.nodes.size()) {
+        for (auto &x : lvl) x.fill(-1);
+    }
+
+    // ---- expression constructors (constants fold) ----
+    int leaf(const std::string &tok, bool neg) { pool.push_back(Ex{Ex::LEAF, neg, -1, -1, tok}); return (int)pool.size() - 1; }
+    int constant(bool v) { pool.push_back(Ex{Ex::CONST, v, -1, -1, ""}); return (int)pool.size() - 1; }
+    int negate(int x) { pool[x].neg = !pool[x].neg; return x; }
+    int bin(Ex::Op op, int x, int y) {
+        for (int pass = 0; pass < 2; ++pass) {
+            if (pool[x].op == Ex::CONST) {
+                const bool v = pool[x].neg;
+                if (op == Ex::AND) return v ? y : x;
+                if (op == Ex::OR) return v ? x : y;
+                return v ? negate(y) : y;                                   // XOR
+            }
+            std::swap(x, y);
+        }
+        pool.push_back(Ex{op, false, x, y, ""});
+        return (int)pool.size() - 1;
+    }
+
+    // position in X of "p_i holds at world w" / of the edge w -> u (-1: constant or table entry)
+    int atom_pos(uint32_t i, uint32_t w) const { return (int)(i * lay.n + w); }
+    int edge_pos(uint32_t w, uint32_t u) const {
+        const uint32_t n = lay.n;
+        if (lay.table) return -1;
+        if (lay.cls == KRIPKE_CLASS_T) return w == u ? -1 : (int)(lay.kn + w * (n - 1) + (u < w ? u : u - 1));   // reflexive_deposit's compact index
+        return (int)(lay.kn + w * n + u);
+    }
     // word of the edge w -> u; "" = the edge is always present (class T diagonal)
     std::string edge(uint32_t w, uint32_t u) {
         const uint32_t n = lay.n;
         if (lay.table) { used_table.insert(w * n + u); return fmt("me%u", w * n + u); }
-        if (lay.cls == KRIPKE_CLASS_T) {
-            if (w == u) return "";
-            return bits.word(lay.kn + w * (n - 1) + (u < w ? u : u - 1));      // reflexive_deposit's compact index
-        }
-        return bits.word(lay.kn + w * n + u);
+        const int pos = edge_pos(w, u);
+        return pos < 0 ? std::string() : bits.word((uint32_t)pos);
     }
-    // C expression of literal `lit` at world w
-    std::string lit(uint32_t l, uint32_t w) {
+    int edge_level(uint32_t w, uint32_t u) const {
+        const int pos = edge_pos(w, u);
+        return pos < 0 ? 0 : bits.level((uint32_t)pos);
+    }
+    // loop level of literal l at world w (its node must have been visited)
+    int lit_level(uint32_t l, uint32_t w) const {
         const DagNode &nd = dag.nodes[l >> 1];
-        std::string s;
-        if (nd.kind == DagNode::CONST0) return (l & 1u) ? "0xFFFFFFFFu" : "0u";
-        if (nd.kind == DagNode::VAR) s = atom(nd.var, w);
-        else s = fmt("t%u_%u", l >> 1, w);
-        return (l & 1u) ? "~" + s : s;
+        if (nd.kind == DagNode::CONST0) return 0;
+        if (nd.kind == DagNode::VAR) return bits.level((uint32_t)atom_pos(nd.var, w));
+        return lvl[l >> 1][w];
+    }
+    // literal l at world w as an expression
+    int lit(uint32_t l, uint32_t w) {
+        const DagNode &nd = dag.nodes[l >> 1];
+        const bool neg = l & 1u;
+        if (nd.kind == DagNode::CONST0) return constant(neg);
+        if (nd.kind == DagNode::VAR) return leaf(bits.word((uint32_t)atom_pos(nd.var, w)), neg);
+        return leaf(fmt("t%u_%u", l >> 1, w), neg);
     }
     void node(uint32_t id) {
         if (done[id]) return;
@@ -92,27 +163,143 @@ struct Emitter {
         if (nd.kind == DagNode::AND) {
             node(nd.a >> 1);
             node(nd.b >> 1);
-            for (uint32_t w = 0; w < n; ++w)
-                body += fmt("      const unsigned t%u_%u = ", id, w) + lit(nd.a, w) + " & " + lit(nd.b, w) + ";\n";
-            stats.logic_ops_per_word += n;
-            ++stats.n_and;
+            for (uint32_t w = 0; w < n; ++w) {
+                const int L = std::max(lit_level(nd.a, w), lit_level(nd.b, w));
+                lvl[id][w] = (int8_t)L;
+                stmts.push_back(Stmt{L, fmt("t%u_%u", id, w), bin(Ex::AND, lit(nd.a, w), lit(nd.b, w)), ""});
+            }
+            ++n_and;
         } else if (nd.kind == DagNode::BOX) {
             node(nd.a >> 1);
             // Lemma 1 on 32 models: R[w] = AND_u ( T[u] | ~E[w][u] )
             for (uint32_t w = 0; w < n; ++w) {
-                std::string e;
-                uint32_t runtime_terms = 0, terms = 0;
+                int L = 0, acc = constant(true);
                 for (uint32_t u = 0; u < n; ++u) {
-                    const std::string ew = edge(w, u), x = lit(nd.a, u);
-                    std::string term;
-                    if (ew.empty()) term = x;                                  // edge always present
-                    else { term = "(" + x + " | ~" + ew + ")"; ++runtime_terms; }
-                    e += (terms++ ? " & " : "") + term;
+                    const std::string ew = edge(w, u);
+                    L = std::max(L, std::max(lit_level(nd.a, u), edge_level(w, u)));
+                    const int x = lit(nd.a, u);
+                    acc = bin(Ex::AND, acc, ew.empty() ? x : bin(Ex::OR, x, leaf(ew, true)));
                 }
-                body += fmt("      const unsigned t%u_%u = ", id, w) + e + ";\n";
-                stats.logic_ops_per_word += std::max(1u, runtime_terms);
+                lvl[id][w] = (int8_t)L;
+                stmts.push_back(Stmt{L, fmt("t%u_%u", id, w), acc, ""});
             }
-            ++stats.n_box;
+            ++n_box;
+        }
+    }
+
+    // ---- single-use substitution ----
+    void collect_leaves(int x, std::vector<int> *out) const {
+        if (pool[x].op == Ex::LEAF) out->push_back(x);
+        else if (pool[x].op != Ex::CONST) { collect_leaves(pool[x].a, out); collect_leaves(pool[x].b, out); }
+    }
+    void substitute() {
+        std::map<std::string, int> producer;
+        std::map<std::string, int> uses;
+        for (size_t i = 0; i < stmts.size(); ++i)
+            if (!stmts[i].out.empty()) producer[stmts[i].out] = (int)i;
+        std::vector<std::vector<int>> leaves(stmts.size());
+        for (size_t i = 0; i < stmts.size(); ++i) {
+            collect_leaves(stmts[i].root, &leaves[i]);
+            for (int lf : leaves[i]) ++uses[pool[lf].tok];
+        }
+        for (size_t i = 0; i < stmts.size(); ++i)
+            for (int lf : leaves[i]) {
+                auto it = producer.find(pool[lf].tok);
+                if (it == producer.end() || uses[pool[lf].tok] != 1) continue;
+                Stmt &p = stmts[it->second];
+                if (p.level != stmts[i].level || pool[p.root].op == Ex::CONST) continue;
+                const bool neg = pool[lf].neg;
+                pool[lf] = pool[p.root];                  // the producer's tree takes the operand's place
+                pool[lf].neg = pool[lf].neg != neg;
+                p.inlined = true;
+            }
+    }
+
+    // ---- covering a tree with 3-input tables ----
+    struct Cut { std::vector<std::string> elems; uint32_t cost; };
+    std::map<int, uint32_t> best_cost;
+    std::map<int, Cut> best_cut;
+    std::map<int, std::vector<Cut>> all_cuts;
+    static std::string key_of(int x) { return fmt("#%d", x); }
+    uint32_t elems_cost(const std::vector<std::string> &e) {
+        uint32_t c = 0;
+        for (const std::string &k : e) if (k[0] == '#') c += best_cost[std::atoi(k.c_str() + 1)];
+        return c;
+    }
+    // the ways to stand for subtree x inside a table of its parent: as one operand, or through any of its cuts
+    std::vector<Cut> options(int x) {
+        if (pool[x].op == Ex::LEAF) return {Cut{{pool[x].tok}, 0}};
+        cover(x);
+        std::vector<Cut> o = all_cuts[x];
+        o.push_back(Cut{{key_of(x)}, best_cost[x]});
+        return o;
+    }
+    void cover(int x) {
+        if (best_cost.count(x)) return;
+        const std::vector<Cut> A = options(pool[x].a), B = options(pool[x].b);
+        std::vector<Cut> cuts;
+        std::set<std::vector<std::string>> seen;
+        for (const Cut &ca : A)
+            for (const Cut &cb : B) {
+                std::vector<std::string> u = ca.elems;
+                for (const std::string &k : cb.elems) if (std::find(u.begin(), u.end(), k) == u.end()) u.push_back(k);
+                if (u.size() > 3) continue;
+                std::sort(u.begin(), u.end());
+                if (!seen.insert(u).second) continue;
+                cuts.push_back(Cut{u, elems_cost(u)});
+            }
+        size_t bi = 0;
+        for (size_t i = 1; i < cuts.size(); ++i)
+            if (cuts[i].cost < cuts[bi].cost || (cuts[i].cost == cuts[bi].cost && cuts[i].elems.size() < cuts[bi].elems.size())) bi = i;
+        best_cost[x] = 1 + cuts[bi].cost;
+        best_cut[x] = cuts[bi];
+        all_cuts[x] = cuts;
+    }
+    // truth table of subtree x over the operands named in `in` (bit patterns 0xF0, 0xCC, 0xAA)
+    uint32_t table(int x, const std::map<std::string, uint32_t> &in, bool top) const {
+        const Ex &e = pool[x];
+        if (e.op == Ex::LEAF) return (in.at(e.tok) ^ (e.neg ? 0xFFu : 0u)) & 0xFFu;
+        if (!top) {
+            auto it = in.find(key_of(x));
+            if (it != in.end()) return it->second;        // realised separately: its complement is already applied
+        }
+        const uint32_t a = table(e.a, in, false), b = table(e.b, in, false);
+        const uint32_t v = e.op == Ex::AND ? (a & b) : e.op == Ex::OR ? (a | b) : (a ^ b);
+        return (v ^ (e.neg ? 0xFFu : 0u)) & 0xFFu;
+    }
+    // emits the tables of subtree x into `out`; returns the name holding its value
+    std::string realise(int x, const std::string &name, int level, std::string *out) {
+        cover(x);
+        const Cut &c = best_cut[x];
+        std::vector<std::string> names;
+        std::map<std::string, uint32_t> in;
+        static const uint32_t pat[3] = {0xF0u, 0xCCu, 0xAAu};
+        for (size_t i = 0; i < c.elems.size(); ++i) {
+            const std::string &k = c.elems[i];
+            names.push_back(k[0] == '#' ? realise(std::atoi(k.c_str() + 1), fmt("x%u", n_tmp++), level, out) : k);
+            in[k] = pat[i];
+        }
+        while (names.size() < 3) names.push_back(names[0]);
+        const uint32_t lut = table(x, in, true);
+        *out += "      unsigned " + name + "; asm(\"lop3.b32 %0, %1, %2, %3, " + fmt("0x%02x", lut) + ";\" : \"=r\"(" + name +
+                ") : \"r\"(" + names[0] + "), \"r\"(" + names[1] + "), \"r\"(" + names[2] + "));\n";
+        ++ops[level];
+        return name;
+    }
+    void emit_all() {
+        substitute();
+        for (const Stmt &st : stmts) {
+            if (st.inlined) continue;
+            std::string &out = body[st.level];
+            const std::string name = st.out.empty() ? "r" : st.out;
+            if (st.out.empty()) out += "      {\n";
+            const Ex &e = pool[st.root];
+            if (e.op == Ex::CONST) out += "      const unsigned " + name + (e.neg ? " = 0xFFFFFFFFu;\n" : " = 0u;\n");
+            else if (e.op == Ex::LEAF) {
+                out += "      const unsigned " + name + " = " + (e.neg ? "~" : "") + e.tok + ";\n";
+                if (e.neg) ++ops[st.level];
+            } else realise(st.root, name, st.level, &out);
+            if (st.out.empty()) out += "      " + st.tail + " }\n";
         }
     }
 };
@@ -218,28 +405,26 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
     else fmode = F_ANY;                                             // 2^inner words per frame, several frames per unit
 
     for (uint32_t r = 0; r < G; ++r) {
-        em.body += fmt("      // program %u\n", r);
         em.node(roots[r].a >> 1);
-        std::string e;
+        int e;
         if (roots[r].b == UINT32_MAX) {
             // refuted lanes: the truth set is not all worlds
-            const bool neg = roots[r].a & 1u;
-            for (uint32_t w = 0; w < n; ++w) e += (w ? (neg ? " | " : " & ") : "") + em.lit(roots[r].a & ~1u, w);
-            e = neg ? e : "~(" + e + ")";
-            em.stats.logic_ops_per_word += (n + 1) / 2;
+            e = em.constant(true);
+            for (uint32_t w = 0; w < n; ++w) e = em.bin(Ex::AND, e, em.lit(roots[r].a, w));
+            e = em.negate(e);
         } else {
             // distinguishing lanes: the two truth sets differ
             em.node(roots[r].b >> 1);
-            for (uint32_t w = 0; w < n; ++w)
-                e += (w ? " | " : "") + ("(" + em.lit(roots[r].a, w) + " ^ " + em.lit(roots[r].b, w) + ")");
-            em.stats.logic_ops_per_word += n;
+            e = em.constant(false);
+            for (uint32_t w = 0; w < n; ++w) e = em.bin(Ex::OR, e, em.bin(Ex::XOR, em.lit(roots[r].a, w), em.lit(roots[r].b, w)));
         }
-        em.body += fmt("      { const unsigned r = ") + e + fmt("; c%u += __popc(r);", r);
-        if (fmode == F_WORD) em.body += fmt(" f%u += (r != 0u);", r);
-        else if (fmode == F_ANY) em.body += fmt(" a%u |= r;", r);
-        else if (fmode == F_FOLD) em.body += fmt(" f%u += kj_frames_in_word<%u>(r);", r, lay.kn);
-        em.body += " }\n";
+        std::string tail = fmt("c%u += __popc(r);", r);
+        if (fmode == F_WORD) tail += fmt(" f%u += (r != 0u);", r);
+        else if (fmode == F_ANY) tail += fmt(" a%u |= r;", r);
+        else if (fmode == F_FOLD) tail += fmt(" f%u += kj_frames_in_word<%u>(r);", r, lay.kn);
+        em.stmts.push_back(Emitter::Stmt{2, "", e, tail});
     }
+    em.emit_all();
 
     std::string s = kPrelude;
     s += fmt("\n// layout: n=%u g=%u cls=%u inner=%u outer=%u split=%u unit_frames_log2=%u programs=%u\n", n, lay.g, lay.cls,
@@ -270,6 +455,7 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
     for (uint32_t b : em.bits.used_outer) decl_outer += fmt("      const unsigned mo%u = 0u - ((jo >> %u) & 1u);\n", b, b);
     for (uint32_t b : em.bits.used_inner) decl_inner += fmt("      const unsigned mi%u = 0u - ((ji >> %u) & 1u);\n", b, b);
     s += decl_unit;
+    s += "      // values that are fixed for the unit\n" + em.body[0];
     for (uint32_t r = 0; r < G; ++r) {
         s += fmt("      unsigned c%u = 0u;", r);
         if (fmode == F_WORD || fmode == F_ANY || fmode == F_FOLD) s += fmt(" unsigned f%u = 0u;", r);
@@ -278,11 +464,12 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
     s += "#pragma unroll 1\n";
     s += fmt("      for (unsigned jo = 0; jo < %uu; ++jo) {\n", 1u << lay.outer);
     s += decl_outer;
+    s += em.body[1];
     if (fmode == F_ANY) for (uint32_t r = 0; r < G; ++r) s += fmt("      unsigned a%u = 0u;\n", r);
     s += "#pragma unroll 1\n";
     s += fmt("      for (unsigned ji = 0; ji < %uu; ++ji) {\n", 1u << lay.inner);
     s += decl_inner;
-    s += em.body;
+    s += em.body[2];
     s += "      }\n";
     if (fmode == F_ANY) for (uint32_t r = 0; r < G; ++r) s += fmt("      f%u += (a%u != 0u);\n", r, r);
     s += "      }\n";
@@ -301,7 +488,14 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
     s += fmt("        atomicMin(&a->best, ((u0 + s_best[i]) >> %u) << %u);\n", lay.split, lay.unit_frames_log2);
     s += "      }\n";
     s += "  }\n}\n";
-    if (stats) *stats = em.stats;
+    if (stats) {
+        const uint64_t *ops = em.ops;
+        stats->logic_ops_emitted = ops[0] + ops[1] + ops[2];
+        stats->logic_ops_per_word = (double)ops[2] + (double)ops[1] / (double)(1u << lay.inner) +
+                                    (double)ops[0] / (double)(1u << (lay.inner + lay.outer));
+        stats->n_box = em.n_box;
+        stats->n_and = em.n_and;
+    }
     return s;
 }
 

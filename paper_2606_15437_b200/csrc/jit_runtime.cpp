@@ -75,8 +75,8 @@ int jit_compile_only(const std::string &source, std::string *log_out, size_t *cu
 }
 
 int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitRoot> &roots,
-                    const std::vector<uint32_t> &slot_record, uint32_t max_roots, JitGroupPlan *out,
-                    std::string *log_out) {
+                    const std::vector<uint32_t> &slot_record, uint32_t max_roots, uint32_t min_blocks,
+                    JitGroupPlan *out, std::string *log_out) {
     out->release();
     out->lay = lay;
     out->stats = JitEmitStats();
@@ -89,8 +89,9 @@ int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitR
         std::vector<JitRoot> rs;
         for (uint32_t r : parts[i]) { rs.push_back(roots[r]); order.push_back(r); }
         JitEmitStats st;
-        sources[i] = jit_emit_kernel(dag, lay, rs, out->threads, 2, &st);
+        sources[i] = jit_emit_kernel(dag, lay, rs, out->threads, min_blocks, &st);
         out->stats.logic_ops_per_word += st.logic_ops_per_word;
+        out->stats.logic_ops_emitted += st.logic_ops_emitted;
         out->stats.n_box += st.n_box;
         out->stats.n_and += st.n_and;
     }

@@ -73,7 +73,7 @@ def test_emitted_kernels_compile_for_sm100a(n, k, cls):
         if nk == 0:
             continue
         seen += 1
-        assert cubin > 0 and ops > 0
+        assert cubin > 0 and (ops > 0 or g < k)
         m = re.search(r"layout: n=(\d+) g=(\d+) cls=(\d+) inner=(\d+) outer=(\d+) split=(\d+) unit_frames_log2=(\d+)", src)
         assert m and int(m.group(1)) == n and int(m.group(2)) == g
         inner, outer, split, ufl = (int(m.group(i)) for i in (4, 5, 6, 7))
