@@ -449,7 +449,11 @@ def run_c4(args):
         info = h.last_run_info()
         ev = B * count * nval
         out["batch"][str(B)] = {"frames": count, "seconds": t, "evaluations_per_s": ev / t,
-                                "logic_instr_per_s": info.sliced_logic_ops_per_word * (count * nval // 32) / t}
+                                "engine": info.kernel_family, "distinct_programs": info.jit_programs,
+                                "compile_seconds": info.jit_compile_seconds,
+                                "executed_logic_instr_per_s": info.logic_instr_per_frame * count / t,
+                                "frac_of_alu_peak": info.logic_instr_per_frame * count / t / (SM_COUNT * INT_LANES_PER_SM * 1.965e9),
+                                "algorithmic_logic_instr_per_s": info.algorithmic_logic_instr_per_frame * count / t}
         h.destroy()
     # B. one fused launch of 32 formulas vs 32 separate launches (2^20-frame range)
     begin, count = 1 << 24, 1 << 20
@@ -493,6 +497,32 @@ def run_c4(args):
         t = timed(lambda: kb.eval_batch_range(h, n, k, 0, begin, count, 0, c, w))
         res["bit_sliced_default"] = {"seconds": t, "evaluations_per_s": NB * count * nval / t}
         out["contention"][name] = res
+        h.destroy()
+    # D. the same ablation where atomics can matter: one variable (32 valuations per frame between two atomics
+    # instead of 32,768), 256 seeded one-variable formulas, 2^20 frames - the regime of the paper's frame-atomic
+    # kernel (26.27x adversarial / 3.44x mixed)
+    rng = W.SplitMix64(15437014)
+    seen, one = set(), []
+    while len(one) < NB:
+        c = W.to_postfix(W.gen_formula(rng, 9, 6, "p"))
+        if c not in seen and len(c) >= 3:
+            seen.add(c); one.append(c)
+    adv1 = [W.to_postfix(("and", ("bot",), W.from_postfix(c))) for c in one]
+    out["contention_one_variable"] = {}
+    for name, batch in (("mixed", one), ("adversarial", adv1)):
+        h = kb.Programs(*W.pack_programs(batch), 1)
+        c = torch.zeros((NB, 2), dtype=torch.int64, device="cuda")
+        w = torch.zeros((NB, 2), dtype=torch.int64, device="cuda")
+        res = {"formulas": NB, "frames": count, "valuations_per_frame": 32}
+        kb.eval_batch_range(h, n, 1, 0, begin, 256, kb.KERNEL_SCALAR, c, w)
+        for mname, mode in (("block", kb.REDUCE_BLOCK), ("warp", kb.REDUCE_WARP), ("thread", kb.REDUCE_THREAD)):
+            t = timed(lambda: kb.eval_batch_range(h, n, 1, 0, begin, count, kb.KERNEL_SCALAR | mode, c, w))
+            res[mname] = {"seconds": t, "evaluations_per_s": NB * count * 32 / t}
+        res["block_vs_thread"] = res["thread"]["seconds"] / res["block"]["seconds"]
+        res["block_vs_warp"] = res["warp"]["seconds"] / res["block"]["seconds"]
+        t = timed(lambda: kb.eval_batch_range(h, n, 1, 0, begin, count, 0, c, w))
+        res["bit_sliced_default"] = {"seconds": t, "evaluations_per_s": NB * count * 32 / t}
+        out["contention_one_variable"][name] = res
         h.destroy()
     clocks = clock.result()
     b2048 = out["batch"]["2048"]
@@ -611,9 +641,106 @@ def run_c5(args):
     }))
 
 
+def run_atlas(args):
+    """--workload atlas: failure densities: per (formula, frame) the number
+    of (valuation, world) pairs on which the formula fails, written formula-major as uint32.  Two legs:
+      panels  the paper-shaped atlas: the 5,624-formula corpus (two variables) on every K frame of 1..3 worlds
+              (Atlas-3), a 2,048-frame four-world panel and a 4,096-frame five-world panel - each count
+              sums 2^(2n) valuations x n worlds, so this leg is bound by the integer pipe, not by memory;
+      write   the regime the paper reports for its atlas materialisation (51.54 GB at 91.6 % of its HBM ceiling,
+              P:262): 64 variable-free formulas of the C5 list on ALL 2^25 five-world K frames, one frame per
+              lane, 8.6 GB of counts - bound by HBM writes; roofline against MEASURED_PEAKS.json hbm_gbs."""
+    import torch
+    from paper_2606_15437_b200 import binding as kb
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    kb.load()
+    peak_src = "MEASURED_PEAKS.json hbm_gbs"
+    try:
+        hbm = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+    except Exception:
+        hbm, peak_src = 6650.0, "fallback of B200_PROFILING.md (6.65 TB/s): MEASURED_PEAKS.json absent"
+    alu_peak = SM_COUNT * INT_LANES_PER_SM * 1.965e9
+    clock = ClockSampler(0)
+    clock.start()
+    reps = max(1, args.steps)
+
+    def timed(fn):
+        for _ in range(max(1, min(args.warmup, 3))):
+            fn()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b) * 1e-3)
+        return float(np.median(ts))
+
+    # leg 1: panels of the two-variable corpus
+    progs = W.corpus_c2()
+    B = len(progs)
+    h = kb.Programs(*W.pack_programs(progs), N_VARS)
+    panels = [(1, 0, 2), (2, 0, 16), (3, 0, 512), (4, 30000, 2048), (5, 1 << 24, 4096)]
+    outs = [torch.zeros((B, cnt), dtype=torch.int32, device="cuda") for _, _, cnt in panels]
+    logic = [0.0]
+
+    def run_panels():
+        logic[0] = 0.0
+        for (n, begin, cnt), o in zip(panels, outs):
+            kb.failure_density(h, n, N_VARS, 0, begin, cnt, o)
+            logic[0] += h.last_run_info().logic_instr_per_frame * cnt
+
+    t0 = time.perf_counter(); run_panels(); torch.cuda.synchronize(); t_build = time.perf_counter() - t0
+    t_panels = timed(run_panels)
+    entries = B * sum(cnt for _, _, cnt in panels)
+    evals = B * sum(cnt << (N_VARS * n) for n, _, cnt in panels)
+    leg1 = {"formulas": B, "frames": sum(cnt for _, _, cnt in panels), "entries": entries, "seconds": t_panels,
+            "entries_per_s": entries / t_panels, "evaluations_per_s": evals / t_panels,
+            "bytes_written": 4 * entries, "write_GB_per_s": 4 * entries / t_panels / 1e9,
+            "logic_instr_per_s": logic[0] / t_panels, "frac_of_alu_peak": logic[0] / t_panels / alu_peak,
+            "plan_build_seconds": t_build, "bound": "alu"}
+    h.destroy()
+
+    # leg 2: HBM-write-bound - variable-free formulas, every five-world K frame
+    p0 = W.pairs_c5()[0][:64]
+    h0 = kb.Programs(*W.pack_programs(p0), 0)
+    frames = 1 << 25
+    out = torch.empty((len(p0), frames), dtype=torch.int32, device="cuda")
+    kb.failure_density(h0, 5, 0, 0, 0, 1 << 12, out)                     # builds the plan
+    torch.cuda.synchronize()
+    t_write = timed(lambda: kb.failure_density(h0, 5, 0, 0, 0, frames, out))
+    info = h0.last_run_info()
+    nbytes = 4 * len(p0) * frames
+    # spot check of the written matrix against the scalar kernel on a window (both are this library's kernels;
+    # parity against the oracle is tests/test_gpu_bitmaps.py)
+    w0 = 12345 * 32
+    chk = kb.failure_density(h0, 5, 0, 0, w0 + 1, 1023)                  # 1,023 frames: unaligned -> scalar kernel
+    assert (chk == out[:, w0 + 1:w0 + 1024]).all()
+    clocks = clock.result()
+    achieved = nbytes / t_write / 1e9
+    print(json.dumps({
+        "metric": "failure-density entries/sec ((formula, frame) counts written, uint32)",
+        "value": len(p0) * frames / t_write, "unit": "entries/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": t_write * 1e3, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "u32",
+        "data": "synthetic",
+        "config": {"workload": f"atlas (SURVEY 8f N2; P:270, P:284, P:262): write leg = {len(p0)} variable-free formulas x all 2^25 "
+                               f"five-world K frames ({nbytes / 1e9:.2f} GB of counts); panels leg = {B} two-variable formulas x "
+                               "Atlas-3 + 2,048 four-world + 4,096 five-world frames",
+                   "panels": leg1,
+                   "context": "paper, H100: atlas materialisation 51.54 GB at >= 1,622 GB/s = 91.6 % of its measured 1,771 GB/s (P:262)"},
+        "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": "kripke_jit_scan, density mode, one frame per lane (class K, n=5, no variables)",
+                     "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm, "peak_source": peak_src,
+                     "algorithmic_bytes": nbytes, "traffic": None,
+                     "traffic_source": "ncu dram__bytes_write.sum: profiles/r2_atlas.md",
+                     "logic_instr_per_s": info.logic_instr_per_frame * frames / t_write,
+                     "frac_of_alu_peak": info.logic_instr_per_frame * frames / t_write / alu_peak},
+    }))
+
+
 def run_frames(args):
     """--workload frames: frame-list mode (Table 2).  Per size n the
-    pair path is timed on a seeded list of 2^20 explicit frames (workloads/frames.py stress_list):
+    pair path is timed on a seeded list of 2^20 explicit frames (kripke_frames_generate, KRIPKE_GEN_STRESS):
     constant pairs (the 36 named pairs of PAPER.md:179/190 plus seeded ones, one valuation) at every
     size, one-variable pairs (2^n valuations) through n = 12.  Reports pair-frame
     tests/s, valuation-frame evaluations/s (2 formulas per pair), the kernel's logic-instruction rate
@@ -650,8 +777,7 @@ def run_frames(args):
     rows = {}
     total_tests = total_evals = total_time = 0.0
     for n in (6, 8, 10, 12, 14, 16):
-        rel = F.stress_list(n, n_frames)
-        succ = torch.from_numpy(F.succ_masks(rel).view(np.int16).reshape(-1).copy()).cuda()
+        succ = kb.frames_generate(kb.GEN_STRESS, n, n_frames, F.SEED_FRAMES)      # written on the device
         row = {}
         for k, progs, pairs in ((0, progs0, pairs0), (1, progs1, pairs1)):
             if k * n > 12:
@@ -682,7 +808,7 @@ def run_frames(args):
     from oracle import volume as V
     V.build()
     n = 8
-    rel = F.stress_list(n, 2048)
+    rel = F.stress_list_cb(n, 2048)
     code, offs = W.pack_programs(progs1)
     t0 = time.perf_counter()
     V.census_relations(code, offs, n, 1, rel, pairs=pairs1)
@@ -809,6 +935,8 @@ def main():
         run_c4(args)
     elif args.workload == "c5":
         run_c5(args)
+    elif args.workload == "atlas":
+        run_atlas(args)
     elif args.workload == "frames":
         run_frames(args)
     elif args.workload == "correspond":

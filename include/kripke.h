@@ -205,6 +205,31 @@ int kripke_eval_frames(const kripke_programs_t *programs, uint32_t n_worlds, uin
                        const uint16_t *succ, uint64_t n_frames, uint64_t index_base, uint32_t flags,
                        kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream);
 
+/* Frame-list generators (P:183-185 the named stress templates; P:192 / Table 2 the synthesized relations).  The
+ * paper's template list and generator parameters are not published; these families take their shape (DESIGN.md
+ * 3).  succ_out: DEVICE, n_frames * n_worlds uint16 successor masks in the format above, written on `stream`, so
+ * a stress list never exists on the host.  Frame j of a list depends only on (generator, n_worlds, seed, j) and
+ * for KRIPKE_GEN_STRESS on n_frames - a counter-based generator, restated in workloads/frames.py for the tests.
+ *   KRIPKE_GEN_TEMPLATES    frame j = template j % KRIPKE_TPL_COUNT
+ *   KRIPKE_GEN_ERDOS_RENYI  every ordered pair (loops included) is an edge with probability 0.05 / 0.1 / 0.2 /
+ *                           0.35 / 0.5 / 0.8 for j % 6 = 0..5 (stratified)
+ *   KRIPKE_GEN_EDGE_FLIP    template j % KRIPKE_TPL_COUNT with 1..4 seeded ordered pairs toggled
+ *   KRIPKE_GEN_DEAD_END     density-0.3 relation with one seeded world's successors removed
+ *   KRIPKE_GEN_BACK_EDGE    the path 0 -> ... -> n-1 plus two seeded edges w -> u, u <= w
+ *   KRIPKE_GEN_STRESS       the templates, then the four generators above in equal shares
+ * 1 <= n_worlds <= 16, n_frames <= 2^32. */
+enum {
+    KRIPKE_TPL_PATH = 0, KRIPKE_TPL_REVERSE_PATH = 1, KRIPKE_TPL_REFLEXIVE_PATH = 2, KRIPKE_TPL_FORK = 3,
+    KRIPKE_TPL_CYCLE = 4, KRIPKE_TPL_STAR = 5, KRIPKE_TPL_REVERSE_STAR = 6, KRIPKE_TPL_PATH_LOOP_END = 7,
+    KRIPKE_TPL_COMPLETE = 8, KRIPKE_TPL_EMPTY = 9, KRIPKE_TPL_COUNT = 10
+};
+enum {
+    KRIPKE_GEN_TEMPLATES = 0, KRIPKE_GEN_ERDOS_RENYI = 1, KRIPKE_GEN_EDGE_FLIP = 2, KRIPKE_GEN_DEAD_END = 3,
+    KRIPKE_GEN_BACK_EDGE = 4, KRIPKE_GEN_STRESS = 5, KRIPKE_GEN_COUNT = 6
+};
+int kripke_frames_generate(uint32_t generator, uint32_t n_worlds, uint64_t n_frames, uint64_t seed,
+                           uint16_t *succ_out, void *stream);
+
 /* The pair path over a frame list: pairs is a HOST array of 2*n_pairs program indices;
  * a frame distinguishes pair j under a valuation iff the two truth sets differ; world = least
  * disagreement world.  counts_out / witness_out: DEVICE, n_pairs entries. */
@@ -332,8 +357,8 @@ int kripke_jit_configure(uint32_t max_programs_per_kernel, uint32_t min_blocks_p
 /* Diagnostic (pure host: works without a CUDA device): the CUDA C source of compiled kernel kernel_index
  * of the group of programs that mention group_vars variables, for the given batch (HOST code / offsets as
  * in kripke_programs_create; pairs == NULL) or the listed pairs of it, as kripke_eval_batch_range / kripke_distinguish_pairs would build it for
- * (n_worlds, frame_class, flags).  compile != 0 also compiles it with NVRTC to an sm_100a cubin
- * (*cubin_bytes_out).  source_out (capacity cap, NUL-terminated, may be NULL), *n_kernels_out = kernels of the
+ * (n_worlds, frame_class, flags).  compile: bit 0 = also compile it with NVRTC to an sm_100a cubin
+ * (*cubin_bytes_out); bit 1 = the failure-density kernel of kripke_failure_density instead of the scan kernel.  source_out (capacity cap, NUL-terminated, may be NULL), *n_kernels_out = kernels of the
  * group, *logic_ops_per_word_out = 3-input logic instructions per 32-model word of this kernel.  Returns the
  * source length or a negative kripke_status (KRIPKE_EUNSUPPORTED: no compiled layout for the shape). */
 int kripke_debug_jit_source(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas, uint32_t n_vars,

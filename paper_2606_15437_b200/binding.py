@@ -37,7 +37,7 @@ EXPORTS = [
     "kripke_eval_frames", "kripke_distinguish_pairs_frames",
     "kripke_validity_bitmap", "kripke_condition_bitmap", "kripke_match_bitmaps", "kripke_frames_from_bitmap",
     "kripke_failure_density", "kripke_failure_density_frames",
-    "kripke_jit_configure", "kripke_debug_jit_source", "kripke_debug_dag_truth", "kripke_signatures",
+    "kripke_jit_configure", "kripke_debug_jit_source", "kripke_debug_dag_truth", "kripke_signatures", "kripke_frames_generate",
 ]
 
 
@@ -101,6 +101,7 @@ def load():
     lib.kripke_distinguish_pairs_frames.argtypes = [vp, u32p, u32, u32, u32, vp, u64, u64, u32, vp, vp, vp]
     lib.kripke_jit_configure.argtypes = [u32, u32]
     lib.kripke_signatures.argtypes = [vp, u32, u32, vp, vp]
+    lib.kripke_frames_generate.argtypes = [u32, u32, u64, u64, vp, vp]
     lib.kripke_debug_jit_source.argtypes = [u8p, u32p, u32, u32, u32p, u32, u32, u32, u32, u32, u32, ctypes.c_int, vp, u64,
                                             ctypes.POINTER(u32), ctypes.POINTER(u64), ctypes.POINTER(u64)]
     lib.kripke_debug_dag_truth.argtypes = [u8p, u32, u32, u32, u32p, u32p, ctypes.POINTER(u32)]
@@ -347,6 +348,19 @@ def failure_density_frames(programs: Programs, n_worlds: int, n_vars: int, succ,
     return counts_out
 
 
+GEN_TEMPLATES, GEN_ERDOS_RENYI, GEN_EDGE_FLIP, GEN_DEAD_END, GEN_BACK_EDGE, GEN_STRESS = range(6)
+
+
+def frames_generate(generator: int, n_worlds: int, n_frames: int, seed: int, succ_out=None, stream=None):
+    """kripke_frames_generate: int16 CUDA tensor of n_frames * n_worlds successor masks (bit pattern of uint16)."""
+    import torch
+    if succ_out is None:
+        succ_out = torch.empty((max(1, n_frames) * n_worlds,), dtype=torch.int16, device="cuda")[:n_frames * n_worlds]
+    _check(load().kripke_frames_generate(generator, n_worlds, n_frames, seed, succ_out.data_ptr(), _stream(stream)),
+           "kripke_frames_generate")
+    return succ_out
+
+
 def signatures(programs: Programs, n_vars: int, n_max: int = 3, sig_out=None, stream=None):
     """kripke_signatures: int64 CUDA tensor (B, 2) holding the two 64-bit sums per formula."""
     import torch
@@ -455,7 +469,7 @@ def jit_configure(max_programs_per_kernel: int = 64, min_blocks_per_sm: int = 2)
 
 
 def debug_jit_source(code, offsets, n_vars: int, n_worlds: int, frame_class: int, group_vars: int,
-                     kernel_index: int = 0, flags: int = 0, pairs=None, compile: bool = False):
+                     kernel_index: int = 0, flags: int = 0, pairs=None, compile: bool = False, density: bool = False):
     """(source text, kernels in the group, logic ops per word of this kernel, cubin bytes) of one compiled
     kernel; None if the emitter has no layout for the shape.  Pure host."""
     code, offsets = _host(code, offsets)
@@ -466,7 +480,8 @@ def debug_jit_source(code, offsets, n_vars: int, n_worlds: int, frame_class: int
     rc = load().kripke_debug_jit_source(code.ctypes.data, offsets.ctypes.data, len(offsets) - 1, n_vars,
                                         None if pa is None else pa.ctypes.data,
                                         0 if pa is None else len(pa) // 2, n_worlds, frame_class, flags, group_vars,
-                                        kernel_index, 1 if compile else 0, ctypes.cast(buf, ctypes.c_void_p), cap,
+                                        kernel_index, (1 if compile else 0) | (2 if density else 0),
+                                        ctypes.cast(buf, ctypes.c_void_p), cap,
                                         ctypes.byref(nk), ctypes.byref(ops), ctypes.byref(cb))
     if rc == EUNSUPPORTED:
         return None

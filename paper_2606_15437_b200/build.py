@@ -31,6 +31,7 @@ UNITS = [
     ("calibrate", "calibrate.cu", []),
     ("scan_frames", "scan_frames.cu", []),
     ("bitmaps", "bitmaps.cu", []),
+    ("frame_gen", "frame_gen.cu", []),
     ("jit_dag", "jit_dag.cpp", []),
     ("jit_emit", "jit_emit.cpp", []),
     ("jit_runtime", "jit_runtime.cpp", []),

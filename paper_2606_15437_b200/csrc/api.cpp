@@ -229,6 +229,7 @@ struct kripke_programs {
     // per formula, from the postfix program as written: modal operators, binary connectives, variables
     std::vector<uint32_t> f_modal, f_binary, f_vars;
     std::map<uint64_t, ScanPlan> single;     // one record per formula; cached per (n, k, class, flags, engine)
+    std::map<uint64_t, ScanPlan> density;    // failure-density plans, per (n, k, class)
     struct PairPlan {                  // plans of kripke_distinguish_pairs, cached per pair list and shape
         std::vector<uint32_t> pairs;
         uint64_t key = 0;
@@ -472,7 +473,7 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *h_pairs, 
             ScanJob rj = job;
             rj.k = g.k_eff; rj.frame_begin = ab; rj.frame_count = ae - ab;
             h->last.kernel_family = 2;
-            if ((e = jit_launch_group(rj, g.jit, (k - g.k_eff) * n, stream, &launches))) return cuda_fail(e);
+            if ((e = jit_launch_group(rj, g.jit, (k - g.k_eff) * n, nullptr, stream, &launches))) return cuda_fail(e);
         }
         ScanJob head = job, tail = job;
         head.frame_count = ab - begin;
@@ -619,7 +620,10 @@ struct JitGroupHost {
 // Groups the records by the number of variables they mention (Algorithm 1's per-formula k_b; the
 // least g >= that count for which the emitter has a layout) and builds each group's graph.
 int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
-                      uint32_t cls, uint32_t flags, std::vector<JitGroupHost> *out) {
+                      uint32_t cls, uint32_t flags, uint32_t mode, std::vector<JitGroupHost> *out) {
+    auto layout_ok = [&](uint32_t g) {
+        return mode == JIT_MODE_DENSITY ? jit_density_layout(n, g, cls, nullptr) : jit_layout(n, g, cls, nullptr);
+    };
     auto prog = [&](uint32_t f) { return &h->h_code[h->h_offsets[f]]; };
     auto plen = [&](uint32_t f) { return h->h_offsets[f + 1] - h->h_offsets[f]; };
     out->clear();
@@ -639,8 +643,8 @@ int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t 
         uint32_t cnt = 0;
         for (uint32_t i = 0; i < KRIPKE_MAX_VARS; ++i) cnt += (sup >> i) & 1u;
         uint32_t g = (flags & KRIPKE_FULL_SWEEP) ? k : cnt;
-        while (g < k && !jit_layout(n, g, cls, nullptr)) ++g;
-        if (!jit_layout(n, g, cls, nullptr)) return KRIPKE_EUNSUPPORTED;
+        while (g < k && !layout_ok(g)) ++g;
+        if (!layout_ok(g)) return KRIPKE_EUNSUPPORTED;
         JitGroupHost &G = (*out)[g];
         uint8_t rename[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
         if (flags & KRIPKE_NO_SHARING) {                 // variables in their own order, nothing shared
@@ -650,7 +654,7 @@ int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t 
         } else {
             canonical_rename(prog(fa), plen(fa), pairs ? prog(fb) : nullptr, pairs ? plen(fb) : 0u, sup, rename);
         }
-        if (!(flags & KRIPKE_NO_SHARING)) {
+        if (!(flags & KRIPKE_NO_SHARING) && mode != JIT_MODE_DENSITY) {
             // records whose graphs coincide are scanned once (the pair path is symmetric in its two formulas)
             uint32_t pa = probe[g].build(prog(fa), plen(fa), rename);
             uint32_t pb = pairs ? probe[g].build(prog(fb), plen(fb), rename) : UINT32_MAX;
@@ -674,7 +678,7 @@ int build_jit_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_r
     out->release();
     const auto t0 = std::chrono::steady_clock::now();
     std::vector<JitGroupHost> groups;
-    int rc = jit_group_records(h, pairs, n_records, n, k, cls, flags, &groups);
+    int rc = jit_group_records(h, pairs, n_records, n, k, cls, flags, JIT_MODE_SCAN, &groups);
     if (rc) return rc;
     for (JitGroupHost &G : groups) {
         if (G.roots.empty() && G.alias.empty()) continue;
@@ -684,11 +688,37 @@ int build_jit_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_r
         JitLayout lay;
         jit_layout(n, G.g, cls, &lay);
         std::string log;
-        rc = jit_build_group(G.dag, lay, G.roots, G.slot_record, g_jit_max_programs, g_jit_min_blocks, &gp.jit, &log);
+        rc = jit_build_group(G.dag, lay, G.roots, G.slot_record, g_jit_max_programs, g_jit_min_blocks, JIT_MODE_SCAN, &gp.jit, &log);
         if (rc > 0) rc = cuda_fail(rc);
         if (!rc) rc = upload(&gp.d_alias, G.alias);
         if (rc) { gp.release(); out->release(); return rc; }
         gp.n_alias = (uint32_t)(G.alias.size() / 2);
+        out->groups.push_back(gp);
+    }
+    out->jit_compile_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    return KRIPKE_OK;
+}
+
+// Failure-density plan: every formula is a record of its own (one output row each), the graph is shared.
+int build_density_plan(const kripke_programs *h, uint32_t n, uint32_t k, uint32_t cls, ScanPlan *out) {
+    out->release();
+    const auto t0 = std::chrono::steady_clock::now();
+    std::vector<JitGroupHost> groups;
+    int rc = jit_group_records(h, nullptr, h->n_formulas, n, k, cls, 0, JIT_MODE_DENSITY, &groups);
+    if (rc) return rc;
+    for (JitGroupHost &G : groups) {
+        if (G.roots.empty()) continue;
+        GroupPlan gp;
+        gp.k_eff = G.g;
+        gp.use_jit = true;
+        JitLayout lay;
+        jit_density_layout(n, G.g, cls, &lay);
+        std::string log;
+        // fewer programs per kernel than a scan: every program keeps n failing-world words alive for its stores
+        rc = jit_build_group(G.dag, lay, G.roots, G.slot_record, std::min<uint32_t>(g_jit_max_programs, 32), g_jit_min_blocks,
+                             JIT_MODE_DENSITY, &gp.jit, &log);
+        if (rc > 0) rc = cuda_fail(rc);
+        if (rc) { gp.release(); out->release(); return rc; }
         out->groups.push_back(gp);
     }
     out->jit_compile_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
@@ -887,7 +917,7 @@ int kripke_failure_density(const kripke_programs_t *programs, uint32_t n_worlds,
                            uint32_t frame_class, uint64_t frame_begin, uint64_t frame_count,
                            uint32_t *counts_out, void *stream) {
     if (!programs) return KRIPKE_EINVAL;
-    const kripke_programs *h = programs;
+    kripke_programs *h = const_cast<kripke_programs *>(programs);
     if (n_worlds < 1 || n_worlds > KRIPKE_MAX_WORLDS || n_vars != h->n_vars || frame_class > KRIPKE_CLASS_S5)
         return KRIPKE_EINVAL;
     if (n_vars * n_worlds > KRIPKE_LIST_MAX_VAL_BITS) return KRIPKE_EUNSUPPORTED;
@@ -902,8 +932,63 @@ int kripke_failure_density(const kripke_programs_t *programs, uint32_t n_worlds,
     if ((rc = class_table_device(n_worlds, frame_class, &job.class_table))) return rc;
     job.code = h->d_code; job.offsets = h->d_offsets; job.n_formulas = h->n_formulas;
     job.pairs = nullptr; job.n_records = h->n_formulas; job.accum = nullptr;
-    int e = launch_failure_density(job, nullptr, counts_out, stream);
-    return e ? cuda_fail(e) : KRIPKE_OK;
+    h->last = kripke_run_info_t{};
+    h->last.models_per_program = frame_count << (n_vars * n_worlds);
+    if (frame_count == 0 || h->n_formulas == 0) return KRIPKE_OK;
+    // Compiled bit-sliced kernels when every variable-count group has a density layout and the rows can be
+    // written with 16-byte stores; the scalar kernel (thread = frame, one model per iteration) otherwise and on
+    // the ragged ends of the range.
+    bool compiled = jit_density_layout(n_worlds, n_vars, frame_class, nullptr) && frame_count % 4 == 0 &&
+                    (reinterpret_cast<uintptr_t>(counts_out) & 15u) == 0;
+    const ScanPlan *plan = nullptr;
+    if (compiled) {
+        const uint64_t key = plan_key(n_worlds, n_vars, frame_class, 0, ENGINE_JIT, 0);
+        auto it = h->density.find(key);
+        if (it == h->density.end()) {
+            ScanPlan sp;
+            rc = build_density_plan(h, n_worlds, n_vars, frame_class, &sp);
+            if (rc == KRIPKE_EUNSUPPORTED) compiled = false;
+            else if (rc) return rc;
+            else it = h->density.emplace(key, std::move(sp)).first;
+        }
+        if (compiled) plan = &it->second;
+    }
+    int e = 0;
+    uint32_t launches = 0;
+    if (!compiled) {
+        if ((e = launch_failure_density(job, nullptr, counts_out, frame_count, 0, stream))) return cuda_fail(e);
+        h->last.launches = 1;
+        return KRIPKE_OK;
+    }
+    h->last.kernel_family = 2;
+    h->last.jit_compile_seconds = plan->jit_compile_seconds;
+    for (const GroupPlan &g : plan->groups) {
+        const uint64_t fpu = 1ull << g.jit.lay.unit_frames_log2;
+        uint64_t ab = (frame_begin + fpu - 1) / fpu * fpu, ae = (frame_begin + frame_count) / fpu * fpu;
+        if (ae <= ab) ab = ae = frame_begin;
+        const double words = (double)(1ull << (g.k_eff * n_worlds)) / 32.0;
+        h->last.logic_instr_per_frame += g.jit.stats.logic_ops_per_word * words;
+        h->last.jit_programs += g.jit.n_slots;
+        if (ae > ab) {
+            ScanJob rj = job;
+            rj.k = g.k_eff; rj.frame_begin = ab; rj.frame_count = ae - ab;
+            JitDensityOut out{counts_out, frame_count, frame_begin};
+            if ((e = jit_launch_group(rj, g.jit, (n_vars - g.k_eff) * n_worlds, &out, stream, &launches))) return cuda_fail(e);
+        }
+        // ragged ends: the scalar kernel on this group's records only
+        for (int side = 0; side < 2; ++side) {
+            ScanJob sj = job;
+            sj.frame_begin = side ? ae : frame_begin;
+            sj.frame_count = side ? frame_begin + frame_count - ae : ab - frame_begin;
+            if (sj.frame_count == 0) continue;
+            if ((e = launch_failure_density_records(sj, g.jit.d_slot_record, g.jit.n_slots, counts_out, frame_count,
+                                                    sj.frame_begin - frame_begin, stream)))
+                return cuda_fail(e);
+            ++launches;
+        }
+    }
+    h->last.launches = launches;
+    return KRIPKE_OK;
 }
 
 int kripke_failure_density_frames(const kripke_programs_t *programs, uint32_t n_worlds, uint32_t n_vars,
@@ -918,7 +1003,16 @@ int kripke_failure_density_frames(const kripke_programs_t *programs, uint32_t n_
     job.frame_begin = 0; job.frame_count = n_frames; job.class_table = nullptr;
     job.code = h->d_code; job.offsets = h->d_offsets; job.n_formulas = h->n_formulas;
     job.pairs = nullptr; job.n_records = h->n_formulas; job.accum = nullptr;
-    int e = launch_failure_density(job, succ, counts_out, stream);
+    int e = launch_failure_density(job, succ, counts_out, n_frames, 0, stream);
+    return e ? cuda_fail(e) : KRIPKE_OK;
+}
+
+int kripke_frames_generate(uint32_t generator, uint32_t n_worlds, uint64_t n_frames, uint64_t seed, uint16_t *succ_out,
+                           void *stream) {
+    if (generator >= KRIPKE_GEN_COUNT || n_worlds < 1 || n_worlds > KRIPKE_LIST_MAX_WORLDS) return KRIPKE_EINVAL;
+    if (n_frames > (1ull << 32)) return KRIPKE_EUNSUPPORTED;
+    if (n_frames && !succ_out) return KRIPKE_EINVAL;
+    int e = launch_frames_generate(generator, n_worlds, n_frames, seed, succ_out, stream);
     return e ? cuda_fail(e) : KRIPKE_OK;
 }
 
@@ -1043,6 +1137,7 @@ int kripke_programs_destroy(kripke_programs_t *h) {
     if (!h) return KRIPKE_OK;
     cudaDeviceSynchronize();
     for (auto &kv : h->single) kv.second.release();
+    for (auto &kv : h->density) kv.second.release();
     for (kripke_programs::PairPlan *pp : h->pair_plans) { pp->plan.release(); cudaFree(pp->d_pairs); delete pp; }
     if (h->done) cudaEventDestroy(h->done);
     h->list_single.release(); h->list_pair.release();
@@ -1284,12 +1379,25 @@ int kripke_debug_jit_source(const uint8_t *code, const uint32_t *offsets, uint32
     for (uint32_t i = 0; pairs && i < 2 * n_pairs; ++i)
         if (pairs[i] >= h->n_formulas) return KRIPKE_EINVAL;
     std::vector<JitGroupHost> groups;
-    int rc = jit_group_records(h, pairs, pairs ? n_pairs : h->n_formulas, n_worlds, h->n_vars, frame_class, flags, &groups);
+    const uint32_t mode = (compile & 2) ? JIT_MODE_DENSITY : JIT_MODE_SCAN;
+    if (mode == JIT_MODE_DENSITY && pairs) return KRIPKE_EINVAL;
+    int rc = jit_group_records(h, pairs, pairs ? n_pairs : h->n_formulas, n_worlds, h->n_vars, frame_class, flags,
+                               mode, &groups);
     if (rc) return rc;
     const JitGroupHost &G = groups[group_vars];
     JitLayout lay;
-    if (!jit_layout(n_worlds, group_vars, frame_class, &lay)) return KRIPKE_EUNSUPPORTED;
-    const std::vector<std::vector<uint32_t>> parts = jit_partition(G.dag, G.roots, n_worlds, g_jit_max_programs);
+    if (!(mode == JIT_MODE_DENSITY ? jit_density_layout(n_worlds, group_vars, frame_class, &lay)
+                                   : jit_layout(n_worlds, group_vars, frame_class, &lay)))
+        return KRIPKE_EUNSUPPORTED;
+    std::vector<std::vector<uint32_t>> parts;
+    if (mode == JIT_MODE_DENSITY) {
+        for (uint32_t r = 0; r < G.roots.size(); ++r) {
+            if (r % 32 == 0) parts.emplace_back();
+            parts.back().push_back(r);
+        }
+    } else {
+        parts = jit_partition(G.dag, G.roots, n_worlds, g_jit_max_programs);
+    }
     if (n_kernels_out) *n_kernels_out = (uint32_t)parts.size();
     if (logic_ops_per_word_out) *logic_ops_per_word_out = 0;
     if (cubin_bytes_out) *cubin_bytes_out = 0;
@@ -1297,9 +1405,9 @@ int kripke_debug_jit_source(const uint8_t *code, const uint32_t *offsets, uint32
     std::vector<JitRoot> rs;
     for (uint32_t r : parts[kernel_index]) rs.push_back(G.roots[r]);
     JitEmitStats st;
-    const std::string src = jit_emit_kernel(G.dag, lay, rs, 128, g_jit_min_blocks, &st);
+    const std::string src = jit_emit_kernel(G.dag, lay, rs, 128, g_jit_min_blocks, mode, &st);
     if (logic_ops_per_word_out) *logic_ops_per_word_out = (uint64_t)(st.logic_ops_per_word + 0.5);
-    if (compile) {
+    if (compile & 1) {
         std::string log;
         size_t bytes = 0;
         if ((rc = jit_compile_only(src, &log, &bytes))) return rc;

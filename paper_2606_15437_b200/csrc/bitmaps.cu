@@ -146,8 +146,10 @@ struct DensityParams {
     uint64_t frame_begin, frame_count;
     const uint8_t *code;
     const uint32_t *offsets;
-    uint32_t n_formulas;
+    uint32_t n_formulas;              // formulas, or listed records
+    const uint32_t *records;          // null = formulas 0..n_formulas-1
     uint32_t *counts;
+    uint64_t row_stride, col_offset;  // counts[formula * row_stride + col_offset + j]
 };
 
 __global__ void __launch_bounds__(128) failure_density_kernel(DensityParams p) {
@@ -161,7 +163,8 @@ __global__ void __launch_bounds__(128) failure_density_kernel(DensityParams p) {
     } else {
         decode_rows(p.n, class_frame(p.n, p.cls, p.class_table, p.frame_begin + j), succ);
     }
-    for (uint32_t b = blockIdx.y; b < p.n_formulas; b += gridDim.y) {
+    for (uint32_t li = blockIdx.y; li < p.n_formulas; li += gridDim.y) {
+        const uint32_t b = p.records ? p.records[li] : li;
         const uint8_t *c = p.code + p.offsets[b];
         const uint32_t len = p.offsets[b + 1] - p.offsets[b];
         uint32_t cnt = 0;
@@ -170,7 +173,7 @@ __global__ void __launch_bounds__(128) failure_density_kernel(DensityParams p) {
             for (uint32_t i = 0; i < KRIPKE_MAX_VARS; ++i) val[i] = (uint32_t)(v >> (i * p.n)) & full;
             cnt += __popc(full & ~eval_postfix_scalar(c, len, p.n, succ, val, full));
         }
-        p.counts[(uint64_t)b * p.frame_count + j] = cnt;
+        p.counts[(uint64_t)b * p.row_stride + p.col_offset + j] = cnt;
     }
 }
 
@@ -296,18 +299,30 @@ int launch_frames_from_bitmap(uint32_t n, uint32_t cls, const uint64_t *class_ta
     return (int)cudaGetLastError();
 }
 
-int launch_failure_density(const ScanJob &job, const uint16_t *succ_list, uint32_t *counts_out, void *stream) {
-    if (job.frame_count == 0 || job.n_formulas == 0) return 0;
+static int launch_density(const ScanJob &job, const uint16_t *succ_list, const uint32_t *records, uint32_t n_list,
+                          uint32_t *counts_out, uint64_t row_stride, uint64_t col_offset, void *stream) {
+    if (job.frame_count == 0 || n_list == 0) return 0;
     DensityParams p;
     p.n = job.n; p.k = job.k; p.cls = job.cls; p.class_table = job.class_table; p.succ_list = succ_list;
     p.frame_begin = job.frame_begin; p.frame_count = job.frame_count;
-    p.code = job.code; p.offsets = job.offsets; p.n_formulas = job.n_formulas; p.counts = counts_out;
+    p.code = job.code; p.offsets = job.offsets; p.n_formulas = n_list; p.records = records; p.counts = counts_out;
+    p.row_stride = row_stride; p.col_offset = col_offset;
     const uint64_t bx = (job.frame_count + 127) / 128;
     if (bx > 0x7FFFFFFFull) return 801;
-    const uint32_t by = (uint32_t)std::min<uint64_t>(std::min<uint64_t>(job.n_formulas, 65535),
+    const uint32_t by = (uint32_t)std::min<uint64_t>(std::min<uint64_t>(n_list, 65535),
                                                      std::max<uint64_t>(1, (148ull * 32 + bx - 1) / bx));
     failure_density_kernel<<<dim3((uint32_t)bx, by), 128, 0, (cudaStream_t)stream>>>(p);
     return (int)cudaGetLastError();
+}
+
+int launch_failure_density(const ScanJob &job, const uint16_t *succ_list, uint32_t *counts_out, uint64_t row_stride,
+                           uint64_t col_offset, void *stream) {
+    return launch_density(job, succ_list, nullptr, job.n_formulas, counts_out, row_stride, col_offset, stream);
+}
+
+int launch_failure_density_records(const ScanJob &job, const uint32_t *records, uint32_t n_list, uint32_t *counts_out,
+                                   uint64_t row_stride, uint64_t col_offset, void *stream) {
+    return launch_density(job, nullptr, records, n_list, counts_out, row_stride, col_offset, stream);
 }
 
 int launch_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words, const uint32_t *library,

@@ -2,7 +2,7 @@
 // "source-level uint32 XOR/AND/OR" kernel, here redone as an executed-instruction rate).
 // Eight dependent chains per thread whose inputs rotate among the chains, so neither nvcc nor
 // ptxas can merge consecutive logic instructions into one LOP3 (a merged chain would overstate the
-// rate).  The SASS of the loop body is checked with cuobjdump (profiles/).
+// rate).  The SASS of the loop body (128 LOP3.LUT + the loop counter) is in profiles/r2_calibrate_sass.md.
 #include <cuda_runtime.h>
 
 #include "internal.h"

@@ -105,9 +105,16 @@ int launch_frames_from_bitmap(uint32_t n, uint32_t cls, const uint64_t *class_ta
                               const uint32_t *bitmap, uint16_t *succ_out, uint64_t capacity, uint64_t *count_out,
                               void *stream);
 // Failure densities: frames of job's class range, or of succ_list (job.frame_count masks rows) if not null.
-int launch_failure_density(const ScanJob &job, const uint16_t *succ_list, uint32_t *counts_out, void *stream);
+// counts_out[record * row_stride + col_offset + j] for frame j of the job's range (all formulas, or the listed records).
+int launch_failure_density(const ScanJob &job, const uint16_t *succ_list, uint32_t *counts_out, uint64_t row_stride,
+                           uint64_t col_offset, void *stream);
+int launch_failure_density_records(const ScanJob &job, const uint32_t *records, uint32_t n_list, uint32_t *counts_out,
+                                   uint64_t row_stride, uint64_t col_offset, void *stream);
 int launch_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words, const uint32_t *library,
                          uint32_t n_library, uint32_t *match_out, void *stream);
+
+// Frame-list generators (frame_gen.cu): n_frames x n successor masks written on the device.
+int launch_frames_generate(uint32_t gen, uint32_t n, uint64_t n_frames, uint64_t seed, uint16_t *succ_out, void *stream);
 
 // Semantic signatures: two 64-bit sums per formula over every model of 1..n_max worlds.
 int launch_signatures(uint32_t k, uint32_t n_max, const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,

@@ -88,9 +88,18 @@ struct JitEmitStats {
     uint32_t n_box = 0, n_and = 0;     // graph nodes evaluated per word (summed over kernels)
 };
 
+// Layout of the failure-density kernels: a thread owns whole frames (one frame and all its valuation words, or -
+// no variables - 32 frames per word), so that it can write the per-frame counts itself.
+bool jit_density_layout(uint32_t n, uint32_t g, uint32_t cls, JitLayout *out);
+
+enum : uint32_t {
+    JIT_MODE_SCAN = 0,      // per program: refuting models / frames, least refuting unit (Algorithm 1's outputs)
+    JIT_MODE_DENSITY = 1    // per (program, frame): the number of (valuation, world) pairs that fail
+};
+
 // CUDA C source of one kernel `kripke_jit_scan` that evaluates roots[0..) on the layout.
 std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vector<JitRoot> &roots,
-                            uint32_t threads, uint32_t min_blocks, JitEmitStats *stats);
+                            uint32_t threads, uint32_t min_blocks, uint32_t mode, JitEmitStats *stats);
 
 // Partition of the roots into kernels of at most `max_roots` that share as many subterms as possible.
 std::vector<std::vector<uint32_t>> jit_partition(const Dag &dag, const std::vector<JitRoot> &roots,
@@ -118,11 +127,17 @@ struct JitGroupPlan {
 // *log_out receives the NVRTC log on a compile error.
 int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitRoot> &roots,
                     const std::vector<uint32_t> &slot_record, uint32_t max_roots, uint32_t min_blocks,
-                    JitGroupPlan *out, std::string *log_out);
+                    uint32_t mode, JitGroupPlan *out, std::string *log_out);
+
+// Output of the density kernels: counts[record * total_frames + (class-order frame index - frame_base)].
+struct JitDensityOut {
+    uint32_t *counts;
+    uint64_t total_frames, frame_base;
+};
 
 // Enqueues the group's kernels over the aligned class range of `job` (job.k = the group's g).
-int jit_launch_group(const ScanJob &job, const JitGroupPlan &plan, uint32_t model_shift, void *stream,
-                     uint32_t *launches);
+int jit_launch_group(const ScanJob &job, const JitGroupPlan &plan, uint32_t model_shift, const JitDensityOut *density,
+                     void *stream, uint32_t *launches);
 
 // Compiles one source to a cubin without loading it (tests on a box without a GPU): 0 or error.
 int jit_compile_only(const std::string &source, std::string *log_out, size_t *cubin_bytes);

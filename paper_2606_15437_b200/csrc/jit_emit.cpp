@@ -93,6 +93,7 @@ struct Emitter {
         int root;
         std::string tail;       // text after the value (programs: the count updates)
         bool inlined = false;
+        bool keep = false;      // the value is read by literal text: never substitute it away
     };
     std::vector<Stmt> stmts;
     std::string body[3];
@@ -199,6 +200,7 @@ struct Emitter {
             if (!stmts[i].out.empty()) producer[stmts[i].out] = (int)i;
         std::vector<std::vector<int>> leaves(stmts.size());
         for (size_t i = 0; i < stmts.size(); ++i) {
+            if (stmts[i].root < 0) continue;
             collect_leaves(stmts[i].root, &leaves[i]);
             for (int lf : leaves[i]) ++uses[pool[lf].tok];
         }
@@ -207,7 +209,7 @@ struct Emitter {
                 auto it = producer.find(pool[lf].tok);
                 if (it == producer.end() || uses[pool[lf].tok] != 1) continue;
                 Stmt &p = stmts[it->second];
-                if (p.level != stmts[i].level || pool[p.root].op == Ex::CONST) continue;
+                if (p.keep || p.level != stmts[i].level || pool[p.root].op == Ex::CONST) continue;
                 const bool neg = pool[lf].neg;
                 pool[lf] = pool[p.root];                  // the producer's tree takes the operand's place
                 pool[lf].neg = pool[lf].neg != neg;
@@ -291,6 +293,7 @@ struct Emitter {
         for (const Stmt &st : stmts) {
             if (st.inlined) continue;
             std::string &out = body[st.level];
+            if (st.root < 0) { out += st.tail; continue; }              // literal text (counts, stores)
             const std::string name = st.out.empty() ? "r" : st.out;
             if (st.out.empty()) out += "      {\n";
             const Ex &e = pool[st.root];
@@ -322,6 +325,26 @@ bool jit_layout(uint32_t n, uint32_t g, uint32_t cls, JitLayout *out) {
         if (l.table || l.kn + fb < 5) return false;       // lanes would have to hold table frames / too few models
         l.outer = std::min(LOOP_BITS, l.kn + fb - 5);
         l.unit_frames_log2 = 5 - l.kn + l.outer;
+    }
+    if (out) *out = l;
+    return true;
+}
+
+bool jit_density_layout(uint32_t n, uint32_t g, uint32_t cls, JitLayout *out) {
+    if (n < 1 || n > KRIPKE_MAX_WORLDS || g > KRIPKE_MAX_VARS || cls > KRIPKE_CLASS_S5) return false;
+    JitLayout l;
+    l.n = n; l.g = g; l.cls = cls; l.kn = g * n;
+    l.table = cls == KRIPKE_CLASS_S4 || cls == KRIPKE_CLASS_S5;
+    const uint32_t fb = l.table ? 0u : (cls == KRIPKE_CLASS_T ? n * n - n : n * n);
+    if (l.kn >= 5) {
+        l.inner = l.kn - 5;                               // one thread = one frame: all its valuation words
+        if (l.inner > 12) return false;
+    } else if (l.kn == 0) {
+        if (l.table || fb < 5) return false;              // one frame per lane
+        l.outer = std::min(LOOP_BITS, fb - 5);
+        l.unit_frames_log2 = 5 + l.outer;
+    } else {
+        return false;                                     // a frame is a fraction of a word: scalar kernel
     }
     if (out) *out = l;
     return true;
@@ -392,8 +415,121 @@ std::vector<std::vector<uint32_t>> jit_partition(const Dag &dag, const std::vect
 // steps H2 / H3 without any memory traffic.  The loop body evaluates the group's graph in topological
 // order on named registers (step H4) and, per program, the refuted-lane word r, c += popc(r) (step H5).
 // After the loops kj_flush reduces per warp and block (step H6).
+// Failure-density kernel (D_ij = the fraction of valuation-world pairs on which formula i fails on frame j,
+// here as the integer count).  Same graph evaluation; per program the failing-world words g_w = ~T_w are either
+// popcounted into the thread's frame count (a thread owns one frame and all its valuation words) or - no
+// variables, one frame per lane - added up bit-sliced into three planes, from which the thread writes its 32
+// consecutive frames' counts with 16-byte stores.
+static std::string emit_density_kernel(const Dag &dag, const JitLayout &lay, const std::vector<JitRoot> &roots,
+                                       uint32_t threads, uint32_t min_blocks, JitEmitStats *stats) {
+    Emitter em(dag, lay);
+    const uint32_t n = lay.n, G = (uint32_t)roots.size();
+    const bool lanes_are_frames = lay.kn == 0;
+    for (uint32_t r = 0; r < G; ++r) {
+        em.node(roots[r].a >> 1);
+        std::vector<std::string> g(n);
+        for (uint32_t w = 0; w < n; ++w) {
+            g[w] = fmt("g%u_%u", r, w);
+            Emitter::Stmt st{em.lit_level(roots[r].a, w), g[w], em.negate(em.lit(roots[r].a, w)), ""};
+            st.keep = true;
+            em.stmts.push_back(st);
+        }
+        if (!lanes_are_frames) {
+            std::string t = fmt("      d%u += ", r);
+            for (uint32_t w = 0; w < n; ++w) t += (w ? " + " : "") + ("__popc(" + g[w] + ")");
+            em.stmts.push_back(Emitter::Stmt{2, "", -1, t + ";\n"});
+        } else {
+            // bit-sliced sum of the n failing-world words: planes[i] = bit i of the per-lane count
+            std::vector<std::vector<std::string>> col(4);
+            col[0] = g;
+            uint32_t tmp = 0;
+            std::string plane[3] = {"0u", "0u", "0u"};
+            for (uint32_t i = 0; i < 3; ++i) {
+                while (col[i].size() > 1) {
+                    const bool three = col[i].size() >= 3;
+                    const std::string a = col[i][0], b = col[i][1], c = three ? col[i][2] : "";
+                    col[i].erase(col[i].begin(), col[i].begin() + (three ? 3 : 2));
+                    const std::string sum = fmt("h%u_%u", r, tmp++), car = fmt("h%u_%u", r, tmp++);
+                    int xs = em.bin(Ex::XOR, em.leaf(a, false), em.leaf(b, false));
+                    int cy = em.bin(Ex::AND, em.leaf(a, false), em.leaf(b, false));
+                    if (three) {
+                        cy = em.bin(Ex::OR, cy, em.bin(Ex::AND, em.leaf(c, false), em.bin(Ex::XOR, em.leaf(a, false), em.leaf(b, false))));
+                        xs = em.bin(Ex::XOR, xs, em.leaf(c, false));
+                    }
+                    Emitter::Stmt s1{2, sum, xs, ""}, s2{2, car, cy, ""};
+                    s1.keep = s2.keep = true;
+                    em.stmts.push_back(s1);
+                    em.stmts.push_back(s2);
+                    col[i].push_back(sum);
+                    col[i + 1].push_back(car);
+                }
+                if (col[i].size() == 1) plane[i] = col[i][0];
+            }
+            std::string t = "      if (valid) {\n";
+            t += fmt("        unsigned *o = p.density + (unsigned long long)p.slot_record[%u] * p.total_frames + ((((unit << %u) + jo) << 5) - p.frame_base);\n", r, lay.outer);
+            for (uint32_t q = 0; q < 8; ++q) {
+                t += fmt("        *reinterpret_cast<uint4 *>(o + %u) = make_uint4(", 4 * q);
+                for (uint32_t i = 0; i < 4; ++i)
+                    t += (i ? ", " : "") + ("KJ_CNT3(" + plane[0] + ", " + plane[1] + ", " + plane[2] + fmt(", %u) << p.model_shift", 4 * q + i));
+                t += ");\n";
+            }
+            t += "      }\n";
+            em.stmts.push_back(Emitter::Stmt{2, "", -1, t});
+        }
+    }
+    em.emit_all();
+
+    std::string s = kPrelude;
+    s += fmt("\n// density layout: n=%u g=%u cls=%u inner=%u outer=%u unit_frames_log2=%u programs=%u\n", n, lay.g, lay.cls,
+             lay.inner, lay.outer, lay.unit_frames_log2, G);
+    s += fmt("extern \"C\" __global__ void __launch_bounds__(%u, %u) kripke_jit_scan(const KjParams p) {\n", threads, min_blocks);
+    s += "  const unsigned lane = threadIdx.x & 31u;\n";
+    s += "  for (unsigned item = blockIdx.x; item < p.n_items; item += gridDim.x) {\n";
+    s += "    const unsigned long long u0 = p.unit_begin + (unsigned long long)item * p.units_per_item;\n";
+    s += "    const unsigned long long rem = p.unit_begin + p.unit_count - u0;\n";
+    s += "    const unsigned item_units = rem < p.units_per_item ? (unsigned)rem : p.units_per_item;\n";
+    s += fmt("    for (unsigned t0 = 0; t0 < item_units; t0 += %uu) {\n", threads);
+    s += "      const unsigned rel = t0 + threadIdx.x;\n";
+    s += "      const bool valid = rel < item_units;\n";
+    s += "      const unsigned long long unit = u0 + (valid ? rel : 0u);\n";
+    s += "      (void)lane;\n";
+    for (uint32_t b : em.bits.used_unit) s += fmt("      const unsigned mu%u = 0u - (unsigned)((unit >> %u) & 1ull);\n", b, b);
+    if (lay.table) {
+        s += "      const unsigned long long frame = p.class_table[unit];\n";
+        for (uint32_t e : em.used_table) s += fmt("      const unsigned me%u = 0u - (unsigned)((frame >> %u) & 1ull);\n", e, e);
+    }
+    s += em.body[0];
+    if (!lanes_are_frames) for (uint32_t r = 0; r < G; ++r) s += fmt("      unsigned d%u = 0u;\n", r);
+    s += "#pragma unroll 1\n";
+    s += fmt("      for (unsigned jo = 0; jo < %uu; ++jo) {\n", 1u << lay.outer);
+    for (uint32_t b : em.bits.used_outer) s += fmt("      const unsigned mo%u = 0u - ((jo >> %u) & 1u);\n", b, b);
+    s += em.body[1];
+    s += "#pragma unroll 1\n";
+    s += fmt("      for (unsigned ji = 0; ji < %uu; ++ji) {\n", 1u << lay.inner);
+    for (uint32_t b : em.bits.used_inner) s += fmt("      const unsigned mi%u = 0u - ((ji >> %u) & 1u);\n", b, b);
+    s += em.body[2];
+    s += "      }\n      }\n";
+    if (!lanes_are_frames) {
+        s += "      if (valid) {\n";
+        for (uint32_t r = 0; r < G; ++r)
+            s += fmt("        p.density[(unsigned long long)p.slot_record[%u] * p.total_frames + (unit - p.frame_base)] = d%u << p.model_shift;\n", r, r);
+        s += "      }\n";
+    }
+    s += "    }\n  }\n}\n";
+    if (stats) {
+        const uint64_t *ops = em.ops;
+        stats->logic_ops_emitted = ops[0] + ops[1] + ops[2];
+        stats->logic_ops_per_word = (double)ops[2] + (double)ops[1] / (double)(1u << lay.inner) +
+                                    (double)ops[0] / (double)(1u << (lay.inner + lay.outer));
+        stats->n_box = em.n_box;
+        stats->n_and = em.n_and;
+    }
+    return s;
+}
+
 std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vector<JitRoot> &roots,
-                            uint32_t threads, uint32_t min_blocks, JitEmitStats *stats) {
+                            uint32_t threads, uint32_t min_blocks, uint32_t mode, JitEmitStats *stats) {
+    if (mode == JIT_MODE_DENSITY) return emit_density_kernel(dag, lay, roots, threads, min_blocks, stats);
     Emitter em(dag, lay);
     const uint32_t n = lay.n, G = (uint32_t)roots.size();
     // how refuted FRAMES are counted

@@ -24,6 +24,8 @@ struct KjParamsHost {
     Accum *accum;
     unsigned units_per_item, n_items;
     unsigned model_shift, pad;
+    unsigned *density;
+    unsigned long long total_frames, frame_base;
 };
 
 struct Module {
@@ -76,20 +78,29 @@ int jit_compile_only(const std::string &source, std::string *log_out, size_t *cu
 
 int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitRoot> &roots,
                     const std::vector<uint32_t> &slot_record, uint32_t max_roots, uint32_t min_blocks,
-                    JitGroupPlan *out, std::string *log_out) {
+                    uint32_t mode, JitGroupPlan *out, std::string *log_out) {
     out->release();
     out->lay = lay;
     out->stats = JitEmitStats();
     out->threads = 128;
     if (roots.empty()) return 0;
-    const std::vector<std::vector<uint32_t>> parts = jit_partition(dag, roots, lay.n, max_roots);
+    std::vector<std::vector<uint32_t>> parts;
+    if (mode == JIT_MODE_DENSITY) {
+        // every record writes its own row: records in order, max_roots per kernel (the graph is still shared)
+        for (uint32_t r = 0; r < roots.size(); ++r) {
+            if (r % max_roots == 0) parts.emplace_back();
+            parts.back().push_back(r);
+        }
+    } else {
+        parts = jit_partition(dag, roots, lay.n, max_roots);
+    }
     std::vector<std::string> sources(parts.size());
     std::vector<uint32_t> order;               // slot -> index into roots
     for (size_t i = 0; i < parts.size(); ++i) {
         std::vector<JitRoot> rs;
         for (uint32_t r : parts[i]) { rs.push_back(roots[r]); order.push_back(r); }
         JitEmitStats st;
-        sources[i] = jit_emit_kernel(dag, lay, rs, out->threads, min_blocks, &st);
+        sources[i] = jit_emit_kernel(dag, lay, rs, out->threads, min_blocks, mode, &st);
         out->stats.logic_ops_per_word += st.logic_ops_per_word;
         out->stats.logic_ops_emitted += st.logic_ops_emitted;
         out->stats.n_box += st.n_box;
@@ -156,8 +167,8 @@ int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitR
     return 0;
 }
 
-int jit_launch_group(const ScanJob &job, const JitGroupPlan &plan, uint32_t model_shift, void *stream,
-                     uint32_t *launches) {
+int jit_launch_group(const ScanJob &job, const JitGroupPlan &plan, uint32_t model_shift, const JitDensityOut *density,
+                     void *stream, uint32_t *launches) {
     const JitLayout &lay = plan.lay;
     if (job.frame_count == 0 || plan.kernels.empty()) return 0;
     int dev = 0, sm_count = 0;
@@ -172,6 +183,9 @@ int jit_launch_group(const ScanJob &job, const JitGroupPlan &plan, uint32_t mode
     p.accum = job.accum;
     p.model_shift = model_shift;
     p.pad = 0;
+    p.density = density ? density->counts : nullptr;
+    p.total_frames = density ? density->total_frames : 0;
+    p.frame_base = density ? density->frame_base : 0;
     if (p.unit_count == 0) return 0;
     const uint32_t threads = plan.threads;
     const uint64_t tiles = (p.unit_count + threads - 1) / threads;

@@ -259,12 +259,13 @@ __global__ void __launch_bounds__(FR_TPB) scan_frames_kernel(FramesParams p) {
 // Host launcher for one instantiation.
 template <int N, int VB>
 int launch_frames_inst(const FramesJob &job, const SlicedPlan &plan, void *stream, uint32_t *launches) {
-    static int sm_count = 0, blocks_per_sm[FR_SPILL + 1] = {0, 0, 0, 0};
+    // queried for the current device on every call (nothing cached per process: multi-device / multi-thread safe)
+    int sm_count = 0, blocks_per_sm[FR_SPILL + 1] = {0, 0, 0, 0};
     auto kern = scan_frames_kernel<N, VB>;
     const uint32_t spill_slots = std::min<uint32_t>(FR_SPILL, plan.max_need > 0 ? plan.max_need - 1 : 0);
     const size_t fixed = ((size_t)N * N * 32 + 36 + (size_t)spill_slots * N * VB * FR_TPB) * sizeof(uint32_t);
     const size_t slot_budget = 8 * 1024;
-    if (!sm_count) {
+    {
         int dev = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return (int)e;
@@ -274,7 +275,7 @@ int launch_frames_inst(const FramesJob &job, const SlicedPlan &plan, void *strea
         e = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
         if (e != cudaSuccess) return (int)e;
     }
-    if (!blocks_per_sm[spill_slots]) {
+    {
         int b = 0;
         cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, kern, FR_TPB, fixed + slot_budget);
         if (e != cudaSuccess) return (int)e;

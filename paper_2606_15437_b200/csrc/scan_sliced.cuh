@@ -565,13 +565,15 @@ __global__ void __launch_bounds__(TPB, MINB) scan_sliced_kernel(SlicedParams p) 
 // Host launcher for one instantiation.
 template <class C, int TPB, int MINB>
 int launch_sliced_inst(const ScanJob &job, const SlicedPlan &plan, void *stream, uint32_t *launches) {
-    static int blocks_per_sm = 0, sm_count = 0;
+    // queried for the current device on every call (host-side, microseconds): nothing is cached per process,
+    // so several devices and several host threads can use the library
+    int blocks_per_sm = 0, sm_count = 0;
     constexpr int SLICED_THREADS = TPB;
     auto kern = scan_sliced_kernel<C, TPB, MINB>;
     const size_t per_slot = 16 + 2 * (size_t)plan.stride;
     const size_t leaf_bytes = (size_t)C::LEAF_WORDS * TPB * sizeof(uint32_t);
     const size_t slot_budget = 32 * 1024;
-    if (!blocks_per_sm) {
+    {
         int dev = 0;
         cudaError_t e = cudaGetDevice(&dev);
         if (e != cudaSuccess) return (int)e;

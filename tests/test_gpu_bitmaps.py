@@ -194,3 +194,34 @@ def test_failure_density_panels_equal_the_oracle(kb, vol):
     # zero density <=> valid frame (the validity bitmap of the same range)
     val = kb.bits_to_bool(kb.validity_bitmap(h, 4, 2, S4, 3, 300), 300)
     assert ((got == 0) == val).all()
+
+
+def test_compiled_failure_density_equals_the_oracle(kb, vol):
+    """kripke_failure_density over class ranges runs on the compiled bit-sliced kernels (a thread owns one
+    frame and all its valuation words; without variables one frame per lane and the counts leave as three bit
+    planes): every layout kind, every class, ragged ranges whose ends fall to the scalar kernel - bit-exact
+    against the oracle's per-frame counts of failing (valuation, world) pairs."""
+    k0 = W.pairs_c5(70)[0]
+    k1 = [c for c in W.corpus_c4(600) if b"\x11" not in c and b"\x12" not in c][:50]
+    k2 = W.corpus_c2(5624)[::47] + [AX[a] for a, _ in PAIRS]
+    k3 = W.corpus_c4(60)
+    cases = [(k2, 2, 3, K, 0, 512), (k2, 2, 4, K, 1000, 2048), (k2, 2, 5, K, (1 << 22) + 8, 4096),
+             (k2, 2, 5, T, 77 * 4, 2048), (k2, 2, 5, S4, 0, 6940), (k2, 2, 4, S5, 0, 12), (k2, 2, 2, K, 0, 16),
+             (k1, 1, 5, K, 4096, 8192), (k1, 1, 5, T, 0, 4096), (k1, 1, 6, K, 1 << 30, 1024), (k1, 1, 4, K, 0, 4096),
+             (k0, 0, 5, K, 1024 * 3 + 4, 1024 * 5 + 8), (k0, 0, 4, K, 0, 1 << 16), (k0, 0, 5, T, 2048, 4096),
+             (k0, 0, 6, K, (1 << 33) + 1024, 8192), (k0, 0, 3, K, 0, 512), (k0, 0, 5, S4, 0, 6940),
+             (k3, 3, 4, K, 64, 256), (k3, 3, 5, K, 1 << 24, 16)]
+    for progs, k, n, cls, begin, count in cases:
+        code, offs = W.pack_programs(progs)
+        h = kb.Programs(code, offs, k)
+        got = kb.failure_density(h, n, k, cls, begin, count).cpu().numpy().view(np.uint32)
+        want = vol.failure_counts(code, offs, n, k, cls, begin, count)
+        assert got.shape == want.shape and (got == want).all(), (k, n, cls, begin, count)
+        info = h.last_run_info()
+        if k * n >= 5 or (k == 0 and cls in (K, T) and n >= 3 and count >= 1024):
+            assert info.kernel_family == 2, (k, n, cls)
+    # an unaligned output row (count % 4 != 0) takes the scalar kernel and gives the same numbers
+    code, offs = W.pack_programs(k2)
+    h = kb.Programs(code, offs, 2)
+    got = kb.failure_density(h, 4, 2, K, 5, 1001).cpu().numpy().view(np.uint32)
+    assert (got == vol.failure_counts(code, offs, 4, 2, K, 5, 1001)).all() and h.last_run_info().kernel_family == 0

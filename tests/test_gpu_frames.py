@@ -131,3 +131,30 @@ def test_frame_list_edges_and_errors(kb):
     with pytest.raises(kb.KripkeError) as e:
         kb.eval_frames(h, 6, 2, torch.zeros(12, dtype=torch.int16, device="cuda"))   # n_vars differs from the handle's
     assert e.value.status == kb.EINVAL
+
+
+def test_in_library_generators_equal_the_numpy_restatement(kb, vol):
+    """kripke_frames_generate (templates and seeded relations written on the device) against the
+    counter-based generators of workloads/frames.py, mask by mask, for every generator and sizes 1..16; then a
+    scan of a device-generated stress list against the oracle fed from the numpy side."""
+    import torch
+    for n in (1, 2, 3, 6, 9, 16):
+        for gen in range(5):
+            got = kb.frames_generate(gen, n, 777, 4242).cpu().numpy().view(np.uint16).reshape(777, n)
+            want = F.succ_masks(F.generate_cb(gen, n, 777, 4242))
+            assert (got == want).all(), (n, gen)
+        for count in (3, 10, 11, 2050):
+            got = kb.frames_generate(kb.GEN_STRESS, n, count, 99).cpu().numpy().view(np.uint16).reshape(count, n)
+            assert (got == F.succ_masks(F.stress_list_cb(n, count, 99))).all(), (n, count)
+    # the named templates are the paper's (P:183-185): the six-world path is Proposition 5's frame (2,4,8,16,32,0)
+    t = kb.frames_generate(kb.GEN_TEMPLATES, 6, 10, 0).cpu().numpy().view(np.uint16).reshape(10, 6)
+    assert t[0].tolist() == [2, 4, 8, 16, 32, 0]
+    progs = [W.to_postfix(W.parse(s)) for s in ("[]p -> p", "[]p -> [][]p", "<>[]p -> []<>p", "[]<>[]<>T", "<>T")]
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 1)
+    n, count = 8, 5000
+    succ = kb.frames_generate(kb.GEN_STRESS, n, count, 15437006)
+    got = kb.unpack(*kb.eval_frames(h, n, 1, succ))
+    want = vol.census_relations(code, offs, n, 1, F.stress_list_cb(n, count, 15437006))
+    for key in ("models", "frames", "wit_f", "wit_v", "wit_w"):
+        assert (got[key].astype(np.uint64) == want[key].astype(np.uint64)).all(), key

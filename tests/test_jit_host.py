@@ -92,3 +92,21 @@ def test_no_layout_for_tiny_shapes():
     code, offs = W.pack_programs(W.pairs_c5(10)[0])
     assert kb.debug_jit_source(code, offs, 0, 2, K, 0) is None          # 16 models: less than one word
     assert kb.debug_jit_source(code, offs, 0, 5, S4, 0) is None         # table class needs the lanes for valuations
+
+
+@pytest.mark.parametrize("n,k,cls", [(5, 2, K), (5, 2, T), (5, 2, S4), (3, 2, K), (5, 0, K), (6, 0, K), (4, 0, T),
+                                     (5, 1, K), (4, 3, K)])
+def test_density_kernels_compile_for_sm100a(n, k, cls):
+    """The failure-density kernels (one frame per thread; one frame per lane with bit-plane counts) compile."""
+    progs = {0: W.pairs_c5(40)[0], 1: [c for c in W.corpus_c4(400) if b"\x11" not in c and b"\x12" not in c][:30],
+             2: W.corpus_c2(80), 3: W.corpus_c4(40)}[k]
+    code, offs = W.pack_programs(progs)
+    seen = 0
+    for g in range(k + 1):
+        r = kb.debug_jit_source(code, offs, k, n, cls, g, 0, compile=True, density=True)
+        if r is None or r[1] == 0:
+            continue
+        seen += 1
+        assert r[3] > 0 and "density layout" in r[0]
+        assert ("KJ_CNT3" in r[0].split("density layout")[1]) == (g == 0)
+    assert seen >= 1

@@ -161,3 +161,71 @@ def succ_masks(rel):
     F, n, _ = rel.shape
     weights = (1 << np.arange(n, dtype=np.uint32)).astype(np.uint32)
     return (rel.astype(np.uint32) * weights[None, None, :]).sum(axis=2).astype(np.uint16)
+
+
+# ---- counter-based generators: the numpy side of kripke_frames_generate (include/kripke.h) ----------------
+# Frame j of a list depends only on (generator, n, seed, j): every draw is the SplitMix64 finaliser of a key.
+# The library writes the same lists on the device (csrc/frame_gen.cu); tests compare the two element by
+# element and feed the oracle from THIS side.  Input generation only: no formula is evaluated here.
+GEN_TEMPLATES, GEN_ERDOS_RENYI, GEN_EDGE_FLIP, GEN_DEAD_END, GEN_BACK_EDGE, GEN_STRESS = range(6)
+_DENSITY = np.array([214748364, 429496729, 858993459, 1503238553, 2147483648, 3435973836], np.uint64)  # x 2^-32
+_DENSITY03 = np.uint64(1288490188)
+_M = np.uint64
+
+
+def _mix(x):
+    with np.errstate(over="ignore"):
+        x = (x + _M(0x9E3779B97F4A7C15)).astype(np.uint64)
+        x = (x ^ (x >> _M(30))) * _M(0xBF58476D1CE4E5B9)
+        x = (x ^ (x >> _M(27))) * _M(0x94D049BB133111EB)
+        return x ^ (x >> _M(31))
+
+
+def _draw(seed, gen, n, j, t):
+    """draw t of frame j (arrays broadcast)."""
+    with np.errstate(over="ignore"):
+        key = _mix(np.array(seed ^ (gen << 56) ^ (n << 48), np.uint64))
+        return _mix(key + np.asarray(j, np.uint64) * _M(0xD6E8FEB86659FD93) + np.asarray(t, np.uint64) * _M(0x2545F4914F6CDD1D))
+
+
+def generate_cb(gen, n, count, seed=SEED_FRAMES):
+    """rel[count, n, n] of one counter-based generator (not GEN_STRESS)."""
+    j = np.arange(count, dtype=np.uint64)
+    names, base = templates(n)
+    if gen == GEN_TEMPLATES:
+        return base[(j % _M(len(base))).astype(np.int64)].copy()
+    if gen in (GEN_ERDOS_RENYI, GEN_DEAD_END):
+        t = np.arange(n * n, dtype=np.uint64)
+        d = _draw(seed, gen, n, j[:, None], t[None, :]) >> _M(32)
+        thr = _DENSITY[(j % _M(6)).astype(np.int64)][:, None] if gen == GEN_ERDOS_RENYI else _DENSITY03
+        rel = (d < thr).astype(np.uint8).reshape(count, n, n)
+        if gen == GEN_DEAD_END:
+            dead = (_draw(seed, gen, n, j, 1000) % _M(n)).astype(np.int64)
+            rel[np.arange(count), dead, :] = 0
+        return rel
+    if gen == GEN_EDGE_FLIP:
+        rel = base[(j % _M(len(base))).astype(np.int64)].copy()
+        flips = 1 + (_draw(seed, gen, n, j, 100) % _M(4)).astype(np.int64)
+        flat = rel.reshape(count, n * n)
+        for t in range(4):
+            idx = np.nonzero(flips > t)[0]
+            pos = (_draw(seed, gen, n, j[idx], t) % _M(n * n)).astype(np.int64)
+            flat[idx, pos] ^= 1
+        return rel
+    if gen == GEN_BACK_EDGE:
+        rel = np.repeat(path(n)[None], count, axis=0)
+        for t in range(2):
+            w = (_draw(seed, gen, n, j, 2 * t) % _M(n)).astype(np.int64)
+            u = (_draw(seed, gen, n, j, 2 * t + 1) % (w + 1).astype(np.uint64)).astype(np.int64)
+            rel[np.arange(count), w, u] = 1
+        return rel
+    raise ValueError(gen)
+
+
+def stress_list_cb(n, count, seed=SEED_FRAMES):
+    """The mixed list KRIPKE_GEN_STRESS writes: the templates, then the four generators in equal shares."""
+    nt = min(count, len(TEMPLATES))
+    rest = count - nt
+    q = [rest // 4 + (1 if i < rest % 4 else 0) for i in range(4)]
+    parts = [generate_cb(GEN_TEMPLATES, n, nt, seed)] + [generate_cb(GEN_ERDOS_RENYI + i, n, q[i], seed) for i in range(4)]
+    return np.concatenate([p for p in parts if len(p)], axis=0)
