@@ -939,7 +939,7 @@ int kripke_failure_density(const kripke_programs_t *programs, uint32_t n_worlds,
     // written with 16-byte stores; the scalar kernel (thread = frame, one model per iteration) otherwise and on
     // the ragged ends of the range.
     bool compiled = jit_density_layout(n_worlds, n_vars, frame_class, nullptr) && frame_count % 4 == 0 &&
-                    (reinterpret_cast<uintptr_t>(counts_out) & 15u) == 0;
+                    frame_begin % 4 == 0 && (reinterpret_cast<uintptr_t>(counts_out) & 15u) == 0;
     const ScanPlan *plan = nullptr;
     if (compiled) {
         const uint64_t key = plan_key(n_worlds, n_vars, frame_class, 0, ENGINE_JIT, 0);

@@ -71,6 +71,8 @@ struct JitLayout {
     uint32_t kn = 0;               // g * n
     uint32_t inner = 0, outer = 0, split = 0;
     uint32_t unit_frames_log2 = 0; // frames per unit = 2^this (0 when a unit is one frame or part of it)
+    uint32_t lane_bits = 0;        // density kernels, one frame per lane: bits 5.. of X taken from the thread's lane
+                                   // (= the low bits of its unit index), so that a warp's words are consecutive
     bool table = false;            // frames come from the class table (S4 / S5)
 };
 // Is there a compiled layout for (n, g, class)?  Fills *out.

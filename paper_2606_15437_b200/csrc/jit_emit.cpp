@@ -49,6 +49,8 @@ struct BitSource {
         pos -= 5;
         if (pos < lay.inner) return 2;
         pos -= lay.inner;
+        if (pos < lay.lane_bits) return 0;
+        pos -= lay.lane_bits;
         return pos < lay.outer ? 1 : 0;
     }
     std::string word(uint32_t pos) {
@@ -56,10 +58,12 @@ struct BitSource {
         pos -= 5;
         if (pos < lay.inner) { used_inner.insert(pos); return fmt("mi%u", pos); }
         pos -= lay.inner;
+        if (pos < lay.lane_bits) { used_unit.insert(pos); return fmt("mu%u", pos); }      // low unit bits = the lane
+        pos -= lay.lane_bits;
         if (pos < lay.outer) { used_outer.insert(pos); return fmt("mo%u", pos); }
         pos -= lay.outer;
-        used_unit.insert(pos);
-        return fmt("mu%u", pos);
+        used_unit.insert(pos + lay.lane_bits);
+        return fmt("mu%u", pos + lay.lane_bits);
     }
 };
 
@@ -341,8 +345,10 @@ bool jit_density_layout(uint32_t n, uint32_t g, uint32_t cls, JitLayout *out) {
         if (l.inner > 12) return false;
     } else if (l.kn == 0) {
         if (l.table || fb < 5) return false;              // one frame per lane
-        l.outer = std::min(LOOP_BITS, fb - 5);
-        l.unit_frames_log2 = 5 + l.outer;
+        // a warp's 32 words are consecutive (1,024 frames = 4 KB of one output row): coalesced stores
+        if (fb >= 10) { l.lane_bits = 5; l.split = 5; }
+        l.outer = std::min(LOOP_BITS, fb - 5 - l.lane_bits);
+        l.unit_frames_log2 = 5 + l.outer + l.lane_bits;   // of the split threads together
     } else {
         return false;                                     // a frame is a fraction of a word: scalar kernel
     }
@@ -465,15 +471,48 @@ static std::string emit_density_kernel(const Dag &dag, const JitLayout &lay, con
                 }
                 if (col[i].size() == 1) plane[i] = col[i][0];
             }
-            std::string t = "      if (valid) {\n";
-            t += fmt("        unsigned *o = p.density + (unsigned long long)p.slot_record[%u] * p.total_frames + ((((unit << %u) + jo) << 5) - p.frame_base);\n", r, lay.outer);
-            for (uint32_t q = 0; q < 8; ++q) {
-                t += fmt("        *reinterpret_cast<uint4 *>(o + %u) = make_uint4(", 4 * q);
-                for (uint32_t i = 0; i < 4; ++i)
-                    t += (i ? ", " : "") + ("KJ_CNT3(" + plane[0] + ", " + plane[1] + ", " + plane[2] + fmt(", %u) << p.model_shift", 4 * q + i));
-                t += ");\n";
+            std::string t;
+            if (lay.lane_bits == 5) {
+                // The count of frame l as a 4-bit field at bit l (mod 32) of word z[l % 4]: plane 0 where it is,
+                // planes 1 and 2 rotated up by one and two.  The thread's 32 counts go to the warp's staging
+                // rows (16-byte chunks, XOR-swizzled: conflict-free both ways), and come back transposed so
+                // that every store instruction of the warp writes 512 consecutive bytes of the output row.
+                t += "      {\n";
+                t += "        const unsigned q1 = __funnelshift_l(" + plane[1] + ", " + plane[1] + ", 1), q2 = __funnelshift_l(" +
+                     plane[2] + ", " + plane[2] + ", 2);\n";
+                for (uint32_t m = 0; m < 4; ++m) {
+                    const uint32_t a0 = 0x11111111u << m, a1 = (a0 << 1) | (a0 >> 31), a2 = (a0 << 2) | (a0 >> 30);
+                    t += fmt("        const unsigned z%u = (", m) + plane[0] + fmt(" & 0x%08xu) | (q1 & 0x%08xu) | (q2 & 0x%08xu);\n", a0, a1, a2);
+                }
+                t += "        __syncwarp();\n";
+                for (uint32_t c = 0; c < 8; ++c) {
+                    t += fmt("        st_w[%uu ^ sw] = make_uint4(", c);
+                    for (uint32_t i = 0; i < 4; ++i) {
+                        const uint32_t l = 4 * c + i;
+                        t += (i ? ", " : "") + (l ? fmt("__funnelshift_r(z%u, z%u, %u) & 7u", l % 4, l % 4, l) : std::string("z0 & 7u"));
+                    }
+                    t += ");\n";
+                }
+                t += "        __syncwarp();\n";
+                t += "        if (valid) {\n";
+                t += fmt("          uint4 *o = reinterpret_cast<uint4 *>(p.density + (unsigned long long)p.slot_record[%u] * p.total_frames + "
+                         "(((((unit >> 5) << %u) + jo) << 10) - p.frame_base)) + lane;\n", r, lay.outer);
+                for (uint32_t q = 0; q < 8; ++q) {
+                    t += fmt("          { uint4 v = ld_w[%uu ^ lw%u]; v.x <<= p.model_shift; v.y <<= p.model_shift; v.z <<= p.model_shift; "
+                             "v.w <<= p.model_shift; __stcs(o + %u, v); }\n", 32 * q, q & 1u, 32 * q);
+                }
+                t += "        }\n      }\n";
+            } else {
+                t += "      if (valid) {\n";
+                t += fmt("        unsigned *o = p.density + (unsigned long long)p.slot_record[%u] * p.total_frames + ((((unit << %u) + jo) << 5) - p.frame_base);\n", r, lay.outer);
+                for (uint32_t q = 0; q < 8; ++q) {
+                    t += fmt("        *reinterpret_cast<uint4 *>(o + %u) = make_uint4(", 4 * q);
+                    for (uint32_t i = 0; i < 4; ++i)
+                        t += (i ? ", " : "") + ("KJ_CNT3(" + plane[0] + ", " + plane[1] + ", " + plane[2] + fmt(", %u) << p.model_shift", 4 * q + i));
+                    t += ");\n";
+                }
+                t += "      }\n";
             }
-            t += "      }\n";
             em.stmts.push_back(Emitter::Stmt{2, "", -1, t});
         }
     }
@@ -484,6 +523,15 @@ static std::string emit_density_kernel(const Dag &dag, const JitLayout &lay, con
              lay.inner, lay.outer, lay.unit_frames_log2, G);
     s += fmt("extern \"C\" __global__ void __launch_bounds__(%u, %u) kripke_jit_scan(const KjParams p) {\n", threads, min_blocks);
     s += "  const unsigned lane = threadIdx.x & 31u;\n";
+    if (lay.lane_bits == 5) {
+        // staging rows of the warp: thread t owns chunks 8t..8t+7 (its 32 counts); store step q reads chunk (lane & 7) of
+        // row 4q + (lane >> 3).  Chunk c of row t lives at 8t + (c ^ (t & 7)).
+        s += fmt("  __shared__ uint4 s_stage[%u];\n", threads * 8);
+        s += "  uint4 *const st_w = s_stage + (threadIdx.x & ~31u) * 8u + lane * 8u;\n";
+        s += "  const unsigned sw = lane & 7u;\n";
+        s += "  const uint4 *const ld_w = s_stage + (threadIdx.x & ~31u) * 8u + (lane >> 3) * 8u;\n";
+        s += "  const unsigned lw0 = (lane & 7u) ^ (lane >> 3), lw1 = (lane & 7u) ^ (4u + (lane >> 3));\n";
+    }
     s += "  for (unsigned item = blockIdx.x; item < p.n_items; item += gridDim.x) {\n";
     s += "    const unsigned long long u0 = p.unit_begin + (unsigned long long)item * p.units_per_item;\n";
     s += "    const unsigned long long rem = p.unit_begin + p.unit_count - u0;\n";

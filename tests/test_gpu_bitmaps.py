@@ -210,7 +210,12 @@ def test_compiled_failure_density_equals_the_oracle(kb, vol):
              (k1, 1, 5, K, 4096, 8192), (k1, 1, 5, T, 0, 4096), (k1, 1, 6, K, 1 << 30, 1024), (k1, 1, 4, K, 0, 4096),
              (k0, 0, 5, K, 1024 * 3 + 4, 1024 * 5 + 8), (k0, 0, 4, K, 0, 1 << 16), (k0, 0, 5, T, 2048, 4096),
              (k0, 0, 6, K, (1 << 33) + 1024, 8192), (k0, 0, 3, K, 0, 512), (k0, 0, 5, S4, 0, 6940),
-             (k3, 3, 4, K, 64, 256), (k3, 3, 5, K, 1 << 24, 16)]
+             (k3, 3, 4, K, 64, 256), (k3, 3, 5, K, 1 << 24, 16),
+             # one frame per lane with a warp's words consecutive (units of 2^15 frames, rows staged through shared
+             # memory and written 512 bytes per warp instruction): aligned units between two ragged ends; the same
+             # programs in a one-variable batch (every count x 2^n)
+             (k0, 0, 5, K, 3 * 32768 - 4000, 2 * 32768 + 8000), (k0, 0, 5, T, 32768 - 8, 2 * 32768 + 16),
+             (k0, 0, 6, K, (1 << 35) - 32768, 3 * 32768), (k0[:20] + k1[:20], 1, 5, K, 5 * 32768 - 12, 32768 + 24)]
     for progs, k, n, cls, begin, count in cases:
         code, offs = W.pack_programs(progs)
         h = kb.Programs(code, offs, k)
@@ -225,3 +230,8 @@ def test_compiled_failure_density_equals_the_oracle(kb, vol):
     h = kb.Programs(code, offs, 2)
     got = kb.failure_density(h, 4, 2, K, 5, 1001).cpu().numpy().view(np.uint32)
     assert (got == vol.failure_counts(code, offs, 4, 2, K, 5, 1001)).all() and h.last_run_info().kernel_family == 0
+    # so does a range whose first frame is not a multiple of four (the rows' 16-byte chunks would be misaligned)
+    code, offs = W.pack_programs(k0)
+    h = kb.Programs(code, offs, 0)
+    got = kb.failure_density(h, 5, 0, K, 32768 + 2, 32768).cpu().numpy().view(np.uint32)
+    assert (got == vol.failure_counts(code, offs, 5, 0, K, 32768 + 2, 32768)).all() and h.last_run_info().kernel_family == 0
