@@ -509,6 +509,7 @@ def run_c4(args):
             seen.add(c); one.append(c)
     adv1 = [W.to_postfix(("and", ("bot",), W.from_postfix(c))) for c in one]
     out["contention_one_variable"] = {}
+    count = 1 << 20
     for name, batch in (("mixed", one), ("adversarial", adv1)):
         h = kb.Programs(*W.pack_programs(batch), 1)
         c = torch.zeros((NB, 2), dtype=torch.int64, device="cuda")
@@ -690,15 +691,17 @@ def run_atlas(args):
             kb.failure_density(h, n, N_VARS, 0, begin, cnt, o)
             logic[0] += h.last_run_info().logic_instr_per_frame * cnt
 
-    t0 = time.perf_counter(); run_panels(); torch.cuda.synchronize(); t_build = time.perf_counter() - t0
-    t_panels = timed(run_panels)
-    entries = B * sum(cnt for _, _, cnt in panels)
-    evals = B * sum(cnt << (N_VARS * n) for n, _, cnt in panels)
-    leg1 = {"formulas": B, "frames": sum(cnt for _, _, cnt in panels), "entries": entries, "seconds": t_panels,
-            "entries_per_s": entries / t_panels, "evaluations_per_s": evals / t_panels,
-            "bytes_written": 4 * entries, "write_GB_per_s": 4 * entries / t_panels / 1e9,
-            "logic_instr_per_s": logic[0] / t_panels, "frac_of_alu_peak": logic[0] / t_panels / alu_peak,
-            "plan_build_seconds": t_build, "bound": "alu"}
+    leg1 = None
+    if not args.atlas_skip_panels:
+        t0 = time.perf_counter(); run_panels(); torch.cuda.synchronize(); t_build = time.perf_counter() - t0
+        t_panels = timed(run_panels)
+        entries = B * sum(cnt for _, _, cnt in panels)
+        evals = B * sum(cnt << (N_VARS * n) for n, _, cnt in panels)
+        leg1 = {"formulas": B, "frames": sum(cnt for _, _, cnt in panels), "entries": entries, "seconds": t_panels,
+                "entries_per_s": entries / t_panels, "evaluations_per_s": evals / t_panels,
+                "bytes_written": 4 * entries, "write_GB_per_s": 4 * entries / t_panels / 1e9,
+                "logic_instr_per_s": logic[0] / t_panels, "frac_of_alu_peak": logic[0] / t_panels / alu_peak,
+                "plan_build_seconds": t_build, "bound": "alu"}
     h.destroy()
 
     # leg 2: HBM-write-bound - variable-free formulas, every five-world K frame
@@ -927,7 +930,10 @@ def main():
     ap.add_argument("--workload", default="c3", choices=["c3", "c3_paper", "c3_small", "c4", "c5", "atlas", "frames", "correspond"])
     ap.add_argument("--e2e-steps", type=int, default=1)
     ap.add_argument("--ref-frames", type=int, default=256)
-    ap.add_argument("--c4-contention-frames", type=int, default=1 << 20)
+    ap.add_argument("--c4-contention-frames", type=int, default=1 << 16,
+                    help="frames of the three-variable contention leg on the scalar kernel (SURVEY 8(d) shape: 2^20, "
+                         "about 20 minutes; recorded once in profiles/)")
+    ap.add_argument("--atlas-skip-panels", action="store_true", help="atlas: only the HBM-write leg (for ncu captures)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

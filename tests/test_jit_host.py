@@ -108,5 +108,8 @@ def test_density_kernels_compile_for_sm100a(n, k, cls):
             continue
         seen += 1
         assert r[3] > 0 and "density layout" in r[0]
-        assert ("KJ_CNT3" in r[0].split("density layout")[1]) == (g == 0)
+        body = r[0].split("density layout")[1]
+        # no variables: one frame per lane, counts leave as bit planes (staged through shared memory when
+        # the warp's words are consecutive, else unpacked per lane)
+        assert ("KJ_CNT3" in body or "s_stage" in body) == (g == 0)
     assert seen >= 1
