@@ -104,7 +104,13 @@ enum {
     KRIPKE_REDUCE_WARP = 1u << 8,     /* one atomic pair per (warp, formula)                      */
     KRIPKE_REDUCE_THREAD = 2u << 8,   /* one per failing (frame, formula): the paper's original
                                          frame-atomic variant, kept for ablation   */
-    KRIPKE_REDUCE_MASK = 3u << 8
+    KRIPKE_REDUCE_MASK = 3u << 8,
+    KRIPKE_NO_GUARDED_ROOTS = 1u << 10, /* compiled kernels only, ablation: test every formula's full truth set (default:
+                                         the refutation test is pushed through the conjunctions and boxes at the
+                                         top of a formula - box x is refuted by a model iff x fails at a world that
+                                         has a predecessor - so those boxes are never evaluated)    */
+    KRIPKE_NO_BOX_DISTRIBUTION = 1u << 11 /* compiled kernels only, ablation: evaluate box (x & y) as written (default:
+                                         as box x & box y wherever the batch's other formulas make that cheaper)    */
 };
 
 /* Outputs, 16 bytes each ("16 bytes per formula"; layout is reading R18). */
@@ -370,6 +376,14 @@ int kripke_debug_jit_source(const uint8_t *code, const uint32_t *offsets, uint32
  * compiled scans computes it - after every rewrite (negation edges, and / box normal form, box
  * distribution, canonical variable order).  succ: n_worlds successor masks; val: n_vars variable masks.
  * Returns the number of graph nodes or a negative kripke_status. */
+/* Diagnostic, host only: for every formula of a batch, whether the model (succ[w] successor masks, val[i] variable
+ * masks) refutes it, evaluated on the forms the compiled kernels of (n_worlds, frame_class, flags) evaluate - the
+ * batch graph after the guarded-root and box-distribution rewrites, under each record's canonical variable
+ * order.  refuted_out: n_formulas bytes (0 / 1).  Returns the number of rewrites applied (>= 0) or an error. */
+int kripke_debug_batch_refuted(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas, uint32_t n_vars,
+                               uint32_t n_worlds, uint32_t frame_class, uint32_t flags, const uint32_t *succ,
+                               const uint32_t *val, uint8_t *refuted_out);
+
 int kripke_debug_dag_truth(const uint8_t *code, uint32_t len, uint32_t n_vars, uint32_t n_worlds,
                            const uint32_t *succ, const uint32_t *val, uint32_t *truth_out);
 

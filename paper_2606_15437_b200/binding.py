@@ -21,6 +21,8 @@ ACCUMULATE = 1 << 0
 FULL_SWEEP = 1 << 1
 NO_SHARING = 1 << 2
 NO_SUBTERM_SHARING = 1 << 3
+NO_GUARDED_ROOTS = 1 << 10
+NO_BOX_DISTRIBUTION = 1 << 11
 KERNEL_AUTO, KERNEL_SCALAR, KERNEL_SLICED, KERNEL_JIT = 0 << 4, 1 << 4, 2 << 4, 3 << 4
 REDUCE_BLOCK, REDUCE_WARP, REDUCE_THREAD = 0 << 8, 1 << 8, 2 << 8
 NO_WITNESS = (1 << 64) - 1
@@ -38,6 +40,7 @@ EXPORTS = [
     "kripke_validity_bitmap", "kripke_condition_bitmap", "kripke_match_bitmaps", "kripke_frames_from_bitmap",
     "kripke_failure_density", "kripke_failure_density_frames",
     "kripke_jit_configure", "kripke_debug_jit_source", "kripke_debug_dag_truth", "kripke_signatures", "kripke_frames_generate",
+    "kripke_debug_batch_refuted",
 ]
 
 
@@ -105,6 +108,7 @@ def load():
     lib.kripke_debug_jit_source.argtypes = [u8p, u32p, u32, u32, u32p, u32, u32, u32, u32, u32, u32, ctypes.c_int, vp, u64,
                                             ctypes.POINTER(u32), ctypes.POINTER(u64), ctypes.POINTER(u64)]
     lib.kripke_debug_dag_truth.argtypes = [u8p, u32, u32, u32, u32p, u32p, ctypes.POINTER(u32)]
+    lib.kripke_debug_batch_refuted.argtypes = [vp, vp, u32, u32, u32, u32, u32, vp, vp, vp]
     for name in EXPORTS:
         if name not in ("kripke_version",):
             getattr(lib, name).restype = ctypes.c_int
@@ -488,6 +492,20 @@ def debug_jit_source(code, offsets, n_vars: int, n_worlds: int, frame_class: int
     if rc < 0:
         raise KripkeError(rc, "kripke_debug_jit_source")
     return buf.value.decode(), nk.value, ops.value, cb.value
+
+
+def debug_batch_refuted(code, offsets, n_vars: int, n_worlds: int, frame_class: int, succ, val, flags: int = 0):
+    """(refuted flag per formula, rewrites applied): does the model refute each formula, evaluated on the forms
+    the compiled kernels evaluate (guarded roots, redistributed boxes, canonical variable order)?  Pure host."""
+    code, offsets = _host(code, offsets)
+    s = np.ascontiguousarray(succ, dtype=np.uint32)
+    v = np.ascontiguousarray(list(val) + [0] * (4 - len(val)), dtype=np.uint32)
+    out = np.zeros(len(offsets) - 1, dtype=np.uint8)
+    rc = load().kripke_debug_batch_refuted(code.ctypes.data, offsets.ctypes.data, len(offsets) - 1, n_vars, n_worlds,
+                                           frame_class, flags, s.ctypes.data, v.ctypes.data, out.ctypes.data)
+    if rc < 0:
+        raise KripkeError(rc, "kripke_debug_batch_refuted")
+    return out.astype(bool), rc
 
 
 def debug_dag_truth(code: bytes, n_vars: int, n_worlds: int, succ, val) -> int:

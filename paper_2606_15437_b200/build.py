@@ -34,6 +34,7 @@ UNITS = [
     ("frame_gen", "frame_gen.cu", []),
     ("jit_dag", "jit_dag.cpp", []),
     ("jit_emit", "jit_emit.cpp", []),
+    ("jit_opt", "jit_opt.cpp", []),
     ("jit_runtime", "jit_runtime.cpp", []),
 ] + [(f"scan_sliced_inst{g}", "scan_sliced_inst.cu", [f"-DKRIPKE_INST_GROUP={g}"]) for g in range(4)] \
   + [(f"scan_frames_inst{g}", "scan_frames_inst.cu", [f"-DKRIPKE_FR_GROUP={g}"]) for g in range(4)]

@@ -295,6 +295,7 @@ int build_jit_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_r
                    uint32_t cls, uint32_t flags, ScanPlan *out);
 
 constexpr uint32_t SCAN_FLAGS = KRIPKE_ACCUMULATE | KRIPKE_FULL_SWEEP | KRIPKE_NO_SHARING | KRIPKE_NO_SUBTERM_SHARING |
+                                KRIPKE_NO_GUARDED_ROOTS | KRIPKE_NO_BOX_DISTRIBUTION |
                                 KRIPKE_KERNEL_MASK | KRIPKE_REDUCE_MASK;
 
 // Argument checks of every class scan - before any plan is built or cached.
@@ -615,12 +616,20 @@ struct JitGroupHost {
     std::vector<JitRoot> roots;          // distinct roots = the programs that are scanned
     std::vector<uint32_t> slot_record;   // representative record of each root
     std::vector<uint32_t> alias;         // (record, representative) pairs
+    JitOptStats opt;
+};
+
+// Where a record went, and the variable order it is evaluated under (host checks only).
+struct JitRecordInfo {
+    uint32_t group = 0, slot = 0, support = 0;
+    uint8_t rename[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
 };
 
 // Groups the records by the number of variables they mention (Algorithm 1's per-formula k_b; the
 // least g >= that count for which the emitter has a layout) and builds each group's graph.
 int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
-                      uint32_t cls, uint32_t flags, uint32_t mode, std::vector<JitGroupHost> *out) {
+                      uint32_t cls, uint32_t flags, uint32_t mode, std::vector<JitGroupHost> *out,
+                      std::vector<JitRecordInfo> *info_out = nullptr) {
     auto layout_ok = [&](uint32_t g) {
         return mode == JIT_MODE_DENSITY ? jit_density_layout(n, g, cls, nullptr) : jit_layout(n, g, cls, nullptr);
     };
@@ -631,6 +640,7 @@ int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t 
     for (uint32_t g = 0; g <= k; ++g) (*out)[g].g = g;
     std::vector<Dag> probe(k + 1);       // unsalted graphs: which records are the same program
     std::vector<std::map<std::pair<uint32_t, uint32_t>, uint32_t>> seen(k + 1);
+    if (info_out) info_out->assign(n_records, JitRecordInfo());
     for (uint32_t r = 0; r < n_records; ++r) {
         const uint32_t fa = pairs ? pairs[2 * r] : r, fb = pairs ? pairs[2 * r + 1] : r;
         // the variables the record's GRAPH mentions (the rewrites fold more than the syntax shows: x & ~x, box T)
@@ -654,13 +664,24 @@ int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t 
         } else {
             canonical_rename(prog(fa), plen(fa), pairs ? prog(fb) : nullptr, pairs ? plen(fb) : 0u, sup, rename);
         }
+        if (info_out) {
+            JitRecordInfo &ri = (*info_out)[r];
+            ri.group = g;
+            ri.support = sup;
+            for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v) ri.rename[v] = rename[v];
+            ri.slot = (uint32_t)G.roots.size();
+        }
         if (!(flags & KRIPKE_NO_SHARING) && mode != JIT_MODE_DENSITY) {
             // records whose graphs coincide are scanned once (the pair path is symmetric in its two formulas)
             uint32_t pa = probe[g].build(prog(fa), plen(fa), rename);
             uint32_t pb = pairs ? probe[g].build(prog(fb), plen(fb), rename) : UINT32_MAX;
             if (pairs && pb < pa) std::swap(pa, pb);
             auto it = seen[g].find(std::make_pair(pa, pb));
-            if (it != seen[g].end()) { G.alias.push_back(r); G.alias.push_back(it->second); continue; }
+            if (it != seen[g].end()) {
+                G.alias.push_back(r); G.alias.push_back(it->second);
+                if (info_out) (*info_out)[r].slot = (*info_out)[it->second].slot;
+                continue;
+            }
             seen[g].emplace(std::make_pair(pa, pb), r);
         }
         G.dag.salt = (flags & (KRIPKE_NO_SHARING | KRIPKE_NO_SUBTERM_SHARING)) ? r + 1 : 0u;
@@ -669,6 +690,22 @@ int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t 
         root.b = pairs ? G.dag.build(prog(fb), plen(fb), rename) : UINT32_MAX;
         G.roots.push_back(root);
         G.slot_record.push_back(r);
+    }
+    // evaluation forms (jit.h): the refutation test pushed through the top of each formula, then box
+    // redistributed over conjunctions where the batch makes that cheaper
+    for (JitGroupHost &G : *out) {
+        if (G.roots.empty()) continue;
+        JitLayout lay;
+        if (!(mode == JIT_MODE_DENSITY ? jit_density_layout(n, G.g, cls, &lay) : jit_layout(n, G.g, cls, &lay))) continue;
+        // (with no variables the frame bits are the lanes and the word loop: the guard sets of class K would be
+        // recomputed per word)
+        if (mode == JIT_MODE_SCAN && !pairs && !(flags & KRIPKE_NO_GUARDED_ROOTS) && (lay.kn >= 5 || cls != KRIPKE_CLASS_K))
+            jit_guard_roots(G.dag, &G.roots);
+        if (!(flags & (KRIPKE_NO_SHARING | KRIPKE_NO_SUBTERM_SHARING | KRIPKE_NO_BOX_DISTRIBUTION))) {
+            Dag opt;
+            jit_optimize(G.dag, lay, &G.roots, &opt, &G.opt);
+            G.dag = std::move(opt);
+        }
     }
     return KRIPKE_OK;
 }
@@ -726,7 +763,8 @@ int build_density_plan(const kripke_programs *h, uint32_t n, uint32_t k, uint32_
 }
 
 uint64_t plan_key(uint32_t n, uint32_t k, uint32_t cls, uint32_t flags, uint32_t engine, uint32_t shapes) {
-    const uint32_t fl = flags & (KRIPKE_FULL_SWEEP | KRIPKE_NO_SHARING | KRIPKE_NO_SUBTERM_SHARING);
+    const uint32_t fl = flags & (KRIPKE_FULL_SWEEP | KRIPKE_NO_SHARING | KRIPKE_NO_SUBTERM_SHARING | KRIPKE_NO_GUARDED_ROOTS |
+                                 KRIPKE_NO_BOX_DISTRIBUTION);
     return (uint64_t)n | ((uint64_t)k << 4) | ((uint64_t)cls << 8) | ((uint64_t)engine << 12) | ((uint64_t)fl << 16) |
            ((uint64_t)shapes << 32);
 }
@@ -1419,6 +1457,36 @@ int kripke_debug_jit_source(const uint8_t *code, const uint32_t *offsets, uint32
         source_out[m] = 0;
     }
     return (int)std::min<size_t>(src.size(), 0x7FFFFFFF);
+}
+
+int kripke_debug_batch_refuted(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas, uint32_t n_vars,
+                               uint32_t n_worlds, uint32_t frame_class, uint32_t flags, const uint32_t *succ,
+                               const uint32_t *val, uint8_t *refuted_out) {
+    if (!succ || !refuted_out || n_worlds < 1 || n_worlds > KRIPKE_MAX_WORLDS || frame_class > KRIPKE_CLASS_S5 ||
+        (n_vars && !val))
+        return KRIPKE_EINVAL;
+    int rc = validate_programs(code, offsets, n_formulas, n_vars, nullptr);
+    if (rc) return rc;
+    kripke_programs tmp;                       // host fields only
+    tmp.n_formulas = n_formulas; tmp.n_vars = n_vars;
+    tmp.h_offsets.assign(offsets, offsets + n_formulas + 1);
+    tmp.h_code.assign(code + offsets[0], code + offsets[n_formulas]);
+    for (auto &o : tmp.h_offsets) o -= offsets[0];
+    std::vector<JitGroupHost> groups;
+    std::vector<JitRecordInfo> info;
+    rc = jit_group_records(&tmp, nullptr, n_formulas, n_worlds, n_vars, frame_class, flags, JIT_MODE_SCAN, &groups, &info);
+    if (rc) return rc;
+    int rewrites = 0;
+    for (const JitGroupHost &G : groups) rewrites += (int)G.opt.rewrites;
+    for (uint32_t r = 0; r < n_formulas; ++r) {
+        const JitRecordInfo &ri = info[r];
+        uint32_t pv[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
+        for (uint32_t v = 0; v < n_vars; ++v)
+            if ((ri.support >> v) & 1u) pv[ri.rename[v]] = val[v];
+        const JitGroupHost &G = groups[ri.group];
+        refuted_out[r] = jit_root_refuted(G.dag, G.roots[ri.slot], n_worlds, succ, pv) ? 1 : 0;
+    }
+    return rewrites;
 }
 
 int kripke_debug_dag_truth(const uint8_t *code, uint32_t len, uint32_t n_vars, uint32_t n_worlds,

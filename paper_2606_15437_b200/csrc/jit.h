@@ -33,6 +33,7 @@ struct DagNode {
     uint8_t var;            // VAR: index in the group's valuation
     uint32_t a, b;          // operand literals (AND: a < b)
     uint32_t salt;          // 0, or the owner record + 1 when subterm sharing is off
+    uint8_t rank;           // loop level of the variables below it (not part of the node's identity)
 };
 
 struct Dag {
@@ -48,6 +49,12 @@ struct Dag {
     // Truth set (n-bit mask) of a literal on one model: succ[w] successor masks, val[i] variable masks.
     uint32_t eval(uint32_t lit, uint32_t n, const uint32_t *succ, const uint32_t *val) const;
     uint32_t salt = 0;      // applied to new AND / BOX nodes
+    // Canonical graphs (the default) rewrite box x & box y into box (x & y) and order conjuncts by literal.  An
+    // implementation graph (jit_opt.cpp) keeps conjunctions of boxes as they are and folds the conjuncts of low
+    // loop level first (var_rank[i] = level of variable i), so that loop-invariant partial conjunctions are hoisted.
+    bool merge_boxes = true;
+    std::vector<uint8_t> var_rank;
+    uint8_t rank_of(uint32_t lit) const { return nodes[lit >> 1].rank; }
     // Canonical text of a literal's cone (conjunctions flattened, operands sorted by text).
     std::string text(uint32_t lit) const;
   private:
@@ -61,6 +68,20 @@ struct Dag {
 // support_mask: variables mentioned; rename_out[v] = index in the reduced valuation (g = popcount).
 void canonical_rename(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b,
                       uint32_t support_mask, uint8_t *rename_out);
+
+// ---- cost-driven redistribution of box over conjunction (jit_opt.cpp) -------------------------------
+struct JitLayout;
+struct JitRoot;
+struct JitOptStats {
+    uint32_t rewrites = 0;
+    double cost_before = 0, cost_after = 0;   // logic instructions per 32-model word of the needed graph nodes
+};
+// box (x1 & ... & xk) = box (S1) & ... & box (Sm) for every partition of the conjuncts, on every frame.  Which
+// side is cheaper depends on what else the batch evaluates: the left side costs one box (n^2 instructions per
+// word), the right side m boxes - but only those that no other formula needs anyway, and only at the loop level
+// of their own variables.  Starting from the canonical graph (left sides only), applies the rewrite with the
+// largest saving until none is left.  *roots is replaced by the roots in *out.
+void jit_optimize(const Dag &in, const JitLayout &lay, std::vector<JitRoot> *roots, Dag *out, JitOptStats *stats);
 
 // ---- layout (jit_emit.cpp) ------------------------------------------------------------------------
 // Model index X = (class-order frame index << g*n) | v.  Bits 0..4 of X vary inside a word, the next
@@ -78,10 +99,47 @@ struct JitLayout {
 // Is there a compiled layout for (n, g, class)?  Fills *out.
 bool jit_layout(uint32_t n, uint32_t g, uint32_t cls, JitLayout *out);
 
+// Loop level at which a bit of the model index changes in a thread (0 = fixed for the unit, 1 = outer loop,
+// 2 = inner loop) for "p_i at world w" and for the edge w -> u (0 where the edge is no index bit: class T's
+// diagonal, the table classes), and the cost of one instruction at a level per 32-model word.
+int jit_atom_level(const JitLayout &lay, uint32_t var, uint32_t w);
+int jit_edge_level(const JitLayout &lay, uint32_t w, uint32_t u);
+double jit_level_weight(const JitLayout &lay, int level);
+
 // One record of a group: a single formula (b == UINT32_MAX) or a pair.
-struct JitRoot {
-    uint32_t a, b;                 // literals
+//
+// A single formula may be given in guarded form instead of by its root literal: a model refutes it iff its truth
+// set is not W, i.e. iff the root fails at some world.  A positive conjunction fails somewhere iff one
+// conjunct does, and box x fails somewhere iff x fails at a world that has a predecessor, so the
+// test is pushed through the positive conjunctions and boxes at the top of the formula:
+//     refuted  <=>  OR over (depth, lit) in guarded of  OR_u ( S_depth[u] & ~lit[u] ),
+// S_0 = W, S_(d+1) = the successors of S_d - sets that depend on the frame only and are shared by every record.
+// The boxes at the top of a formula are then never evaluated (n instructions per obligation instead of n^2 per box).
+struct JitGuarded {
+    uint32_t depth, lit;
+    bool operator<(const JitGuarded &o) const { return depth != o.depth ? depth < o.depth : lit < o.lit; }
+    bool operator==(const JitGuarded &o) const { return depth == o.depth && lit == o.lit; }
 };
+struct JitRoot {
+    uint32_t a = 0, b = UINT32_MAX;        // literals (a is unused when guarded is not empty)
+    std::vector<JitGuarded> guarded;
+    // every literal whose value the record reads
+    template <class F> void for_each_lit(F f) const {
+        if (!guarded.empty()) { for (const JitGuarded &g : guarded) f(g.lit); return; }
+        f(a);
+        if (b != UINT32_MAX) f(b);
+    }
+    template <class F> void map_lits(F f) {
+        if (!guarded.empty()) { for (JitGuarded &g : guarded) g.lit = f(g.lit); return; }
+        a = f(a);
+        if (b != UINT32_MAX) b = f(b);
+    }
+};
+// Rewrites the single-formula roots into guarded form (pairs and roots that are a bare literal stay as they are).
+void jit_guard_roots(const Dag &dag, std::vector<JitRoot> *roots);
+// Does the model (succ[w] successor masks, val[i] variable masks) refute the record, evaluated as the compiled
+// kernels evaluate it?  (host check of the guarded form and of the optimised graph)
+bool jit_root_refuted(const Dag &dag, const JitRoot &root, uint32_t n, const uint32_t *succ, const uint32_t *val);
 
 struct JitEmitStats {
     double logic_ops_per_word = 0;     // 3-input logic instructions executed per 32-model word: statements of the

@@ -26,12 +26,12 @@ uint32_t Dag::intern(const DagNode &nd) {
 }
 
 uint32_t Dag::lit_const(bool v) {
-    DagNode nd{DagNode::CONST0, 0, 0, 0, 0};
+    DagNode nd{DagNode::CONST0, 0, 0, 0, 0, 0};
     return intern(nd) * 2 + (v ? 1u : 0u);
 }
 
 uint32_t Dag::lit_var(uint32_t i) {
-    DagNode nd{DagNode::VAR, (uint8_t)i, 0, 0, 0};
+    DagNode nd{DagNode::VAR, (uint8_t)i, 0, 0, 0, i < var_rank.size() ? var_rank[i] : (uint8_t)0};
     return intern(nd) * 2;
 }
 
@@ -48,7 +48,7 @@ void Dag::conjuncts(uint32_t lit, std::vector<uint32_t> *out) const {
 
 uint32_t Dag::mk_box(uint32_t x) {
     if (nodes[x >> 1].kind == DagNode::CONST0 && (x & 1u)) return x;       // box T = T
-    DagNode nd{DagNode::BOX, 0, x, 0, salt};
+    DagNode nd{DagNode::BOX, 0, x, 0, salt, rank_of(x)};
     return intern(nd) * 2;
 }
 
@@ -68,7 +68,7 @@ uint32_t Dag::mk_and(uint32_t x, uint32_t y) {
                 continue;                                                  // ... and T
             }
             if (i + 1 < c.size() && c[i + 1] == (l ^ 1u)) return lit_const(false);   // x and not x
-            if (!(l & 1u) && nd.kind == DagNode::BOX && nd.salt == salt) boxed.push_back(nd.a);
+            if (merge_boxes && !(l & 1u) && nd.kind == DagNode::BOX && nd.salt == salt) boxed.push_back(nd.a);
             else keep.push_back(l);
         }
         if (boxed.size() < 2) {
@@ -84,9 +84,11 @@ uint32_t Dag::mk_and(uint32_t x, uint32_t y) {
     std::sort(c.begin(), c.end());
     c.erase(std::unique(c.begin(), c.end()), c.end());
     if (c.empty()) return lit_const(true);
+    // fold order: conjuncts of low loop level first (all ranks are 0 in a canonical graph: literal order)
+    std::stable_sort(c.begin(), c.end(), [&](uint32_t p, uint32_t q) { return rank_of(p) < rank_of(q); });
     uint32_t acc = c[0];
     for (size_t i = 1; i < c.size(); ++i) {
-        DagNode nd{DagNode::AND, 0, std::min(acc, c[i]), std::max(acc, c[i]), salt};
+        DagNode nd{DagNode::AND, 0, std::min(acc, c[i]), std::max(acc, c[i]), salt, std::max(rank_of(acc), rank_of(c[i]))};
         acc = intern(nd) * 2;
     }
     return acc;

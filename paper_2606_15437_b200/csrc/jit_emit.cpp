@@ -192,6 +192,31 @@ struct Emitter {
         }
     }
 
+    // ---- guard sets of the guarded roots (jit.h): S_d[u] = "world u is reachable in exactly d steps" ----
+    // Only class K needs them: T, S4 and S5 frames are reflexive, so every S_d is W.
+    std::vector<std::array<int8_t, KRIPKE_MAX_WORLDS>> guard_lvl;       // guard_lvl[d - 1][u]
+    int guard(uint32_t d, uint32_t u) {
+        if (d == 0 || lay.cls != KRIPKE_CLASS_K) return constant(true);
+        const uint32_t n = lay.n;
+        while (guard_lvl.size() < d) {
+            const uint32_t k = (uint32_t)guard_lvl.size() + 1;          // builds S_k from S_(k-1)
+            std::array<int8_t, KRIPKE_MAX_WORLDS> lv;
+            lv.fill(0);
+            for (uint32_t v = 0; v < n; ++v) {
+                int L = 0, acc = constant(false);
+                for (uint32_t w = 0; w < n; ++w) {
+                    L = std::max(L, std::max(edge_level(w, v), k > 1 ? (int)guard_lvl[k - 2][w] : 0));
+                    const int e = leaf(edge(w, v), false);
+                    acc = bin(Ex::OR, acc, k > 1 ? bin(Ex::AND, leaf(fmt("s%u_%u", k - 1, w), false), e) : e);
+                }
+                lv[v] = (int8_t)L;
+                stmts.push_back(Stmt{L, fmt("s%u_%u", k, v), acc, ""});
+            }
+            guard_lvl.push_back(lv);
+        }
+        return leaf(fmt("s%u_%u", d, u), false);
+    }
+
     // ---- single-use substitution ----
     void collect_leaves(int x, std::vector<int> *out) const {
         if (pool[x].op == Ex::LEAF) out->push_back(x);
@@ -313,6 +338,21 @@ struct Emitter {
 
 }  // namespace
 
+int jit_atom_level(const JitLayout &lay, uint32_t var, uint32_t w) {
+    return BitSource(lay).level(var * lay.n + w);
+}
+
+int jit_edge_level(const JitLayout &lay, uint32_t w, uint32_t u) {
+    const uint32_t n = lay.n;
+    if (lay.table) return 0;
+    if (lay.cls == KRIPKE_CLASS_T) return w == u ? 0 : BitSource(lay).level(lay.kn + w * (n - 1) + (u < w ? u : u - 1));
+    return BitSource(lay).level(lay.kn + w * n + u);
+}
+
+double jit_level_weight(const JitLayout &lay, int level) {
+    return level >= 2 ? 1.0 : level == 1 ? 1.0 / (double)(1u << lay.inner) : 1.0 / (double)(1u << (lay.inner + lay.outer));
+}
+
 bool jit_layout(uint32_t n, uint32_t g, uint32_t cls, JitLayout *out) {
     if (n < 1 || n > KRIPKE_MAX_WORLDS || g > KRIPKE_MAX_VARS || cls > KRIPKE_CLASS_S5) return false;
     JitLayout l;
@@ -368,8 +408,7 @@ std::vector<std::vector<uint32_t>> jit_partition(const Dag &dag, const std::vect
         std::vector<uint32_t> stamp(dag.nodes.size(), UINT32_MAX), stack;
         for (size_t r = 0; r < R; ++r) {
             stack.clear();
-            stack.push_back(roots[r].a >> 1);
-            if (roots[r].b != UINT32_MAX) stack.push_back(roots[r].b >> 1);
+            roots[r].for_each_lit([&](uint32_t l) { stack.push_back(l >> 1); });
             while (!stack.empty()) {
                 const uint32_t id = stack.back(); stack.pop_back();
                 if (stamp[id] == r) continue;
@@ -589,15 +628,24 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
     else fmode = F_ANY;                                             // 2^inner words per frame, several frames per unit
 
     for (uint32_t r = 0; r < G; ++r) {
-        em.node(roots[r].a >> 1);
         int e;
-        if (roots[r].b == UINT32_MAX) {
+        if (!roots[r].guarded.empty()) {
+            // refuted lanes of a guarded root: some obligation fails at a world of its guard set (jit.h)
+            e = em.constant(false);
+            for (const JitGuarded &g : roots[r].guarded) {
+                em.node(g.lit >> 1);
+                for (uint32_t u = 0; u < n; ++u)
+                    e = em.bin(Ex::OR, e, em.bin(Ex::AND, em.guard(g.depth, u), em.negate(em.lit(g.lit, u))));
+            }
+        } else if (roots[r].b == UINT32_MAX) {
+            em.node(roots[r].a >> 1);
             // refuted lanes: the truth set is not all worlds
             e = em.constant(true);
             for (uint32_t w = 0; w < n; ++w) e = em.bin(Ex::AND, e, em.lit(roots[r].a, w));
             e = em.negate(e);
         } else {
             // distinguishing lanes: the two truth sets differ
+            em.node(roots[r].a >> 1);
             em.node(roots[r].b >> 1);
             e = em.constant(false);
             for (uint32_t w = 0; w < n; ++w) e = em.bin(Ex::OR, e, em.bin(Ex::XOR, em.lit(roots[r].a, w), em.lit(roots[r].b, w)));

@@ -42,6 +42,44 @@ def test_batch_graph_truth_equals_oracle(vol):
                     assert got == want, (W.to_text(W.from_postfix(c)), n, f, v)
 
 
+@pytest.mark.parametrize("flags", [0, kb.NO_GUARDED_ROOTS, kb.NO_BOX_DISTRIBUTION])
+def test_evaluation_forms_refute_exactly_the_oracles_models(vol, flags):
+    """kripke_debug_batch_refuted: the forms the compiled kernels evaluate - the refutation test pushed through the
+    conjunctions and boxes at the top of each formula (guard sets S_d = worlds reachable in exactly d steps) and box
+    redistributed over conjunctions by the batch's cost - refute exactly the models the oracle's truth set
+    refutes, for every formula of a batch on random models (classes K and T, n = 3..6), and rewrites do happen."""
+    rng = W.SplitMix64(77002)
+    extra = ["[]p", "[][]p", "[](p & q)", "[]p & []q", "[][](p -> q) & p", "[]F", "[][]F", "[]T", "[]([]p & q)",
+             "[]([]F | p)", "[]p & ([]q & ~[](p & q))", "[](p & []q) -> [](q & []p)", "<>p -> []<>p", "[](p & q & []p)"]
+    sets = [(W.corpus_c2(700), 2), (W.corpus_c1(300) + [W.to_postfix(W.parse(t)) for t in extra], 2),
+            (W.corpus_c4(200), 3), (W.pairs_c5(150)[0], 0)]
+    total_rewrites = 0
+    for progs, k in sets:
+        code, offs = W.pack_programs(progs)
+        for n, cls in ((3, K), (5, K), (5, T), (4, T), (6, K)):
+            if n * n + k * n > 61:
+                continue
+            for f, v, succ, vals in _models(rng, n, k, 4):
+                if cls == T:
+                    f |= sum(1 << (w * n + w) for w in range(n))
+                    succ = [(f >> (w * n)) & ((1 << n) - 1) for w in range(n)]
+                got, rewrites = kb.debug_batch_refuted(code, offs, k, n, cls, succ, vals, flags)
+                total_rewrites += rewrites
+                for i, c in enumerate(progs):
+                    want = not all(vol.truth(c, n, f, k, v))
+                    assert bool(got[i]) == want, (W.to_text(W.from_postfix(c)), n, cls, f, v)
+    assert (total_rewrites > 0) == (not (flags & kb.NO_BOX_DISTRIBUTION))
+
+
+def test_guarded_roots_drop_the_top_boxes():
+    """A formula that is a box of a variable costs n instructions per word in guarded form (no box is evaluated),
+    n^2 + the test when its full truth set is computed."""
+    code, offs = W.pack_programs([W.to_postfix(W.parse("[][](p | q)"))])
+    guarded = kb.debug_jit_source(code, offs, 2, 5, K, 2)[2]
+    plain = kb.debug_jit_source(code, offs, 2, 5, K, 2, 0, kb.NO_GUARDED_ROOTS)[2]
+    assert guarded <= 12 and plain >= 50
+
+
 def test_box_distribution_shares_nodes():
     """[]p & []q and [](p & q) are the same graph node; alpha-equivalent programs coincide after the
     canonical renaming (one compiled program for the two of them)."""
