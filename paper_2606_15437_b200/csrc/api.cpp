@@ -710,56 +710,118 @@ int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t 
     return KRIPKE_OK;
 }
 
-int build_jit_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
-                   uint32_t cls, uint32_t flags, ScanPlan *out) {
-    out->release();
-    const auto t0 = std::chrono::steady_clock::now();
-    std::vector<JitGroupHost> groups;
-    int rc = jit_group_records(h, pairs, n_records, n, k, cls, flags, JIT_MODE_SCAN, &groups);
-    if (rc) return rc;
-    for (JitGroupHost &G : groups) {
-        if (G.roots.empty() && G.alias.empty()) continue;
+// Process-wide cache of compiled plans, keyed by everything a plan depends on (the programs' bytes, the record
+// list, shape, class, flags, emitter configuration) and compared in full: the same batch staged again - a new
+// handle for the next class range, shard or call of kripke_eval_batch_host - skips graph building, rewriting,
+// emission and compilation and only uploads its slot tables.  The kernels themselves live in the module cache of
+// jit_runtime.cpp and are never unloaded.
+struct CachedJitGroup {
+    uint32_t g = 0;
+    JitGroupPlan jit;                 // d_slot_record is null here
+    std::vector<uint32_t> alias;
+};
+struct CachedJitPlan {
+    std::vector<CachedJitGroup> groups;
+    uint64_t stamp = 0;
+};
+std::mutex g_plan_cache_mutex;
+std::map<std::string, CachedJitPlan> g_plan_cache;
+uint64_t g_plan_cache_clock = 0;
+constexpr size_t PLAN_CACHE_ENTRIES = 32;
+
+std::string jit_plan_key(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
+                         uint32_t cls, uint32_t flags, uint32_t mode) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const uint32_t head[] = {n_records, n, k, cls, flags, mode, g_jit_max_programs, g_jit_min_blocks, (uint32_t)dev,
+                             h->n_formulas, pairs ? 1u : 0u};
+    std::string key((const char *)head, sizeof(head));
+    key.append((const char *)h->h_offsets.data(), h->h_offsets.size() * sizeof(uint32_t));
+    key.append((const char *)h->h_code.data(), h->h_code.size());
+    if (pairs) key.append((const char *)pairs, 2 * (size_t)n_records * sizeof(uint32_t));
+    return key;
+}
+
+// Instantiates a cached plan for this handle (device copies of the slot and alias tables).
+int instantiate_jit_plan(const CachedJitPlan &cp, ScanPlan *out) {
+    for (const CachedJitGroup &cg : cp.groups) {
         GroupPlan gp;
-        gp.k_eff = G.g;
+        gp.k_eff = cg.g;
         gp.use_jit = true;
-        JitLayout lay;
-        jit_layout(n, G.g, cls, &lay);
-        std::string log;
-        rc = jit_build_group(G.dag, lay, G.roots, G.slot_record, g_jit_max_programs, g_jit_min_blocks, JIT_MODE_SCAN, &gp.jit, &log);
+        gp.jit = cg.jit;
+        gp.jit.d_slot_record = nullptr;
+        int rc = jit_upload_slots(&gp.jit);
         if (rc > 0) rc = cuda_fail(rc);
-        if (!rc) rc = upload(&gp.d_alias, G.alias);
+        if (!rc) rc = upload(&gp.d_alias, cg.alias);
         if (rc) { gp.release(); out->release(); return rc; }
-        gp.n_alias = (uint32_t)(G.alias.size() / 2);
+        gp.n_alias = (uint32_t)(cg.alias.size() / 2);
         out->groups.push_back(gp);
     }
-    out->jit_compile_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
     return KRIPKE_OK;
+}
+
+int build_jit_plan_mode(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
+                        uint32_t cls, uint32_t flags, uint32_t mode, ScanPlan *out) {
+    out->release();
+    const auto t0 = std::chrono::steady_clock::now();
+    const uint32_t plan_flags = flags & (KRIPKE_FULL_SWEEP | KRIPKE_NO_SHARING | KRIPKE_NO_SUBTERM_SHARING |
+                                         KRIPKE_NO_GUARDED_ROOTS | KRIPKE_NO_BOX_DISTRIBUTION);
+    const std::string key = jit_plan_key(h, pairs, n_records, n, k, cls, plan_flags, mode);
+    {
+        std::lock_guard<std::mutex> lock(g_plan_cache_mutex);
+        auto it = g_plan_cache.find(key);
+        if (it != g_plan_cache.end()) {
+            it->second.stamp = ++g_plan_cache_clock;
+            return instantiate_jit_plan(it->second, out);          // jit_compile_seconds stays 0: nothing was compiled
+        }
+    }
+    std::vector<JitGroupHost> groups;
+    int rc = jit_group_records(h, pairs, n_records, n, k, cls, flags, mode, &groups);
+    if (rc) return rc;
+    CachedJitPlan cp;
+    for (JitGroupHost &G : groups) {
+        if (G.roots.empty() && G.alias.empty()) continue;
+        CachedJitGroup cg;
+        cg.g = G.g;
+        cg.alias = G.alias;
+        JitLayout lay;
+        if (mode == JIT_MODE_DENSITY) jit_density_layout(n, G.g, cls, &lay);
+        else jit_layout(n, G.g, cls, &lay);
+        std::string log;
+        // density: fewer programs per kernel than a scan - every program keeps n failing-world words alive for its stores
+        const uint32_t max_programs = mode == JIT_MODE_DENSITY ? std::min<uint32_t>(g_jit_max_programs, 32) : g_jit_max_programs;
+        rc = jit_build_group(G.dag, lay, G.roots, G.slot_record, max_programs, g_jit_min_blocks, mode, &cg.jit, &log);
+        cudaFree(cg.jit.d_slot_record);                             // the cache keeps host data only
+        cg.jit.d_slot_record = nullptr;
+        if (rc > 0) rc = cuda_fail(rc);
+        if (rc) return rc;
+        cp.groups.push_back(std::move(cg));
+    }
+    rc = instantiate_jit_plan(cp, out);
+    if (rc) return rc;
+    out->jit_compile_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    {
+        std::lock_guard<std::mutex> lock(g_plan_cache_mutex);
+        if (g_plan_cache.size() >= PLAN_CACHE_ENTRIES) {
+            auto victim = g_plan_cache.begin();
+            for (auto it = g_plan_cache.begin(); it != g_plan_cache.end(); ++it)
+                if (it->second.stamp < victim->second.stamp) victim = it;
+            g_plan_cache.erase(victim);
+        }
+        cp.stamp = ++g_plan_cache_clock;
+        g_plan_cache.emplace(key, std::move(cp));
+    }
+    return KRIPKE_OK;
+}
+
+int build_jit_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_records, uint32_t n, uint32_t k,
+                   uint32_t cls, uint32_t flags, ScanPlan *out) {
+    return build_jit_plan_mode(h, pairs, n_records, n, k, cls, flags, JIT_MODE_SCAN, out);
 }
 
 // Failure-density plan: every formula is a record of its own (one output row each), the graph is shared.
 int build_density_plan(const kripke_programs *h, uint32_t n, uint32_t k, uint32_t cls, ScanPlan *out) {
-    out->release();
-    const auto t0 = std::chrono::steady_clock::now();
-    std::vector<JitGroupHost> groups;
-    int rc = jit_group_records(h, nullptr, h->n_formulas, n, k, cls, 0, JIT_MODE_DENSITY, &groups);
-    if (rc) return rc;
-    for (JitGroupHost &G : groups) {
-        if (G.roots.empty()) continue;
-        GroupPlan gp;
-        gp.k_eff = G.g;
-        gp.use_jit = true;
-        JitLayout lay;
-        jit_density_layout(n, G.g, cls, &lay);
-        std::string log;
-        // fewer programs per kernel than a scan: every program keeps n failing-world words alive for its stores
-        rc = jit_build_group(G.dag, lay, G.roots, G.slot_record, std::min<uint32_t>(g_jit_max_programs, 32), g_jit_min_blocks,
-                             JIT_MODE_DENSITY, &gp.jit, &log);
-        if (rc > 0) rc = cuda_fail(rc);
-        if (rc) { gp.release(); out->release(); return rc; }
-        out->groups.push_back(gp);
-    }
-    out->jit_compile_seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
-    return KRIPKE_OK;
+    return build_jit_plan_mode(h, nullptr, h->n_formulas, n, k, cls, 0, JIT_MODE_DENSITY, out);
 }
 
 uint64_t plan_key(uint32_t n, uint32_t k, uint32_t cls, uint32_t flags, uint32_t engine, uint32_t shapes) {

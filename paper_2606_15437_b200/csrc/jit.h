@@ -176,6 +176,7 @@ struct JitGroupPlan {
     JitLayout lay;
     std::vector<JitKernel> kernels;
     uint32_t *d_slot_record = nullptr;   // device: record per slot
+    std::vector<uint32_t> h_slot_record; // the same on the host (a cached plan is re-uploaded from it)
     uint32_t n_slots = 0;
     uint32_t threads = 128;
     JitEmitStats stats;
@@ -188,6 +189,9 @@ struct JitGroupPlan {
 int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitRoot> &roots,
                     const std::vector<uint32_t> &slot_record, uint32_t max_roots, uint32_t min_blocks,
                     uint32_t mode, JitGroupPlan *out, std::string *log_out);
+
+// Device copy of plan->h_slot_record (a plan taken from the process-wide cache owns no device memory yet).
+int jit_upload_slots(JitGroupPlan *plan);
 
 // Output of the density kernels: counts[record * total_frames + (class-order frame index - frame_base)].
 struct JitDensityOut {

@@ -157,14 +157,21 @@ int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitR
             out->kernels.push_back(k);
         }
     }
-    std::vector<uint32_t> records(order.size());
-    for (size_t s = 0; s < order.size(); ++s) records[s] = slot_record[order[s]];
-    cudaError_t e = cudaMalloc((void **)&out->d_slot_record, records.size() * sizeof(uint32_t));
+    out->h_slot_record.resize(order.size());
+    for (size_t s = 0; s < order.size(); ++s) out->h_slot_record[s] = slot_record[order[s]];
+    return jit_upload_slots(out);
+}
+
+int jit_upload_slots(JitGroupPlan *plan) {
+    cudaFree(plan->d_slot_record);
+    plan->d_slot_record = nullptr;
+    const std::vector<uint32_t> &records = plan->h_slot_record;
+    plan->n_slots = (uint32_t)records.size();
+    if (records.empty()) return 0;
+    cudaError_t e = cudaMalloc((void **)&plan->d_slot_record, records.size() * sizeof(uint32_t));
     if (e == cudaSuccess)
-        e = cudaMemcpy(out->d_slot_record, records.data(), records.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
-    if (e != cudaSuccess) return (int)e;
-    out->n_slots = (uint32_t)records.size();
-    return 0;
+        e = cudaMemcpy(plan->d_slot_record, records.data(), records.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
+    return (int)e;
 }
 
 int jit_launch_group(const ScanJob &job, const JitGroupPlan &plan, uint32_t model_shift, const JitDensityOut *density,

@@ -103,6 +103,29 @@ def test_compiled_equals_interpreted_and_scalar_on_c2(kb):
             same(a, scan(kb, h, n, 2, cls, begin, count, kb.KERNEL_SCALAR), f"compiled vs scalar n={n} cls={cls}")
 
 
+def test_rewrites_and_plan_cache_give_the_same_records(kb, vol):
+    """The guarded-root and box-distribution rewrites (on by default) leave every record unchanged: default =
+    each ablation flag = the oracle, on windows of K and T at n = 5 and on all of S4; a second handle over the same
+    bytes takes its plan from the process-wide cache (nothing is compiled) and gives the same records."""
+    extra = ["[]p", "[][]p", "[](p & q)", "[]p & []q", "[][](p -> q) & p", "[]F", "[][]F", "[]([]p & q)",
+             "[]([]F | p)", "[]p & ([]q & ~[](p & q))", "[](p & []q) -> [](q & []p)", "[](p & q & []p)", "[][][]q"]
+    progs = W.corpus_c2(5624)[::13] + [W.to_postfix(W.parse(t)) for t in extra]
+    code, offs = W.pack_programs(progs)
+    h = kb.Programs(code, offs, 2)
+    for cls, begin, count in ((K, 1024 * 77, 2048), (T, 1024 * 3, 2048), (S4, 0, 6942)):
+        want = vol.census(code, offs, 5, 2, cls, begin, count)
+        same(scan(kb, h, 5, 2, cls, begin, count), want, f"default cls={cls}")
+        assert h.last_run_info().kernel_family == 2
+        ops = h.last_run_info().logic_instr_per_frame
+        for fl in (kb.NO_GUARDED_ROOTS, kb.NO_BOX_DISTRIBUTION, kb.NO_GUARDED_ROOTS | kb.NO_BOX_DISTRIBUTION):
+            same(scan(kb, h, 5, 2, cls, begin, count, fl), want, f"flags={fl} cls={cls}")
+        assert h.last_run_info().logic_instr_per_frame > ops          # the rewrites do remove work
+    h2 = kb.Programs(code, offs, 2)
+    got = scan(kb, h2, 5, 2, K, 1024 * 77, 2048)
+    assert h2.last_run_info().jit_compile_seconds == 0.0
+    same(got, vol.census(code, offs, 5, 2, K, 1024 * 77, 2048), "plan from the cache")
+
+
 def test_compiled_pairs_equal_oracle(kb, vol):
     progs, pairs, _ = W.pairs_c5(400)
     pairs = np.array(pairs, np.uint32)
