@@ -621,7 +621,7 @@ struct JitGroupHost {
 
 // Where a record went, and the variable order it is evaluated under (host checks only).
 struct JitRecordInfo {
-    uint32_t group = 0, slot = 0, support = 0;
+    uint32_t group = 0, slot = 0, support = 0, neg = 0;
     uint8_t rename[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
 };
 
@@ -639,6 +639,15 @@ int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t 
     out->resize(k + 1);
     for (uint32_t g = 0; g <= k; ++g) (*out)[g].g = g;
     std::vector<Dag> probe(k + 1);       // unsalted graphs: which records are the same program
+    // per group: which of its variables change inside a thread's word loop on the group's layout
+    std::vector<uint32_t> loop_vars(k + 1, 0);
+    for (uint32_t g = 0; g <= k; ++g) {
+        JitLayout lay;
+        if (!(mode == JIT_MODE_DENSITY ? jit_density_layout(n, g, cls, &lay) : jit_layout(n, g, cls, &lay))) continue;
+        for (uint32_t v = 0; v < g; ++v)
+            for (uint32_t w = 0; w < n; ++w)
+                if (jit_atom_level(lay, v, w) > 0) loop_vars[g] |= 1u << v;
+    }
     std::vector<std::map<std::pair<uint32_t, uint32_t>, uint32_t>> seen(k + 1);
     if (info_out) info_out->assign(n_records, JitRecordInfo());
     for (uint32_t r = 0; r < n_records; ++r) {
@@ -657,24 +666,26 @@ int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t 
         if (!layout_ok(g)) return KRIPKE_EUNSUPPORTED;
         JitGroupHost &G = (*out)[g];
         uint8_t rename[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
+        uint32_t neg = 0;
         if (flags & KRIPKE_NO_SHARING) {                 // variables in their own order, nothing shared
             uint8_t next = 0;
             for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v)
                 if ((sup >> v) & 1u) rename[v] = next++;
         } else {
-            canonical_rename(prog(fa), plen(fa), pairs ? prog(fb) : nullptr, pairs ? plen(fb) : 0u, sup, rename);
+            canonical_rename(prog(fa), plen(fa), pairs ? prog(fb) : nullptr, pairs ? plen(fb) : 0u, sup, n, loop_vars[g], rename, &neg);
         }
         if (info_out) {
             JitRecordInfo &ri = (*info_out)[r];
             ri.group = g;
             ri.support = sup;
+            ri.neg = neg;
             for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v) ri.rename[v] = rename[v];
             ri.slot = (uint32_t)G.roots.size();
         }
         if (!(flags & KRIPKE_NO_SHARING) && mode != JIT_MODE_DENSITY) {
             // records whose graphs coincide are scanned once (the pair path is symmetric in its two formulas)
-            uint32_t pa = probe[g].build(prog(fa), plen(fa), rename);
-            uint32_t pb = pairs ? probe[g].build(prog(fb), plen(fb), rename) : UINT32_MAX;
+            uint32_t pa = probe[g].build(prog(fa), plen(fa), rename, neg);
+            uint32_t pb = pairs ? probe[g].build(prog(fb), plen(fb), rename, neg) : UINT32_MAX;
             if (pairs && pb < pa) std::swap(pa, pb);
             auto it = seen[g].find(std::make_pair(pa, pb));
             if (it != seen[g].end()) {
@@ -686,8 +697,8 @@ int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t 
         }
         G.dag.salt = (flags & (KRIPKE_NO_SHARING | KRIPKE_NO_SUBTERM_SHARING)) ? r + 1 : 0u;
         JitRoot root;
-        root.a = G.dag.build(prog(fa), plen(fa), rename);
-        root.b = pairs ? G.dag.build(prog(fb), plen(fb), rename) : UINT32_MAX;
+        root.a = G.dag.build(prog(fa), plen(fa), rename, neg);
+        root.b = pairs ? G.dag.build(prog(fb), plen(fb), rename, neg) : UINT32_MAX;
         G.roots.push_back(root);
         G.slot_record.push_back(r);
     }
@@ -1496,7 +1507,7 @@ int kripke_debug_jit_source(const uint8_t *code, const uint32_t *offsets, uint32
             parts.back().push_back(r);
         }
     } else {
-        parts = jit_partition(G.dag, G.roots, n_worlds, g_jit_max_programs);
+        parts = jit_partition(G.dag, G.roots, lay, g_jit_max_programs);
     }
     if (n_kernels_out) *n_kernels_out = (uint32_t)parts.size();
     if (logic_ops_per_word_out) *logic_ops_per_word_out = 0;
@@ -1544,7 +1555,7 @@ int kripke_debug_batch_refuted(const uint8_t *code, const uint32_t *offsets, uin
         const JitRecordInfo &ri = info[r];
         uint32_t pv[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
         for (uint32_t v = 0; v < n_vars; ++v)
-            if ((ri.support >> v) & 1u) pv[ri.rename[v]] = val[v];
+            if ((ri.support >> v) & 1u) pv[ri.rename[v]] = ((ri.neg >> v) & 1u) ? ~val[v] : val[v];
         const JitGroupHost &G = groups[ri.group];
         refuted_out[r] = jit_root_refuted(G.dag, G.roots[ri.slot], n_worlds, succ, pv) ? 1 : 0;
     }
@@ -1564,7 +1575,7 @@ int kripke_debug_dag_truth(const uint8_t *code, uint32_t len, uint32_t n_vars, u
         Dag sd;
         sup = sd.support(sd.build(code, len, nullptr));
     }
-    canonical_rename(code, len, nullptr, 0, sup, rename);
+    canonical_rename(code, len, nullptr, 0, sup, n_worlds, 0, rename);
     uint32_t pv[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
     for (uint32_t v = 0; v < n_vars; ++v)
         if ((sup >> v) & 1u) pv[rename[v]] = val[v];

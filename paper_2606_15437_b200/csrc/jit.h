@@ -42,8 +42,9 @@ struct Dag {
     uint32_t lit_var(uint32_t i);
     uint32_t mk_and(uint32_t x, uint32_t y);
     uint32_t mk_box(uint32_t x);
-    // Postfix program -> literal.  rename: variable index -> index in the group's valuation.
-    uint32_t build(const uint8_t *code, uint32_t len, const uint8_t *rename);
+    // Postfix program -> literal.  rename: variable index -> index in the group's valuation; neg_mask: bit v =
+    // variable v (as written) is read complemented.
+    uint32_t build(const uint8_t *code, uint32_t len, const uint8_t *rename, uint32_t neg_mask = 0);
     // Variables a literal's cone mentions (bit i).
     uint32_t support(uint32_t lit) const;
     // Truth set (n-bit mask) of a literal on one model: succ[w] successor masks, val[i] variable masks.
@@ -63,11 +64,18 @@ struct Dag {
     std::map<std::array<uint32_t, 5>, uint32_t> index_;
 };
 
-// Canonical variable order of one program (or pair): the permutation of the variables it mentions
-// under which its graph has the least canonical text; alpha-equivalent programs get the same graph.
-// support_mask: variables mentioned; rename_out[v] = index in the reduced valuation (g = popcount).
+// Canonical variable order of one program (or pair): among the permutations of the variables it mentions, the one
+// whose graph does the least work inside the loops (loop_var_mask: bit i = renamed variable i changes inside a
+// thread's word loop on the layout in use; a subterm over the other variables is evaluated once per unit), ties
+// broken by the least canonical text.  The choice depends on the alpha-equivalence class only, so alpha-equivalent
+// programs get the same graph.  support_mask: variables mentioned; rename_out[v] = index in the reduced valuation.
+// neg_out (may be null): also the variables to complement - v -> v XOR (the worlds of p_i) is a bijection of the
+// valuations of every frame, so phi(p) and phi(~p) have the same refuting-model and refuting-frame counts, the
+// same first refuting frame and the same failure densities; with neg_out the canonical form is taken over
+// permutations and complementations, and more programs of a batch coincide.
 void canonical_rename(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b,
-                      uint32_t support_mask, uint8_t *rename_out);
+                      uint32_t support_mask, uint32_t n, uint32_t loop_var_mask, uint8_t *rename_out,
+                      uint32_t *neg_out = nullptr);
 
 // ---- cost-driven redistribution of box over conjunction (jit_opt.cpp) -------------------------------
 struct JitLayout;
@@ -163,7 +171,10 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
 
 // Partition of the roots into kernels of at most `max_roots` that share as many subterms as possible.
 std::vector<std::vector<uint32_t>> jit_partition(const Dag &dag, const std::vector<JitRoot> &roots,
-                                                 uint32_t n, uint32_t max_roots);
+                                                 const JitLayout &lay, uint32_t max_roots);
+// Logic instructions per 32-model word the emitter generates for every node of the graph on this layout (a node
+// that does not change inside the loops is charged its share of a word).
+std::vector<double> jit_node_costs(const Dag &dag, const JitLayout &lay);
 
 // ---- runtime (jit_runtime.cpp) --------------------------------------------------------------------
 struct JitKernel {

@@ -94,14 +94,15 @@ uint32_t Dag::mk_and(uint32_t x, uint32_t y) {
     return acc;
 }
 
-uint32_t Dag::build(const uint8_t *code, uint32_t len, const uint8_t *rename) {
+uint32_t Dag::build(const uint8_t *code, uint32_t len, const uint8_t *rename, uint32_t neg_mask) {
     std::vector<uint32_t> st;
     for (uint32_t i = 0; i < len; ++i) {
         const uint8_t c = code[i];
         if (c == KRIPKE_OP_TOP) st.push_back(lit_const(true));
         else if (c == KRIPKE_OP_BOT) st.push_back(lit_const(false));
         else if (c >= KRIPKE_OP_VAR0 && c < KRIPKE_OP_VAR0 + KRIPKE_MAX_VARS)
-            st.push_back(lit_var(rename ? rename[c - KRIPKE_OP_VAR0] : (uint32_t)(c - KRIPKE_OP_VAR0)));
+            st.push_back(lit_var(rename ? rename[c - KRIPKE_OP_VAR0] : (uint32_t)(c - KRIPKE_OP_VAR0)) ^
+                         ((neg_mask >> (c - KRIPKE_OP_VAR0)) & 1u));
         else if (c == KRIPKE_OP_NOT) st.back() ^= 1u;
         else if (c == KRIPKE_OP_BOX) st.back() = mk_box(st.back());
         else if (c == KRIPKE_OP_DIA) st.back() = mk_box(st.back() ^ 1u) ^ 1u;
@@ -164,8 +165,30 @@ std::string Dag::text(uint32_t lit) const {
     }
 }
 
+namespace {
+
+// Work a literal's cone does inside the loops: box n*n, conjunction n, for the nodes that mention a loop variable.
+// `value`: false while still inside the positive conjunctions and boxes at the top of a single formula, which the
+// guarded form never evaluates (jit.h).
+void loop_cost(const Dag &d, uint32_t lit, bool value, uint32_t n, uint32_t loop_var_mask, std::vector<char> *seen, uint64_t *cost) {
+    const DagNode &nd = d.nodes[lit >> 1];
+    if (nd.kind != DagNode::AND && nd.kind != DagNode::BOX) return;
+    if (!value && !(lit & 1u)) {
+        loop_cost(d, nd.a, false, n, loop_var_mask, seen, cost);
+        if (nd.kind == DagNode::AND) loop_cost(d, nd.b, false, n, loop_var_mask, seen, cost);
+        return;
+    }
+    if ((*seen)[lit >> 1]) return;
+    (*seen)[lit >> 1] = 1;
+    if (d.support(lit) & loop_var_mask) *cost += nd.kind == DagNode::BOX ? n * n : n;
+    loop_cost(d, nd.a, true, n, loop_var_mask, seen, cost);
+    if (nd.kind == DagNode::AND) loop_cost(d, nd.b, true, n, loop_var_mask, seen, cost);
+}
+
+}  // namespace
+
 void canonical_rename(const uint8_t *code_a, uint32_t len_a, const uint8_t *code_b, uint32_t len_b,
-                      uint32_t support_mask, uint8_t *rename_out) {
+                      uint32_t support_mask, uint32_t n, uint32_t loop_var_mask, uint8_t *rename_out, uint32_t *neg_out) {
     uint8_t vars[KRIPKE_MAX_VARS];
     uint32_t g = 0;
     for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v) {
@@ -174,21 +197,40 @@ void canonical_rename(const uint8_t *code_a, uint32_t len_a, const uint8_t *code
     }
     uint8_t perm[KRIPKE_MAX_VARS] = {0, 1, 2, 3};
     std::string best;
+    uint64_t best_cost = 0;
     bool have = false;
+    if (neg_out) *neg_out = 0;
     do {
+      for (uint32_t pol = 0; pol < (neg_out ? 1u << g : 1u); ++pol) {
         uint8_t rn[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
-        for (uint32_t i = 0; i < g; ++i) rn[vars[i]] = perm[i];
-        Dag d;
-        std::string t = d.text(d.build(code_a, len_a, rn));
-        if (code_b) {
-            const std::string tb = d.text(d.build(code_b, len_b, rn));
-            t = (t < tb) ? t + "#" + tb : tb + "#" + t;
+        uint32_t neg = 0;
+        for (uint32_t i = 0; i < g; ++i) {
+            rn[vars[i]] = perm[i];
+            if ((pol >> i) & 1u) neg |= 1u << vars[i];
         }
-        if (!have || t < best) {
+        Dag d;
+        const uint32_t la = d.build(code_a, len_a, rn, neg);
+        std::string t = d.text(la);
+        uint64_t cost = 0;
+        if (code_b) {
+            const uint32_t lb = d.build(code_b, len_b, rn, neg);
+            const std::string tb = d.text(lb);
+            t = (t < tb) ? t + "#" + tb : tb + "#" + t;
+            std::vector<char> seen(d.nodes.size(), 0);
+            loop_cost(d, la, true, n, loop_var_mask, &seen, &cost);
+            loop_cost(d, lb, true, n, loop_var_mask, &seen, &cost);
+        } else {
+            std::vector<char> seen(d.nodes.size(), 0);
+            loop_cost(d, la, false, n, loop_var_mask, &seen, &cost);
+        }
+        if (!have || cost < best_cost || (cost == best_cost && t < best)) {
             best = t;
+            best_cost = cost;
             have = true;
             for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v) rename_out[v] = rn[v];
+            if (neg_out) *neg_out = neg;
         }
+      }
     } while (std::next_permutation(perm, perm + g));
 }
 

@@ -217,6 +217,108 @@ struct Emitter {
         return leaf(fmt("s%u_%u", d, u), false);
     }
 
+    // conjuncts of a positive conjunction (flattened)
+    void flat_conjuncts(uint32_t l, std::vector<uint32_t> *out) const {
+        const DagNode &nd = dag.nodes[l >> 1];
+        if (!(l & 1u) && nd.kind == DagNode::AND) { flat_conjuncts(nd.a, out); flat_conjuncts(nd.b, out); }
+        else out->push_back(l);
+    }
+    // Conjunction of operands that change at different loop levels: the operands of the lower levels are folded
+    // first and become a value of their own at that level, so the inner loop only pays for what changes in it.
+    int and_by_level(std::vector<std::pair<int, int>> items, int *level_out) {
+        std::stable_sort(items.begin(), items.end(), [](const std::pair<int, int> &x, const std::pair<int, int> &y) { return x.first < y.first; });
+        int acc = constant(true), L = 0, leaves = 0;
+        for (const auto &it : items) {
+            if (it.first > L && leaves >= 2 && pool[acc].op != Ex::CONST && pool[acc].op != Ex::LEAF) {
+                const std::string name = fmt("y%u", n_tmp++);
+                stmts.push_back(Stmt{L, name, acc, ""});
+                acc = leaf(name, false);
+                leaves = 1;
+            }
+            L = std::max(L, it.first);
+            acc = bin(Ex::AND, acc, it.second);
+            ++leaves;
+        }
+        *level_out = L;
+        return acc;
+    }
+    // fail word of one obligation: OR_u ( S_depth[u] & ~lit[u] )
+    std::map<std::pair<uint32_t, uint32_t>, std::string> obligation_name;
+    std::vector<uint32_t> value_uses;       // readers of every node's value other than guarded obligations that fold it themselves
+    void count_uses(const std::vector<JitRoot> &roots) {
+        value_uses.assign(dag.nodes.size(), 0);
+        std::vector<char> seen(dag.nodes.size(), 0);
+        std::vector<uint32_t> stack;
+        auto visit = [&](uint32_t l) { if (!seen[l >> 1]) { seen[l >> 1] = 1; stack.push_back(l >> 1); } };
+        auto ref = [&](uint32_t l) { ++value_uses[l >> 1]; visit(l); };
+        for (const JitRoot &r : roots) {
+            if (r.guarded.empty()) { r.for_each_lit(ref); continue; }
+            for (const JitGuarded &g : r.guarded) {
+                const bool folds = g.depth > 0 && lay.cls == KRIPKE_CLASS_K && (g.lit & 1u) && dag.nodes[g.lit >> 1].kind == DagNode::AND;
+                if (!folds) { ref(g.lit); continue; }
+                std::vector<uint32_t> conj;
+                flat_conjuncts(g.lit ^ 1u, &conj);
+                for (uint32_t c : conj) ref(c);
+            }
+        }
+        while (!stack.empty()) {
+            const DagNode &nd = dag.nodes[stack.back()];
+            stack.pop_back();
+            if (nd.kind == DagNode::AND) { ref(nd.a); ref(nd.b); }
+            else if (nd.kind == DagNode::BOX) ref(nd.a);
+        }
+    }
+    int obligation(const JitGuarded &g) {
+        const auto key = std::make_pair(g.depth, g.lit);
+        auto it = obligation_name.find(key);
+        if (it == obligation_name.end()) {
+            const bool guarded = g.depth > 0 && lay.cls == KRIPKE_CLASS_K;
+            // ~lit is a conjunction: S & x & y is folded by loop level (the guard and the in-word variable do not
+            // change inside the loops)
+            std::vector<uint32_t> conj;
+            // (only when nothing else reads the conjunction's value)
+            if (guarded && (g.lit & 1u) && dag.nodes[g.lit >> 1].kind == DagNode::AND) {
+                flat_conjuncts(g.lit ^ 1u, &conj);
+                for (uint32_t c : conj) node(c >> 1);
+                // where another reader needs the conjunction's value anyway, fold only if at most one conjunct
+                // changes in the innermost loop (the fold then costs no more than reading that value)
+                if (!value_uses.empty() && value_uses[g.lit >> 1] > 0) {
+                    int top = 0, at_top = 0;
+                    for (uint32_t c : conj)
+                        for (uint32_t u = 0; u < lay.n; ++u) top = std::max(top, lit_level(c, u));
+                    for (uint32_t c : conj) {
+                        int lc = 0;
+                        for (uint32_t u = 0; u < lay.n; ++u) lc = std::max(lc, lit_level(c, u));
+                        at_top += lc == top;
+                    }
+                    if (at_top > 1) conj.clear();
+                }
+            }
+            if (conj.empty()) node(g.lit >> 1);
+            int L = 0, acc = constant(false);
+            for (uint32_t u = 0; u < lay.n; ++u) {
+                int term, lu = 0;
+                if (conj.empty()) {
+                    term = bin(Ex::AND, guard(g.depth, u), negate(lit(g.lit, u)));
+                    lu = lit_level(g.lit, u);
+                    if (guarded) lu = std::max(lu, (int)guard_lvl[g.depth - 1][u]);
+                } else {
+                    std::vector<std::pair<int, int>> items;
+                    const int gx = guard(g.depth, u);
+                    items.emplace_back((int)guard_lvl[g.depth - 1][u], gx);
+                    for (uint32_t c : conj) items.emplace_back(lit_level(c, u), lit(c, u));
+                    term = and_by_level(items, &lu);
+                }
+                acc = bin(Ex::OR, acc, term);
+                L = std::max(L, lu);
+            }
+            const std::string name = fmt("o%u_%u", g.depth, g.lit);
+            stmts.push_back(Stmt{L, name, acc, ""});
+            it = obligation_name.emplace(key, name).first;
+        }
+        return leaf(it->second, false);
+    }
+
     // ---- single-use substitution ----
     void collect_leaves(int x, std::vector<int> *out) const {
         if (pool[x].op == Ex::LEAF) out->push_back(x);
@@ -397,14 +499,19 @@ bool jit_density_layout(uint32_t n, uint32_t g, uint32_t cls, JitLayout *out) {
 }
 
 std::vector<std::vector<uint32_t>> jit_partition(const Dag &dag, const std::vector<JitRoot> &roots,
-                                                 uint32_t n, uint32_t max_roots) {
+                                                 const JitLayout &lay, uint32_t max_roots) {
+    const uint32_t n = lay.n;
     const size_t R = roots.size();
-    // cone of every root: its AND / BOX nodes, with the cost model of the emitter (box n*n, and n)
+    // cone of every root: its AND / BOX nodes, with the cost model of the emitter (box n*n, and n), and its
+    // obligations (guarded roots: one fail word each, n instructions, shared by the records that carry it)
     std::vector<std::vector<uint32_t>> cone(R);
-    std::vector<uint32_t> cost(dag.nodes.size(), 0);
-    for (size_t i = 0; i < dag.nodes.size(); ++i)
-        cost[i] = dag.nodes[i].kind == DagNode::BOX ? n * n : dag.nodes[i].kind == DagNode::AND ? n : 0;
+    std::vector<uint64_t> cost(dag.nodes.size(), 0);                 // in 1/1024 of an instruction per word
     {
+        const std::vector<double> c = jit_node_costs(dag, lay);
+        for (size_t i = 0; i < dag.nodes.size(); ++i) cost[i] = (uint64_t)(c[i] * 1024.0 + 0.5);
+    }
+    {
+        std::map<std::pair<uint32_t, uint32_t>, uint32_t> obligation_id;
         std::vector<uint32_t> stamp(dag.nodes.size(), UINT32_MAX), stack;
         for (size_t r = 0; r < R; ++r) {
             stack.clear();
@@ -417,16 +524,24 @@ std::vector<std::vector<uint32_t>> jit_partition(const Dag &dag, const std::vect
                 if (nd.kind == DagNode::AND) { cone[r].push_back(id); stack.push_back(nd.a >> 1); stack.push_back(nd.b >> 1); }
                 else if (nd.kind == DagNode::BOX) { cone[r].push_back(id); stack.push_back(nd.a >> 1); }
             }
+            for (const JitGuarded &g : roots[r].guarded) {
+                auto it = obligation_id.find(std::make_pair(g.depth, g.lit));
+                if (it == obligation_id.end()) {
+                    it = obligation_id.emplace(std::make_pair(g.depth, g.lit), (uint32_t)cost.size()).first;
+                    cost.push_back((uint64_t)n * 1024u);
+                }
+                cone[r].push_back(it->second);
+            }
         }
     }
-    auto total = [&](size_t r) { uint32_t c = 0; for (uint32_t id : cone[r]) c += cost[id]; return c; };
+    auto total = [&](size_t r) { uint64_t c = 0; for (uint32_t id : cone[r]) c += cost[id]; return c; };
     std::vector<std::vector<uint32_t>> groups;
-    std::vector<char> left(R, 1), in_union(dag.nodes.size(), 0);
+    std::vector<char> left(R, 1), in_union(cost.size(), 0);
     size_t n_left = R;
     while (n_left) {
         // seed: the most expensive root left; then repeatedly the root that adds the least new work
         size_t seed = R;
-        uint32_t seed_cost = 0;
+        uint64_t seed_cost = 0;
         for (size_t r = 0; r < R; ++r)
             if (left[r] && (seed == R || total(r) > seed_cost)) { seed = r; seed_cost = total(r); }
         std::vector<uint32_t> members, touched;
@@ -438,10 +553,10 @@ std::vector<std::vector<uint32_t>> jit_partition(const Dag &dag, const std::vect
         take(seed);
         while (members.size() < max_roots && n_left) {
             size_t best = R;
-            uint32_t best_add = 0;
+            uint64_t best_add = 0;
             for (size_t r = 0; r < R; ++r) {
                 if (!left[r]) continue;
-                uint32_t add = 0;
+                uint64_t add = 0;
                 for (uint32_t id : cone[r]) if (!in_union[id]) add += cost[id];
                 if (best == R || add < best_add) { best = r; best_add = add; if (add == 0) break; }
             }
@@ -627,16 +742,15 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
     else if (lay.inner == 0) fmode = F_WORD;                        // one word per frame
     else fmode = F_ANY;                                             // 2^inner words per frame, several frames per unit
 
+    em.count_uses(roots);
     for (uint32_t r = 0; r < G; ++r) {
         int e;
         if (!roots[r].guarded.empty()) {
             // refuted lanes of a guarded root: some obligation fails at a world of its guard set (jit.h)
+            // Every obligation's fail word is a value of its own: shared by the records of the kernel that carry the
+            // same obligation, and computed once per unit when its literal does not change inside the loops.
             e = em.constant(false);
-            for (const JitGuarded &g : roots[r].guarded) {
-                em.node(g.lit >> 1);
-                for (uint32_t u = 0; u < n; ++u)
-                    e = em.bin(Ex::OR, e, em.bin(Ex::AND, em.guard(g.depth, u), em.negate(em.lit(g.lit, u))));
-            }
+            for (const JitGuarded &g : roots[r].guarded) e = em.bin(Ex::OR, e, em.obligation(g));
         } else if (roots[r].b == UINT32_MAX) {
             em.node(roots[r].a >> 1);
             // refuted lanes: the truth set is not all worlds
@@ -720,6 +834,8 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
     s += fmt("        atomicMin(&a->best, ((u0 + s_best[i]) >> %u) << %u);\n", lay.split, lay.unit_frames_log2);
     s += "      }\n";
     s += "  }\n}\n";
+    s += fmt("// graph nodes evaluated: box=%u and=%u; lop3 per unit=%llu, per outer iteration=%llu, per word=%llu\n", em.n_box,
+             em.n_and, (unsigned long long)em.ops[0], (unsigned long long)em.ops[1], (unsigned long long)em.ops[2]);
     if (stats) {
         const uint64_t *ops = em.ops;
         stats->logic_ops_emitted = ops[0] + ops[1] + ops[2];

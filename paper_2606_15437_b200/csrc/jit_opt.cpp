@@ -233,6 +233,13 @@ void jit_optimize(const Dag &in, const JitLayout &lay, std::vector<JitRoot> *roo
     if (stats) *stats = st;
 }
 
+std::vector<double> jit_node_costs(const Dag &dag, const JitLayout &lay) {
+    Levels lv(lay);
+    std::vector<double> c(dag.nodes.size(), 0.0);
+    for (uint32_t id = 0; id < dag.nodes.size(); ++id) c[id] = lv.cost(dag, id);
+    return c;
+}
+
 // ---- guarded roots (jit.h) -------------------------------------------------------------------------
 namespace {
 

@@ -92,7 +92,7 @@ int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitR
             parts.back().push_back(r);
         }
     } else {
-        parts = jit_partition(dag, roots, lay.n, max_roots);
+        parts = jit_partition(dag, roots, lay, max_roots);
     }
     std::vector<std::string> sources(parts.size());
     std::vector<uint32_t> order;               // slot -> index into roots
