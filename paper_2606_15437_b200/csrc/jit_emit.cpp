@@ -741,6 +741,8 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
     else if (lay.kn < 5) fmode = F_FOLD;                            // several frames per word
     else if (lay.inner == 0) fmode = F_WORD;                        // one word per frame
     else fmode = F_ANY;                                             // 2^inner words per frame, several frames per unit
+    const bool has_f = fmode == F_WORD || fmode == F_ANY || fmode == F_FOLD;
+    const bool packed = lay.inner + lay.outer <= 10;                // models of a unit < 2^16
 
     em.count_uses(roots);
     for (uint32_t r = 0; r < G; ++r) {
@@ -764,10 +766,23 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
             e = em.constant(false);
             for (uint32_t w = 0; w < n; ++w) e = em.bin(Ex::OR, e, em.bin(Ex::XOR, em.lit(roots[r].a, w), em.lit(roots[r].b, w)));
         }
-        std::string tail = fmt("c%u += __popc(r);", r);
-        if (fmode == F_WORD) tail += fmt(" f%u += (r != 0u);", r);
-        else if (fmode == F_ANY) tail += fmt(" a%u |= r;", r);
-        else if (fmode == F_FOLD) tail += fmt(" f%u += kj_frames_in_word<%u>(r);", r, lay.kn);
+        // Counters of a unit are 16-bit fields where they fit (a unit has 2^(5+inner+outer) models): with a frame
+        // count, models in the low half and frames in the high half of one register; without, two programs per
+        // register - half the registers the counters would take.
+        std::string tail;
+        if (!packed) {
+            tail = fmt("c%u += __popc(r);", r);
+            if (fmode == F_WORD) tail += fmt(" f%u += (r != 0u);", r);
+            else if (fmode == F_ANY) tail += fmt(" a%u |= r;", r);
+            else if (fmode == F_FOLD) tail += fmt(" f%u += kj_frames_in_word<%u>(r);", r, lay.kn);
+        } else if (has_f) {
+            tail = fmt("c%u += __popc(r);", r);
+            if (fmode == F_WORD) tail += fmt(" if (r != 0u) c%u += 65536u;", r);
+            else if (fmode == F_ANY) tail += fmt(" a%u |= r;", r);
+            else tail += fmt(" c%u += kj_frames_in_word<%u>(r) << 16;", r, lay.kn);
+        } else {
+            tail = (r & 1u) ? fmt("c%u += __popc(r) << 16;", r >> 1) : fmt("c%u += __popc(r);", r >> 1);
+        }
         em.stmts.push_back(Emitter::Stmt{2, "", e, tail});
     }
     em.emit_all();
@@ -803,8 +818,9 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
     s += decl_unit;
     s += "      // values that are fixed for the unit\n" + em.body[0];
     for (uint32_t r = 0; r < G; ++r) {
+        if (packed && !has_f) { if (!(r & 1u)) s += fmt("      unsigned c%u = 0u;\n", r >> 1); continue; }
         s += fmt("      unsigned c%u = 0u;", r);
-        if (fmode == F_WORD || fmode == F_ANY || fmode == F_FOLD) s += fmt(" unsigned f%u = 0u;", r);
+        if (has_f && !packed) s += fmt(" unsigned f%u = 0u;", r);
         s += "\n";
     }
     s += "#pragma unroll 1\n";
@@ -817,12 +833,14 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
     s += decl_inner;
     s += em.body[2];
     s += "      }\n";
-    if (fmode == F_ANY) for (uint32_t r = 0; r < G; ++r) s += fmt("      f%u += (a%u != 0u);\n", r, r);
+    if (fmode == F_ANY) for (uint32_t r = 0; r < G; ++r) s += packed ? fmt("      if (a%u != 0u) c%u += 65536u;\n", r, r) : fmt("      f%u += (a%u != 0u);\n", r, r);
     s += "      }\n";
     for (uint32_t r = 0; r < G; ++r) {
         const char *fm = fmode == F_MODELS ? "0" : fmode == F_THREAD ? "1" : "2";
-        const std::string f = (fmode == F_MODELS || fmode == F_THREAD) ? "0u" : fmt("f%u", r);
-        s += fmt("      kj_flush<%u, %s>(%uu, c%u, ", lay.split, fm, r, r) + f + ", valid, warp_rel, lane, s_models, s_frames, s_best);\n";
+        std::string c = fmt("c%u", r), f = has_f ? fmt("f%u", r) : std::string("0u");
+        if (packed && has_f) { f = fmt("(c%u >> 16)", r); c = fmt("(c%u & 0xFFFFu)", r); }
+        else if (packed) c = (r & 1u) ? fmt("(c%u >> 16)", r >> 1) : fmt("(c%u & 0xFFFFu)", r >> 1);
+        s += fmt("      kj_flush<%u, %s>(%uu, ", lay.split, fm, r) + c + ", " + f + ", valid, warp_rel, lane, s_models, s_frames, s_best);\n";
     }
     s += "    }\n";
     s += "    __syncthreads();\n";

@@ -32,6 +32,7 @@ struct Module {
     cudaLibrary_t lib = nullptr;
     cudaKernel_t kernel = nullptr;
     int regs = 0;
+    int local_bytes = 0;       // per-thread local memory: nonzero = ptxas spilled registers
 };
 
 std::mutex g_cache_mutex;
@@ -94,61 +95,87 @@ int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitR
     } else {
         parts = jit_partition(dag, roots, lay, max_roots);
     }
-    std::vector<std::string> sources(parts.size());
+    // Emit, compile (what the process has not seen yet, in parallel host threads) and load; a kernel that ptxas
+    // could only fit by spilling registers to local memory is split into two halves and redone.
+    std::vector<std::string> sources;
+    std::vector<JitEmitStats> stats;
+    for (int round = 0;; ++round) {
+        sources.assign(parts.size(), std::string());
+        stats.assign(parts.size(), JitEmitStats());
+        for (size_t i = 0; i < parts.size(); ++i) {
+            std::vector<JitRoot> rs;
+            for (uint32_t r : parts[i]) rs.push_back(roots[r]);
+            sources[i] = jit_emit_kernel(dag, lay, rs, out->threads, min_blocks, mode, &stats[i]);
+        }
+        std::vector<size_t> todo;
+        {
+            std::lock_guard<std::mutex> lock(g_cache_mutex);
+            for (size_t i = 0; i < sources.size(); ++i)
+                if (!g_cache.count(sources[i]) &&
+                    std::find_if(todo.begin(), todo.end(), [&](size_t j) { return sources[j] == sources[i]; }) == todo.end())
+                    todo.push_back(i);
+        }
+        std::vector<std::vector<char>> cubins(todo.size());
+        std::vector<int> rcs(todo.size(), 0);
+        std::vector<std::string> logs(todo.size());
+        {
+            std::atomic<size_t> next{0};
+            const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
+            const size_t n_threads = std::min<size_t>(todo.size(), hw);
+            std::vector<std::thread> pool;
+            auto work = [&]() {
+                for (size_t t = next++; t < todo.size(); t = next++) rcs[t] = compile(sources[todo[t]], &cubins[t], &logs[t]);
+            };
+            for (size_t t = 1; t < n_threads; ++t) pool.emplace_back(work);
+            if (n_threads) work();
+            for (auto &th : pool) th.join();
+        }
+        for (size_t t = 0; t < todo.size(); ++t)
+            if (rcs[t]) {
+                if (log_out) *log_out = logs[t];
+                return rcs[t];
+            }
+        bool split = false;
+        {
+            std::lock_guard<std::mutex> lock(g_cache_mutex);
+            for (size_t t = 0; t < todo.size(); ++t) {
+                Module m;
+                cudaError_t e = cudaLibraryLoadData(&m.lib, cubins[t].data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+                if (e == cudaSuccess) e = cudaLibraryGetKernel(&m.kernel, m.lib, "kripke_jit_scan");
+                cudaFuncAttributes attr;
+                if (e == cudaSuccess) e = cudaFuncGetAttributes(&attr, (const void *)m.kernel);
+                if (e != cudaSuccess) return (int)e;
+                m.regs = attr.numRegs;
+                m.local_bytes = (int)attr.localSizeBytes;
+                g_cache.emplace(sources[todo[t]], m);
+            }
+            if (mode != JIT_MODE_DENSITY && round < 4) {
+                std::vector<std::vector<uint32_t>> next_parts;
+                for (size_t i = 0; i < parts.size(); ++i) {
+                    if (g_cache[sources[i]].local_bytes > 0 && parts[i].size() >= 16) {
+                        const size_t half = parts[i].size() / 2;
+                        next_parts.emplace_back(parts[i].begin(), parts[i].begin() + half);
+                        next_parts.emplace_back(parts[i].begin() + half, parts[i].end());
+                        split = true;
+                    } else {
+                        next_parts.push_back(parts[i]);
+                    }
+                }
+                if (split) parts.swap(next_parts);
+            }
+        }
+        if (!split) break;
+    }
     std::vector<uint32_t> order;               // slot -> index into roots
-    for (size_t i = 0; i < parts.size(); ++i) {
-        std::vector<JitRoot> rs;
-        for (uint32_t r : parts[i]) { rs.push_back(roots[r]); order.push_back(r); }
-        JitEmitStats st;
-        sources[i] = jit_emit_kernel(dag, lay, rs, out->threads, min_blocks, mode, &st);
-        out->stats.logic_ops_per_word += st.logic_ops_per_word;
-        out->stats.logic_ops_emitted += st.logic_ops_emitted;
-        out->stats.n_box += st.n_box;
-        out->stats.n_and += st.n_and;
-    }
-    // compile what the process has not seen yet, in parallel host threads
-    std::vector<size_t> todo;
     {
         std::lock_guard<std::mutex> lock(g_cache_mutex);
-        for (size_t i = 0; i < sources.size(); ++i)
-            if (!g_cache.count(sources[i]) &&
-                std::find_if(todo.begin(), todo.end(), [&](size_t j) { return sources[j] == sources[i]; }) == todo.end())
-                todo.push_back(i);
-    }
-    std::vector<std::vector<char>> cubins(todo.size());
-    std::vector<int> rcs(todo.size(), 0);
-    std::vector<std::string> logs(todo.size());
-    {
-        std::atomic<size_t> next{0};
-        const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
-        const size_t n_threads = std::min<size_t>(todo.size(), hw);
-        std::vector<std::thread> pool;
-        auto work = [&]() {
-            for (size_t t = next++; t < todo.size(); t = next++) rcs[t] = compile(sources[todo[t]], &cubins[t], &logs[t]);
-        };
-        for (size_t t = 1; t < n_threads; ++t) pool.emplace_back(work);
-        if (n_threads) work();
-        for (auto &th : pool) th.join();
-    }
-    for (size_t t = 0; t < todo.size(); ++t)
-        if (rcs[t]) {
-            if (log_out) *log_out = logs[t];
-            return rcs[t];
-        }
-    {
-        std::lock_guard<std::mutex> lock(g_cache_mutex);
-        for (size_t t = 0; t < todo.size(); ++t) {
-            Module m;
-            cudaError_t e = cudaLibraryLoadData(&m.lib, cubins[t].data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
-            if (e == cudaSuccess) e = cudaLibraryGetKernel(&m.kernel, m.lib, "kripke_jit_scan");
-            cudaFuncAttributes attr;
-            if (e == cudaSuccess) e = cudaFuncGetAttributes(&attr, (const void *)m.kernel);
-            if (e != cudaSuccess) return (int)e;
-            m.regs = attr.numRegs;
-            g_cache.emplace(sources[todo[t]], m);
-        }
         uint32_t base = 0;
         for (size_t i = 0; i < parts.size(); ++i) {
+            for (uint32_t r : parts[i]) order.push_back(r);
+            out->stats.logic_ops_per_word += stats[i].logic_ops_per_word;
+            out->stats.logic_ops_emitted += stats[i].logic_ops_emitted;
+            out->stats.n_box += stats[i].n_box;
+            out->stats.n_and += stats[i].n_and;
             JitKernel k;
             k.kernel = (void *)g_cache[sources[i]].kernel;
             k.slot_base = base;
