@@ -31,7 +31,7 @@ import workloads as W  # noqa: E402
 
 CLASSES = (("K", 0), ("T", 1), ("S4", 2), ("S5", 3))
 N_WORLDS, N_VARS = 5, 2
-NCU_TRAFFIC_BYTES = None                     # class-K launches of one step, set from profiles/r2_jit_launches_c3.md
+NCU_TRAFFIC_BYTES = 3176192                  # class-K launches of one step, from profiles/r2_jit_launches_c3.md
 SM_COUNT, INT_LANES_PER_SM = 148, 64       # 4 sub-partitions x 16 lanes/clk on the ALU pipe (B300_MICROARCH.md)
 
 
@@ -245,7 +245,8 @@ def run_ours(args):
 
     # calibration: the measured integer-pipe rate, right before the timed runs
     cal = {}
-    for variant, name in ((0, "lop3"), (1, "iadd3"), (2, "shf"), (3, "lop3+imad")):
+    for variant, name in ((0, "lop3"), (1, "iadd3"), (2, "shf"), (3, "lop3+imad"), (4, "lop3_with_1_popc_per_8"),
+                          (5, "lop3_with_2_popc_per_8")):
         cal[name] = kb.calibrate_int32(variant)[0]
 
     t_first = time.perf_counter()
@@ -734,8 +735,10 @@ def run_atlas(args):
         "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": "kripke_jit_scan, density mode, one frame per lane (class K, n=5, no variables)",
                      "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm, "peak_source": peak_src,
-                     "algorithmic_bytes": nbytes, "traffic": None,
-                     "traffic_source": "ncu dram__bytes_write.sum: profiles/r2_atlas.md",
+                     "algorithmic_bytes": nbytes, "traffic": 8471674000,
+                     "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum of the two density kernels of one pass: "
+                                       "profiles/r2_atlas_full.md (the tail of the last rows is still in the 126 MB L2 when the "
+                                       "kernel ends)",
                      "logic_instr_per_s": info.logic_instr_per_frame * frames / t_write,
                      "frac_of_alu_peak": info.logic_instr_per_frame * frames / t_write / alu_peak},
     }))

@@ -390,7 +390,9 @@ int kripke_debug_dag_truth(const uint8_t *code, uint32_t len, uint32_t n_vars, u
 /* Integer-pipe calibration ("source-level uint32 XOR/AND/OR" re-done as an instruction
  * rate): runs a register-resident loop of independent 3-input logic instructions on every SM and
  * reports executed thread-instructions per second.  variant: 0 = LOP3 only, 1 = IADD3 only,
- * 2 = SHF only, 3 = LOP3 interleaved with IMAD (reports LOP3+IMAD).  Synchronous. */
+ * 2 = SHF only, 3 = LOP3 interleaved with IMAD (reports LOP3+IMAD), 4 / 5 = LOP3 with one / two population
+ * counts (each added to a counter with an IMAD) per eight logic instructions - the census loop's own mix; these
+ * two report the LOP3 rate alone, so the cost of a POPC shows as the drop against variant 0.  Synchronous. */
 int kripke_calibrate_int32(uint32_t variant, double *thread_instr_per_s_out, double *elapsed_ms_out,
                            void *stream);
 

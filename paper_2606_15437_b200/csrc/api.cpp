@@ -682,8 +682,9 @@ int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t 
             for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v) ri.rename[v] = rename[v];
             ri.slot = (uint32_t)G.roots.size();
         }
-        if (!(flags & KRIPKE_NO_SHARING) && mode != JIT_MODE_DENSITY) {
-            // records whose graphs coincide are scanned once (the pair path is symmetric in its two formulas)
+        if (!(flags & KRIPKE_NO_SHARING)) {
+            // records whose graphs coincide are scanned once (the pair path is symmetric in its two formulas;
+            // density mode: the representative's row is copied)
             uint32_t pa = probe[g].build(prog(fa), plen(fa), rename, neg);
             uint32_t pb = pairs ? probe[g].build(prog(fb), plen(fb), rename, neg) : UINT32_MAX;
             if (pairs && pb < pa) std::swap(pa, pb);
@@ -1095,6 +1096,12 @@ int kripke_failure_density(const kripke_programs_t *programs, uint32_t n_worlds,
             if ((e = launch_failure_density_records(sj, g.jit.d_slot_record, g.jit.n_slots, counts_out, frame_count,
                                                     sj.frame_begin - frame_begin, stream)))
                 return cuda_fail(e);
+            ++launches;
+        }
+        // formulas whose program is another formula's (equal graphs under the canonical variable order and polarity:
+        // the count of a frame is invariant under both) receive a copy of its row
+        if (g.n_alias) {
+            if ((e = launch_density_alias_rows(counts_out, frame_count, g.d_alias, g.n_alias, stream))) return cuda_fail(e);
             ++launches;
         }
     }
@@ -1587,7 +1594,7 @@ int kripke_debug_dag_truth(const uint8_t *code, uint32_t len, uint32_t n_vars, u
 
 int kripke_calibrate_int32(uint32_t variant, double *thread_instr_per_s_out, double *elapsed_ms_out,
                            void *stream) {
-    if (variant > 3 || !thread_instr_per_s_out) return KRIPKE_EINVAL;
+    if (variant > 5 || !thread_instr_per_s_out) return KRIPKE_EINVAL;
     int e = run_calibration(variant, thread_instr_per_s_out, elapsed_ms_out, stream);
     if (e) return cuda_fail(e);
     return KRIPKE_OK;

@@ -325,6 +325,33 @@ int launch_failure_density_records(const ScanJob &job, const uint32_t *records, 
     return launch_density(job, nullptr, records, n_list, counts_out, row_stride, col_offset, stream);
 }
 
+// One row copy per alias pair (blockIdx.y), 16 bytes per thread where the rows allow it.
+__global__ void density_alias_rows_kernel(uint32_t *counts, uint64_t row_stride, const uint32_t *alias) {
+    const uint32_t *src = counts + (uint64_t)alias[2 * blockIdx.y + 1] * row_stride;
+    uint32_t *dst = counts + (uint64_t)alias[2 * blockIdx.y] * row_stride;
+    const uint64_t step = (uint64_t)gridDim.x * blockDim.x, t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (((row_stride & 3u) | (reinterpret_cast<uintptr_t>(counts) & 15u)) == 0) {
+        const uint4 *s4 = reinterpret_cast<const uint4 *>(src);
+        uint4 *d4 = reinterpret_cast<uint4 *>(dst);
+        for (uint64_t i = t; i < row_stride / 4; i += step) __stcs(d4 + i, __ldcs(s4 + i));
+    } else {
+        for (uint64_t i = t; i < row_stride; i += step) dst[i] = src[i];
+    }
+}
+
+int launch_density_alias_rows(uint32_t *counts, uint64_t row_stride, const uint32_t *alias, uint32_t n_alias, void *stream) {
+    if (n_alias == 0 || row_stride == 0) return 0;
+    const uint64_t want = (row_stride / 4 + 255) / 256;
+    for (uint32_t a0 = 0; a0 < n_alias; a0 += 65535u) {
+        const uint32_t na = n_alias - a0 < 65535u ? n_alias - a0 : 65535u;
+        dim3 grid((unsigned)(want < 1 ? 1 : want > 1024 ? 1024 : want), na);
+        density_alias_rows_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(counts, row_stride, alias + 2 * (size_t)a0);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return (int)e;
+    }
+    return 0;
+}
+
 int launch_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words, const uint32_t *library,
                          uint32_t n_library, uint32_t *match_out, void *stream) {
     if (n_records == 0) return 0;

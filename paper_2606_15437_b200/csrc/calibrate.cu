@@ -29,11 +29,15 @@ __global__ void __launch_bounds__(CAL_THREADS) calib_kernel(uint32_t *out, uint3
 #pragma unroll
             for (int j = 0; j < CAL_CHAINS; ++j) {
                 const uint32_t a = x[(j + 1) % CAL_CHAINS], b = x[(j + 3) % CAL_CHAINS];
-                if (VARIANT == 0 || VARIANT == 3) {
+                if (VARIANT == 0 || VARIANT == 3 || VARIANT == 4 || VARIANT == 5) {
                     if (j & 1) asm volatile("lop3.b32 %0, %0, %1, %2, 0xE8;" : "+r"(x[j]) : "r"(a), "r"(b));
                     else asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(x[j]) : "r"(a), "r"(b));
                     if (VARIANT == 3)
                         asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(y[j]) : "r"(y[(j + 1) % CAL_CHAINS]), "r"(y[(j + 3) % CAL_CHAINS]));
+                    // the census loop's own mix: one (variant 4) or two (variant 5) population counts, each added to
+                    // a counter on the FMA pipe, per eight logic instructions
+                    if ((VARIANT == 4 && j == 7) || (VARIANT == 5 && (j & 3) == 3))
+                        asm volatile("{ .reg .u32 t; popc.b32 t, %1; mad.lo.u32 %0, t, %2, %0; }" : "+r"(y[j]) : "r"(x[j]), "r"(shift));
                 } else if (VARIANT == 1) {
                     asm volatile("{ .reg .u32 t; add.u32 t, %0, %1; add.u32 %0, t, %2; }" : "+r"(x[j]) : "r"(a), "r"(b));
                 } else {
@@ -72,7 +76,9 @@ int run_calibration(uint32_t variant, double *rate_out, double *ms_out, void *st
         case 0: calib_kernel<0><<<blocks, CAL_THREADS, 0, stream>>>(out, 12345u + rep, 7u, iters); break;
         case 1: calib_kernel<1><<<blocks, CAL_THREADS, 0, stream>>>(out, 12345u + rep, 7u, iters); break;
         case 2: calib_kernel<2><<<blocks, CAL_THREADS, 0, stream>>>(out, 12345u + rep, 7u, iters); break;
-        default: calib_kernel<3><<<blocks, CAL_THREADS, 0, stream>>>(out, 12345u + rep, 7u, iters); break;
+        case 3: calib_kernel<3><<<blocks, CAL_THREADS, 0, stream>>>(out, 12345u + rep, 7u, iters); break;
+        case 4: calib_kernel<4><<<blocks, CAL_THREADS, 0, stream>>>(out, 12345u + rep, 7u, iters); break;
+        default: calib_kernel<5><<<blocks, CAL_THREADS, 0, stream>>>(out, 12345u + rep, 7u, iters); break;
         }
         cudaEventRecord(t1, stream);
         e = cudaEventSynchronize(t1);
@@ -87,6 +93,7 @@ int run_calibration(uint32_t variant, double *rate_out, double *ms_out, void *st
     if (e != cudaSuccess) return (int)e;
     e = cudaGetLastError();
     if (e != cudaSuccess) return (int)e;
+    // variants 4 / 5 report the LOGIC instructions only: what a POPC costs shows as the drop against variant 0
     const double per_thread = (double)iters * CAL_UNROLL * CAL_CHAINS * (variant == 3 ? 2.0 : 1.0);
     const double total = per_thread * (double)blocks * CAL_THREADS;
     if (ms_out) *ms_out = best;
