@@ -682,9 +682,10 @@ int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t 
             for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v) ri.rename[v] = rename[v];
             ri.slot = (uint32_t)G.roots.size();
         }
-        if (!(flags & KRIPKE_NO_SHARING)) {
+        if (!(flags & KRIPKE_NO_SHARING) && (mode != JIT_MODE_DENSITY || g > 0)) {
             // records whose graphs coincide are scanned once (the pair path is symmetric in its two formulas;
-            // density mode: the representative's row is copied)
+            // density mode: the representative's row is copied - except with no variable, where a row is written
+            // at the HBM rate and recomputing it is cheaper than the copy's read + write)
             uint32_t pa = probe[g].build(prog(fa), plen(fa), rename, neg);
             uint32_t pb = pairs ? probe[g].build(prog(fb), plen(fb), rename, neg) : UINT32_MAX;
             if (pairs && pb < pa) std::swap(pa, pb);

@@ -319,6 +319,27 @@ def test_c_invariants(vol):
     assert (w3["models"] == 3 * w1["models"]).all() and (w3["frames"] == 3 * w1["frames"]).all()
 
 
+def test_c_variable_complementation_invariance(vol):
+    """v -> v XOR (worlds of p_i) is a bijection of the valuations of every frame, so phi(p, q), phi(~p, q) and
+    phi(~p, ~q) have the same refuting-model count, refuting-frame count, first refuting frame and per-frame
+    failure counts (what the CUDA path's canonical polarity relies on); the first valuation differs."""
+    neg = lambda t, m: (("not", t) if (m >> t[1]) & 1 else t) if t[0] == "var" else (t[0],) + tuple(neg(c, m) for c in t[1:])
+    sub = [W.from_postfix(c) for c in W.corpus_c2(400)[100:160]]
+    progs = []
+    for t in sub:
+        progs += [W.to_postfix(t), W.to_postfix(neg(t, 1)), W.to_postfix(neg(t, 2)), W.to_postfix(neg(t, 3))]
+    code, offs = W.pack_programs(progs)
+    for n, cls in ((3, K), (4, T), (4, S4)):
+        r = vol.census(code, offs, n, 2, cls)
+        for key in ("models", "frames", "wit_f"):
+            a = r[key].reshape(-1, 4)
+            assert (a == a[:, :1]).all(), (n, cls, key)
+        fc = vol.failure_counts(code, offs, n, 2, cls).reshape(len(sub), 4, -1)
+        assert (fc == fc[:, :1, :]).all()
+    v = vol.census(code, offs, 3, 2, K)["wit_v"].reshape(-1, 4)
+    assert (v != v[:, :1]).any()
+
+
 def test_c_filter_consistency(vol):
     """Counting over the class enumerator = counting over K restricted to class members."""
     c2 = W.corpus_c2(200)
