@@ -53,16 +53,19 @@ struct HostPlan {
     uint64_t n_modal = 0, n_bool = 0;
 };
 
-void build_plan(const std::vector<Lowered> &low, const std::vector<bool> &fits, HostPlan *hp) {
+// skip (may be null): records that are not scanned at all (their program is another record's)
+void build_plan(const std::vector<Lowered> &low, const std::vector<bool> &fits, HostPlan *hp,
+                const std::vector<bool> *skip = nullptr) {
+    auto skipped = [&](size_t i) { return skip && (*skip)[i]; };
     size_t longest = 1;
     for (size_t i = 0; i < low.size(); ++i)
-        if (fits[i]) longest = std::max(longest, low[i].ucode.size());
+        if (fits[i] && !skipped(i)) longest = std::max(longest, low[i].ucode.size());
     hp->stride = (uint32_t)((longest + 1 + 1) / 2 * 2);        // one spare entry after FIN (prefetch)
     for (size_t i = 0; i < low.size(); ++i)
-        if (!fits[i]) hp->unfit.push_back((uint32_t)i);
+        if (!fits[i] && !skipped(i)) hp->unfit.push_back((uint32_t)i);
     for (int need = 1; need <= UC_DMAX; ++need) {
         for (size_t i = 0; i < low.size(); ++i) {
-            if (!fits[i] || low[i].need != need) continue;
+            if (!fits[i] || skipped(i) || low[i].need != need) continue;
             hp->slot_record.push_back((uint32_t)i);
             size_t at = hp->ucode.size();
             hp->ucode.resize(at + hp->stride, (uint16_t)UC_FIN_ALL);
@@ -78,12 +81,13 @@ struct DevicePlan {
     uint16_t *ucode = nullptr;
     uint32_t *slot_record = nullptr;
     uint32_t *unfit = nullptr;
-    uint32_t n_slots = 0, n_unfit = 0, stride = 2;
+    uint32_t *alias = nullptr;         // frame-list plans: (record, representative) pairs of records not scanned themselves
+    uint32_t n_slots = 0, n_unfit = 0, stride = 2, n_alias = 0;
     uint32_t need_end[UC_DMAX + 1] = {0, 0, 0, 0, 0};
     uint64_t n_modal = 0, n_bool = 0;
     void release() {
-        cudaFree(ucode); cudaFree(slot_record); cudaFree(unfit);
-        ucode = nullptr; slot_record = nullptr; unfit = nullptr; n_slots = n_unfit = 0;
+        cudaFree(ucode); cudaFree(slot_record); cudaFree(unfit); cudaFree(alias);
+        ucode = nullptr; slot_record = nullptr; unfit = nullptr; alias = nullptr; n_slots = n_unfit = n_alias = 0;
     }
 };
 
@@ -244,7 +248,9 @@ struct kripke_programs {
     bool has_last = false;
     DevicePlan list_single;            // frame-list mode: every formula lowered without derived leaves
     bool list_single_built = false;
-    DevicePlan list_pair;              // rebuilt by each kripke_distinguish_pairs_frames call
+    DevicePlan list_pair;              // plan of the last pair list given to kripke_distinguish_pairs_frames
+    std::vector<uint32_t> list_pair_key;   // that list (a call with the same list reuses the plan and enqueues only)
+    bool list_pair_built = false;
     uint32_t *d_pairs = nullptr;
     uint32_t pairs_cap = 0;
     Accum *d_accum = nullptr;
@@ -682,10 +688,9 @@ int jit_group_records(const kripke_programs *h, const uint32_t *pairs, uint32_t 
             for (uint32_t v = 0; v < KRIPKE_MAX_VARS; ++v) ri.rename[v] = rename[v];
             ri.slot = (uint32_t)G.roots.size();
         }
-        if (!(flags & KRIPKE_NO_SHARING) && (mode != JIT_MODE_DENSITY || g > 0)) {
+        if (!(flags & KRIPKE_NO_SHARING)) {
             // records whose graphs coincide are scanned once (the pair path is symmetric in its two formulas;
-            // density mode: the representative's row is copied - except with no variable, where a row is written
-            // at the HBM rate and recomputing it is cheaper than the copy's read + write)
+            // density mode: the program writes the rows of all its records)
             uint32_t pa = probe[g].build(prog(fa), plen(fa), rename, neg);
             uint32_t pb = pairs ? probe[g].build(prog(fb), plen(fb), rename, neg) : UINT32_MAX;
             if (pairs && pb < pa) std::swap(pa, pb);
@@ -762,7 +767,7 @@ int instantiate_jit_plan(const CachedJitPlan &cp, ScanPlan *out) {
         gp.k_eff = cg.g;
         gp.use_jit = true;
         gp.jit = cg.jit;
-        gp.jit.d_slot_record = nullptr;
+        gp.jit.d_slot_record = gp.jit.d_row_begin = gp.jit.d_rows = nullptr;
         int rc = jit_upload_slots(&gp.jit);
         if (rc > 0) rc = cuda_fail(rc);
         if (!rc) rc = upload(&gp.d_alias, cg.alias);
@@ -808,6 +813,20 @@ int build_jit_plan_mode(const kripke_programs *h, const uint32_t *pairs, uint32_
         cg.jit.d_slot_record = nullptr;
         if (rc > 0) rc = cuda_fail(rc);
         if (rc) return rc;
+        if (mode == JIT_MODE_DENSITY) {
+            // a program writes its own record's row and the rows of the records that share it: no accumulators
+            // to copy, and every row is written exactly once (write-only HBM traffic)
+            std::map<uint32_t, std::vector<uint32_t>> followers;
+            for (size_t i = 0; i + 1 < G.alias.size(); i += 2) followers[G.alias[i + 1]].push_back(G.alias[i]);
+            for (uint32_t rec : cg.jit.h_slot_record) {
+                cg.jit.h_row_begin.push_back((uint32_t)cg.jit.h_rows.size());
+                cg.jit.h_rows.push_back(rec);
+                auto it = followers.find(rec);
+                if (it != followers.end()) cg.jit.h_rows.insert(cg.jit.h_rows.end(), it->second.begin(), it->second.end());
+            }
+            cg.jit.h_row_begin.push_back((uint32_t)cg.jit.h_rows.size());
+            cg.alias.clear();
+        }
         cp.groups.push_back(std::move(cg));
     }
     rc = instantiate_jit_plan(cp, out);
@@ -922,17 +941,47 @@ int build_list_plan(const kripke_programs *h, const uint32_t *pairs, uint32_t n_
     auto prog = [&](uint32_t f) { return &h->h_code[h->h_offsets[f]]; };
     auto plen = [&](uint32_t f) { return h->h_offsets[f + 1] - h->h_offsets[f]; };
     const uint8_t rename[KRIPKE_MAX_VARS] = {0, 1, 2, 3};
+    // Records whose graphs coincide under the canonical variable order and polarity (jit.h) have the same counts
+    // and the same first refuting list position on every list: one of them is scanned, the others copy its
+    // accumulators before the finish step completes each record's own witness.
+    std::vector<bool> skip(n_records, false);
+    std::vector<uint32_t> alias;
+    {
+        Dag probe;
+        std::map<std::pair<uint32_t, uint32_t>, uint32_t> seen;
+        for (uint32_t r = 0; r < n_records; ++r) {
+            const uint32_t fa = pairs ? pairs[2 * r] : r, fb = pairs ? pairs[2 * r + 1] : r;
+            uint32_t sup;
+            {
+                Dag sd;
+                sup = sd.support(sd.build(prog(fa), plen(fa), nullptr));
+                if (pairs) sup |= sd.support(sd.build(prog(fb), plen(fb), nullptr));
+            }
+            uint8_t rn[KRIPKE_MAX_VARS] = {0, 0, 0, 0};
+            uint32_t neg = 0;
+            canonical_rename(prog(fa), plen(fa), pairs ? prog(fb) : nullptr, pairs ? plen(fb) : 0u, sup, 1, 0, rn, &neg);
+            uint32_t pa = probe.build(prog(fa), plen(fa), rn, neg);
+            uint32_t pb = pairs ? probe.build(prog(fb), plen(fb), rn, neg) : UINT32_MAX;
+            if (pairs && pb < pa) std::swap(pa, pb);
+            auto it = seen.find(std::make_pair(pa, pb));
+            if (it != seen.end()) { skip[r] = true; alias.push_back(r); alias.push_back(it->second); }
+            else seen.emplace(std::make_pair(pa, pb), r);
+        }
+    }
     std::vector<Lowered> low(n_records);
     std::vector<bool> fits(n_records);
     for (uint32_t r = 0; r < n_records; ++r)
-        fits[r] = pairs ? lower_pair(prog(pairs[2 * r]), plen(pairs[2 * r]), prog(pairs[2 * r + 1]),
-                                     plen(pairs[2 * r + 1]), 0u, rename, &low[r])
-                        : lower_single(prog(r), plen(r), 0u, rename, &low[r]);
+        if (!skip[r])
+            fits[r] = pairs ? lower_pair(prog(pairs[2 * r]), plen(pairs[2 * r]), prog(pairs[2 * r + 1]),
+                                         plen(pairs[2 * r + 1]), 0u, rename, &low[r])
+                            : lower_single(prog(r), plen(r), 0u, rename, &low[r]);
     HostPlan hp;
-    build_plan(low, fits, &hp);
-    return upload_plan(hp, out);
+    build_plan(low, fits, &hp, &skip);
+    int rc = upload_plan(hp, out);
+    if (!rc) rc = upload(&out->alias, alias);
+    if (!rc) out->n_alias = (uint32_t)(alias.size() / 2);
+    return rc;
 }
-
 int run_frames(kripke_programs *h, const DevicePlan &dp, const uint32_t *d_pairs, uint32_t n_records,
                uint32_t n, uint32_t k, const uint16_t *succ, uint64_t n_frames, uint64_t index_base,
                uint32_t flags, kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream) {
@@ -946,7 +995,7 @@ int run_frames(kripke_programs *h, const DevicePlan &dp, const uint32_t *d_pairs
     if (family == KRIPKE_KERNEL_SLICED && dp.n_unfit) return KRIPKE_EUNSUPPORTED;
     h->last = kripke_run_info_t{};
     h->last.models_per_program = n_frames << (k * n);
-    h->last.executed_models = (uint64_t)n_records * h->last.models_per_program;
+    h->last.executed_models = (uint64_t)(n_records - (family == KRIPKE_KERNEL_SCALAR ? 0u : dp.n_alias)) * h->last.models_per_program;
     h->last.sliced_logic_ops_per_word = dp.n_modal * n * n + dp.n_bool * n + (uint64_t)dp.n_slots * (n + 1);
     h->last.logic_instr_per_frame = (double)h->last.sliced_logic_ops_per_word * (double)(1ull << (k * n)) / 32.0;
     h->last.dense_logic_instr_per_frame = h->last.logic_instr_per_frame;
@@ -974,6 +1023,10 @@ int run_frames(kripke_programs *h, const DevicePlan &dp, const uint32_t *d_pairs
             if (dp.need_end[d] > dp.need_end[d - 1]) sp.max_need = d;
         if ((e = launch_frames(job, sp, stream, &launches))) return cuda_fail(e);
         if (dp.n_unfit && (e = launch_frames_scalar(job, dp.unfit, dp.n_unfit, stream, &launches))) return cuda_fail(e);
+        if (dp.n_alias) {
+            if ((e = launch_alias_accum(job.accum, dp.alias, dp.n_alias, stream))) return cuda_fail(e);
+            ++launches;
+        }
     }
     if ((e = launch_frames_finish(job, (flags & KRIPKE_ACCUMULATE) != 0, counts_out, witness_out, stream)))
         return cuda_fail(e);
@@ -1094,15 +1147,9 @@ int kripke_failure_density(const kripke_programs_t *programs, uint32_t n_worlds,
             sj.frame_begin = side ? ae : frame_begin;
             sj.frame_count = side ? frame_begin + frame_count - ae : ab - frame_begin;
             if (sj.frame_count == 0) continue;
-            if ((e = launch_failure_density_records(sj, g.jit.d_slot_record, g.jit.n_slots, counts_out, frame_count,
-                                                    sj.frame_begin - frame_begin, stream)))
+            if ((e = launch_failure_density_records(sj, g.jit.d_slot_record, g.jit.n_slots, g.jit.d_row_begin, g.jit.d_rows,
+                                                    counts_out, frame_count, sj.frame_begin - frame_begin, stream)))
                 return cuda_fail(e);
-            ++launches;
-        }
-        // formulas whose program is another formula's (equal graphs under the canonical variable order and polarity:
-        // the count of a frame is invariant under both) receive a copy of its row
-        if (g.n_alias) {
-            if ((e = launch_density_alias_rows(counts_out, frame_count, g.d_alias, g.n_alias, stream))) return cuda_fail(e);
             ++launches;
         }
     }
@@ -1193,16 +1240,23 @@ int kripke_distinguish_pairs_frames(const kripke_programs_t *programs, const uin
     kripke_programs *h = const_cast<kripke_programs *>(programs);
     for (uint32_t i = 0; i < 2 * n_pairs; ++i)
         if (pairs[i] >= h->n_formulas) return KRIPKE_EINVAL;
-    if (h->has_last) CU(cudaEventSynchronize(h->done));   // the previous call's plan may still be in use
-    int rc = build_list_plan(h, pairs, n_pairs, &h->list_pair);
-    if (rc) return rc;
-    if (n_pairs > h->pairs_cap) {
-        cudaFree(h->d_pairs);
-        h->d_pairs = nullptr; h->pairs_cap = 0;
-        CU(cudaMalloc((void **)&h->d_pairs, (size_t)2 * n_pairs * sizeof(uint32_t)));
-        h->pairs_cap = n_pairs;
+    const bool same = h->list_pair_built && h->list_pair_key.size() == 2 * (size_t)n_pairs &&
+                      std::equal(h->list_pair_key.begin(), h->list_pair_key.end(), pairs);
+    if (!same) {
+        if (h->has_last) CU(cudaEventSynchronize(h->done));   // the previous call's plan may still be in use
+        h->list_pair_built = false;
+        int rc = build_list_plan(h, pairs, n_pairs, &h->list_pair);
+        if (rc) return rc;
+        if (n_pairs > h->pairs_cap) {
+            cudaFree(h->d_pairs);
+            h->d_pairs = nullptr; h->pairs_cap = 0;
+            CU(cudaMalloc((void **)&h->d_pairs, (size_t)2 * n_pairs * sizeof(uint32_t)));
+            h->pairs_cap = n_pairs;
+        }
+        if (n_pairs) CU(cudaMemcpy(h->d_pairs, pairs, (size_t)2 * n_pairs * sizeof(uint32_t), cudaMemcpyHostToDevice));
+        h->list_pair_key.assign(pairs, pairs + 2 * (size_t)n_pairs);
+        h->list_pair_built = true;
     }
-    if (n_pairs) CU(cudaMemcpy(h->d_pairs, pairs, (size_t)2 * n_pairs * sizeof(uint32_t), cudaMemcpyHostToDevice));
     return run_frames(h, h->list_pair, h->d_pairs, n_pairs, n_worlds, n_vars, succ, n_frames, index_base, flags,
                       counts_out, witness_out, stream);
 }

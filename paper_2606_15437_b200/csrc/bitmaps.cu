@@ -148,6 +148,7 @@ struct DensityParams {
     const uint32_t *offsets;
     uint32_t n_formulas;              // formulas, or listed records
     const uint32_t *records;          // null = formulas 0..n_formulas-1
+    const uint32_t *row_begin, *rows; // not null: listed record i is written to the rows rows[row_begin[i] .. row_begin[i+1])
     uint32_t *counts;
     uint64_t row_stride, col_offset;  // counts[formula * row_stride + col_offset + j]
 };
@@ -173,7 +174,12 @@ __global__ void __launch_bounds__(128) failure_density_kernel(DensityParams p) {
             for (uint32_t i = 0; i < KRIPKE_MAX_VARS; ++i) val[i] = (uint32_t)(v >> (i * p.n)) & full;
             cnt += __popc(full & ~eval_postfix_scalar(c, len, p.n, succ, val, full));
         }
-        p.counts[(uint64_t)b * p.row_stride + p.col_offset + j] = cnt;
+        if (p.rows) {
+            for (uint32_t t = p.row_begin[li]; t < p.row_begin[li + 1]; ++t)
+                p.counts[(uint64_t)p.rows[t] * p.row_stride + p.col_offset + j] = cnt;
+        } else {
+            p.counts[(uint64_t)b * p.row_stride + p.col_offset + j] = cnt;
+        }
     }
 }
 
@@ -300,12 +306,14 @@ int launch_frames_from_bitmap(uint32_t n, uint32_t cls, const uint64_t *class_ta
 }
 
 static int launch_density(const ScanJob &job, const uint16_t *succ_list, const uint32_t *records, uint32_t n_list,
+                          const uint32_t *row_begin, const uint32_t *rows,
                           uint32_t *counts_out, uint64_t row_stride, uint64_t col_offset, void *stream) {
     if (job.frame_count == 0 || n_list == 0) return 0;
     DensityParams p;
     p.n = job.n; p.k = job.k; p.cls = job.cls; p.class_table = job.class_table; p.succ_list = succ_list;
     p.frame_begin = job.frame_begin; p.frame_count = job.frame_count;
     p.code = job.code; p.offsets = job.offsets; p.n_formulas = n_list; p.records = records; p.counts = counts_out;
+    p.row_begin = row_begin; p.rows = rows;
     p.row_stride = row_stride; p.col_offset = col_offset;
     const uint64_t bx = (job.frame_count + 127) / 128;
     if (bx > 0x7FFFFFFFull) return 801;
@@ -317,39 +325,13 @@ static int launch_density(const ScanJob &job, const uint16_t *succ_list, const u
 
 int launch_failure_density(const ScanJob &job, const uint16_t *succ_list, uint32_t *counts_out, uint64_t row_stride,
                            uint64_t col_offset, void *stream) {
-    return launch_density(job, succ_list, nullptr, job.n_formulas, counts_out, row_stride, col_offset, stream);
+    return launch_density(job, succ_list, nullptr, job.n_formulas, nullptr, nullptr, counts_out, row_stride, col_offset, stream);
 }
 
-int launch_failure_density_records(const ScanJob &job, const uint32_t *records, uint32_t n_list, uint32_t *counts_out,
-                                   uint64_t row_stride, uint64_t col_offset, void *stream) {
-    return launch_density(job, nullptr, records, n_list, counts_out, row_stride, col_offset, stream);
-}
-
-// One row copy per alias pair (blockIdx.y), 16 bytes per thread where the rows allow it.
-__global__ void density_alias_rows_kernel(uint32_t *counts, uint64_t row_stride, const uint32_t *alias) {
-    const uint32_t *src = counts + (uint64_t)alias[2 * blockIdx.y + 1] * row_stride;
-    uint32_t *dst = counts + (uint64_t)alias[2 * blockIdx.y] * row_stride;
-    const uint64_t step = (uint64_t)gridDim.x * blockDim.x, t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (((row_stride & 3u) | (reinterpret_cast<uintptr_t>(counts) & 15u)) == 0) {
-        const uint4 *s4 = reinterpret_cast<const uint4 *>(src);
-        uint4 *d4 = reinterpret_cast<uint4 *>(dst);
-        for (uint64_t i = t; i < row_stride / 4; i += step) __stcs(d4 + i, __ldcs(s4 + i));
-    } else {
-        for (uint64_t i = t; i < row_stride; i += step) dst[i] = src[i];
-    }
-}
-
-int launch_density_alias_rows(uint32_t *counts, uint64_t row_stride, const uint32_t *alias, uint32_t n_alias, void *stream) {
-    if (n_alias == 0 || row_stride == 0) return 0;
-    const uint64_t want = (row_stride / 4 + 255) / 256;
-    for (uint32_t a0 = 0; a0 < n_alias; a0 += 65535u) {
-        const uint32_t na = n_alias - a0 < 65535u ? n_alias - a0 : 65535u;
-        dim3 grid((unsigned)(want < 1 ? 1 : want > 1024 ? 1024 : want), na);
-        density_alias_rows_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(counts, row_stride, alias + 2 * (size_t)a0);
-        cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess) return (int)e;
-    }
-    return 0;
+int launch_failure_density_records(const ScanJob &job, const uint32_t *records, uint32_t n_list, const uint32_t *row_begin,
+                                   const uint32_t *rows, uint32_t *counts_out, uint64_t row_stride, uint64_t col_offset,
+                                   void *stream) {
+    return launch_density(job, nullptr, records, n_list, row_begin, rows, counts_out, row_stride, col_offset, stream);
 }
 
 int launch_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words, const uint32_t *library,

@@ -108,10 +108,10 @@ int launch_frames_from_bitmap(uint32_t n, uint32_t cls, const uint64_t *class_ta
 // counts_out[record * row_stride + col_offset + j] for frame j of the job's range (all formulas, or the listed records).
 int launch_failure_density(const ScanJob &job, const uint16_t *succ_list, uint32_t *counts_out, uint64_t row_stride,
                            uint64_t col_offset, void *stream);
-// Rows of records whose program is another record's (alias[2i] receives the row of alias[2i+1]): row copies.
-int launch_density_alias_rows(uint32_t *counts, uint64_t row_stride, const uint32_t *alias, uint32_t n_alias, void *stream);
-int launch_failure_density_records(const ScanJob &job, const uint32_t *records, uint32_t n_list, uint32_t *counts_out,
-                                   uint64_t row_stride, uint64_t col_offset, void *stream);
+// records[i] is evaluated once and written to the rows rows[row_begin[i] .. row_begin[i+1]) (row tables null: to its own row)
+int launch_failure_density_records(const ScanJob &job, const uint32_t *records, uint32_t n_list, const uint32_t *row_begin,
+                                   const uint32_t *rows, uint32_t *counts_out, uint64_t row_stride, uint64_t col_offset,
+                                   void *stream);
 int launch_match_bitmaps(const uint32_t *bitmaps, uint32_t n_records, uint64_t words, const uint32_t *library,
                          uint32_t n_library, uint32_t *match_out, void *stream);
 

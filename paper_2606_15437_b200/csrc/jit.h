@@ -188,6 +188,10 @@ struct JitGroupPlan {
     std::vector<JitKernel> kernels;
     uint32_t *d_slot_record = nullptr;   // device: record per slot
     std::vector<uint32_t> h_slot_record; // the same on the host (a cached plan is re-uploaded from it)
+    // density plans: program (slot) s writes the rows h_rows[h_row_begin[s] .. h_row_begin[s+1]) - its own record and
+    // the records whose program it is (equal graphs under the canonical variable order and polarity)
+    std::vector<uint32_t> h_row_begin, h_rows;
+    uint32_t *d_row_begin = nullptr, *d_rows = nullptr;
     uint32_t n_slots = 0;
     uint32_t threads = 128;
     JitEmitStats stats;

@@ -648,17 +648,17 @@ static std::string emit_density_kernel(const Dag &dag, const JitLayout &lay, con
                     t += ");\n";
                 }
                 t += "        __syncwarp();\n";
-                t += "        if (valid) {\n";
-                t += fmt("          uint4 *o = reinterpret_cast<uint4 *>(p.density + (unsigned long long)p.slot_record[%u] * p.total_frames + "
-                         "(((((unit >> 5) << %u) + jo) << 10) - p.frame_base)) + lane;\n", r, lay.outer);
+                t += fmt("        if (valid) for (unsigned row = p.row_begin[%u]; row < p.row_begin[%u]; ++row) {\n", r, r + 1);
+                t += fmt("          uint4 *o = reinterpret_cast<uint4 *>(p.density + (unsigned long long)p.rows[row] * p.total_frames + "
+                         "(((((unit >> 5) << %u) + jo) << 10) - p.frame_base)) + lane;\n", lay.outer);
                 for (uint32_t q = 0; q < 8; ++q) {
                     t += fmt("          { uint4 v = ld_w[%uu ^ lw%u]; v.x <<= p.model_shift; v.y <<= p.model_shift; v.z <<= p.model_shift; "
                              "v.w <<= p.model_shift; __stcs(o + %u, v); }\n", 32 * q, q & 1u, 32 * q);
                 }
                 t += "        }\n      }\n";
             } else {
-                t += "      if (valid) {\n";
-                t += fmt("        unsigned *o = p.density + (unsigned long long)p.slot_record[%u] * p.total_frames + ((((unit << %u) + jo) << 5) - p.frame_base);\n", r, lay.outer);
+                t += fmt("      if (valid) for (unsigned row = p.row_begin[%u]; row < p.row_begin[%u]; ++row) {\n", r, r + 1);
+                t += fmt("        unsigned *o = p.density + (unsigned long long)p.rows[row] * p.total_frames + ((((unit << %u) + jo) << 5) - p.frame_base);\n", lay.outer);
                 for (uint32_t q = 0; q < 8; ++q) {
                     t += fmt("        *reinterpret_cast<uint4 *>(o + %u) = make_uint4(", 4 * q);
                     for (uint32_t i = 0; i < 4; ++i)
@@ -714,7 +714,8 @@ static std::string emit_density_kernel(const Dag &dag, const JitLayout &lay, con
     if (!lanes_are_frames) {
         s += "      if (valid) {\n";
         for (uint32_t r = 0; r < G; ++r)
-            s += fmt("        p.density[(unsigned long long)p.slot_record[%u] * p.total_frames + (unit - p.frame_base)] = d%u << p.model_shift;\n", r, r);
+            s += fmt("        for (unsigned row = p.row_begin[%u]; row < p.row_begin[%u]; ++row) "
+                     "p.density[(unsigned long long)p.rows[row] * p.total_frames + (unit - p.frame_base)] = d%u << p.model_shift;\n", r, r + 1, r);
         s += "      }\n";
     }
     s += "    }\n  }\n}\n";

@@ -26,6 +26,7 @@ struct KjParamsHost {
     unsigned model_shift, pad;
     unsigned *density;
     unsigned long long total_frames, frame_base;
+    const unsigned *row_begin, *rows;
 };
 
 struct Module {
@@ -65,7 +66,9 @@ int compile(const std::string &src, std::vector<char> *cubin, std::string *log) 
 
 void JitGroupPlan::release() {
     cudaFree(d_slot_record);
-    d_slot_record = nullptr;
+    cudaFree(d_row_begin);
+    cudaFree(d_rows);
+    d_slot_record = d_row_begin = d_rows = nullptr;
     kernels.clear();
     n_slots = 0;
 }
@@ -190,14 +193,20 @@ int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitR
 }
 
 int jit_upload_slots(JitGroupPlan *plan) {
-    cudaFree(plan->d_slot_record);
-    plan->d_slot_record = nullptr;
     const std::vector<uint32_t> &records = plan->h_slot_record;
     plan->n_slots = (uint32_t)records.size();
     if (records.empty()) return 0;
-    cudaError_t e = cudaMalloc((void **)&plan->d_slot_record, records.size() * sizeof(uint32_t));
-    if (e == cudaSuccess)
-        e = cudaMemcpy(plan->d_slot_record, records.data(), records.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
+    auto up = [](uint32_t **dst, const std::vector<uint32_t> &src) {
+        cudaFree(*dst);
+        *dst = nullptr;
+        if (src.empty()) return cudaSuccess;
+        cudaError_t e = cudaMalloc((void **)dst, src.size() * sizeof(uint32_t));
+        if (e == cudaSuccess) e = cudaMemcpy(*dst, src.data(), src.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
+        return e;
+    };
+    cudaError_t e = up(&plan->d_slot_record, records);
+    if (e == cudaSuccess) e = up(&plan->d_row_begin, plan->h_row_begin);
+    if (e == cudaSuccess) e = up(&plan->d_rows, plan->h_rows);
     return (int)e;
 }
 
@@ -220,6 +229,8 @@ int jit_launch_group(const ScanJob &job, const JitGroupPlan &plan, uint32_t mode
     p.density = density ? density->counts : nullptr;
     p.total_frames = density ? density->total_frames : 0;
     p.frame_base = density ? density->frame_base : 0;
+    p.row_begin = nullptr;
+    p.rows = nullptr;
     if (p.unit_count == 0) return 0;
     const uint32_t threads = plan.threads;
     const uint64_t tiles = (p.unit_count + threads - 1) / threads;
@@ -244,6 +255,8 @@ int jit_launch_group(const ScanJob &job, const JitGroupPlan &plan, uint32_t mode
             q.unit_count = std::min<uint64_t>(p.unit_count - i0 * q.units_per_item, ni * q.units_per_item);
             q.n_items = (unsigned)ni;
             q.slot_record = plan.d_slot_record + k.slot_base;
+            q.row_begin = plan.d_row_begin ? plan.d_row_begin + k.slot_base : nullptr;
+            q.rows = plan.d_rows;
             void *args[] = {&q};
             const unsigned grid = (unsigned)std::min<uint64_t>(ni, grid_full);
             e = cudaLaunchKernel((const void *)k.kernel, dim3(grid), dim3(threads), args, 0, (cudaStream_t)stream);
