@@ -354,7 +354,7 @@ int kripke_last_run_info(const kripke_programs_t *programs, kripke_run_info_t *i
  * (handle, n, class, flags) combination is scanned and cached per process by source text.  That first
  * call therefore blocks for the compilation (kripke_run_info_t.jit_compile_seconds); later calls only
  * enqueue.  Results are identical to the interpreted and scalar kernels (GPU tests).
- * kripke_jit_configure: 1 <= max_programs_per_kernel <= 160 (default 64; more programs per kernel share
+ * kripke_jit_configure: 1 <= max_programs_per_kernel <= 160 (default 48; more programs per kernel share
  * more subterms and need more registers); 1 <= min_blocks_per_sm <= 8 = the __launch_bounds__ occupancy
  * request of the generated kernels (128 threads per block; default 2, i.e. up to 255 registers per thread).
  * Affects plans built afterwards. */

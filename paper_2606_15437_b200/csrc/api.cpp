@@ -291,7 +291,7 @@ uint32_t reduced_shapes(uint32_t n, uint32_t k, uint32_t cls, uint32_t flags) {
 enum : uint32_t { ENGINE_INTERPRETED = 0, ENGINE_JIT = 1 };
 
 // Tunables of the compiled scans (kripke_jit_configure).
-uint32_t g_jit_max_programs = 64;
+uint32_t g_jit_max_programs = 48;
 uint32_t g_jit_min_blocks = 2;
 
 // Lowers the records (formulas, or pairs if `pairs` != null) into one GroupPlan per variable count.

@@ -47,7 +47,7 @@ struct BitSource {
     int level(uint32_t pos) const {
         if (pos < 5) return 0;
         pos -= 5;
-        if (pos < lay.inner) return 2;
+        if (pos < lay.inner) return 2 + (int)std::min(lay.inner - 1 - pos, lay.nest_bits);
         pos -= lay.inner;
         if (pos < lay.lane_bits) return 0;
         pos -= lay.lane_bits;
@@ -100,8 +100,10 @@ struct Emitter {
         bool keep = false;      // the value is read by literal text: never substitute it away
     };
     std::vector<Stmt> stmts;
-    std::string body[3];
-    uint64_t ops[3] = {0, 0, 0};
+    static constexpr int MAX_LEVELS = 2 + 16;
+    std::string body[MAX_LEVELS];
+    uint64_t ops[MAX_LEVELS] = {0};
+    int deep() const { return lay.nest_bits >= lay.inner && lay.inner ? 1 + (int)lay.inner : 2 + (int)lay.nest_bits; }   // level of the innermost loop
     uint32_t n_tmp = 0;
 
     Emitter(const Dag &d, const JitLayout &l) : dag(d), lay(l), bits(l), done(d.nodes.size(), 0), lvl(d.nodes.size()) {
@@ -178,13 +180,15 @@ struct Emitter {
             node(nd.a >> 1);
             // Lemma 1 on 32 models: R[w] = AND_u ( T[u] | ~E[w][u] )
             for (uint32_t w = 0; w < n; ++w) {
-                int L = 0, acc = constant(true);
+                std::vector<std::pair<int, int>> terms;
                 for (uint32_t u = 0; u < n; ++u) {
                     const std::string ew = edge(w, u);
-                    L = std::max(L, std::max(lit_level(nd.a, u), edge_level(w, u)));
                     const int x = lit(nd.a, u);
-                    acc = bin(Ex::AND, acc, ew.empty() ? x : bin(Ex::OR, x, leaf(ew, true)));
+                    terms.emplace_back(std::max(lit_level(nd.a, u), edge_level(w, u)),
+                                       ew.empty() ? x : bin(Ex::OR, x, leaf(ew, true)));
                 }
+                int L = 0;
+                const int acc = fold_by_level(Ex::AND, terms, &L);
                 lvl[id][w] = (int8_t)L;
                 stmts.push_back(Stmt{L, fmt("t%u_%u", id, w), acc, ""});
             }
@@ -223,27 +227,28 @@ struct Emitter {
         if (!(l & 1u) && nd.kind == DagNode::AND) { flat_conjuncts(nd.a, out); flat_conjuncts(nd.b, out); }
         else out->push_back(l);
     }
-    // Conjunction of operands that change at different loop levels: the operands of the lower levels are folded
-    // first and become a value of their own at that level, so the inner loop only pays for what changes in it.
-    int and_by_level(std::vector<std::pair<int, int>> items, int *level_out) {
+    // Conjunction / disjunction of operands that change at different loop levels: the operands of the lower levels
+    // are folded first and become a value of their own at that level, so an inner loop only pays for what
+    // changes in it.
+    int fold_by_level(Ex::Op op, std::vector<std::pair<int, int>> items, int *level_out) {
         std::stable_sort(items.begin(), items.end(), [](const std::pair<int, int> &x, const std::pair<int, int> &y) { return x.first < y.first; });
-        int acc = constant(true), L = 0, leaves = 0;
+        int acc = constant(op == Ex::AND), L = 0;
         for (const auto &it : items) {
-            if (it.first > L && leaves >= 2 && pool[acc].op != Ex::CONST && pool[acc].op != Ex::LEAF) {
+            if (it.first > L && pool[acc].op != Ex::CONST && pool[acc].op != Ex::LEAF) {
                 const std::string name = fmt("y%u", n_tmp++);
                 stmts.push_back(Stmt{L, name, acc, ""});
                 acc = leaf(name, false);
-                leaves = 1;
             }
             L = std::max(L, it.first);
-            acc = bin(Ex::AND, acc, it.second);
-            ++leaves;
+            acc = bin(op, acc, it.second);
         }
         *level_out = L;
         return acc;
     }
+    int and_by_level(std::vector<std::pair<int, int>> items, int *level_out) { return fold_by_level(Ex::AND, std::move(items), level_out); }
     // fail word of one obligation: OR_u ( S_depth[u] & ~lit[u] )
     std::map<std::pair<uint32_t, uint32_t>, std::string> obligation_name;
+    std::map<std::pair<uint32_t, uint32_t>, int> obligation_level;
     std::vector<uint32_t> value_uses;       // readers of every node's value other than guarded obligations that fold it themselves
     void count_uses(const std::vector<JitRoot> &roots) {
         value_uses.assign(dag.nodes.size(), 0);
@@ -295,7 +300,8 @@ struct Emitter {
                 }
             }
             if (conj.empty()) node(g.lit >> 1);
-            int L = 0, acc = constant(false);
+            int L = 0;
+            std::vector<std::pair<int, int>> terms;
             for (uint32_t u = 0; u < lay.n; ++u) {
                 int term, lu = 0;
                 if (conj.empty()) {
@@ -309,12 +315,13 @@ struct Emitter {
                     for (uint32_t c : conj) items.emplace_back(lit_level(c, u), lit(c, u));
                     term = and_by_level(items, &lu);
                 }
-                acc = bin(Ex::OR, acc, term);
-                L = std::max(L, lu);
+                terms.emplace_back(lu, term);
             }
+            const int acc = fold_by_level(Ex::OR, terms, &L);
             const std::string name = fmt("o%u_%u", g.depth, g.lit);
             stmts.push_back(Stmt{L, name, acc, ""});
             it = obligation_name.emplace(key, name).first;
+            obligation_level[key] = L;
         }
         return leaf(it->second, false);
     }
@@ -452,7 +459,13 @@ int jit_edge_level(const JitLayout &lay, uint32_t w, uint32_t u) {
 }
 
 double jit_level_weight(const JitLayout &lay, int level) {
-    return level >= 2 ? 1.0 : level == 1 ? 1.0 / (double)(1u << lay.inner) : 1.0 / (double)(1u << (lay.inner + lay.outer));
+    if (level <= 0) return 1.0 / (double)(1u << (lay.inner + lay.outer));
+    if (level == 1) return 1.0 / (double)(1u << lay.inner);
+    // level 2 + j, j < nest_bits = the loop of the j-th slowest inner bit: its body runs 2^(j+1) times per 2^inner
+    // words; the loop over the remaining bits runs once per word
+    const uint32_t j = (uint32_t)level - 2u;
+    if (j >= lay.nest_bits || j + 1u >= lay.inner) return 1.0;
+    return (double)(1u << (j + 1u)) / (double)(1u << lay.inner);
 }
 
 bool jit_layout(uint32_t n, uint32_t g, uint32_t cls, JitLayout *out) {
@@ -472,6 +485,7 @@ bool jit_layout(uint32_t n, uint32_t g, uint32_t cls, JitLayout *out) {
         l.outer = std::min(LOOP_BITS, l.kn + fb - 5);
         l.unit_frames_log2 = 5 - l.kn + l.outer;
     }
+    l.nest_bits = l.inner >= 2 ? l.inner : 0;
     if (out) *out = l;
     return true;
 }
@@ -752,20 +766,30 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
             // refuted lanes of a guarded root: some obligation fails at a world of its guard set (jit.h)
             // Every obligation's fail word is a value of its own: shared by the records of the kernel that carry the
             // same obligation, and computed once per unit when its literal does not change inside the loops.
-            e = em.constant(false);
-            for (const JitGuarded &g : roots[r].guarded) e = em.bin(Ex::OR, e, em.obligation(g));
+            std::vector<std::pair<int, int>> items;
+            for (const JitGuarded &g : roots[r].guarded) {
+                const int x = em.obligation(g);
+                items.emplace_back(em.obligation_level[std::make_pair(g.depth, g.lit)], x);
+            }
+            int L = 0;
+            e = em.fold_by_level(Ex::OR, items, &L);
         } else if (roots[r].b == UINT32_MAX) {
             em.node(roots[r].a >> 1);
             // refuted lanes: the truth set is not all worlds
-            e = em.constant(true);
-            for (uint32_t w = 0; w < n; ++w) e = em.bin(Ex::AND, e, em.lit(roots[r].a, w));
-            e = em.negate(e);
+            std::vector<std::pair<int, int>> items;
+            for (uint32_t w = 0; w < n; ++w) items.emplace_back(em.lit_level(roots[r].a, w), em.lit(roots[r].a, w));
+            int L = 0;
+            e = em.negate(em.fold_by_level(Ex::AND, items, &L));
         } else {
             // distinguishing lanes: the two truth sets differ
             em.node(roots[r].a >> 1);
             em.node(roots[r].b >> 1);
-            e = em.constant(false);
-            for (uint32_t w = 0; w < n; ++w) e = em.bin(Ex::OR, e, em.bin(Ex::XOR, em.lit(roots[r].a, w), em.lit(roots[r].b, w)));
+            std::vector<std::pair<int, int>> items;
+            for (uint32_t w = 0; w < n; ++w)
+                items.emplace_back(std::max(em.lit_level(roots[r].a, w), em.lit_level(roots[r].b, w)),
+                                   em.bin(Ex::XOR, em.lit(roots[r].a, w), em.lit(roots[r].b, w)));
+            int L = 0;
+            e = em.fold_by_level(Ex::OR, items, &L);
         }
         // Counters of a unit are 16-bit fields where they fit (a unit has 2^(5+inner+outer) models): with a frame
         // count, models in the low half and frames in the high half of one register; without, two programs per
@@ -784,7 +808,7 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
         } else {
             tail = (r & 1u) ? fmt("c%u += __popc(r) << 16;", r >> 1) : fmt("c%u += __popc(r);", r >> 1);
         }
-        em.stmts.push_back(Emitter::Stmt{2, "", e, tail});
+        em.stmts.push_back(Emitter::Stmt{em.deep(), "", e, tail});
     }
     em.emit_all();
 
@@ -815,7 +839,7 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
         for (uint32_t e : em.used_table) decl_unit += fmt("      const unsigned me%u = 0u - (unsigned)((frame >> %u) & 1ull);\n", e, e);
     }
     for (uint32_t b : em.bits.used_outer) decl_outer += fmt("      const unsigned mo%u = 0u - ((jo >> %u) & 1u);\n", b, b);
-    for (uint32_t b : em.bits.used_inner) decl_inner += fmt("      const unsigned mi%u = 0u - ((ji >> %u) & 1u);\n", b, b);
+    if (!lay.nest_bits) for (uint32_t b : em.bits.used_inner) decl_inner += fmt("      const unsigned mi%u = 0u - ((ji >> %u) & 1u);\n", b, b);
     s += decl_unit;
     s += "      // values that are fixed for the unit\n" + em.body[0];
     for (uint32_t r = 0; r < G; ++r) {
@@ -829,11 +853,32 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
     s += decl_outer;
     s += em.body[1];
     if (fmode == F_ANY) for (uint32_t r = 0; r < G; ++r) s += fmt("      unsigned a%u = 0u;\n", r);
-    s += "#pragma unroll 1\n";
-    s += fmt("      for (unsigned ji = 0; ji < %uu; ++ji) {\n", 1u << lay.inner);
-    s += decl_inner;
-    s += em.body[2];
-    s += "      }\n";
+    if (!lay.nest_bits) {
+        s += "#pragma unroll 1\n";
+        s += fmt("      for (unsigned ji = 0; ji < %uu; ++ji) {\n", 1u << lay.inner);
+        s += decl_inner;
+        s += em.body[2];
+        s += "      }\n";
+    } else {
+        // one two-iteration loop per slow valuation bit, the slowest outermost, then one loop over the remaining
+        // bits: the body of the loop of bit b holds the values whose fastest-changing input is bit b
+        const uint32_t rest = lay.inner - lay.nest_bits;
+        for (uint32_t j = 0; j < lay.nest_bits; ++j) {
+            const uint32_t b = lay.inner - 1 - j;
+            s += "#pragma unroll 1\n";
+            s += fmt("      for (unsigned jb%u = 0; jb%u < 2u; ++jb%u) {\n", b, b, b);
+            if (em.bits.used_inner.count(b)) s += fmt("      const unsigned mi%u = 0u - jb%u;\n", b, b);
+            s += em.body[2 + j];
+        }
+        if (rest) {
+            s += "#pragma unroll 1\n";
+            s += fmt("      for (unsigned ji = 0; ji < %uu; ++ji) {\n", 1u << rest);
+            for (uint32_t b : em.bits.used_inner) if (b < rest) s += fmt("      const unsigned mi%u = 0u - ((ji >> %u) & 1u);\n", b, b);
+            s += em.body[2 + lay.nest_bits];
+            s += "      }\n";
+        }
+        for (uint32_t j = 0; j < lay.nest_bits; ++j) s += "      }\n";
+    }
     if (fmode == F_ANY) for (uint32_t r = 0; r < G; ++r) s += packed ? fmt("      if (a%u != 0u) c%u += 65536u;\n", r, r) : fmt("      f%u += (a%u != 0u);\n", r, r);
     s += "      }\n";
     for (uint32_t r = 0; r < G; ++r) {
@@ -853,15 +898,23 @@ std::string jit_emit_kernel(const Dag &dag, const JitLayout &lay, const std::vec
     s += fmt("        atomicMin(&a->best, ((u0 + s_best[i]) >> %u) << %u);\n", lay.split, lay.unit_frames_log2);
     s += "      }\n";
     s += "  }\n}\n";
-    s += fmt("// graph nodes evaluated: box=%u and=%u; lop3 per unit=%llu, per outer iteration=%llu, per word=%llu\n", em.n_box,
-             em.n_and, (unsigned long long)em.ops[0], (unsigned long long)em.ops[1], (unsigned long long)em.ops[2]);
-    if (stats) {
-        const uint64_t *ops = em.ops;
-        stats->logic_ops_emitted = ops[0] + ops[1] + ops[2];
-        stats->logic_ops_per_word = (double)ops[2] + (double)ops[1] / (double)(1u << lay.inner) +
-                                    (double)ops[0] / (double)(1u << (lay.inner + lay.outer));
-        stats->n_box = em.n_box;
-        stats->n_and = em.n_and;
+    {
+        double per_word = 0;
+        uint64_t emitted = 0;
+        std::string by_level;
+        for (int L = 0; L <= em.deep(); ++L) {
+            per_word += (double)em.ops[L] * jit_level_weight(lay, L);
+            emitted += em.ops[L];
+            by_level += fmt(" %llu", (unsigned long long)em.ops[L]);
+        }
+        s += fmt("// graph nodes evaluated: box=%u and=%u; lop3 by loop level (unit, outer, inner bits slowest first):%s; per word %.1f\n",
+                 em.n_box, em.n_and, by_level.c_str(), per_word);
+        if (stats) {
+            stats->logic_ops_emitted = emitted;
+            stats->logic_ops_per_word = per_word;
+            stats->n_box = em.n_box;
+            stats->n_and = em.n_and;
+        }
     }
     return s;
 }

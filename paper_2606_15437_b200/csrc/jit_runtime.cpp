@@ -156,9 +156,13 @@ int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitR
                 std::vector<std::vector<uint32_t>> next_parts;
                 for (size_t i = 0; i < parts.size(); ++i) {
                     if (g_cache[sources[i]].local_bytes > 0 && parts[i].size() >= 16) {
-                        const size_t half = parts[i].size() / 2;
-                        next_parts.emplace_back(parts[i].begin(), parts[i].begin() + half);
-                        next_parts.emplace_back(parts[i].begin() + half, parts[i].end());
+                        // its programs are partitioned again, into two kernels with about the same work
+                        std::vector<JitRoot> sub;
+                        for (uint32_t r : parts[i]) sub.push_back(roots[r]);
+                        for (const auto &sp : jit_partition(dag, sub, lay, (uint32_t)(parts[i].size() + 1) / 2)) {
+                            next_parts.emplace_back();
+                            for (uint32_t j : sp) next_parts.back().push_back(parts[i][j]);
+                        }
                         split = true;
                     } else {
                         next_parts.push_back(parts[i]);
