@@ -31,7 +31,7 @@ import workloads as W  # noqa: E402
 
 CLASSES = (("K", 0), ("T", 1), ("S4", 2), ("S5", 3))
 N_WORLDS, N_VARS = 5, 2
-NCU_TRAFFIC_BYTES = 3176192                  # class-K launches of one step, from profiles/r2_jit_launches_c3.md
+NCU_TRAFFIC_BYTES = 4239616                  # class-K launches of one step, from profiles/r2_jit_launches_c3.md
 SM_COUNT, INT_LANES_PER_SM = 148, 64       # 4 sub-partitions x 16 lanes/clk on the ALU pipe (B300_MICROARCH.md)
 
 
@@ -228,6 +228,7 @@ def run_ours(args):
             if cname == "K":
                 k_info["instr_per_frame"] = info.logic_instr_per_frame
                 k_info["alg_instr_per_frame"] = info.algorithmic_logic_instr_per_frame
+                k_info["popc_per_frame"] = info.popc_instr_per_frame
                 k_info["frames"] = count
                 k_info["family"] = info.kernel_family
                 k_info["programs"] = info.jit_programs
@@ -386,6 +387,13 @@ def run_ours(args):
                 "executed_ops": "3-input logic (LOP3) thread-instructions the compiled kernels execute: one per emitted "
                                 "lop3.b32 (the emitter covers every expression tree with 3-input tables itself), weighted by "
                                 "loop level; cross-checked against ncu's opcode count in profiles/r2_jit_full.md",
+                "xu_pipe": {"popc_per_s_T": k_info["popc_per_frame"] * k_info["frames"] / (k_ms * 1e-3) / 1e12,
+                            "peak_T": peak / 4, "frac": k_info["popc_per_frame"] * k_info["frames"] / (k_ms * 1e-3) / 1e12 / (peak / 4),
+                            "what": "one POPC per scanned program and 32-model word counts the refuting models; POPC issues on "
+                                    "the XU pipe at 16 lanes/clk/SM (a quarter of the ALU rate).  At the two warps per "
+                                    "scheduler these kernels run with, ALU and XU time barely overlap (ncu: "
+                                    "profiles/r2_jit_perkernel.md), so frac + xu_pipe.frac is the share of the step the two "
+                                    "pipes account for"},
                 "frac_algorithmic": k_alg / (k_ms * 1e-3) / 1e12 / peak,
                 "algorithmic_ops": "SURVEY 8(d): every formula as written, (d n^2 + b n + n + 1) logic instructions per "
                                    "32-model word x 2^(k_b n)/32 words per frame - work the method defines per peak-second; "

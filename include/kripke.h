@@ -334,7 +334,9 @@ typedef struct {
                                              variable-count group): EXECUTED logic thread-instructions   */
     uint32_t jit_programs;                /* distinct programs the compiled kernels evaluated          */
     uint32_t reserved;
-    double dense_logic_instr_per_frame;   /* = logic_instr_per_frame (kept for layout compatibility)   */
+    double popc_instr_per_frame;          /* population-count thread-instructions per frame of the range: one per
+                                             scanned program and 32-model word (the refuting-model count); they
+                                             issue on the quarter-rate XU pipe (16 lanes per clock per SM)       */
     double algorithmic_logic_instr_per_frame; /* SURVEY.md 8(d)'s ALGORITHMIC count: every formula of the
                                              batch as written, no sharing and no folding - (d n^2 + b n +
                                              n + 1) logic instructions per 32-model word (d modal operators,

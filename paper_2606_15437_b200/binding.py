@@ -57,7 +57,7 @@ class RunInfo(ctypes.Structure):
                 ("sliced_logic_ops_per_word", ctypes.c_uint64), ("models_per_program", ctypes.c_uint64),
                 ("executed_models", ctypes.c_uint64), ("logic_instr_per_frame", ctypes.c_double),
                 ("jit_programs", ctypes.c_uint32), ("reserved", ctypes.c_uint32),
-                ("dense_logic_instr_per_frame", ctypes.c_double),
+                ("popc_instr_per_frame", ctypes.c_double),
                 ("algorithmic_logic_instr_per_frame", ctypes.c_double),
                 ("jit_compile_seconds", ctypes.c_double)]
 

@@ -364,6 +364,7 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *h_pairs, 
         if (g.use_jit) {
             h->last.sliced_logic_ops_per_word += g.jit.stats.logic_ops_emitted;
             h->last.logic_instr_per_frame += g.jit.stats.logic_ops_per_word * words;
+            h->last.popc_instr_per_frame += (double)g.jit.n_slots * words;
             h->last.executed_models += (uint64_t)g.jit.n_slots * (count << (g.k_eff * n));
             h->last.jit_programs += g.jit.n_slots;
             continue;
@@ -373,9 +374,9 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *h_pairs, 
         };
         h->last.sliced_logic_ops_per_word += g.dp.n_modal * n * n + g.dp.n_bool * n + (uint64_t)g.dp.n_slots * (n + 1);
         h->last.logic_instr_per_frame += dense(g.dp);
+        h->last.popc_instr_per_frame += (double)g.dp.n_slots * words;
         h->last.executed_models += (uint64_t)(g.dp.n_slots + g.dp.n_unfit) * (count << (g.k_eff * n));
     }
-    h->last.dense_logic_instr_per_frame = h->last.logic_instr_per_frame;
     if (n_records == 0) return KRIPKE_OK;
 
     // One scan at a time per handle (its accumulators are shared): a call on another stream waits for
@@ -998,7 +999,7 @@ int run_frames(kripke_programs *h, const DevicePlan &dp, const uint32_t *d_pairs
     h->last.executed_models = (uint64_t)(n_records - (family == KRIPKE_KERNEL_SCALAR ? 0u : dp.n_alias)) * h->last.models_per_program;
     h->last.sliced_logic_ops_per_word = dp.n_modal * n * n + dp.n_bool * n + (uint64_t)dp.n_slots * (n + 1);
     h->last.logic_instr_per_frame = (double)h->last.sliced_logic_ops_per_word * (double)(1ull << (k * n)) / 32.0;
-    h->last.dense_logic_instr_per_frame = h->last.logic_instr_per_frame;
+    h->last.popc_instr_per_frame = (double)dp.n_slots * (double)(1ull << (k * n)) / 32.0;
     h->last.kernel_family = family == KRIPKE_KERNEL_SCALAR ? 0 : 1;
     if (n_records == 0) return KRIPKE_OK;
     if (!h->done) CU(cudaEventCreateWithFlags(&h->done, cudaEventDisableTiming));
