@@ -103,16 +103,16 @@ struct JitLayout {
     uint32_t lane_bits = 0;        // density kernels, one frame per lane: bits 5.. of X taken from the thread's lane
                                    // (= the low bits of its unit index), so that a warp's words are consecutive
     bool table = false;            // frames come from the class table (S4 / S5)
-    uint32_t nest_bits = 0;        // the nest_bits slowest bits of the inner loop get a two-iteration loop each, the slowest
-                                   // outermost, around one loop over the remaining bits: a value that depends only on slow
-                                   // bits is computed in the loop of the fastest bit it depends on (levels 2 .. 2 + nest_bits),
-                                   // not once per word
+    uint32_t nest_first = 0;       // 0: the inner loop is one loop.  Else it is a nest: one loop over the nest_first slowest
+                                   // valuation bits, then a two-iteration loop for each remaining bit, slower bits outside:
+                                   // a value that depends only on slow bits is computed in the loop of the fastest bit it
+                                   // depends on (levels 2 .. 2 + inner - nest_first), not once per word
 };
 // Is there a compiled layout for (n, g, class)?  Fills *out.
 bool jit_layout(uint32_t n, uint32_t g, uint32_t cls, JitLayout *out);
 
 // Loop level at which a bit of the model index changes in a thread (0 = fixed for the unit, 1 = outer loop,
-// 2 = inner loop; nested layouts: 2 + j for the j-th slowest bit of the inner loop, 2 + nest_bits for the rest) for "p_i at world w" and for the edge w -> u (0 where the edge is no index bit: class T's
+// 2 = inner loop; nested layouts: 2 for the nest_first slowest bits of the inner loop, then one level per bit) for "p_i at world w" and for the edge w -> u (0 where the edge is no index bit: class T's
 // diagonal, the table classes), and the cost of one instruction at a level per 32-model word.
 int jit_atom_level(const JitLayout &lay, uint32_t var, uint32_t w);
 int jit_edge_level(const JitLayout &lay, uint32_t w, uint32_t u);
