@@ -317,6 +317,47 @@ int kripke_eval_batch_host(const uint8_t *code, const uint32_t *offsets, uint32_
                            uint32_t n_worlds, uint32_t n_vars, uint32_t frame_class,
                            kripke_count_t *counts_host, kripke_witness_t *witness_host);
 
+/* The corpus scan for callers that cannot allocate device memory (Algorithm 1, on the scalar
+ * kernel; same results as kripke_eval_batch_range, bit for bit).
+ *
+ * Why it exists: kripke_programs_create and the scans on a handle call cudaMalloc - for the device copy of
+ * the programs, the per-formula accumulators, the S4 / S5 class table, compiled modules.  That rules the
+ * handle API out for a process whose device memory is entirely in the hands of another allocator (a torch
+ * job whose caching allocator owns the card, a server that reserved its HBM at start-up: cudaMalloc fails
+ * there, or takes memory the pool believes is its own), and for a loop that must not stall its other
+ * streams (cudaMalloc / cudaFree synchronise the whole device).  This call needs no handle and calls no
+ * cudaMalloc, cudaFree or allocating library routine: its working memory - accumulators, the staged
+ * programs, the class table - is one fixed block of KRIPKE_STATIC_SCRATCH_BYTES (about 0.8 MB) inside the
+ * library image.  Every GPU that loads the library holds that block until the process exits, used or not.
+ *
+ * Inputs: code / offsets are HOST pointers in the format of kripke_programs_create; they are validated the
+ * same way (same status codes) and read before the call returns - unless they lie in page-locked memory,
+ * in which case they must stay unchanged until `stream` has passed this call.  Outputs: counts_out /
+ * witness_out are the caller's DEVICE arrays of n_formulas entries, written on `stream`.  flags:
+ * KRIPKE_ACCUMULATE and KRIPKE_REDUCE_* only (anything else: KRIPKE_EINVAL).
+ *
+ * Limits, checked on the host before any CUDA call; beyond them the call returns KRIPKE_EUNSUPPORTED and
+ * touches nothing: n_formulas <= KRIPKE_STATIC_MAX_FORMULAS; for S4 / S5 the class must have at most
+ * KRIPKE_STATIC_MAX_CLASS_FRAMES frames (true for n_worlds <= 5: 6,942 preorders, 52 equivalences).
+ *
+ * First call on a device: looks up the device address of the block (cudaGetSymbolAddress) with that device
+ * current and remembers it; make that first call outside any stream capture.
+ *
+ * Sharing: all calls on a device use the same block, and it still holds the previous call's contents when
+ * the next one starts; each call re-initialises what it reads.  Calls whose device work can overlap -
+ * different streams with no event between them, concurrent host threads - race on the block and produce
+ * garbage: keep them on one stream or order them with events.
+ *
+ * Throughput is the scalar kernel's (one model per thread iteration), far below the compiled engine's:
+ * this is the escape hatch, not the fast path. */
+#define KRIPKE_STATIC_MAX_FORMULAS 8192u
+#define KRIPKE_STATIC_MAX_CLASS_FRAMES 8192u
+#define KRIPKE_STATIC_SCRATCH_BYTES 819456u
+int kripke_eval_batch_static(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,
+                             uint32_t n_worlds, uint32_t n_vars, uint32_t frame_class,
+                             uint64_t frame_begin, uint64_t frame_count, uint32_t flags,
+                             kripke_count_t *counts_out, kripke_witness_t *witness_out, void *stream);
+
 /* What the last eval / pairs call on this handle executed (host-side bookkeeping, valid right
  * after the call returns). */
 typedef struct {

@@ -40,7 +40,7 @@ EXPORTS = [
     "kripke_validity_bitmap", "kripke_condition_bitmap", "kripke_match_bitmaps", "kripke_frames_from_bitmap",
     "kripke_failure_density", "kripke_failure_density_frames",
     "kripke_jit_configure", "kripke_debug_jit_source", "kripke_debug_dag_truth", "kripke_signatures", "kripke_frames_generate",
-    "kripke_debug_batch_refuted",
+    "kripke_debug_batch_refuted", "kripke_eval_batch_static",
 ]
 
 
@@ -109,6 +109,7 @@ def load():
                                             ctypes.POINTER(u32), ctypes.POINTER(u64), ctypes.POINTER(u64)]
     lib.kripke_debug_dag_truth.argtypes = [u8p, u32, u32, u32, u32p, u32p, ctypes.POINTER(u32)]
     lib.kripke_debug_batch_refuted.argtypes = [vp, vp, u32, u32, u32, u32, u32, vp, vp, vp]
+    lib.kripke_eval_batch_static.argtypes = [u8p, u32p, u32, u32, u32, u32, u64, u64, u32, vp, vp, vp]
     for name in EXPORTS:
         if name not in ("kripke_version",):
             getattr(lib, name).restype = ctypes.c_int
@@ -220,6 +221,30 @@ def eval_batch_range(programs: Programs, n_worlds: int, n_vars: int, frame_class
                                           frame_count, flags, counts_out.data_ptr(),
                                           witness_out.data_ptr(), _stream(stream)),
            "kripke_eval_batch_range")
+    return counts_out, witness_out
+
+
+STATIC_MAX_FORMULAS = 8192
+STATIC_MAX_CLASS_FRAMES = 8192
+STATIC_SCRATCH_BYTES = 819456
+
+
+def eval_batch_static(code, offsets, n_worlds: int, n_vars: int, frame_class: int, frame_begin: int,
+                      frame_count: int, counts_out, witness_out, flags: int = 0, stream=None):
+    """kripke_eval_batch_static: the scan for callers that cannot allocate device memory (their memory
+    belongs to another pool, or they cannot take cudaMalloc's device-wide synchronisation).  No handle:
+    code / offsets are the HOST program arrays, counts_out / witness_out the caller's own int64 CUDA
+    tensors of shape (B, 2) - unlike the other wrappers this one never creates a tensor, so the call
+    allocates nothing on the device.  Working memory is the library's fixed static block; calls that
+    overlap on the GPU race on it."""
+    code, offsets = _host(code, offsets)
+    n = len(offsets) - 1
+    assert counts_out is not None and witness_out is not None, "the caller provides the output tensors"
+    _outputs(n, counts_out, witness_out)
+    _check(load().kripke_eval_batch_static(code.ctypes.data, offsets.ctypes.data, n, n_worlds, n_vars,
+                                           frame_class, frame_begin, frame_count, flags,
+                                           counts_out.data_ptr(), witness_out.data_ptr(), _stream(stream)),
+           "kripke_eval_batch_static")
     return counts_out, witness_out
 
 

@@ -28,6 +28,7 @@ UNITS = [
     ("lower", "lower.cpp", []),
     ("sliced_dispatch", "sliced_dispatch.cpp", []),
     ("scan_scalar", "scan_scalar.cu", []),
+    ("scan_static", "scan_static.cu", []),
     ("calibrate", "calibrate.cu", []),
     ("scan_frames", "scan_frames.cu", []),
     ("bitmaps", "bitmaps.cu", []),

@@ -176,6 +176,10 @@ std::map<std::tuple<int, uint32_t, uint32_t>, uint64_t *> g_tables_dev;
 
 namespace kripke {
 
+// For entry points that live in other translation units (scan_static.cu): record a cudaError_t where
+// kripke_last_cuda_error() finds it and return KRIPKE_ECUDA.
+int note_cuda_error(int e) { return cuda_fail(e); }
+
 const std::vector<uint64_t> *class_table_host(uint32_t n, uint32_t cls) {
     std::lock_guard<std::mutex> lock(g_table_mutex);
     auto key = std::make_pair(n, cls);

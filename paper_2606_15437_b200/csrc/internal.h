@@ -136,6 +136,10 @@ int launch_witness_keys(bool to_keys, const void *src, uint32_t n_records, uint3
 // Calibration kernels.
 int run_calibration(uint32_t variant, double *rate_out, double *ms_out, void *stream);
 
+// ---- error bookkeeping (api.cpp) ---------------------------------------------------------------
+// Stores e (a cudaError_t) as this thread's last CUDA error and returns KRIPKE_ECUDA.
+int note_cuda_error(int e);
+
 // ---- class tables (api.cpp) --------------------------------------------------------------------
 // Host: ascending K-indices of the class members (S4 / S5), n <= 5 here; cached.
 const std::vector<uint64_t> *class_table_host(uint32_t n, uint32_t cls);
