@@ -403,22 +403,24 @@ int kripke_last_run_info(const kripke_programs_t *programs, kripke_run_info_t *i
  * Affects plans built afterwards. */
 int kripke_jit_configure(uint32_t max_programs_per_kernel, uint32_t min_blocks_per_sm);
 
-/* Diagnostic (pure host: works without a CUDA device): the CUDA C source of compiled kernel kernel_index
- * of the group of programs that mention group_vars variables, for the given batch (HOST code / offsets as
- * in kripke_programs_create; pairs == NULL) or the listed pairs of it, as kripke_eval_batch_range / kripke_distinguish_pairs would build it for
- * (n_worlds, frame_class, flags).  compile: bit 0 = also compile it with NVRTC to an sm_100a cubin
- * (*cubin_bytes_out); bit 1 = the failure-density kernel of kripke_failure_density instead of the scan kernel.  source_out (capacity cap, NUL-terminated, may be NULL), *n_kernels_out = kernels of the
- * group, *logic_ops_per_word_out = 3-input logic instructions per 32-model word of this kernel.  Returns the
- * source length or a negative kripke_status (KRIPKE_EUNSUPPORTED: no compiled layout for the shape). */
+/* Diagnostic (pure host: works without a CUDA device): the CUDA C source of one compiled kernel, exactly as
+ * kripke_eval_batch_range / kripke_distinguish_pairs would build it for (n_worlds, frame_class, flags).
+ *   batch:        HOST code / offsets as in kripke_programs_create; pairs == NULL for the batch itself, or a
+ *                 HOST list of n_pairs pairs of it.
+ *   group_vars:   the group of programs that mention this many variables.
+ *   kernel_index: which kernel of that group.
+ *   compile:      bit 0 = also compile the source with NVRTC to an sm_100a cubin (*cubin_bytes_out);
+ *                 bit 1 = the failure-density kernel of kripke_failure_density instead of the scan kernel.
+ *   source_out:   capacity cap, NUL-terminated, may be NULL.
+ *   *n_kernels_out = kernels of the group; *logic_ops_per_word_out = 3-input logic instructions per 32-model
+ *                 word of this kernel.
+ * Returns the source length or a negative kripke_status (KRIPKE_EUNSUPPORTED: no compiled layout for the
+ * shape). */
 int kripke_debug_jit_source(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas, uint32_t n_vars,
                             const uint32_t *pairs, uint32_t n_pairs, uint32_t n_worlds, uint32_t frame_class, uint32_t flags, uint32_t group_vars,
                             uint32_t kernel_index, int compile, char *source_out, uint64_t cap,
                             uint32_t *n_kernels_out, uint64_t *logic_ops_per_word_out, uint64_t *cubin_bytes_out);
 
-/* Diagnostic (pure host): the truth set (n-bit mask) of one program on one model as the batch graph of the
- * compiled scans computes it - after every rewrite (negation edges, and / box normal form, box
- * distribution, canonical variable order).  succ: n_worlds successor masks; val: n_vars variable masks.
- * Returns the number of graph nodes or a negative kripke_status. */
 /* Diagnostic, host only: for every formula of a batch, whether the model (succ[w] successor masks, val[i] variable
  * masks) refutes it, evaluated on the forms the compiled kernels of (n_worlds, frame_class, flags) evaluate - the
  * batch graph after the guarded-root and box-distribution rewrites, under each record's canonical variable
@@ -427,6 +429,10 @@ int kripke_debug_batch_refuted(const uint8_t *code, const uint32_t *offsets, uin
                                uint32_t n_worlds, uint32_t frame_class, uint32_t flags, const uint32_t *succ,
                                const uint32_t *val, uint8_t *refuted_out);
 
+/* Diagnostic (pure host): the truth set (n-bit mask) of one program on one model as the batch graph of the
+ * compiled scans computes it - after every rewrite (negation edges, and / box normal form, box
+ * distribution, canonical variable order).  succ: n_worlds successor masks; val: n_vars variable masks.
+ * Returns the number of graph nodes or a negative kripke_status. */
 int kripke_debug_dag_truth(const uint8_t *code, uint32_t len, uint32_t n_vars, uint32_t n_worlds,
                            const uint32_t *succ, const uint32_t *val, uint32_t *truth_out);
 
