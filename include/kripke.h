@@ -149,7 +149,11 @@ int kripke_validate_programs(const uint8_t *code, const uint32_t *offsets, uint3
  * device memory owned by the handle).  code / offsets are HOST pointers and are not retained. */
 int kripke_programs_create(const uint8_t *code, const uint32_t *offsets, uint32_t n_formulas,
                            uint32_t n_vars, kripke_programs_t **programs_out);
-int kripke_programs_destroy(kripke_programs_t *programs);   /* synchronises the device first */
+/* Waits until the device has finished the work enqueued on this handle, then frees what it holds.  A handle
+ * that only ran scans (kripke_eval_batch*, kripke_distinguish_pairs*, kripke_eval_frames) waits for its own
+ * last scan and does not disturb other streams; one that also ran bitmaps, densities, signatures or the size
+ * loop waits for the whole device. */
+int kripke_programs_destroy(kripke_programs_t *programs);
 
 /* Number of distinct labelled frames in a class (2^(n*n), 2^(n*n-n), preorders, equivalences). */
 int kripke_class_size(uint32_t n_worlds, uint32_t frame_class, uint64_t *size_out);
@@ -402,6 +406,16 @@ int kripke_last_run_info(const kripke_programs_t *programs, kripke_run_info_t *i
  * request of the generated kernels (128 threads per block; default 2, i.e. up to 255 registers per thread).
  * Affects plans built afterwards. */
 int kripke_jit_configure(uint32_t max_programs_per_kernel, uint32_t min_blocks_per_sm);
+
+/* Drops everything the process has cached about compiled scans: the plans kept per batch (keyed by the batch's
+ * bytes, shape, class and flags) and every loaded module, which is unloaded from the device.  The caches never
+ * shrink by themselves - a process that stages corpus after corpus calls this between them to give the host and
+ * device memory back - and the next scan of any batch pays the emitter, NVRTC and the module load again (it is
+ * also how bench.py measures that cold cost).  Plans cached inside live handles hold kernels of these modules,
+ * so the call is refused with KRIPKE_EINVAL while any kripke_programs_t exists; it waits for the device to go
+ * idle first (a destroyed handle's last scan may still be running).  *modules_unloaded_out (optional) = number of
+ * modules that were loaded. */
+int kripke_jit_cache_clear(uint32_t *modules_unloaded_out);
 
 /* Diagnostic (pure host: works without a CUDA device): the CUDA C source of one compiled kernel, exactly as
  * kripke_eval_batch_range / kripke_distinguish_pairs would build it for (n_worlds, frame_class, flags).

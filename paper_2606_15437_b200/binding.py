@@ -41,6 +41,7 @@ EXPORTS = [
     "kripke_failure_density", "kripke_failure_density_frames",
     "kripke_jit_configure", "kripke_debug_jit_source", "kripke_debug_dag_truth", "kripke_signatures", "kripke_frames_generate",
     "kripke_debug_batch_refuted", "kripke_eval_batch_static",
+    "kripke_jit_cache_clear",
 ]
 
 
@@ -103,6 +104,7 @@ def load():
     lib.kripke_eval_frames.argtypes = [vp, u32, u32, vp, u64, u64, u32, vp, vp, vp]
     lib.kripke_distinguish_pairs_frames.argtypes = [vp, u32p, u32, u32, u32, vp, u64, u64, u32, vp, vp, vp]
     lib.kripke_jit_configure.argtypes = [u32, u32]
+    lib.kripke_jit_cache_clear.argtypes = [ctypes.POINTER(u32)]
     lib.kripke_signatures.argtypes = [vp, u32, u32, vp, vp]
     lib.kripke_frames_generate.argtypes = [u32, u32, u64, u64, vp, vp]
     lib.kripke_debug_jit_source.argtypes = [u8p, u32p, u32, u32, u32p, u32, u32, u32, u32, u32, u32, ctypes.c_int, vp, u64,
@@ -222,6 +224,14 @@ def eval_batch_range(programs: Programs, n_worlds: int, n_vars: int, frame_class
                                           witness_out.data_ptr(), _stream(stream)),
            "kripke_eval_batch_range")
     return counts_out, witness_out
+
+
+def jit_cache_clear() -> int:
+    """kripke_jit_cache_clear: forget every cached plan and unload every compiled module (no Programs object
+    may be alive).  Returns the number of modules unloaded."""
+    n = ctypes.c_uint32(0)
+    _check(load().kripke_jit_cache_clear(ctypes.byref(n)), "kripke_jit_cache_clear")
+    return n.value
 
 
 STATIC_MAX_FORMULAS = 8192

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -250,6 +251,8 @@ struct kripke_programs {
     cudaEvent_t done = nullptr;        // end of the last scan enqueued on this handle
     void *last_stream = nullptr;
     bool has_last = false;
+    bool aux_work = false;             // something other than a scan (bitmaps, densities, signatures, the size loop's
+                                       // record kernel) was enqueued on this handle's memory: not covered by `done`
     DevicePlan list_single;            // frame-list mode: every formula lowered without derived leaves
     bool list_single_built = false;
     DevicePlan list_pair;              // plan of the last pair list given to kripke_distinguish_pairs_frames
@@ -397,10 +400,22 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *h_pairs, 
     job.pairs = d_pairs; job.n_records = n_records;
     job.accum = h->d_accum;
 
+    // A forced compiled scan needs a unit-aligned range: refused here, before anything is enqueued.
+    if (family == KRIPKE_KERNEL_JIT)
+        for (const GroupPlan &g : plan.groups)
+            if (g.use_jit) {
+                const uint64_t fpu = 1ull << g.jit.lay.unit_frames_log2;
+                if (begin % fpu || (begin + count) % fpu) return KRIPKE_EUNSUPPORTED;
+            }
+
     int e = launch_init(job.accum, n_records, stream);
     if (e) return cuda_fail(e);
     uint32_t launches = 1;
 
+    // Everything from here on works on the handle's accumulators.  Whatever this call manages to enqueue - also
+    // when it then gives up (a forced family that does not fit, a failed launch) - has to be ordered before the
+    // next call on the handle, so the enqueueing is one function and the event is recorded on every way out.
+    auto enqueue = [&]() -> int {
     if (family == KRIPKE_KERNEL_SCALAR) {
         if ((e = launch_scalar(job, nullptr, n_records, reduce, stream, &launches))) return cuda_fail(e);
     }
@@ -503,10 +518,15 @@ int run_scan(kripke_programs *h, const ScanPlan &plan, const uint32_t *h_pairs, 
             }
     if ((e = launch_finish(job, (flags & KRIPKE_ACCUMULATE) != 0, counts_out, witness_out, stream)))
         return cuda_fail(e);
-    h->last.launches = launches + 1;
-    CU(cudaEventRecord(h->done, (cudaStream_t)stream));
+    return KRIPKE_OK;
+    };
+    rc = enqueue();
+    const cudaError_t recorded = cudaEventRecord(h->done, (cudaStream_t)stream);
     h->last_stream = stream;
     h->has_last = true;
+    if (rc) return rc;
+    if (recorded != cudaSuccess) return cuda_fail((int)recorded);
+    h->last.launches = launches + 1;
     return KRIPKE_OK;
 }
 
@@ -749,6 +769,7 @@ struct CachedJitPlan {
 };
 std::mutex g_plan_cache_mutex;
 std::map<std::string, CachedJitPlan> g_plan_cache;
+std::atomic<int> g_live_handles{0};            // kripke_programs_t objects alive (their plans hold kernel handles)
 uint64_t g_plan_cache_clock = 0;
 constexpr size_t PLAN_CACHE_ENTRIES = 32;
 
@@ -1065,6 +1086,7 @@ int kripke_validity_bitmap(const kripke_programs_t *programs, uint32_t n_worlds,
     if ((rc = class_table_device(n_worlds, frame_class, &job.class_table))) return rc;
     job.code = h->d_code; job.offsets = h->d_offsets; job.n_formulas = h->n_formulas;
     job.pairs = nullptr; job.n_records = h->n_formulas; job.accum = nullptr;
+    const_cast<kripke_programs *>(programs)->aux_work = true;
     int e = launch_validity_bitmap(job, bitmap_out, stream);
     return e ? cuda_fail(e) : KRIPKE_OK;
 }
@@ -1097,6 +1119,7 @@ int kripke_failure_density(const kripke_programs_t *programs, uint32_t n_worlds,
     if (rc) return rc;
     if (frame_begin > csize || frame_count > csize - frame_begin) return KRIPKE_EINVAL;
     if (frame_count && h->n_formulas && !counts_out) return KRIPKE_EINVAL;
+    h->aux_work = true;
     ScanJob job;
     job.n = n_worlds; job.k = n_vars; job.cls = frame_class;
     job.frame_begin = frame_begin; job.frame_count = frame_count;
@@ -1174,6 +1197,7 @@ int kripke_failure_density_frames(const kripke_programs_t *programs, uint32_t n_
     job.frame_begin = 0; job.frame_count = n_frames; job.class_table = nullptr;
     job.code = h->d_code; job.offsets = h->d_offsets; job.n_formulas = h->n_formulas;
     job.pairs = nullptr; job.n_records = h->n_formulas; job.accum = nullptr;
+    const_cast<kripke_programs *>(programs)->aux_work = true;
     int e = launch_failure_density(job, succ, counts_out, n_frames, 0, stream);
     return e ? cuda_fail(e) : KRIPKE_OK;
 }
@@ -1194,6 +1218,7 @@ int kripke_signatures(const kripke_programs_t *programs, uint32_t n_vars, uint32
     if (n_vars != h->n_vars || n_max < 1 || n_max > 4) return KRIPKE_EINVAL;
     if (n_max * n_max + n_vars * n_max > 40) return KRIPKE_EUNSUPPORTED;
     if (h->n_formulas && !sig_out) return KRIPKE_EINVAL;
+    const_cast<kripke_programs *>(programs)->aux_work = true;
     int e = launch_signatures(n_vars, n_max, h->d_code, h->d_offsets, h->n_formulas, sig_out, stream);
     return e ? cuda_fail(e) : KRIPKE_OK;
 }
@@ -1288,6 +1313,7 @@ int kripke_programs_create(const uint8_t *code, const uint32_t *offsets, uint32_
     if (rc) return rc;
     kripke_programs *h = new (std::nothrow) kripke_programs();
     if (!h) return KRIPKE_ENOMEM;
+    ++g_live_handles;
     h->n_formulas = n_formulas;
     h->n_vars = n_vars;
     h->h_offsets.assign(offsets, offsets + n_formulas + 1);
@@ -1313,7 +1339,11 @@ int kripke_programs_create(const uint8_t *code, const uint32_t *offsets, uint32_
 
 int kripke_programs_destroy(kripke_programs_t *h) {
     if (!h) return KRIPKE_OK;
-    cudaDeviceSynchronize();
+    // A handle that only ran scans waits for its own last scan (every scan records h->done, on every exit path)
+    // and leaves other handles' streams alone; one that also enqueued other work on its memory, possibly on
+    // several streams, has no single event for it and waits for the device.
+    if (h->aux_work) cudaDeviceSynchronize();
+    else if (h->has_last && h->done) cudaEventSynchronize(h->done);
     for (auto &kv : h->single) kv.second.release();
     for (auto &kv : h->density) kv.second.release();
     for (kripke_programs::PairPlan *pp : h->pair_plans) { pp->plan.release(); cudaFree(pp->d_pairs); delete pp; }
@@ -1322,6 +1352,20 @@ int kripke_programs_destroy(kripke_programs_t *h) {
     cudaFree(h->d_code); cudaFree(h->d_offsets); cudaFree(h->d_pairs); cudaFree(h->d_accum);
     cudaFree(h->d_tmp_counts); cudaFree(h->d_tmp_wit);
     delete h;
+    --g_live_handles;
+    return KRIPKE_OK;
+}
+
+int kripke_jit_cache_clear(uint32_t *modules_unloaded_out) {
+    if (modules_unloaded_out) *modules_unloaded_out = 0;
+    if (g_live_handles.load() > 0) return KRIPKE_EINVAL;      // their cached plans point into the modules
+    CU(cudaDeviceSynchronize());                              // a destroyed handle's last scan may still be running
+    {
+        std::lock_guard<std::mutex> lock(g_plan_cache_mutex);
+        g_plan_cache.clear();
+    }
+    const size_t n = jit_cache_clear();
+    if (modules_unloaded_out) *modules_unloaded_out = (uint32_t)n;
     return KRIPKE_OK;
 }
 
@@ -1375,6 +1419,7 @@ int kripke_minimal_refutation(const kripke_programs_t *programs, uint32_t n_vars
     kripke_programs *h = const_cast<kripke_programs *>(programs);
     const uint32_t B = h->n_formulas;
     if (B && (!size_out || !counts_out || !witness_out)) return KRIPKE_EINVAL;
+    h->aux_work = true;                       // the record kernel reads d_tmp_* after the scan's event
     if (B > h->tmp_cap) {
         cudaFree(h->d_tmp_counts); cudaFree(h->d_tmp_wit);
         h->d_tmp_counts = nullptr; h->d_tmp_wit = nullptr; h->tmp_cap = 0;

@@ -224,5 +224,9 @@ int jit_launch_group(const ScanJob &job, const JitGroupPlan &plan, uint32_t mode
 
 // Compiles one source to a cubin without loading it (tests on a box without a GPU): 0 or error.
 int jit_compile_only(const std::string &source, std::string *log_out, size_t *cubin_bytes);
+// Unloads every compiled module of the process-wide cache and forgets it; returns how many there were.  Only
+// safe when no plan that holds one of their kernels can be launched again and none is running (api.cpp checks).
+size_t jit_cache_clear();
+size_t jit_cache_modules();
 
 }  // namespace kripke

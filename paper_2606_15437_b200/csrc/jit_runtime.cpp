@@ -37,7 +37,8 @@ struct Module {
 };
 
 std::mutex g_cache_mutex;
-std::map<std::string, Module> g_cache;     // source text -> loaded module (never unloaded: a few MB at most)
+// source text -> loaded module.  Modules stay loaded until jit_cache_clear(): plans hold their kernel handles.
+std::map<std::string, Module> g_cache;
 
 int compile(const std::string &src, std::vector<char> *cubin, std::string *log) {
     nvrtcProgram prog = nullptr;
@@ -71,6 +72,20 @@ void JitGroupPlan::release() {
     d_slot_record = d_row_begin = d_rows = nullptr;
     kernels.clear();
     n_slots = 0;
+}
+
+size_t jit_cache_clear() {
+    std::lock_guard<std::mutex> lock(g_cache_mutex);
+    const size_t n = g_cache.size();
+    for (auto &kv : g_cache)
+        if (kv.second.lib) cudaLibraryUnload(kv.second.lib);
+    g_cache.clear();
+    return n;
+}
+
+size_t jit_cache_modules() {
+    std::lock_guard<std::mutex> lock(g_cache_mutex);
+    return g_cache.size();
 }
 
 int jit_compile_only(const std::string &source, std::string *log_out, size_t *cubin_bytes) {
@@ -142,12 +157,17 @@ int jit_build_group(const Dag &dag, const JitLayout &lay, const std::vector<JitR
         {
             std::lock_guard<std::mutex> lock(g_cache_mutex);
             for (size_t t = 0; t < todo.size(); ++t) {
+                // another thread may have compiled and loaded the same source since `todo` was made: keep its module
+                if (g_cache.count(sources[todo[t]])) continue;
                 Module m;
                 cudaError_t e = cudaLibraryLoadData(&m.lib, cubins[t].data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
                 if (e == cudaSuccess) e = cudaLibraryGetKernel(&m.kernel, m.lib, "kripke_jit_scan");
                 cudaFuncAttributes attr;
                 if (e == cudaSuccess) e = cudaFuncGetAttributes(&attr, (const void *)m.kernel);
-                if (e != cudaSuccess) return (int)e;
+                if (e != cudaSuccess) {
+                    if (m.lib) cudaLibraryUnload(m.lib);
+                    return (int)e;
+                }
                 m.regs = attr.numRegs;
                 m.local_bytes = (int)attr.localSizeBytes;
                 g_cache.emplace(sources[todo[t]], m);

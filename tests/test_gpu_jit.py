@@ -245,3 +245,60 @@ def test_exchange_step_on_one_device(kb, vol):
             second = np.nonzero((first["wit_f"] == O.NO_WITNESS) & (got["wit_f"] != O.NO_WITNESS))[0]
             if cut == 1:
                 assert len(second) >= 3, "records whose least (f, v) lies in the second range"
+
+
+def test_cache_clear_recompiles_and_gives_the_same_records(kb):
+    """kripke_jit_cache_clear: refused while a handle exists (its plans hold kernels of the cached modules);
+    with none alive it unloads the modules, and the next scan of the same batch compiles again and returns the
+    same records."""
+    import gc
+    import torch
+    gc.collect()
+    progs = corpus(2)[:60]
+    h = kb.Programs(*W.pack_programs(progs), 2)
+    before = scan(kb, h, 4, 2, K, 0, 1 << 16)
+    assert h.last_run_info().kernel_family == 2
+    with pytest.raises(kb.KripkeError) as err:
+        kb.jit_cache_clear()
+    assert err.value.status == kb.EINVAL
+    h.destroy()
+    assert kb.jit_cache_clear() >= 1                 # at least this batch's module was loaded
+    assert kb.jit_cache_clear() == 0                 # nothing left
+    h = kb.Programs(*W.pack_programs(progs), 2)
+    after = scan(kb, h, 4, 2, K, 0, 1 << 16)
+    assert h.last_run_info().jit_compile_seconds > 0  # rebuilt, not found in a cache
+    same(after, before, "after a cache clear")
+    again = scan(kb, h, 4, 2, K, 0, 1 << 16)
+    torch.cuda.synchronize()
+    same(again, before, "second scan on the rebuilt plan")
+    h.destroy()
+
+
+def test_two_handles_on_two_streams_and_a_refused_call_in_between(kb, vol):
+    """Two handles scan on their own streams; one is destroyed while the other still has work queued (destroy
+    waits for the handle's own last scan only); a forced-family call that is refused (unaligned range for the
+    compiled kernels) sits between two good scans of the same handle on different streams and must not disturb
+    either.  Every record equals the oracle's."""
+    import torch
+    progs_a, progs_b = corpus(2)[:120], corpus(1)[:40]
+    code_a, offs_a = W.pack_programs(progs_a)
+    code_b, offs_b = W.pack_programs(progs_b)
+    want_a = vol.census(code_a, offs_a, 4, 2, K, 1 << 12, 1 << 13)
+    want_a2 = vol.census(code_a, offs_a, 4, 2, K, 3, 1000)
+    want_b = vol.census(code_b, offs_b, 4, 1, T, 0, 1 << 12)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    ha, hb = kb.Programs(code_a, offs_a, 2), kb.Programs(code_b, offs_b, 1)
+    ca, wa = kb.eval_batch_range(ha, 4, 2, K, 1 << 12, 1 << 13, 0, stream=s1)
+    cb, wb = kb.eval_batch_range(hb, 4, 1, T, 0, 1 << 12, 0, stream=s2)
+    with pytest.raises(kb.KripkeError) as err:                       # 3 is not a multiple of the scan unit
+        kb.eval_batch_range(ha, 4, 2, K, 3, 1000, kb.KERNEL_JIT, stream=s2)
+    assert err.value.status == kb.EUNSUPPORTED
+    hb.destroy()                                                     # ha's scan on s1 may still be running
+    torch.cuda.synchronize()
+    got_a, got_b = kb.unpack(ca, wa), kb.unpack(cb, wb)
+    ca2, wa2 = kb.eval_batch_range(ha, 4, 2, K, 3, 1000, 0, stream=s2)   # same handle, other stream, ragged range
+    torch.cuda.synchronize()
+    same(got_a, want_a, "handle a, stream 1")
+    same(got_b, want_b, "handle b, stream 2")
+    same(kb.unpack(ca2, wa2), want_a2, "handle a again on stream 2 after the refused call")
+    ha.destroy()
