@@ -177,6 +177,41 @@ def paper_corpus(kb):
     return reps + [W.to_postfix(W.named_axioms()["K"])], len(progs), len(reps)
 
 
+def check_results(kb, args, progs, counts, wits):
+    """What the timed steps left in the device tensors, looked at after the timed region: a SHA-256 over the four
+    classes' (models, frames) arrays; the rows with closed forms (F refuted by every model, T and the K axiom by
+    none); and, for the contract corpus, the S4 / S5 records against tests/golden/n5_s4s5.npz (written by the
+    oracle, tests/golden/make_golden.py).  A mismatch ends the run: a wrong scan has no throughput."""
+    import hashlib
+    res = {c: kb.unpack(counts[c], wits[c]) for c, _ in CLASSES}
+    sha = hashlib.sha256()
+    for c, _ in CLASSES:
+        sha.update(np.ascontiguousarray(res[c]["models"]).tobytes())
+        sha.update(np.ascontiguousarray(res[c]["frames"]).tobytes())
+    done = ["sha256 over models|frames of K, T, S4, S5"]
+    if args.workload in ("c3", "c3_paper"):
+        sizes = class_sizes_n5()
+        nval = 1 << (N_VARS * N_WORLDS)
+        probes = {"F": W.to_postfix(W.parse("F")), "T": W.to_postfix(W.parse("T")), "K axiom": W.to_postfix(W.named_axioms()["K"])}
+        for name, code in probes.items():
+            for b in [i for i, p in enumerate(progs) if p == code][:1]:
+                for c, _ in CLASSES:
+                    want_f = sizes[c] if name == "F" else 0
+                    got = (int(res[c]["models"][b]), int(res[c]["frames"][b]))
+                    if got != (want_f * nval, want_f):
+                        raise SystemExit(f"bench.py: result check failed: {name} on class {c}: {got}")
+                done.append(f"closed form: {name} (formula {b}) on all four classes")
+    gold = os.path.join(ROOT, "tests", "golden", "n5_s4s5.npz")
+    if args.workload == "c3" and os.path.exists(gold):
+        g = np.load(gold)
+        for c in ("S4", "S5"):
+            for key in ("models", "frames", "wit_f", "wit_v", "wit_w"):
+                if not np.array_equal(np.asarray(res[c][key]).astype(np.uint64), g[f"{c}_{key}"].astype(np.uint64)):
+                    raise SystemExit(f"bench.py: result check failed: class {c} {key} differs from tests/golden/n5_s4s5.npz")
+        done.append("S4 and S5 records (counts and witnesses, every formula) equal the oracle's golden file")
+    return {"counts_sha256": sha.hexdigest(), "checked": done}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -297,30 +332,40 @@ def run_ours(args):
     ms_per_step = ms_total / args.steps
     value = evals_alg1 / (ms_per_step * 1e-3)
 
-    # end to end through the host-buffer entry point: H2D of programs, plan building, scan, D2H of results.
-    # The compiled kernels are cached per process by source text, so these steps emit the source again and hit
-    # the cache; the one-off NVRTC compilation is reported beside it (jit_compile_seconds).
+    # end to end through the host-buffer entry point (kripke_eval_batch_host): H2D of the programs, plan look-up,
+    # scan, D2H of the records.  These steps are WARM: every call creates a new handle with the same program bytes
+    # and finds the finished plan in the process-wide plan cache (keyed by those bytes), so nothing is emitted or
+    # compiled again - the figure is the cost of a repeated scan of a corpus the process has seen.  The cost of the
+    # first scan of a fresh corpus (emitter + NVRTC + module load) is measured separately below as e2e["cold"].
     e2e = None
+    check = None
     if rank == 0 and args.e2e_steps > 0:
         times = []
-        for _ in range(args.e2e_steps):
+        host_res = {}
+        for _ in range(max(args.e2e_steps, 1)):
             torch.cuda.synchronize()
             t0 = time.perf_counter()
             for cname, cls in CLASSES:
                 if args.workload in ("c3", "c3_paper"):
-                    kb.eval_batch_host(code, offs, N_WORLDS, N_VARS, cls)
+                    host_res[cname] = kb.eval_batch_host(code, offs, N_WORLDS, N_VARS, cls)
                 else:   # reduced ranges are not expressible through the host entry point
                     hh = kb.Programs(code, offs, N_VARS)
                     c, w = kb.eval_batch_range(hh, N_WORLDS, N_VARS, cls, 0, sizes[cname])
                     c.cpu(); w.cpu()
                     hh.destroy()
             times.append(time.perf_counter() - t0)
-        e2e = {"value": evals_alg1 / float(np.mean(times)), "unit": "evaluations/s",
+        e2e = {"value": evals_alg1 / float(np.median(times)), "unit": "evaluations/s",
                "h2d_bytes_per_step": int(4 * (code.nbytes + offs.nbytes)), "d2h_bytes_per_step": int(4 * 32 * B),
-               "seconds_per_step": float(np.mean(times)),
+               "seconds_per_step": float(np.median(times)), "samples": len(times), "statistic": "median",
+               "seconds_per_step_min_max": [float(min(times)), float(max(times))],
+               "state": "warm: amortised over repeated scans of a corpus whose compiled plan is cached in the process",
                "jit": f"kernels compiled with NVRTC once per process ({compile_s[0]:.2f} s for the class-K plan, paid "
-                      f"in the first warm-up step: {t_first:.2f} s); the timed e2e steps create a new handle, emit the "
-                      "sources again and hit the process-wide module cache"}
+                      f"in the first warm-up step: {t_first:.2f} s); the timed e2e steps create a new handle and find "
+                      "the finished plan in the process-wide plan cache"}
+
+    # what the timed region produced, checked after it (world == 1: the full ranges were scanned by this rank)
+    if rank == 0 and world == 1:
+        check = check_results(kb, args, progs, counts, wits)
 
     # ablation, one timed pass each after the timed region; the records are bit-identical in every mode (GPU tests)
     ablation = None
@@ -350,11 +395,29 @@ def run_ours(args):
             ablation[name] = {"what": what, "ms_per_step": ms, "value": evals_alg1 / (ms * 1e-3),
                               "executed_evaluations_per_step": ex, "executed_logic_instr_per_step": ops}
 
+    # cold end-to-end: the same host-buffer calls with every cached plan and compiled module dropped first, i.e.
+    # the first scan of a corpus the process has never seen (a census scans each batch once)
+    if rank == 0 and world == 1 and e2e is not None and args.workload in ("c3", "c3_paper") and not args.no_cold:
+        h.destroy()
+        torch.cuda.synchronize()
+        import gc
+        gc.collect()                     # handles of the ablation passes and of paper_corpus() are gone by now
+        unloaded = kb.jit_cache_clear()  # raises if a handle is still alive: then there is no cold figure to report
+        t0 = time.perf_counter()
+        for cname, cls in CLASSES:
+            kb.eval_batch_host(code, offs, N_WORLDS, N_VARS, cls)
+        cold = time.perf_counter() - t0
+        e2e["cold"] = {"value": evals_alg1 / cold, "unit": "evaluations/s", "seconds_per_step": cold, "samples": 1,
+                       "modules_unloaded_before": unloaded,
+                       "what": "kripke_jit_cache_clear(), then one pass through kripke_eval_batch_host: graph, rewrites, "
+                               "emitter, NVRTC for sm_100a, module load, scan, D2H (CUDA context and library already up)"}
+
     if rank == 0:
         k_exec = k_info["instr_per_frame"] * k_info["frames"]         # logic thread-instructions the class-K launches execute
         k_alg = k_info["alg_instr_per_frame"] * k_info["frames"]      # SURVEY 8(d)'s algorithmic count for the same call
         achieved = k_exec / (k_ms * 1e-3) / 1e12
-        peak = SM_COUNT * INT_LANES_PER_SM * 1.965e9 / 1e12        # derived ALU-pipe peak at max clock
+        peak_derived = SM_COUNT * INT_LANES_PER_SM * 1.965e9 / 1e12   # derived ALU-pipe peak at max clock
+        peak = cal["lop3"] / 1e12                                      # measured in this process, right before the timed runs
         cpu_rate, cpu_dt, cores, cpu_evals, cpu_alg1 = oracle_sample(W.corpus_c2() if args.workload != "c3_paper" else progs,
                                                                      args.ref_frames, repeats=3)
         label = {"c3": "C3 n=5 census layer (BASELINE.json configs[2]): 5,624 seeded formulas x K/T/S4/S5 frames of 5 "
@@ -389,23 +452,25 @@ def run_ours(args):
             },
             "clocks": clocks,
             "e2e": e2e,
+            "result_check": check,
             "gpu_launches": n_launches,
             "roofline": {
                 "bound": "alu", "kernel": "kripke_jit_scan (the compiled class-K launches of one step)",
                 "achieved": achieved, "peak": peak, "unit": "T thread-instr/s", "frac": achieved / peak,
                 "frac_executed": achieved / peak,
-                "frac_executed_of_measured_lop3": achieved / (cal["lop3"] / 1e12),
+                "peak_derived": peak_derived, "frac_of_peak_derived": achieved / peak_derived,
                 "executed_ops": "3-input logic (LOP3) thread-instructions the compiled kernels execute: one per emitted "
                                 "lop3.b32 (the emitter covers every expression tree with 3-input tables itself), weighted by "
                                 "loop level; cross-checked against ncu's opcode count in profiles/r2_jit_full.md",
                 "xu_pipe": {"popc_per_s_T": k_info["popc_per_frame"] * k_info["frames"] / (k_ms * 1e-3) / 1e12,
-                            "peak_T": peak / 4, "frac": k_info["popc_per_frame"] * k_info["frames"] / (k_ms * 1e-3) / 1e12 / (peak / 4),
+                            "peak_T": peak_derived / 4,
+                            "frac": k_info["popc_per_frame"] * k_info["frames"] / (k_ms * 1e-3) / 1e12 / (peak_derived / 4),
                             "what": "one POPC per scanned program and 32-model word counts the refuting models; POPC issues on "
                                     "the XU pipe at 16 lanes/clk/SM (a quarter of the ALU rate).  At the two warps per "
                                     "scheduler these kernels run with, ALU and XU time barely overlap (ncu: "
                                     "profiles/r2_jit_perkernel.md), so frac + xu_pipe.frac is the share of the step the two "
                                     "pipes account for"},
-                "frac_algorithmic": k_alg / (k_ms * 1e-3) / 1e12 / peak,
+                "frac_algorithmic": k_alg / (k_ms * 1e-3) / 1e12 / peak_derived,
                 "algorithmic_ops": "SURVEY 8(d): every formula as written, (d n^2 + b n + n + 1) logic instructions per "
                                    "32-model word x 2^(k_b n)/32 words per frame - work the method defines per peak-second; "
                                    "NOT a pipe fraction (sharing makes it exceed 1)",
@@ -413,7 +478,9 @@ def run_ours(args):
                 "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of the class-K kernels of one step, "
                                   "ncu launch list profiles/r2_jit_launches_c3.csv (bytes; algorithmic HBM bytes = 0)",
                 "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_per_step,
-                "peak_source": "derived: 148 SMs x 4 x 16 ALU lanes/clk x 1.965 GHz (DESIGN.md 6)",
+                "peak_source": "measured: kripke_calibrate_int32 variant 0 (register-resident independent LOP3 on every SM) "
+                               "in this process right before the timed runs; peak_derived = 148 SMs x 4 x 16 ALU "
+                               "lanes/clk x 1.965 GHz (DESIGN.md 6)",
                 "peak_measured_calibration": {k: v / 1e12 for k, v in cal.items()},
             },
             "ablation": ablation,
@@ -950,7 +1017,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c3", choices=["c3", "c3_paper", "c3_small", "c4", "c5", "atlas", "frames", "correspond"])
-    ap.add_argument("--e2e-steps", type=int, default=1)
+    ap.add_argument("--e2e-steps", type=int, default=5, help="warm end-to-end samples (median is reported); 0 = skip e2e, "
+                                                             "ablation and cold e2e")
+    ap.add_argument("--no-cold", action="store_true", help="skip the cold end-to-end pass (cache clear + recompilation)")
     ap.add_argument("--ref-frames", type=int, default=256)
     ap.add_argument("--c4-contention-frames", type=int, default=1 << 16,
                     help="frames of the three-variable contention leg on the scalar kernel (SURVEY 8(d) shape: 2^20, "
