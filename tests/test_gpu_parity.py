@@ -204,6 +204,12 @@ def test_c3_n5_full_corpus_witnesses(kb, vol):
     results = {}
     for cname, cls in CLS.items():
         results[cname] = run(kb, progs, 5, 2, cls, handle=h)
+    # the whole-batch, full-range class-K COUNTS (the graph and kernel partition the bench times) at the seeded
+    # formulas of the orbit golden: equal to the oracle's isomorphism-orbit sums
+    g = gold("n5_orbit.npz")
+    idx = g["index"]
+    same({key: results["K"][key][idx] for key in ("models", "frames")},
+         {key: g[key][:len(idx)] for key in ("models", "frames")}, "n=5 full K, whole batch", keys=("models", "frames"))
     # monotone in the class: refuted in a stronger class => refuted in every weaker one
     for weak, strong in (("K", "T"), ("T", "S4"), ("S4", "S5")):
         assert ((results[strong]["models"] > 0) <= (results[weak]["models"] > 0)).all()

@@ -485,3 +485,33 @@ def test_c_orbit_weighted_census_equals_direct_census(vol):
         w = vol.census_list(code, offs, n, 0, reps, weights=sizes, pairs=pairs)
         d = vol.census(code, offs, n, 0, K, pairs=pairs)
         assert (w["frames"] == d["frames"]).all() and (w["models"] == d["models"]).all()
+
+
+def test_py_distinguish_pinned_directly():
+    """The Python pair path against things fixed outside it (it used to be compared only with
+    distinguish_relations, which shares its formula):
+    - by hand on one world: []p and <>p differ exactly on the dead-end frame (both valuations, at world 0) and
+      coincide with p on the reflexive one;
+    - p and ~p differ at every world of every model; a formula never differs from itself;
+    - phi and T differ where phi fails, so the pair (phi, T) has the census of phi (pinned above by Table 9,
+      closed forms and hand-computed cases), including the witness;
+    - Table 3 / Prop. 5: alpha_1 and alpha_2 agree on every frame of <= 3 worlds and are
+      split by a four-world frame; the first such frame is accepted by the certificate checker."""
+    p, notp = prog("p"), prog("~p")
+    assert O.distinguish(prog("[]p"), prog("<>p"), 1, 1) == (2, 1, (0, 0, 0))
+    for n in (1, 2):
+        frames = 1 << (n * n)
+        assert O.distinguish(p, notp, n, 1) == (frames << n, frames, (0, 0, 0))
+        assert O.distinguish(prog("[]p -> p"), prog("[]p -> p"), n, 1) == (0, 0, (O.NO_WITNESS, 0, 0))
+    for text in ("[]p -> p", "p -> []<>p", "[](p -> q) -> ([]p -> []q)", "<>T"):
+        k = 2 if "q" in text else (1 if "p" in text else 0)
+        for cls in (K, T):
+            assert O.distinguish(prog(text), prog("T"), 2, k, cls) == O.census(prog(text), 2, k, cls), (text, cls)
+    a1, a2 = W.to_postfix(W.alpha(1)), W.to_postfix(W.alpha(2))
+    for n in (1, 2, 3):
+        assert O.distinguish(a1, a2, n, 0) == (0, 0, (O.NO_WITNESS, 0, 0))
+    models, frames, (f, v, w) = O.distinguish(a1, a2, 4, 0)
+    assert models == frames > 0 and v == 0                       # no variables: one valuation per frame
+    assert (frames, f, w) == (768, 328, 1)                       # SURVEY.md 8(c) scratch; the C oracle finds the same
+    assert O.check_pair_witness(a1, a2, 4, 0, K, f, v, w)
+    assert all(not O.check_pair_witness(a1, a2, 4, 0, K, g, 0, u) for g in range(0, f, 37) for u in range(4))
