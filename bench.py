@@ -221,8 +221,12 @@ def run_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started {world} rank(s); n_gpus is what ran")
     if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+        raise SystemExit(f"bench.py: no CUDA device on rank {rank} (there is no CPU fallback)")
+    if local_rank >= torch.cuda.device_count():
+        raise SystemExit(f"bench.py: rank {rank} wants cuda:{local_rank} but the node has {torch.cuda.device_count()} GPU(s)")
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
@@ -1026,6 +1030,20 @@ def main():
                          "about 20 minutes; recorded once in profiles/)")
     ap.add_argument("--atlas-skip-panels", action="store_true", help="atlas: only the HBM-write leg (for ncu captures)")
     args = ap.parse_args()
+    if args.impl == "ours" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # asked for N GPUs without a launcher: start the N ranks ourselves (one process per GPU, NCCL over NVLink)
+        # and let rank 0's line be the output
+        import socket
+        import subprocess
+        with socket.socket() as sock:
+            sock.bind(("127.0.0.1", 0))
+            port = sock.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
+    if args.impl == "ours" and args.workload not in ("c3", "c3_paper", "c3_small") and \
+            (args.gpus > 1 or int(os.environ.get("WORLD_SIZE", "1")) > 1):
+        raise SystemExit(f"bench.py: --workload {args.workload} is a one-GPU measurement; only the census layer shards")
     if args.impl == "reference":
         run_reference(args)
     elif args.workload == "c4":

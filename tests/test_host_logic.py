@@ -229,3 +229,24 @@ def test_no_cpu_fallback_without_cuda():
     with pytest.raises(kb.KripkeError) as e:
         kb.eval_batch_host(code, offs, 3, 2, 0)
     assert e.value.status == kb.ECUDA
+
+
+def test_bench_starts_one_rank_per_gpu_by_itself():
+    """`python bench.py --gpus 2` without a launcher re-executes itself under torch.distributed.run with two
+    ranks (one process per GPU).  On a box without a CUDA device both ranks must say so - there is
+    no CPU fallback (the launcher's failure report proves the run went through it) - and a rank count that differs from --gpus is refused rather than mislabelled."""
+    import subprocess
+    import sys
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("checks the no-device message; on a GPU box the driver's own bench runs cover the launcher")
+    bench = os.path.join(ROOT, "bench.py")
+    r = subprocess.run([sys.executable, bench, "--gpus", "2", "--steps", "1", "--warmup", "1"],
+                       capture_output=True, text=True, timeout=300)
+    assert r.returncode != 0 and not r.stdout.strip().startswith("{")
+    # the launcher stops the other rank as soon as one has failed, so only one of the two messages is certain
+    assert re.search(r"no CUDA device on rank [01]", r.stderr + r.stdout)
+    assert "torch.distributed" in r.stderr or "torchrun" in r.stderr or "ChildFailedError" in r.stderr
+    env = dict(os.environ, WORLD_SIZE="2", RANK="0", LOCAL_RANK="0")
+    r = subprocess.run([sys.executable, bench, "--gpus", "1"], capture_output=True, text=True, timeout=300, env=env)
+    assert r.returncode != 0 and "the launcher started 2 rank(s)" in r.stderr
