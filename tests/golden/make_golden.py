@@ -16,6 +16,12 @@ parts (sizes are oracle evaluations; times are for the 8-core build box at ~0.1 
   c5_counts   config 5: distinguishing-frame counts of every pair for n=1..5 (orbit route at
               n=5) and first witnesses for n<=4
 
+  c3_paper    the paper-shaped census corpus: the 44,678 constant-free formulas of <= 7 nodes over
+              {p, q}, one representative (first in enumeration order) per class of equal truth sets on all
+              models of <= 3 worlds (oracle signatures: 5,621) + the K axiom; at n=5: S4 and S5 in full,
+              8 seeded ranges of 2^10 frames of K and of T for every formula, and full-range K counts of
+              100 seeded two-variable representatives by the orbit route (1.7e11, ~25 min)
+
 Nothing here imports the CUDA path; no value comes from it.  Each .npz stores the corpus SHA-256
 so a test can tell that it is comparing the same bytes.
 """
@@ -136,6 +142,62 @@ def part_n5_orbit(threads):
          models=r["models"], frames=r["frames"])
 
 
+def paper_corpus():
+    """(programs, indices of the representatives in W.enumerate_constant_free(7, 2) order): P:143's reduction
+    done by the oracle's signatures; the K axiom is appended last (R19)."""
+    forms = W.enumerate_constant_free(7, 2)
+    progs = [W.to_postfix(t) for t in forms]
+    a, b = V.signatures(*W.pack_programs(progs), 3, 2)
+    first = {}
+    for i, s in enumerate(zip(a.tolist(), b.tolist())):
+        first.setdefault(s, i)
+    reps = sorted(first.values())
+    return [progs[i] for i in reps] + [W.to_postfix(W.named_axioms()["K"])], np.array(reps, np.uint32), len(progs)
+
+
+def part_c3_paper(threads):
+    progs, reps, n_enum = paper_corpus()
+    print(f"{n_enum} enumerated -> {len(reps)} representatives + K axiom")
+    code, offs = W.pack_programs(progs)
+    out = {"corpus_sha256": np.array(sha(progs)), "rep_index": reps, "n_enumerated": np.array(n_enum)}
+    for cname in ("S4", "S5"):
+        t = time.time()
+        r = V.census(code, offs, 5, 2, CLASSES[cname], threads=threads)
+        print(cname, "%.1fs" % (time.time() - t))
+        for key, val in r.items():
+            out[f"{cname}_{key}"] = val
+    width = 1 << 10
+    out["width"] = np.array(width)
+    for cname, total, seed in (("K", 1 << 25, 511), ("T", 1 << 20, 512)):
+        begins = seeded_ranges(seed, total, width, 8)
+        out[f"{cname}_begin"] = np.array(begins, np.uint64)
+        acc = {}
+        t = time.time()
+        for b in begins:
+            r = V.census(code, offs, 5, 2, CLASSES[cname], b, width, threads=threads)
+            for key, val in r.items():
+                acc.setdefault(key, []).append(val)
+        print(cname, "ranges %.1fs" % (time.time() - t))
+        for key, val in acc.items():
+            out[f"{cname}_{key}"] = np.stack(val)
+    # full-range K counts of 100 seeded representatives over both variables, by the orbit route
+    rng = W.SplitMix64(513)
+    two = [i for i, c in enumerate(progs) if b"\x10" in c and b"\x11" in c]
+    picked = set()
+    while len(picked) < 100:
+        picked.add(two[rng.below(len(two))])
+    idx = sorted(picked)
+    oc, oo = W.pack_programs([progs[i] for i in idx])
+    orb, sizes = V.orbits(5)
+    assert int(sizes.sum()) == 1 << 25
+    t = time.time()
+    r = V.census_list(oc, oo, 5, 2, orb, weights=sizes, threads=threads)
+    print("orbit census %.1fs" % (time.time() - t))
+    out["orbit_index"] = np.array(idx, np.uint32)
+    out["orbit_models"], out["orbit_frames"] = r["models"], r["frames"]
+    save("c3_paper_n5.npz", **out)
+
+
 def part_c4_ranges(threads):
     progs = W.corpus_c4()
     code, offs = W.pack_programs(progs)
@@ -165,7 +227,8 @@ def part_c5_counts(threads):
 
 
 PARTS = {"c2": part_c2, "n5_classes": part_n5_classes, "n5_ranges": part_n5_ranges,
-         "n5_orbit": part_n5_orbit, "n5_t_full": part_n5_t_full, "c4_ranges": part_c4_ranges, "c5_counts": part_c5_counts}
+         "n5_orbit": part_n5_orbit, "n5_t_full": part_n5_t_full, "c4_ranges": part_c4_ranges, "c5_counts": part_c5_counts,
+         "c3_paper": part_c3_paper}
 
 if __name__ == "__main__":
     ap = argparse.ArgumentParser()

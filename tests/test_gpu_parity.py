@@ -452,6 +452,46 @@ def test_h8_paper_frontier_on_gpu(kb, vol):
     assert len(surv["K"]) == 1
 
 
+def test_c3_paper_n5_whole_batch_golden(kb):
+    """The paper-shaped census corpus at n=5 (5,621 constant-free representatives + the K axiom; the second
+    workload bench.py reports) as ONE 5,622-formula batch against the oracle's stored values
+    (tests/golden/make_golden.py c3_paper): S4 and S5 in full, 8 seeded 2^10-frame windows of K and of T for every
+    formula, and the whole batch's full-range class-K counts against the orbit route at 100 seeded two-variable
+    representatives.  The representatives are rebuilt from the stored enumeration indices; the SHA-256 says they
+    are the bytes the oracle saw, and the GPU signature route (what bench.py uses) must pick the same ones."""
+    import hashlib
+    g = gold("c3_paper_n5.npz")
+    forms = W.enumerate_constant_free(7, 2)
+    assert len(forms) == int(g["n_enumerated"])
+    every = [W.to_postfix(t) for t in forms]
+    progs = [every[i] for i in g["rep_index"]] + [W.to_postfix(W.named_axioms()["K"])]
+    assert hashlib.sha256(b"\xff".join(progs)).hexdigest() == str(g["corpus_sha256"])
+    assert len(progs) == 5622
+    hall = kb.Programs(*W.pack_programs(every), 2)
+    first = {}
+    for i, sgn in enumerate(map(tuple, kb.signatures(hall, 2, 3).cpu().numpy().tolist())):
+        first.setdefault(sgn, i)
+    assert sorted(first.values()) == g["rep_index"].tolist()
+    hall.destroy()
+    h = kb.Programs(*W.pack_programs(progs), 2)
+    for cname in ("S4", "S5"):
+        same(run(kb, progs, 5, 2, CLS[cname], handle=h), {key: g[f"{cname}_{key}"] for key in KEYS}, f"C3-paper {cname}")
+    width = int(g["width"])
+    for cname in ("K", "T"):
+        for i, b in enumerate(g[f"{cname}_begin"]):
+            got = run(kb, progs, 5, 2, CLS[cname], int(b), width, handle=h)
+            same(got, {key: g[f"{cname}_{key}"][i] for key in KEYS}, f"C3-paper {cname} window at {int(b)}")
+    full = run(kb, progs, 5, 2, K, handle=h)
+    assert h.last_run_info().kernel_family == 2
+    idx = g["orbit_index"]
+    same({key: full[key][idx] for key in ("models", "frames")},
+         {"models": g["orbit_models"], "frames": g["orbit_frames"]}, "C3-paper full K, whole batch", keys=("models", "frames"))
+    certify(progs, full, 5, 2, K, idx=range(0, len(progs), 53))
+    # p -> p is the only representative no five-world model refutes (P:145), and the K axiom is never refuted
+    never = np.nonzero(full["models"] == 0)[0]
+    assert sorted(W.to_text(W.from_postfix(progs[b])) for b in never[:-1]) == ["(p->p)"] and never[-1] == len(progs) - 1
+
+
 def test_c5_pairs_separation_sizes(kb, vol):
     """Config 5 driver: separation size of every pair through five worlds against the stored oracle
     counts, and the paper's late separations at six worlds."""
